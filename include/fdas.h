@@ -1,0 +1,192 @@
+/*
+ * fdas.h -- C ABI of libfdas: the FDAS (Fourier Domain Acceleration Search) Fourier-domain
+ * convolution stage of arxiv 2206.12205 ("Bits missing: Finding exotic pulsars using
+ * bfloat16 on NVIDIA GPUs"), written from scratch for NVIDIA B200 (sm_100a).
+ *
+ * PAPER.md below is /root/reference/PAPER.md (text of the paper); DESIGN.md is this repo's.
+ *
+ * What the library computes:
+ *   the complex spectrum X[0..M-1] of a time series is convolved with a bank of K
+ *   constant-acceleration response templates h_z (Ransom et al. 2002, cited PAPER.md:37)
+ *   by the overlap-save method (Fig. 1), and the squared magnitude is
+ *   written as the f-fdot power plane
+ *        P[k][r] = | sum_{j=-m_k..m_k} X[r-j] h_{z_k}[j] |^2 ,  k = 0..K-1, r = 0..M-1,
+ *   with X = 0 outside [0, M), z_k = -zmax + k*dz, m_k = ceil(|z_k|/2) + 16, and
+ *   h_z[j] = conj( int_0^1 exp(2 pi i [ j u + (z/2)(u^2 - u) ]) du ).
+ *   Three precisions: fp64 ("gold standard"), fp32, and bf16 storage with
+ *   fp32 accumulation.
+ *
+ * Conventions
+ *   - Every function returns an fdas_status_t as int (0 = FDAS_OK).  The library never
+ *     throws, exits or prints.
+ *   - All pointers named *_dev are DEVICE pointers (e.g. a torch tensor's data_ptr()),
+ *     16-byte aligned.  Pointers named *_host are HOST pointers.  The caller owns them.
+ *     The library owns the plan and everything inside it (template bank, twiddle tables).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  All
+ *     GPU work is enqueued on it.  Only the *_host entry points and fdas_plan_destroy
+ *     synchronise.
+ *   - Output is bit-reproducible run to run (no atomics touch the plane).  The ORDER of
+ *     peak records is unspecified.
+ *   - A plan may be used from one host thread at a time; distinct plans are independent.
+ *   - There is no CPU fallback: without a CUDA device every compute entry point returns
+ *     FDAS_ERR_CUDA.
+ */
+#ifndef FDAS_H_
+#define FDAS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FDAS_VERSION_MAJOR 0
+#define FDAS_VERSION_MINOR 1
+
+typedef struct fdas_plan fdas_plan_t; /* opaque */
+
+/* Arithmetic / storage variant. */
+typedef enum {
+    FDAS_F64 = 0,  /* complex128 spectrum, fp64 bank and FFTs, double plane              */
+    FDAS_F32 = 1,  /* complex64 spectrum, fp32 bank and FFTs, float plane                */
+    FDAS_BF16 = 2  /* complex64 spectrum rounded to bf16 on load (RNE), bf16 bank, bf16
+                      staging between FFT passes, fp32 arithmetic, float plane
+                      ("bf16 storage / fp32 accumulate"; reading A12)          */
+} fdas_precision_t;
+
+typedef enum {
+    FDAS_OK = 0,
+    FDAS_ERR_INVALID_ARG = 1, /* NULL pointer, bad size, illegal parameter combination   */
+    FDAS_ERR_ALLOC = 2,       /* host or device allocation failed                        */
+    FDAS_ERR_CUDA = 3,        /* a CUDA call failed; see fdas_last_cuda_error            */
+    FDAS_ERR_NOT_BUILT = 4,   /* convolve/peaks before fdas_build_templates              */
+    FDAS_ERR_UNSUPPORTED = 5  /* legal request this build has no kernel for              */
+} fdas_status_t;
+
+/* One peak candidate (12 bytes). */
+typedef struct {
+    int32_t z_index; /* k, row of the plane; z = -zmax + k*dz                            */
+    int32_t r;       /* Fourier bin                                                      */
+    float power;     /* P[k][r] (rounded to float in FDAS_F64 mode)                      */
+} fdas_peak_t;
+
+typedef struct {
+    int64_t n_bins;          /* M = N/2 spectrum bins = plane columns                    */
+    int32_t n_templates;     /* K = 2*floor(zmax/dz) + 1                                 */
+    int32_t seglen;          /* S, overlap-save segment FFT length                       */
+    int32_t halfwidth_max;   /* m_max = ceil(zmax/2) + 16                                */
+    int32_t overlap_left;    /* L >= m_max: segment s starts at bin s*V - L              */
+    int32_t valid_per_seg;   /* V <= S - L - m_max: bins written per segment             */
+    int32_t precision;       /* fdas_precision_t                                         */
+    int64_t n_segments;      /* ceil(M / V)                                              */
+    int64_t plane_row_pitch; /* elements between plane rows (= M: rows are contiguous)   */
+    size_t plane_elem_bytes; /* 4 (float) or 8 (double, FDAS_F64)                        */
+    size_t spectrum_elem_bytes; /* 8 (complex64) or 16 (complex128, FDAS_F64)            */
+    size_t bank_bytes;       /* device bytes of the template bank                        */
+} fdas_info_t;
+
+/*
+ * fdas_plan_create -- fix the problem shape (BASELINE.json north_star: "fdas_plan_create(N,
+ * zmax, dz, seglen, precision)").
+ *   N        real samples of the time series; the spectrum has M = N/2 bins (bins
+ *            0..N/2-1 of the real FFT, Nyquist dropped; reading A8).  N even,
+ *            N >= 2*seglen.
+ *   zmax,dz  template grid z_k = -zmax + k*dz (Eq. 1: z = Fourier bin
+ *            drift).  zmax >= 0, dz > 0, K <= 4096.
+ *   seglen   overlap-save FFT length S: one of 256, 512, 1024, 2048,
+ *            4096, and S - 2*m_max >= 32.
+ *   precision fdas_precision_t.
+ * Allocates the template bank and tables on the current CUDA device.  *out is set to NULL
+ * on failure.  Errors: INVALID_ARG, UNSUPPORTED (seglen 8192), ALLOC, CUDA.
+ */
+int fdas_plan_create(fdas_plan_t **out, int64_t N, double zmax, double dz, int seglen,
+                     int precision);
+
+/* Frees the plan and its device memory (synchronises the device first).  NULL is OK. */
+int fdas_plan_destroy(fdas_plan_t *p);
+
+/* Copies the derived sizes into *info. */
+int fdas_plan_info(const fdas_plan_t *p, fdas_info_t *info);
+
+/* z_k = -zmax + k*dz for 0 <= k < K. */
+int fdas_z_of_index(const fdas_plan_t *p, int k, double *z);
+
+/*
+ * fdas_build_templates -- the template builder ("Each template is a 1D array
+ * of complex numbers ... generated ... then ... converted to bfloat16/double-precision by a
+ * tuned GPU kernel"; response function PAPER.md:37).  A GPU kernel evaluates the taps
+ * h_z[j], j = -m_z..m_z, in fp64, a second one takes their length-S DFT with the 1/S of the
+ * inverse transform folded in, H_z[f] = (1/S) sum_j h_z[j] exp(-2 pi i f j / S), and rounds
+ * once to the bank's storage type (fp64 / fp32 / bf16 RNE; reading A11).
+ * Asynchronous on `stream`.  Must complete (stream order) before fdas_convolve.
+ */
+int fdas_build_templates(fdas_plan_t *p, void *stream);
+
+/*
+ * fdas_convolve -- the fused hot path (PAPER.md:65-67 overlap-save; :59 power plane).
+ * One kernel: per segment, load S bins (zero outside [0,M)), forward FFT once, then for
+ * every template multiply by H_z, inverse FFT, |.|^2, and store only the V valid bins.
+ *   spectrum_dev  M interleaved complex (float2 for F32/BF16, double2 for F64)
+ *   plane_dev     [K][M] row-major, float (F32/BF16) or double (F64); fully overwritten
+ * Asynchronous on `stream`; no host synchronisation.
+ * Errors: INVALID_ARG (NULL), NOT_BUILT, CUDA.
+ */
+int fdas_convolve(fdas_plan_t *p, const void *spectrum_dev, void *plane_dev, void *stream);
+
+/*
+ * Batched form for independent series sharing one bank (BASELINE.json config 4):
+ * spectra_dev [batch][M], planes_dev [batch][K][M], both contiguous.  batch >= 1.
+ */
+int fdas_convolve_batched(fdas_plan_t *p, const void *spectra_dev, void *planes_dev, int batch,
+                          void *stream);
+
+/*
+ * fdas_peaks -- threshold / local-maximum pass over one plane (the
+ * analysis takes "the highest point" of a band; reading A14).  (k, r) is reported
+ * iff P[k][r] > threshold and P[k][r] >= each of its (up to 8) existing neighbours, strictly
+ * greater than those that precede it in (k, r) lexicographic order.
+ *   peaks_dev   device array of `capacity` records (may be NULL iff capacity == 0)
+ *   count_dev   device int32: receives the TOTAL number of peaks found (snprintf
+ *               convention: only min(count, capacity) records are written; overflow is not
+ *               an error).  The call zeroes it first, on `stream`.
+ * Record order is unspecified.  Asynchronous on `stream`.
+ */
+int fdas_peaks(fdas_plan_t *p, const void *plane_dev, float threshold, fdas_peak_t *peaks_dev,
+               int capacity, int *count_dev, void *stream);
+
+/*
+ * Host-buffer forms (end-to-end path): copy the spectrum host->device, run fdas_convolve
+ * (and fdas_peaks), copy the result device->host, on `stream`, then synchronise the stream.
+ * Device staging buffers are owned by the plan and allocated on first use.  Pinned host
+ * memory makes the copies asynchronous and fast; pageable memory also works.
+ *   fdas_convolve_host   plane_host receives [K][M]
+ *   fdas_search_host     convolve + peaks; the plane stays on the device; peaks_host
+ *                        receives min(count, capacity) records and *count_host the total.
+ */
+int fdas_convolve_host(fdas_plan_t *p, const void *spectrum_host, void *plane_host, void *stream);
+int fdas_search_host(fdas_plan_t *p, const void *spectrum_host, float threshold,
+                     fdas_peak_t *peaks_host, int capacity, int *count_host, void *stream);
+
+/*
+ * Debug / test access to the bank: copies H_z[f] in NATURAL order, [K][S] interleaved
+ * complex of the storage type (double2 / float2 / 2 x bf16 bit patterns), to host memory.
+ * `bytes` must equal K*S*2*sizeof(storage scalar).  Synchronises.
+ * fdas_taps_host copies the fp64 taps: for template k, 2*m_max+1 complex doubles
+ * (zero-padded beyond m_k), j = -m_max..m_max.  `bytes` = K*(2*m_max+1)*16.
+ */
+int fdas_templates_host(const fdas_plan_t *p, void *dst_host, size_t bytes);
+int fdas_taps_host(const fdas_plan_t *p, void *dst_host, size_t bytes);
+
+/* Number of kernels this plan has launched so far (template build + convolve + peaks). */
+int fdas_launch_count(const fdas_plan_t *p, int64_t *count);
+
+const char *fdas_status_string(int status);
+
+/* Last cudaError_t seen by this plan, as int (0 = cudaSuccess).  -1 if p is NULL. */
+int fdas_last_cuda_error(const fdas_plan_t *p);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FDAS_H_ */

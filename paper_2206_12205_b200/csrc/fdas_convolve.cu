@@ -1,0 +1,430 @@
+// fdas_convolve.cu -- the fused overlap-save convolution kernel (include/fdas.h: fdas_convolve).
+//
+// PAPER.md:65-67 (overlap-save: window the spectrum, convolve each window with every
+// template by FFT, keep the central region) and PAPER.md:59 (the result is the f-fdot power
+// plane).  In AstroAccelerate each arrow of Fig. 1 is a kernel or a library FFT with its
+// intermediate in HBM ("limited by memory bandwidth"); here one CTA does the
+// whole chain for one segment and a group of templates and only the V valid powers per
+// (segment, template) ever reach HBM.
+//
+// Transform structure (S = 16 * 16 * R3, T = S/16 threads, 16 points per thread):
+//   layout A : thread t, slot a  <-> index t + T a                     (input of a transform)
+//   pass 1   : 16-point DFT over a, twiddle W_S^(t k1), exchange through shared memory
+//   pass 2   : thread (k1, n3) = (t / R3, t % R3): 16-point DFT over n2, twiddle
+//              W_(16 R3)^(n3 k2), exchange
+//   pass 3   : R3-point DFTs; output index i = k1 + 16 k2 + 256 k3      (natural order)
+// The forward transform of the segment runs once per CTA through the same passes (real and
+// imaginary parts swapped) and is kept in registers (fp32) or shared memory (fp64) in layout
+// A; the bank is stored in layout A as well, so the per-template work is
+//   G = F * H_k  ->  pass 1..3  ->  |y|^2  ->  store bins [L, L+V).
+#include <cuda_bf16.h>
+#include "fdas_fft.cuh"
+#include "fdas_internal.h"
+
+namespace {
+
+using namespace fdas;
+
+struct ConvParams {
+    const void *spectra;  // [batch][M] complex
+    void *planes;         // [batch][K][M]
+    const void *bank;     // kernel-native order
+    const void *twiddle;  // [S] exp(+2 pi i j / S)
+    long long M;
+    long long n_seg;
+    int K, L, V;
+    int k_per_group;
+};
+
+// ---- per-precision traits -------------------------------------------------------------
+struct TraitsF64 {
+    using CT = double;
+    using CT2 = double2;
+    using PT = double;        // plane element
+    using E = double2;        // exchange element in shared memory
+    static constexpr int VC = 1;              // complexes per 16-byte bank vector
+    static constexpr bool F_IN_REGS = false;
+    static constexpr bool TW_IN_REGS = false;
+    static constexpr bool PREFETCH_H = false;
+    static constexpr bool ROUND_INPUT = false;
+    static constexpr int REG_TARGET = 255;
+    static __device__ __forceinline__ E pack(CT re, CT im) { return make_double2(re, im); }
+    static __device__ __forceinline__ void unpack(E v, CT &re, CT &im) { re = v.x; im = v.y; }
+    static __device__ __forceinline__ void bank_unpack(const uint4 &v, CT *re, CT *im)
+    {
+        re[0] = __longlong_as_double(((long long)v.y << 32) | v.x);
+        im[0] = __longlong_as_double(((long long)v.w << 32) | v.z);
+    }
+};
+
+struct TraitsF32 {
+    using CT = float;
+    using CT2 = float2;
+    using PT = float;
+    using E = float2;
+    static constexpr int VC = 2;
+    static constexpr bool F_IN_REGS = true;
+    static constexpr bool TW_IN_REGS = true;
+    static constexpr bool PREFETCH_H = true;
+    static constexpr bool ROUND_INPUT = false;
+    static constexpr int REG_TARGET = 168;
+    static __device__ __forceinline__ E pack(CT re, CT im) { return make_float2(re, im); }
+    static __device__ __forceinline__ void unpack(E v, CT &re, CT &im) { re = v.x; im = v.y; }
+    static __device__ __forceinline__ void bank_unpack(const uint4 &v, CT *re, CT *im)
+    {
+        re[0] = __uint_as_float(v.x); im[0] = __uint_as_float(v.y);
+        re[1] = __uint_as_float(v.z); im[1] = __uint_as_float(v.w);
+    }
+};
+
+// bf16 storage / fp32 accumulate (reading A12): spectrum rounded on load, bf16
+// bank, bf16 staging of every shared-memory exchange, fp32 arithmetic, fp32 plane.
+struct TraitsBF16 {
+    using CT = float;
+    using CT2 = float2;
+    using PT = float;
+    using E = unsigned int;   // packed bf16x2: low half = re, high half = im
+    static constexpr int VC = 4;
+    static constexpr bool F_IN_REGS = true;
+    static constexpr bool TW_IN_REGS = true;
+    static constexpr bool PREFETCH_H = true;
+    static constexpr bool ROUND_INPUT = true;
+    static constexpr int REG_TARGET = 168;
+    static __device__ __forceinline__ E pack(CT re, CT im)
+    {
+        __nv_bfloat162 v = __floats2bfloat162_rn(re, im);   // .x = re (low), .y = im (high)
+        return *reinterpret_cast<unsigned int *>(&v);
+    }
+    static __device__ __forceinline__ void unpack(E v, CT &re, CT &im)
+    {
+        re = __uint_as_float(v << 16);
+        im = __uint_as_float(v & 0xffff0000u);
+    }
+    static __device__ __forceinline__ void bank_unpack(const uint4 &v, CT *re, CT *im)
+    {
+        unpack(v.x, re[0], im[0]);
+        unpack(v.y, re[1], im[1]);
+        unpack(v.z, re[2], im[2]);
+        unpack(v.w, re[3], im[3]);
+    }
+};
+
+template <typename T> __device__ __forceinline__ T round_bf16(T x) { return x; }
+template <> __device__ __forceinline__ float round_bf16<float>(float x)
+{
+    return __bfloat162float(__float2bfloat16_rn(x));
+}
+
+template <typename PT> __device__ __forceinline__ void store_stream(PT *p, PT v) { __stcs(p, v); }
+__device__ __forceinline__ void store_stream2(float *p, float a, float b) { __stcs((float2 *)p, make_float2(a, b)); }
+__device__ __forceinline__ void store_stream2(double *p, double a, double b) { __stcs((double2 *)p, make_double2(a, b)); }
+
+template <class Tr, int S> struct Geo {
+    static constexpr int T = S / 16;
+    static constexpr int R3 = S / 256;
+    static constexpr int U = 16 / R3;                       // radix-R3 butterflies per thread
+    static constexpr int STR1 = T + R3;                     // exchange-1 row stride (elements)
+    static constexpr int EPW = 128 / (int)sizeof(typename Tr::E);   // elements per 128-byte wavefront
+    static constexpr int PAD2 = (EPW / R3) > 1 ? (EPW / R3) : 1;
+    static constexpr int STR2 = 256 + PAD2;                 // exchange-2 row stride
+    static constexpr int SM1 = 16 * STR1;                   // elements
+    static constexpr int SM2 = R3 * STR2;
+    static constexpr size_t XCH_BYTES = (size_t)(SM1 + SM2) * sizeof(typename Tr::E);
+    static constexpr size_t NAT_BYTES = (size_t)S * sizeof(typename Tr::CT2);   // natural-order view
+    static constexpr size_t XCH_REGION = XCH_BYTES > NAT_BYTES ? XCH_BYTES : NAT_BYTES;
+    static constexpr size_t F_BYTES = Tr::F_IN_REGS ? 0 : NAT_BYTES;
+    static constexpr size_t SMEM_BYTES = ((XCH_REGION + 15) / 16) * 16 + F_BYTES;
+    // resident CTAs per SM the register budget allows at Tr::REG_TARGET registers per thread
+    static constexpr int MIN_BLOCKS_RAW = 65536 / (T * Tr::REG_TARGET);
+    static constexpr int MIN_BLOCKS = MIN_BLOCKS_RAW < 1 ? 1 : (MIN_BLOCKS_RAW > 16 ? 16 : MIN_BLOCKS_RAW);
+    // pass-3 butterfly index handled by thread t, sub-index u
+    static __device__ __forceinline__ int bfly(int t, int u) { return (U <= 2) ? U * t + u : t + T * u; }
+};
+
+// Passes 1 and 2 of the inverse-sign transform.  In: layout A registers.  Out: exchange-2
+// buffer written and the CTA synchronised; pass 3 reads it.
+template <class Tr, int S, bool TWR>
+__device__ __forceinline__ void passes12(typename Tr::CT *re, typename Tr::CT *im, typename Tr::E *sm1,
+                                         typename Tr::E *sm2, const typename Tr::CT2 *__restrict__ tw,
+                                         const typename Tr::CT *tw1r, const typename Tr::CT *tw1i,
+                                         const typename Tr::CT *tw2r, const typename Tr::CT *tw2i, int t)
+{
+    using G = Geo<Tr, S>;
+    using CT = typename Tr::CT;
+    constexpr int R3 = G::R3;
+    const int n3 = t % R3, k1p = t / R3;
+    // ---- pass 1
+    Dft<CT, 16>::run(re, im);
+#pragma unroll
+    for (int k1 = 0; k1 < 16; ++k1) {
+        const int s = DftSlot<16>::of(k1);
+        if (k1 > 0) {
+            if constexpr (TWR) {
+                cmul(re[s], im[s], tw1r[k1], tw1i[k1]);
+            } else {
+                const typename Tr::CT2 w = tw[t * k1];
+                cmul(re[s], im[s], w.x, w.y);
+            }
+        }
+        sm1[k1 * G::STR1 + t] = Tr::pack(re[s], im[s]);
+    }
+    __syncthreads();
+    // ---- pass 2
+#pragma unroll
+    for (int n2 = 0; n2 < 16; ++n2) Tr::unpack(sm1[k1p * G::STR1 + n2 * R3 + n3], re[n2], im[n2]);
+    Dft<CT, 16>::run(re, im);
+#pragma unroll
+    for (int k2 = 0; k2 < 16; ++k2) {
+        const int s = DftSlot<16>::of(k2);
+        if (k2 > 0 && R3 > 1) {
+            if constexpr (TWR) {
+                cmul(re[s], im[s], tw2r[k2], tw2i[k2]);
+            } else {
+                const typename Tr::CT2 w = tw[16 * n3 * k2];
+                cmul(re[s], im[s], w.x, w.y);
+            }
+        }
+        sm2[n3 * G::STR2 + k1p + 16 * k2] = Tr::pack(re[s], im[s]);
+    }
+    __syncthreads();
+}
+
+// Pass 3 for butterfly sub-index u: leaves y[b + 256 k3] in (re, im)[DftSlot<R3>::of(k3)].
+template <class Tr, int S>
+__device__ __forceinline__ void pass3(typename Tr::CT *re, typename Tr::CT *im, const typename Tr::E *sm2, int b)
+{
+    using G = Geo<Tr, S>;
+#pragma unroll
+    for (int n3 = 0; n3 < G::R3; ++n3) Tr::unpack(sm2[n3 * G::STR2 + b], re[n3], im[n3]);
+    Dft<typename Tr::CT, G::R3>::run(re, im);
+}
+
+template <class Tr, int S>
+__global__ void __launch_bounds__(S / 16, Geo<Tr, S>::MIN_BLOCKS) fdas_convolve_kernel(const ConvParams p)
+{
+    using G = Geo<Tr, S>;
+    using CT = typename Tr::CT;
+    using CT2 = typename Tr::CT2;
+    using PT = typename Tr::PT;
+    using E = typename Tr::E;
+    constexpr int T = G::T, R3 = G::R3, U = G::U, VC = Tr::VC, NV = 16 / VC;
+    constexpr bool TWR = Tr::TW_IN_REGS;
+
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    E *sm1 = reinterpret_cast<E *>(smem_raw);
+    E *sm2 = sm1 + G::SM1;
+    CT2 *nat = reinterpret_cast<CT2 *>(smem_raw);  // natural-order view of the exchange region
+    CT2 *smF = reinterpret_cast<CT2 *>(smem_raw + ((G::XCH_REGION + 15) / 16) * 16);
+
+    const int t = threadIdx.x;
+    const long long seg = blockIdx.x % p.n_seg;
+    const long long ser = blockIdx.x / p.n_seg;
+    const int k_begin = blockIdx.y * p.k_per_group;
+    const int k_end = min(p.K, k_begin + p.k_per_group);
+    const CT2 *__restrict__ tw = static_cast<const CT2 *>(p.twiddle);
+    const int n3 = t % R3;
+
+    // twiddles that do not depend on the template
+    CT tw1r[TWR ? 16 : 1], tw1i[TWR ? 16 : 1], tw2r[TWR ? 16 : 1], tw2i[TWR ? 16 : 1];
+    if constexpr (TWR) {
+#pragma unroll
+        for (int k = 1; k < 16; ++k) {
+            CT2 w = tw[t * k];
+            tw1r[k] = w.x; tw1i[k] = w.y;
+            w = tw[16 * n3 * k];
+            tw2r[k] = w.x; tw2i[k] = w.y;
+        }
+    }
+
+    CT re[16], im[16];
+
+    // ---- segment load (layout A), zero outside [0, M)   ("splitting the long
+    //      input signal into windows")
+    {
+        const CT2 *__restrict__ X = static_cast<const CT2 *>(p.spectra) + ser * p.M;
+        const long long g0 = seg * p.V - p.L + t;
+#pragma unroll
+        for (int a = 0; a < 16; ++a) {
+            const long long g = g0 + (long long)T * a;
+            CT2 v;
+            v.x = 0; v.y = 0;
+            if (g >= 0 && g < p.M) v = X[g];
+            if (Tr::ROUND_INPUT) { v.x = round_bf16(v.x); v.y = round_bf16(v.y); }
+            // forward transform by the swap trick: feed (im, re)
+            re[a] = v.y;
+            im[a] = v.x;
+        }
+    }
+    // ---- forward FFT, once per segment
+    passes12<Tr, S, TWR>(re, im, sm1, sm2, tw, tw1r, tw1i, tw2r, tw2i, t);
+    {
+        CT2 fo[16];   // natural-order results of this thread: index bfly(t,u) + 256 k3
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            pass3<Tr, S>(re, im, sm2, G::bfly(t, u));
+#pragma unroll
+            for (int k3 = 0; k3 < R3; ++k3) {
+                const int s = DftSlot<R3>::of(k3);
+                fo[u * R3 + k3].x = im[s];   // un-swap
+                fo[u * R3 + k3].y = re[s];
+            }
+        }
+        __syncthreads();   // everyone is done reading sm2 before the natural-order view overwrites it
+        CT2 *dstF = Tr::F_IN_REGS ? nat : smF;
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+#pragma unroll
+            for (int k3 = 0; k3 < R3; ++k3) dstF[G::bfly(t, u) + 256 * k3] = fo[u * R3 + k3];
+        __syncthreads();
+    }
+    CT Fr[Tr::F_IN_REGS ? 16 : 1], Fi[Tr::F_IN_REGS ? 16 : 1];
+    if constexpr (Tr::F_IN_REGS) {
+#pragma unroll
+        for (int a = 0; a < 16; ++a) {
+            const CT2 v = nat[t + T * a];
+            Fr[a] = v.x; Fi[a] = v.y;
+        }
+        __syncthreads();   // nat aliases the exchange buffers
+    }
+
+    // ---- template loop
+    const uint4 *__restrict__ bank = static_cast<const uint4 *>(p.bank);
+    uint4 hv[Tr::PREFETCH_H ? NV : 1];
+    if constexpr (Tr::PREFETCH_H) if (k_begin < k_end) {
+#pragma unroll
+        for (int v = 0; v < NV; ++v) hv[v] = __ldg(bank + ((size_t)k_begin * NV + v) * T + t);
+    }
+    PT *plane = static_cast<PT *>(p.planes) + (size_t)ser * p.K * p.M;
+    const long long col0 = seg * p.V - p.L;   // plane column of output index i is col0 + i
+
+    for (int k = k_begin; k < k_end; ++k) {
+        // G = F * H_k   (PAPER.md:35 convolution theorem)
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+            uint4 h;
+            if constexpr (Tr::PREFETCH_H) h = hv[v];
+            else h = __ldg(bank + ((size_t)k * NV + v) * T + t);
+            CT hr[VC], hi[VC];
+            Tr::bank_unpack(h, hr, hi);
+#pragma unroll
+            for (int c = 0; c < VC; ++c) {
+                const int a = v * VC + c;
+                CT fr, fi;
+                if constexpr (Tr::F_IN_REGS) { fr = Fr[a]; fi = Fi[a]; }
+                else { const CT2 f = smF[t + T * a]; fr = f.x; fi = f.y; }
+                re[a] = fr * hr[c] - fi * hi[c];
+                im[a] = fr * hi[c] + fi * hr[c];
+            }
+        }
+        if constexpr (Tr::PREFETCH_H) if (k + 1 < k_end) {
+#pragma unroll
+            for (int v = 0; v < NV; ++v) hv[v] = __ldg(bank + ((size_t)(k + 1) * NV + v) * T + t);
+        }
+        // inverse FFT
+        passes12<Tr, S, TWR>(re, im, sm1, sm2, tw, tw1r, tw1i, tw2r, tw2i, t);
+        PT *row = plane + (size_t)k * p.M;
+        if constexpr (U == 2) {
+            CT pw[2][R3];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                pass3<Tr, S>(re, im, sm2, 2 * t + u);
+#pragma unroll
+                for (int k3 = 0; k3 < R3; ++k3) {
+                    const int s = DftSlot<R3>::of(k3);
+                    pw[u][k3] = re[s] * re[s] + im[s] * im[s];
+                }
+            }
+#pragma unroll
+            for (int k3 = 0; k3 < R3; ++k3) {
+                const int i = 2 * t + 256 * k3;
+                const long long col = col0 + i;
+                if (i >= p.L && i < p.L + p.V) {
+                    if (col + 1 < p.M && (p.M & 1) == 0) store_stream2(row + col, (PT)pw[0][k3], (PT)pw[1][k3]);
+                    else {
+                        if (col < p.M) store_stream(row + col, (PT)pw[0][k3]);
+                        if (col + 1 < p.M) store_stream(row + col + 1, (PT)pw[1][k3]);
+                    }
+                }
+            }
+        } else {
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int b = G::bfly(t, u);
+                pass3<Tr, S>(re, im, sm2, b);
+#pragma unroll
+                for (int k3 = 0; k3 < R3; ++k3) {
+                    const int s = DftSlot<R3>::of(k3);
+                    const int i = b + 256 * k3;
+                    const long long col = col0 + i;
+                    if (i >= p.L && i < p.L + p.V && col < p.M)
+                        store_stream(row + col, (PT)(re[s] * re[s] + im[s] * im[s]));
+                }
+            }
+        }
+        // no barrier needed here: the next template's first shared-memory write (exchange 1)
+        // touches sm1, whose last readers finished before this template's second barrier;
+        // sm2 is rewritten only after the next template's first barrier.
+    }
+}
+
+template <class Tr, int S>
+int launch_one(fdas_plan *p, const ConvParams &cp, int batch, int groups, cudaStream_t st)
+{
+    using G = Geo<Tr, S>;
+    auto kern = fdas_convolve_kernel<Tr, S>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        FDAS_CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM_BYTES));
+        attr_done = true;
+    }
+    const long long gx = (long long)batch * p->n_seg;
+    if (gx > 2147483647LL) return FDAS_ERR_INVALID_ARG;
+    kern<<<dim3((unsigned)gx, groups), G::T, G::SMEM_BYTES, st>>>(cp);
+    FDAS_CUDA_TRY(p, cudaGetLastError());
+    p->launches += 1;
+    return FDAS_OK;
+}
+
+template <class Tr>
+int launch_prec(fdas_plan *p, const ConvParams &cp, int batch, int groups, cudaStream_t st)
+{
+    switch (p->S) {
+    case 256: return launch_one<Tr, 256>(p, cp, batch, groups, st);
+    case 512: return launch_one<Tr, 512>(p, cp, batch, groups, st);
+    case 1024: return launch_one<Tr, 1024>(p, cp, batch, groups, st);
+    case 2048: return launch_one<Tr, 2048>(p, cp, batch, groups, st);
+    case 4096: return launch_one<Tr, 4096>(p, cp, batch, groups, st);
+    default: return FDAS_ERR_UNSUPPORTED;
+    }
+}
+
+}  // namespace
+
+int fdas_launch_convolve(fdas_plan *p, const void *spectra, void *planes, int batch, cudaStream_t st)
+{
+    ConvParams cp;
+    cp.spectra = spectra;
+    cp.planes = planes;
+    cp.bank = p->bank;
+    cp.twiddle = p->twiddle;
+    cp.M = p->M;
+    cp.n_seg = p->n_seg;
+    cp.K = p->K;
+    cp.L = p->L;
+    cp.V = p->V;
+    // Template groups: one forward FFT per (segment, group).  Split the K templates only
+    // when there are too few segments to fill the GPU (e.g. config 1: 35 segments).
+    const long long ctas = (long long)batch * p->n_seg;
+    const long long want = 8LL * p->num_sms;
+    int groups = 1;
+    if (ctas < want) groups = (int)((want + ctas - 1) / ctas);
+    if (groups > p->K) groups = p->K;
+    cp.k_per_group = (p->K + groups - 1) / groups;
+    groups = (p->K + cp.k_per_group - 1) / cp.k_per_group;
+    switch (p->precision) {
+    case FDAS_F64: return launch_prec<TraitsF64>(p, cp, batch, groups, st);
+    case FDAS_F32: return launch_prec<TraitsF32>(p, cp, batch, groups, st);
+    case FDAS_BF16: return launch_prec<TraitsBF16>(p, cp, batch, groups, st);
+    default: return FDAS_ERR_INVALID_ARG;
+    }
+}

@@ -1,0 +1,69 @@
+// fdas_internal.h -- plan layout and helpers shared by the libfdas translation units.
+// Product code: never includes or links anything under oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "fdas.h"
+
+// Points of the length-S transforms held per thread, and the derived kernel geometry
+// (DESIGN.md section 5):  S = 16 * 16 * R3,  T = S/16 threads per segment.
+#define FDAS_PTS 16
+
+struct fdas_plan {
+    // problem shape
+    int64_t N, M;
+    double zmax, dz;
+    int K, S, m_max, L, V, precision;
+    int64_t n_seg;
+    int T, R3;
+    // device objects owned by the plan
+    void *bank;        // [K][16/VC][T][VC] complex of the storage type (kernel-native order)
+    size_t bank_bytes;
+    double2 *taps;     // [K][2*m_max+1] fp64 taps h_z[j], zero padded
+    void *twiddle;     // [S] complex of the compute type: exp(+2 pi i j / S)
+    int built;
+    // host-buffer entry points: lazily allocated device staging
+    void *stage_spectrum, *stage_plane;
+    fdas_peak_t *stage_peaks;
+    int *stage_count;
+    int stage_peaks_capacity;
+    // bookkeeping
+    int device, num_sms;
+    cudaError_t last_err;
+    int64_t launches;
+};
+
+static inline size_t fdas_storage_scalar_bytes(int precision)
+{
+    return precision == FDAS_F64 ? 8 : (precision == FDAS_F32 ? 4 : 2);
+}
+
+// complexes of the storage type per 16-byte vector: 1 (fp64), 2 (fp32), 4 (bf16)
+static inline int fdas_bank_vc(int precision)
+{
+    return (int)(16 / (2 * fdas_storage_scalar_bytes(precision)));
+}
+
+// offset (in complex elements) of H_k[f] inside the kernel-native bank:
+// thread t = f % T holds slot a = f / T; slots are grouped VC at a time so that one
+// warp-wide 128-bit load covers 512 contiguous bytes.
+__host__ __device__ static inline size_t fdas_bank_offset(int k, int f, int T, int VC)
+{
+    int t = f % T, a = f / T;
+    return (((size_t)k * (FDAS_PTS / VC) + a / VC) * T + t) * VC + a % VC;
+}
+
+#define FDAS_CUDA_TRY(p, call)                                  \
+    do {                                                        \
+        cudaError_t e__ = (call);                               \
+        if (e__ != cudaSuccess) {                               \
+            if (p) (p)->last_err = e__;                         \
+            return FDAS_ERR_CUDA;                               \
+        }                                                       \
+    } while (0)
+
+// implemented in fdas_templates.cu / fdas_convolve.cu / fdas_peaks.cu
+int fdas_launch_build_templates(fdas_plan *p, cudaStream_t st);
+int fdas_launch_convolve(fdas_plan *p, const void *spectra, void *planes, int batch, cudaStream_t st);
+int fdas_launch_peaks(fdas_plan *p, const void *plane, float thr, fdas_peak_t *peaks, int capacity,
+                      int *count, cudaStream_t st);

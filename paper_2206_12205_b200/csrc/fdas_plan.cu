@@ -1,0 +1,265 @@
+// fdas_plan.cu -- plan lifetime, argument checking and the C-ABI entry points of libfdas.
+// Every entry point is documented in include/fdas.h.
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#include <new>
+#include <vector>
+#include "fdas_internal.h"
+
+static int halfwidth_of(double z) { return (int)ceil(fabs(z) / 2.0) + 16; }
+
+static void free_device_members(fdas_plan *p)
+{
+    cudaFree(p->bank);
+    cudaFree(p->taps);
+    cudaFree(p->twiddle);
+    cudaFree(p->stage_spectrum);
+    cudaFree(p->stage_plane);
+    cudaFree(p->stage_peaks);
+    cudaFree(p->stage_count);
+}
+
+extern "C" int fdas_plan_create(fdas_plan_t **out, int64_t N, double zmax, double dz, int seglen,
+                                int precision)
+{
+    if (!out) return FDAS_ERR_INVALID_ARG;
+    *out = NULL;
+    if (!(zmax >= 0.0) || !(dz > 0.0) || !isfinite(zmax) || !isfinite(dz)) return FDAS_ERR_INVALID_ARG;
+    if (precision != FDAS_F64 && precision != FDAS_F32 && precision != FDAS_BF16) return FDAS_ERR_INVALID_ARG;
+    if (seglen == 8192) return FDAS_ERR_UNSUPPORTED;
+    if (seglen != 256 && seglen != 512 && seglen != 1024 && seglen != 2048 && seglen != 4096)
+        return FDAS_ERR_INVALID_ARG;
+    if (N < 2 * (int64_t)seglen || (N & 1)) return FDAS_ERR_INVALID_ARG;
+    double kk = floor(zmax / dz + 1e-9);
+    if (kk > 2047.0) return FDAS_ERR_INVALID_ARG;
+    const int K = 2 * (int)kk + 1;
+    const int m_max = halfwidth_of(zmax);
+    const int L = (m_max + 31) / 32 * 32;
+    const int V = (seglen - L - m_max) / 32 * 32;
+    if (V < 32) return FDAS_ERR_INVALID_ARG;
+
+    fdas_plan *p = new (std::nothrow) fdas_plan;
+    if (!p) return FDAS_ERR_ALLOC;
+    memset(p, 0, sizeof(*p));
+    p->N = N;
+    p->M = N / 2;
+    p->zmax = zmax;
+    p->dz = dz;
+    p->K = K;
+    p->S = seglen;
+    p->m_max = m_max;
+    p->L = L;
+    p->V = V;
+    p->precision = precision;
+    p->n_seg = (p->M + V - 1) / V;
+    p->T = seglen / FDAS_PTS;
+    p->R3 = seglen / 256;
+    p->last_err = cudaSuccess;
+
+    cudaError_t e = cudaGetDevice(&p->device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, p->device);
+    if (e != cudaSuccess) {
+        delete p;
+        return FDAS_ERR_CUDA;
+    }
+    p->bank_bytes = (size_t)K * seglen * 2 * fdas_storage_scalar_bytes(precision);
+    const size_t tw_bytes = (size_t)seglen * (precision == FDAS_F64 ? sizeof(double2) : sizeof(float2));
+    const size_t taps_bytes = (size_t)K * (2 * m_max + 1) * sizeof(double2);
+    if ((e = cudaMalloc(&p->bank, p->bank_bytes)) != cudaSuccess ||
+        (e = cudaMalloc((void **)&p->taps, taps_bytes)) != cudaSuccess ||
+        (e = cudaMalloc(&p->twiddle, tw_bytes)) != cudaSuccess) {
+        free_device_members(p);
+        delete p;
+        cudaGetLastError();
+        return e == cudaErrorMemoryAllocation ? FDAS_ERR_ALLOC : FDAS_ERR_CUDA;
+    }
+    *out = p;
+    return FDAS_OK;
+}
+
+extern "C" int fdas_plan_destroy(fdas_plan_t *p)
+{
+    if (!p) return FDAS_OK;
+    cudaDeviceSynchronize();
+    free_device_members(p);
+    delete p;
+    return FDAS_OK;
+}
+
+extern "C" int fdas_plan_info(const fdas_plan_t *p, fdas_info_t *info)
+{
+    if (!p || !info) return FDAS_ERR_INVALID_ARG;
+    info->n_bins = p->M;
+    info->n_templates = p->K;
+    info->seglen = p->S;
+    info->halfwidth_max = p->m_max;
+    info->overlap_left = p->L;
+    info->valid_per_seg = p->V;
+    info->precision = p->precision;
+    info->n_segments = p->n_seg;
+    info->plane_row_pitch = p->M;
+    info->plane_elem_bytes = p->precision == FDAS_F64 ? 8 : 4;
+    info->spectrum_elem_bytes = p->precision == FDAS_F64 ? 16 : 8;
+    info->bank_bytes = p->bank_bytes;
+    return FDAS_OK;
+}
+
+extern "C" int fdas_z_of_index(const fdas_plan_t *p, int k, double *z)
+{
+    if (!p || !z || k < 0 || k >= p->K) return FDAS_ERR_INVALID_ARG;
+    *z = -p->zmax + k * p->dz;
+    return FDAS_OK;
+}
+
+extern "C" int fdas_build_templates(fdas_plan_t *p, void *stream)
+{
+    if (!p) return FDAS_ERR_INVALID_ARG;
+    int rc = fdas_launch_build_templates(p, (cudaStream_t)stream);
+    if (rc == FDAS_OK) p->built = 1;
+    return rc;
+}
+
+extern "C" int fdas_convolve_batched(fdas_plan_t *p, const void *spectra_dev, void *planes_dev,
+                                     int batch, void *stream)
+{
+    if (!p || !spectra_dev || !planes_dev || batch < 1) return FDAS_ERR_INVALID_ARG;
+    if (!p->built) return FDAS_ERR_NOT_BUILT;
+    return fdas_launch_convolve(p, spectra_dev, planes_dev, batch, (cudaStream_t)stream);
+}
+
+extern "C" int fdas_convolve(fdas_plan_t *p, const void *spectrum_dev, void *plane_dev, void *stream)
+{
+    return fdas_convolve_batched(p, spectrum_dev, plane_dev, 1, stream);
+}
+
+extern "C" int fdas_peaks(fdas_plan_t *p, const void *plane_dev, float threshold,
+                          fdas_peak_t *peaks_dev, int capacity, int *count_dev, void *stream)
+{
+    if (!p || !plane_dev || !count_dev || capacity < 0 || (capacity > 0 && !peaks_dev))
+        return FDAS_ERR_INVALID_ARG;
+    if (!p->built) return FDAS_ERR_NOT_BUILT;
+    return fdas_launch_peaks(p, plane_dev, threshold, peaks_dev, capacity, count_dev,
+                             (cudaStream_t)stream);
+}
+
+static int ensure_staging(fdas_plan *p, bool want_plane, int peaks_capacity)
+{
+    const size_t spec_bytes = (size_t)p->M * (p->precision == FDAS_F64 ? 16 : 8);
+    const size_t plane_bytes = (size_t)p->K * p->M * (p->precision == FDAS_F64 ? 8 : 4);
+    if (!p->stage_spectrum) FDAS_CUDA_TRY(p, cudaMalloc(&p->stage_spectrum, spec_bytes));
+    if (want_plane && !p->stage_plane) FDAS_CUDA_TRY(p, cudaMalloc(&p->stage_plane, plane_bytes));
+    if (!p->stage_count) FDAS_CUDA_TRY(p, cudaMalloc((void **)&p->stage_count, sizeof(int)));
+    if (peaks_capacity > p->stage_peaks_capacity) {
+        cudaFree(p->stage_peaks);
+        p->stage_peaks = NULL;
+        p->stage_peaks_capacity = 0;
+        FDAS_CUDA_TRY(p, cudaMalloc((void **)&p->stage_peaks, sizeof(fdas_peak_t) * (size_t)peaks_capacity));
+        p->stage_peaks_capacity = peaks_capacity;
+    }
+    return FDAS_OK;
+}
+
+extern "C" int fdas_convolve_host(fdas_plan_t *p, const void *spectrum_host, void *plane_host,
+                                  void *stream)
+{
+    if (!p || !spectrum_host || !plane_host) return FDAS_ERR_INVALID_ARG;
+    if (!p->built) return FDAS_ERR_NOT_BUILT;
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = ensure_staging(p, true, 0);
+    if (rc) return rc;
+    const size_t spec_bytes = (size_t)p->M * (p->precision == FDAS_F64 ? 16 : 8);
+    const size_t plane_bytes = (size_t)p->K * p->M * (p->precision == FDAS_F64 ? 8 : 4);
+    FDAS_CUDA_TRY(p, cudaMemcpyAsync(p->stage_spectrum, spectrum_host, spec_bytes, cudaMemcpyHostToDevice, st));
+    rc = fdas_launch_convolve(p, p->stage_spectrum, p->stage_plane, 1, st);
+    if (rc) return rc;
+    FDAS_CUDA_TRY(p, cudaMemcpyAsync(plane_host, p->stage_plane, plane_bytes, cudaMemcpyDeviceToHost, st));
+    FDAS_CUDA_TRY(p, cudaStreamSynchronize(st));
+    return FDAS_OK;
+}
+
+extern "C" int fdas_search_host(fdas_plan_t *p, const void *spectrum_host, float threshold,
+                                fdas_peak_t *peaks_host, int capacity, int *count_host, void *stream)
+{
+    if (!p || !spectrum_host || !count_host || capacity < 0 || (capacity > 0 && !peaks_host))
+        return FDAS_ERR_INVALID_ARG;
+    if (!p->built) return FDAS_ERR_NOT_BUILT;
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = ensure_staging(p, true, capacity);
+    if (rc) return rc;
+    const size_t spec_bytes = (size_t)p->M * (p->precision == FDAS_F64 ? 16 : 8);
+    FDAS_CUDA_TRY(p, cudaMemcpyAsync(p->stage_spectrum, spectrum_host, spec_bytes, cudaMemcpyHostToDevice, st));
+    rc = fdas_launch_convolve(p, p->stage_spectrum, p->stage_plane, 1, st);
+    if (rc) return rc;
+    rc = fdas_launch_peaks(p, p->stage_plane, threshold, p->stage_peaks, capacity, p->stage_count, st);
+    if (rc) return rc;
+    FDAS_CUDA_TRY(p, cudaMemcpyAsync(count_host, p->stage_count, sizeof(int), cudaMemcpyDeviceToHost, st));
+    FDAS_CUDA_TRY(p, cudaStreamSynchronize(st));
+    int n = *count_host < capacity ? *count_host : capacity;
+    if (n > 0) {
+        FDAS_CUDA_TRY(p, cudaMemcpyAsync(peaks_host, p->stage_peaks, sizeof(fdas_peak_t) * (size_t)n,
+                                         cudaMemcpyDeviceToHost, st));
+        FDAS_CUDA_TRY(p, cudaStreamSynchronize(st));
+    }
+    return FDAS_OK;
+}
+
+extern "C" int fdas_templates_host(const fdas_plan_t *p, void *dst_host, size_t bytes)
+{
+    if (!p || !dst_host) return FDAS_ERR_INVALID_ARG;
+    if (!p->built) return FDAS_ERR_NOT_BUILT;
+    if (bytes != p->bank_bytes) return FDAS_ERR_INVALID_ARG;
+    fdas_plan *q = const_cast<fdas_plan *>(p);
+    std::vector<unsigned char> tmp;
+    try {
+        tmp.resize(bytes);
+    } catch (...) {
+        return FDAS_ERR_ALLOC;
+    }
+    FDAS_CUDA_TRY(q, cudaDeviceSynchronize());
+    FDAS_CUDA_TRY(q, cudaMemcpy(tmp.data(), p->bank, bytes, cudaMemcpyDeviceToHost));
+    // kernel-native order -> natural [K][S]
+    const size_t cb = 2 * fdas_storage_scalar_bytes(p->precision);
+    const int VC = fdas_bank_vc(p->precision);
+    unsigned char *dst = (unsigned char *)dst_host;
+    for (int k = 0; k < p->K; ++k)
+        for (int f = 0; f < p->S; ++f)
+            memcpy(dst + ((size_t)k * p->S + f) * cb, tmp.data() + fdas_bank_offset(k, f, p->T, VC) * cb, cb);
+    return FDAS_OK;
+}
+
+extern "C" int fdas_taps_host(const fdas_plan_t *p, void *dst_host, size_t bytes)
+{
+    if (!p || !dst_host) return FDAS_ERR_INVALID_ARG;
+    if (!p->built) return FDAS_ERR_NOT_BUILT;
+    if (bytes != (size_t)p->K * (2 * p->m_max + 1) * sizeof(double2)) return FDAS_ERR_INVALID_ARG;
+    fdas_plan *q = const_cast<fdas_plan *>(p);
+    FDAS_CUDA_TRY(q, cudaDeviceSynchronize());
+    FDAS_CUDA_TRY(q, cudaMemcpy(dst_host, p->taps, bytes, cudaMemcpyDeviceToHost));
+    return FDAS_OK;
+}
+
+extern "C" int fdas_launch_count(const fdas_plan_t *p, int64_t *count)
+{
+    if (!p || !count) return FDAS_ERR_INVALID_ARG;
+    *count = p->launches;
+    return FDAS_OK;
+}
+
+extern "C" const char *fdas_status_string(int status)
+{
+    switch (status) {
+    case FDAS_OK: return "FDAS_OK";
+    case FDAS_ERR_INVALID_ARG: return "FDAS_ERR_INVALID_ARG";
+    case FDAS_ERR_ALLOC: return "FDAS_ERR_ALLOC";
+    case FDAS_ERR_CUDA: return "FDAS_ERR_CUDA";
+    case FDAS_ERR_NOT_BUILT: return "FDAS_ERR_NOT_BUILT";
+    case FDAS_ERR_UNSUPPORTED: return "FDAS_ERR_UNSUPPORTED";
+    default: return "FDAS_ERR_UNKNOWN";
+    }
+}
+
+extern "C" int fdas_last_cuda_error(const fdas_plan_t *p)
+{
+    return p ? (int)p->last_err : -1;
+}

@@ -1,0 +1,293 @@
+"""Thin ctypes binding over libfdas (include/fdas.h).  Argument marshalling only: every step
+of the path runs in the CUDA library.  The functions carry the C names; ``Plan`` is a small
+convenience wrapper that owns a plan handle and passes torch tensors' ``data_ptr()``.
+
+There is no CPU fallback: if ``libfdas.so`` has not been built, importing the library raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfdas.so")
+
+FDAS_F64, FDAS_F32, FDAS_BF16 = 0, 1, 2
+FDAS_OK, FDAS_ERR_INVALID_ARG, FDAS_ERR_ALLOC, FDAS_ERR_CUDA, FDAS_ERR_NOT_BUILT, FDAS_ERR_UNSUPPORTED = range(6)
+PRECISIONS = {"f64": FDAS_F64, "f32": FDAS_F32, "bf16": FDAS_BF16}
+
+EXPORTS = [
+    "fdas_plan_create", "fdas_plan_destroy", "fdas_plan_info", "fdas_z_of_index",
+    "fdas_build_templates", "fdas_convolve", "fdas_convolve_batched", "fdas_peaks",
+    "fdas_convolve_host", "fdas_search_host", "fdas_templates_host", "fdas_taps_host",
+    "fdas_launch_count", "fdas_status_string", "fdas_last_cuda_error",
+]
+
+
+class fdas_peak_t(ctypes.Structure):
+    _fields_ = [("z_index", ctypes.c_int32), ("r", ctypes.c_int32), ("power", ctypes.c_float)]
+
+
+class fdas_info_t(ctypes.Structure):
+    _fields_ = [
+        ("n_bins", ctypes.c_int64), ("n_templates", ctypes.c_int32), ("seglen", ctypes.c_int32),
+        ("halfwidth_max", ctypes.c_int32), ("overlap_left", ctypes.c_int32),
+        ("valid_per_seg", ctypes.c_int32), ("precision", ctypes.c_int32),
+        ("n_segments", ctypes.c_int64), ("plane_row_pitch", ctypes.c_int64),
+        ("plane_elem_bytes", ctypes.c_size_t), ("spectrum_elem_bytes", ctypes.c_size_t),
+        ("bank_bytes", ctypes.c_size_t),
+    ]
+
+
+_lib: Optional[ctypes.CDLL] = None
+
+
+def lib() -> ctypes.CDLL:
+    """Loads libfdas.so; raises if it is missing (no fallback of any kind)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(
+            f"{LIB_PATH} not found: build it with `python -m paper_2206_12205_b200._build` "
+            "(or __graft_entry__.build()); libfdas has no CPU fallback")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, i, i64, dbl = ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_double
+    L.fdas_plan_create.argtypes = [ctypes.POINTER(vp), i64, dbl, dbl, i, i]
+    L.fdas_plan_destroy.argtypes = [vp]
+    L.fdas_plan_info.argtypes = [vp, ctypes.POINTER(fdas_info_t)]
+    L.fdas_z_of_index.argtypes = [vp, i, ctypes.POINTER(dbl)]
+    L.fdas_build_templates.argtypes = [vp, vp]
+    L.fdas_convolve.argtypes = [vp, vp, vp, vp]
+    L.fdas_convolve_batched.argtypes = [vp, vp, vp, i, vp]
+    L.fdas_peaks.argtypes = [vp, vp, ctypes.c_float, vp, i, vp, vp]
+    L.fdas_convolve_host.argtypes = [vp, vp, vp, vp]
+    L.fdas_search_host.argtypes = [vp, vp, ctypes.c_float, vp, i, ctypes.POINTER(i), vp]
+    L.fdas_templates_host.argtypes = [vp, vp, ctypes.c_size_t]
+    L.fdas_taps_host.argtypes = [vp, vp, ctypes.c_size_t]
+    L.fdas_launch_count.argtypes = [vp, ctypes.POINTER(i64)]
+    L.fdas_status_string.argtypes = [i]
+    L.fdas_status_string.restype = ctypes.c_char_p
+    L.fdas_last_cuda_error.argtypes = [vp]
+    for name in EXPORTS:
+        if name != "fdas_status_string":
+            getattr(L, name).restype = i
+    _lib = L
+    return L
+
+
+class FdasError(RuntimeError):
+    def __init__(self, status: int, where: str, cuda_error: int = 0):
+        self.status = status
+        self.cuda_error = cuda_error
+        msg = lib().fdas_status_string(status).decode()
+        super().__init__(f"{where}: {msg}" + (f" (cudaError {cuda_error})" if cuda_error else ""))
+
+
+# ---- the C entry points under their own names (raw: return the status code) -------------
+def fdas_plan_create(N, zmax, dz, seglen, precision):
+    h = ctypes.c_void_p()
+    rc = lib().fdas_plan_create(ctypes.byref(h), int(N), float(zmax), float(dz), int(seglen), int(precision))
+    return rc, h
+
+
+def fdas_plan_destroy(h):
+    return lib().fdas_plan_destroy(h)
+
+
+def fdas_plan_info(h):
+    info = fdas_info_t()
+    rc = lib().fdas_plan_info(h, ctypes.byref(info))
+    return rc, info
+
+
+def fdas_z_of_index(h, k):
+    z = ctypes.c_double()
+    rc = lib().fdas_z_of_index(h, int(k), ctypes.byref(z))
+    return rc, z.value
+
+
+def fdas_build_templates(h, stream=0):
+    return lib().fdas_build_templates(h, ctypes.c_void_p(stream))
+
+
+def fdas_convolve(h, spectrum_ptr, plane_ptr, stream=0):
+    return lib().fdas_convolve(h, ctypes.c_void_p(spectrum_ptr), ctypes.c_void_p(plane_ptr), ctypes.c_void_p(stream))
+
+
+def fdas_convolve_batched(h, spectra_ptr, planes_ptr, batch, stream=0):
+    return lib().fdas_convolve_batched(h, ctypes.c_void_p(spectra_ptr), ctypes.c_void_p(planes_ptr), int(batch),
+                                       ctypes.c_void_p(stream))
+
+
+def fdas_peaks(h, plane_ptr, threshold, peaks_ptr, capacity, count_ptr, stream=0):
+    return lib().fdas_peaks(h, ctypes.c_void_p(plane_ptr), float(threshold), ctypes.c_void_p(peaks_ptr),
+                            int(capacity), ctypes.c_void_p(count_ptr), ctypes.c_void_p(stream))
+
+
+def fdas_convolve_host(h, spectrum_host_ptr, plane_host_ptr, stream=0):
+    return lib().fdas_convolve_host(h, ctypes.c_void_p(spectrum_host_ptr), ctypes.c_void_p(plane_host_ptr),
+                                    ctypes.c_void_p(stream))
+
+
+def fdas_search_host(h, spectrum_host_ptr, threshold, peaks_host_ptr, capacity, stream=0):
+    n = ctypes.c_int(0)
+    rc = lib().fdas_search_host(h, ctypes.c_void_p(spectrum_host_ptr), float(threshold),
+                                ctypes.c_void_p(peaks_host_ptr), int(capacity), ctypes.byref(n),
+                                ctypes.c_void_p(stream))
+    return rc, n.value
+
+
+def fdas_templates_host(h, dst_ptr, nbytes):
+    return lib().fdas_templates_host(h, ctypes.c_void_p(dst_ptr), int(nbytes))
+
+
+def fdas_taps_host(h, dst_ptr, nbytes):
+    return lib().fdas_taps_host(h, ctypes.c_void_p(dst_ptr), int(nbytes))
+
+
+def fdas_launch_count(h):
+    n = ctypes.c_int64()
+    rc = lib().fdas_launch_count(h, ctypes.byref(n))
+    return rc, n.value
+
+
+def fdas_status_string(status):
+    return lib().fdas_status_string(int(status)).decode()
+
+
+def fdas_last_cuda_error(h):
+    return lib().fdas_last_cuda_error(h)
+
+
+# ---- convenience wrapper ------------------------------------------------------------------
+class Plan:
+    """Owns one fdas_plan_t.  Tensors are torch CUDA tensors (device memory and streams are
+    torch's; all arithmetic is the library's)."""
+
+    def __init__(self, N: int, zmax: float, dz: float, seglen: int, precision="f32", build: bool = True,
+                 stream: int = 0):
+        prec = PRECISIONS[precision] if isinstance(precision, str) else int(precision)
+        rc, self._h = fdas_plan_create(N, zmax, dz, seglen, prec)
+        if rc:
+            self._h = None
+            raise FdasError(rc, "fdas_plan_create")
+        rc, self.info = fdas_plan_info(self._h)
+        self._check(rc, "fdas_plan_info")
+        self.precision = prec
+        if build:
+            self.build_templates(stream)
+
+    def _check(self, rc, where):
+        if rc:
+            raise FdasError(rc, where, fdas_last_cuda_error(self._h))
+
+    # shape helpers
+    @property
+    def M(self): return int(self.info.n_bins)
+    @property
+    def K(self): return int(self.info.n_templates)
+    @property
+    def S(self): return int(self.info.seglen)
+
+    def z_values(self):
+        return [fdas_z_of_index(self._h, k)[1] for k in range(self.K)]
+
+    def plane_dtype(self):
+        import torch
+        return torch.float64 if self.precision == FDAS_F64 else torch.float32
+
+    def spectrum_dtype(self):
+        import torch
+        return torch.complex128 if self.precision == FDAS_F64 else torch.complex64
+
+    def build_templates(self, stream: int = 0):
+        self._check(fdas_build_templates(self._h, stream), "fdas_build_templates")
+
+    def convolve(self, spectrum, plane=None, stream: Optional[int] = None):
+        """spectrum: CUDA tensor [M] (or [B, M]) complex64/complex128; returns plane [K, M] ([B, K, M])."""
+        import torch
+        assert spectrum.is_cuda and spectrum.is_contiguous() and spectrum.dtype == self.spectrum_dtype()
+        batch = 1 if spectrum.dim() == 1 else spectrum.shape[0]
+        assert spectrum.shape[-1] == self.M
+        shape = (self.K, self.M) if spectrum.dim() == 1 else (batch, self.K, self.M)
+        if plane is None:
+            plane = torch.empty(shape, dtype=self.plane_dtype(), device=spectrum.device)
+        assert plane.is_cuda and plane.is_contiguous() and tuple(plane.shape) == shape and plane.dtype == self.plane_dtype()
+        if stream is None:
+            stream = torch.cuda.current_stream().cuda_stream
+        self._check(fdas_convolve_batched(self._h, spectrum.data_ptr(), plane.data_ptr(), batch, stream),
+                    "fdas_convolve")
+        return plane
+
+    def peaks(self, plane, threshold: float, capacity: int = 1 << 16, stream: Optional[int] = None):
+        """Returns (total_count, records) with records a numpy structured array (z_index, r, power)."""
+        import numpy as np
+        import torch
+        assert plane.is_cuda and plane.is_contiguous() and tuple(plane.shape) == (self.K, self.M)
+        if stream is None:
+            stream = torch.cuda.current_stream().cuda_stream
+        buf = torch.empty(max(capacity, 1) * 3, dtype=torch.int32, device=plane.device)
+        cnt = torch.zeros(1, dtype=torch.int32, device=plane.device)
+        self._check(fdas_peaks(self._h, plane.data_ptr(), threshold, buf.data_ptr() if capacity else 0, capacity,
+                               cnt.data_ptr(), stream), "fdas_peaks")
+        n = int(cnt.item())
+        w = min(n, capacity)
+        raw = buf[: 3 * w].cpu().numpy().reshape(w, 3)
+        rec = np.zeros(w, dtype=[("z_index", np.int32), ("r", np.int32), ("power", np.float32)])
+        rec["z_index"] = raw[:, 0]
+        rec["r"] = raw[:, 1]
+        rec["power"] = raw[:, 2].copy().view(np.float32)
+        return n, rec
+
+    def convolve_host(self, spectrum_host, plane_host, stream: int = 0):
+        """numpy or pinned torch CPU buffers; copies are inside the call."""
+        self._check(fdas_convolve_host(self._h, _host_ptr(spectrum_host), _host_ptr(plane_host), stream),
+                    "fdas_convolve_host")
+        return plane_host
+
+    def search_host(self, spectrum_host, threshold: float, peaks_host, capacity: int, stream: int = 0):
+        rc, n = fdas_search_host(self._h, _host_ptr(spectrum_host), threshold, _host_ptr(peaks_host), capacity, stream)
+        self._check(rc, "fdas_search_host")
+        return n
+
+    def templates(self):
+        """Bank in natural order as numpy: complex128/complex64, or uint16 [K, S, 2] bit patterns for bf16."""
+        import numpy as np
+        if self.precision == FDAS_F64:
+            out = np.empty((self.K, self.S), dtype=np.complex128)
+        elif self.precision == FDAS_F32:
+            out = np.empty((self.K, self.S), dtype=np.complex64)
+        else:
+            out = np.empty((self.K, self.S, 2), dtype=np.uint16)
+        self._check(fdas_templates_host(self._h, out.ctypes.data, out.nbytes), "fdas_templates_host")
+        return out
+
+    def taps(self):
+        import numpy as np
+        m = int(self.info.halfwidth_max)
+        out = np.empty((self.K, 2 * m + 1), dtype=np.complex128)
+        self._check(fdas_taps_host(self._h, out.ctypes.data, out.nbytes), "fdas_taps_host")
+        return out
+
+    def launch_count(self) -> int:
+        return fdas_launch_count(self._h)[1]
+
+    def close(self):
+        if getattr(self, "_h", None):
+            fdas_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def _host_ptr(buf) -> int:
+    if hasattr(buf, "data_ptr"):
+        assert not buf.is_cuda
+        return buf.data_ptr()
+    return buf.ctypes.data
