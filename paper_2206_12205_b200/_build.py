@@ -32,28 +32,29 @@ def stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not stale():
+def build(force: bool = False, verbose: bool = False, extra_flags=(), out: str = LIB) -> str:
+    """extra_flags / out: build a tuning variant elsewhere (e.g. -DFDAS_F32_REGS=168)."""
+    if not force and out == LIB and not stale():
         return LIB
     objs = []
     procs = []
     for src in sources():
-        obj = os.path.join(CSRC, os.path.basename(src)[:-3] + ".o")
-        cmd = [NVCC, *FLAGS, "-c", src, "-o", obj]
+        obj = (out[:-3] + "_" if out != LIB else os.path.join(CSRC, "")) + os.path.basename(src)[:-3] + ".o"
+        cmd = [NVCC, *FLAGS, *extra_flags, "-c", src, "-o", obj]
         if verbose:
             cmd[1:1] = ["-Xptxas", "-v"]
         procs.append((src, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
         objs.append(obj)
     failed = False
     for src, pr in procs:
-        out, _ = pr.communicate()
+        log, _ = pr.communicate()
         if verbose or pr.returncode:
-            sys.stderr.write(out)
+            sys.stderr.write(log)
         failed |= pr.returncode != 0
     if failed:
         raise RuntimeError("nvcc failed")
-    subprocess.run([NVCC, "-shared", "-o", LIB, *objs, "-lcudart"], check=True)
-    return LIB
+    subprocess.run([NVCC, "-shared", "-o", out, *objs, "-lcudart"], check=True)
+    return out
 
 
 if __name__ == "__main__":

@@ -25,6 +25,17 @@ namespace {
 
 using namespace fdas;
 
+// Tuning knobs (defaults are the shipped configuration; overridable with -D for sweeps).
+#ifndef FDAS_F32_PREFETCH
+#define FDAS_F32_PREFETCH 1
+#endif
+#ifndef FDAS_F32_REGS
+#define FDAS_F32_REGS 128
+#endif
+#ifndef FDAS_BF16_REGS
+#define FDAS_BF16_REGS 128
+#endif
+
 struct ConvParams {
     const void *spectra;  // [batch][M] complex
     void *planes;         // [batch][K][M]
@@ -65,9 +76,9 @@ struct TraitsF32 {
     static constexpr int VC = 2;
     static constexpr bool F_IN_REGS = true;
     static constexpr bool TW_IN_REGS = true;
-    static constexpr bool PREFETCH_H = true;
+    static constexpr bool PREFETCH_H = FDAS_F32_PREFETCH != 0;
     static constexpr bool ROUND_INPUT = false;
-    static constexpr int REG_TARGET = 168;
+    static constexpr int REG_TARGET = FDAS_F32_REGS;
     static __device__ __forceinline__ E pack(CT re, CT im) { return make_float2(re, im); }
     static __device__ __forceinline__ void unpack(E v, CT &re, CT &im) { re = v.x; im = v.y; }
     static __device__ __forceinline__ void bank_unpack(const uint4 &v, CT *re, CT *im)
@@ -89,7 +100,7 @@ struct TraitsBF16 {
     static constexpr bool TW_IN_REGS = true;
     static constexpr bool PREFETCH_H = true;
     static constexpr bool ROUND_INPUT = true;
-    static constexpr int REG_TARGET = 168;
+    static constexpr int REG_TARGET = FDAS_BF16_REGS;
     static __device__ __forceinline__ E pack(CT re, CT im)
     {
         __nv_bfloat162 v = __floats2bfloat162_rn(re, im);   // .x = re (low), .y = im (high)
@@ -133,7 +144,9 @@ template <class Tr, int S> struct Geo {
     static constexpr size_t NAT_BYTES = (size_t)S * sizeof(typename Tr::CT2);   // natural-order view
     static constexpr size_t XCH_REGION = XCH_BYTES > NAT_BYTES ? XCH_BYTES : NAT_BYTES;
     static constexpr size_t F_BYTES = Tr::F_IN_REGS ? 0 : NAT_BYTES;
-    static constexpr size_t SMEM_BYTES = ((XCH_REGION + 15) / 16) * 16 + F_BYTES;
+    static constexpr size_t XCH_ALIGNED = ((XCH_REGION + 15) / 16) * 16;
+    static constexpr size_t TW2_BYTES = (size_t)16 * R3 * sizeof(typename Tr::CT2);   // [k2][n3] table
+    static constexpr size_t SMEM_BYTES = XCH_ALIGNED + F_BYTES + TW2_BYTES;
     // resident CTAs per SM the register budget allows at Tr::REG_TARGET registers per thread
     static constexpr int MIN_BLOCKS_RAW = 65536 / (T * Tr::REG_TARGET);
     static constexpr int MIN_BLOCKS = MIN_BLOCKS_RAW < 1 ? 1 : (MIN_BLOCKS_RAW > 16 ? 16 : MIN_BLOCKS_RAW);
@@ -142,12 +155,15 @@ template <class Tr, int S> struct Geo {
 };
 
 // Passes 1 and 2 of the inverse-sign transform.  In: layout A registers.  Out: exchange-2
-// buffer written and the CTA synchronised; pass 3 reads it.
+// buffer written and the CTA synchronised; pass 3 reads it.  Pass-1 twiddles W_S^(t k1) are
+// per-thread constants (registers, or the global table in fp64); pass-2 twiddles
+// W_(16 R3)^(n3 k2) come from a 16 x R3 shared-memory table (conflict-free: the R3 distinct
+// entries a warp needs for one k2 are contiguous).
 template <class Tr, int S, bool TWR>
 __device__ __forceinline__ void passes12(typename Tr::CT *re, typename Tr::CT *im, typename Tr::E *sm1,
                                          typename Tr::E *sm2, const typename Tr::CT2 *__restrict__ tw,
                                          const typename Tr::CT *tw1r, const typename Tr::CT *tw1i,
-                                         const typename Tr::CT *tw2r, const typename Tr::CT *tw2i, int t)
+                                         const typename Tr::CT2 *tw2, int t)
 {
     using G = Geo<Tr, S>;
     using CT = typename Tr::CT;
@@ -177,12 +193,8 @@ __device__ __forceinline__ void passes12(typename Tr::CT *re, typename Tr::CT *i
     for (int k2 = 0; k2 < 16; ++k2) {
         const int s = DftSlot<16>::of(k2);
         if (k2 > 0 && R3 > 1) {
-            if constexpr (TWR) {
-                cmul(re[s], im[s], tw2r[k2], tw2i[k2]);
-            } else {
-                const typename Tr::CT2 w = tw[16 * n3 * k2];
-                cmul(re[s], im[s], w.x, w.y);
-            }
+            const typename Tr::CT2 w = tw2[k2 * R3 + n3];
+            cmul(re[s], im[s], w.x, w.y);
         }
         sm2[n3 * G::STR2 + k1p + 16 * k2] = Tr::pack(re[s], im[s]);
     }
@@ -214,7 +226,7 @@ __global__ void __launch_bounds__(S / 16, Geo<Tr, S>::MIN_BLOCKS) fdas_convolve_
     E *sm1 = reinterpret_cast<E *>(smem_raw);
     E *sm2 = sm1 + G::SM1;
     CT2 *nat = reinterpret_cast<CT2 *>(smem_raw);  // natural-order view of the exchange region
-    CT2 *smF = reinterpret_cast<CT2 *>(smem_raw + ((G::XCH_REGION + 15) / 16) * 16);
+    CT2 *smF = reinterpret_cast<CT2 *>(smem_raw + G::XCH_ALIGNED);
 
     const int t = threadIdx.x;
     const long long seg = blockIdx.x % p.n_seg;
@@ -222,19 +234,19 @@ __global__ void __launch_bounds__(S / 16, Geo<Tr, S>::MIN_BLOCKS) fdas_convolve_
     const int k_begin = blockIdx.y * p.k_per_group;
     const int k_end = min(p.K, k_begin + p.k_per_group);
     const CT2 *__restrict__ tw = static_cast<const CT2 *>(p.twiddle);
-    const int n3 = t % R3;
 
     // twiddles that do not depend on the template
-    CT tw1r[TWR ? 16 : 1], tw1i[TWR ? 16 : 1], tw2r[TWR ? 16 : 1], tw2i[TWR ? 16 : 1];
+    CT2 *tw2 = reinterpret_cast<CT2 *>(smem_raw + G::XCH_ALIGNED + G::F_BYTES);
+    for (int e = t; e < 16 * R3; e += T) tw2[e] = tw[16 * (e % R3) * (e / R3)];
+    CT tw1r[TWR ? 16 : 1], tw1i[TWR ? 16 : 1];
     if constexpr (TWR) {
 #pragma unroll
         for (int k = 1; k < 16; ++k) {
-            CT2 w = tw[t * k];
+            const CT2 w = tw[t * k];
             tw1r[k] = w.x; tw1i[k] = w.y;
-            w = tw[16 * n3 * k];
-            tw2r[k] = w.x; tw2i[k] = w.y;
         }
     }
+    // (the first __syncthreads inside passes12 orders the tw2 table writes before its reads)
 
     CT re[16], im[16];
 
@@ -256,7 +268,7 @@ __global__ void __launch_bounds__(S / 16, Geo<Tr, S>::MIN_BLOCKS) fdas_convolve_
         }
     }
     // ---- forward FFT, once per segment
-    passes12<Tr, S, TWR>(re, im, sm1, sm2, tw, tw1r, tw1i, tw2r, tw2i, t);
+    passes12<Tr, S, TWR>(re, im, sm1, sm2, tw, tw1r, tw1i, tw2, t);
     {
         CT2 fo[16];   // natural-order results of this thread: index bfly(t,u) + 256 k3
 #pragma unroll
@@ -294,9 +306,23 @@ __global__ void __launch_bounds__(S / 16, Geo<Tr, S>::MIN_BLOCKS) fdas_convolve_
 #pragma unroll
         for (int v = 0; v < NV; ++v) hv[v] = __ldg(bank + ((size_t)k_begin * NV + v) * T + t);
     }
-    PT *plane = static_cast<PT *>(p.planes) + (size_t)ser * p.K * p.M;
+    // Output bookkeeping that does not depend on the template: which of this thread's 16
+    // outputs (u, k3) -> i = bfly(t,u) + 256 k3 fall in the valid window [L, L+V) and inside
+    // the plane ("discarding the contaminated regions at the edge of the windows").
     const long long col0 = seg * p.V - p.L;   // plane column of output index i is col0 + i
+    const bool vec2 = (U == 2) && ((p.M & 1) == 0);
+    unsigned vmask = 0;
+#pragma unroll
+    for (int u = 0; u < U; ++u)
+#pragma unroll
+        for (int k3 = 0; k3 < R3; ++k3) {
+            const int i = G::bfly(t, u) + 256 * k3;
+            if (i >= p.L && i < p.L + p.V && col0 + i < p.M) vmask |= 1u << (u * R3 + k3);
+        }
+    const long long out_off = (long long)ser * p.K * p.M + col0 + G::bfly(t, 0);   // + k*M per template
+    PT *const plane = static_cast<PT *>(p.planes);
 
+#pragma unroll 1
     for (int k = k_begin; k < k_end; ++k) {
         // G = F * H_k   (PAPER.md:35 convolution theorem)
 #pragma unroll
@@ -321,8 +347,8 @@ __global__ void __launch_bounds__(S / 16, Geo<Tr, S>::MIN_BLOCKS) fdas_convolve_
             for (int v = 0; v < NV; ++v) hv[v] = __ldg(bank + ((size_t)(k + 1) * NV + v) * T + t);
         }
         // inverse FFT
-        passes12<Tr, S, TWR>(re, im, sm1, sm2, tw, tw1r, tw1i, tw2r, tw2i, t);
-        PT *row = plane + (size_t)k * p.M;
+        passes12<Tr, S, TWR>(re, im, sm1, sm2, tw, tw1r, tw1i, tw2, t);
+        PT *const row = plane + (out_off + (long long)k * p.M);   // &P[k][col0 + bfly(t,0)]
         if constexpr (U == 2) {
             CT pw[2][R3];
 #pragma unroll
@@ -334,30 +360,27 @@ __global__ void __launch_bounds__(S / 16, Geo<Tr, S>::MIN_BLOCKS) fdas_convolve_
                     pw[u][k3] = re[s] * re[s] + im[s] * im[s];
                 }
             }
+            if (vec2) {
 #pragma unroll
-            for (int k3 = 0; k3 < R3; ++k3) {
-                const int i = 2 * t + 256 * k3;
-                const long long col = col0 + i;
-                if (i >= p.L && i < p.L + p.V) {
-                    if (col + 1 < p.M && (p.M & 1) == 0) store_stream2(row + col, (PT)pw[0][k3], (PT)pw[1][k3]);
-                    else {
-                        if (col < p.M) store_stream(row + col, (PT)pw[0][k3]);
-                        if (col + 1 < p.M) store_stream(row + col + 1, (PT)pw[1][k3]);
-                    }
+                for (int k3 = 0; k3 < R3; ++k3)
+                    if (vmask & (1u << k3)) store_stream2(row + 256 * k3, (PT)pw[0][k3], (PT)pw[1][k3]);
+            } else {
+#pragma unroll
+                for (int k3 = 0; k3 < R3; ++k3) {
+                    if (vmask & (1u << k3)) store_stream(row + 256 * k3, (PT)pw[0][k3]);
+                    if (vmask & (1u << (R3 + k3))) store_stream(row + 256 * k3 + 1, (PT)pw[1][k3]);
                 }
             }
         } else {
 #pragma unroll
             for (int u = 0; u < U; ++u) {
-                const int b = G::bfly(t, u);
-                pass3<Tr, S>(re, im, sm2, b);
+                pass3<Tr, S>(re, im, sm2, G::bfly(t, u));
 #pragma unroll
                 for (int k3 = 0; k3 < R3; ++k3) {
                     const int s = DftSlot<R3>::of(k3);
-                    const int i = b + 256 * k3;
-                    const long long col = col0 + i;
-                    if (i >= p.L && i < p.L + p.V && col < p.M)
-                        store_stream(row + col, (PT)(re[s] * re[s] + im[s] * im[s]));
+                    if (vmask & (1u << (u * R3 + k3)))
+                        store_stream(row + (G::bfly(t, u) - G::bfly(t, 0)) + 256 * k3,
+                                     (PT)(re[s] * re[s] + im[s] * im[s]));
                 }
             }
         }

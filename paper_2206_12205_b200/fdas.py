@@ -11,7 +11,7 @@ import os
 from typing import Optional
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libfdas.so")
+LIB_PATH = os.environ.get("FDAS_LIBRARY", os.path.join(_HERE, "libfdas.so"))   # FDAS_LIBRARY: alternative build of the same library
 
 FDAS_F64, FDAS_F32, FDAS_BF16 = 0, 1, 2
 FDAS_OK, FDAS_ERR_INVALID_ARG, FDAS_ERR_ALLOC, FDAS_ERR_CUDA, FDAS_ERR_NOT_BUILT, FDAS_ERR_UNSUPPORTED = range(6)
