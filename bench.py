@@ -174,7 +174,7 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_2206_12205_b200 import _build, fdas, workloads
+    from paper_2206_12205_b200 import _build, fdas, sharding, workloads
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: libfdas has no CPU fallback")
@@ -242,11 +242,7 @@ def main():
                 dist.barrier()
         conv_ms = [a.elapsed_time(b) for a, b, c in ev]
         step_ms = [a.elapsed_time(c) for a, b, c in ev]
-        total_ms = float(sum(step_ms))
-        if world > 1:
-            t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            total_ms = float(t.item())
+        total_ms = sharding.max_over_ranks(float(sum(step_ms)), device="cuda")
         n_found = int(count_dev.item())
 
         # ---- end to end through the host-buffer entry point (H2D spectrum, convolve, peaks, D2H result)
@@ -259,10 +255,7 @@ def main():
             n_e2e = plan.search_host(x_pin, THRESH, peaks_pin, PEAK_CAPACITY, sptr)
         torch.cuda.synchronize()
         e2e_s = (time.perf_counter() - t0) / e2e_steps
-        if world > 1:
-            t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e2e_s = float(t.item())
+        e2e_s = sharding.max_over_ranks(e2e_s, device="cuda")
         results[prec] = dict(K=K, M=M, S=S, V=V, conv_ms=float(np.mean(conv_ms)), conv_ms_min=float(np.min(conv_ms)),
                              step_ms=total_ms / args.steps, launches=launches, n_found=n_found,
                              e2e_s=e2e_s, n_e2e=n_e2e)
@@ -293,7 +286,7 @@ def main():
 
     cpu = None
     if not args.no_cpu_baseline:
-        v, dt, cores, desc = time_oracle_sample(w.spectrum, 1 << 20)
+        v, dt, cores, desc = time_oracle_sample(w.spectrum, 1 << 22)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc, "seconds": dt}
 
     line = {

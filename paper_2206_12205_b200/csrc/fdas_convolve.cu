@@ -30,7 +30,7 @@ using namespace fdas;
 #define FDAS_F32_PREFETCH 1
 #endif
 #ifndef FDAS_F32_REGS
-#define FDAS_F32_REGS 128
+#define FDAS_F32_REGS 168
 #endif
 #ifndef FDAS_BF16_REGS
 #define FDAS_BF16_REGS 128
