@@ -50,10 +50,18 @@ typedef struct fdas_plan fdas_plan_t; /* opaque */
 typedef enum {
     FDAS_F64 = 0,  /* complex128 spectrum, fp64 bank and FFTs, double plane              */
     FDAS_F32 = 1,  /* complex64 spectrum, fp32 bank and FFTs, float plane                */
-    FDAS_BF16 = 2  /* complex64 spectrum rounded to bf16 on load (RNE), bf16 bank, bf16
-                      staging between FFT passes, fp32 arithmetic, float plane
-                      ("bf16 storage / fp32 accumulate"; reading A12)          */
+    FDAS_BF16 = 2  /* complex64 spectrum rounded to bf16 on load (RNE), bf16 templates, fp32
+                      accumulation, float plane ("bf16 storage / fp32 accumulate"; DESIGN.md
+                      reading A12); see fdas_set_algorithm for the two evaluation orders     */
 } fdas_precision_t;
+
+/* How fdas_convolve evaluates the convolution (fdas_set_algorithm). */
+typedef enum {
+    FDAS_ALGO_AUTO = 0, /* default: FDAS_ALGO_MMA where it applies (FDAS_BF16), else FDAS_ALGO_FFT */
+    FDAS_ALGO_FFT = 1,  /* overlap-save FFTs on the fp32/fp64 ALUs, all precisions */
+    FDAS_ALGO_MMA = 2   /* FDAS_BF16 only: the same linear convolution as a bf16 x bf16 -> fp32
+                           tensor-core contraction over the taps (tcgen05), no FFT            */
+} fdas_algorithm_t;
 
 typedef enum {
     FDAS_OK = 0,
@@ -102,6 +110,22 @@ typedef struct {
  */
 int fdas_plan_create(fdas_plan_t **out, int64_t N, double zmax, double dz, int seglen,
                      int precision);
+
+/*
+ * fdas_set_algorithm -- choose how fdas_convolve evaluates Y_z[r] = sum_j X[r-j] h_z[j]
+ * (PAPER.md:35, :59).  Both algorithms compute the same plane; they differ in rounding points:
+ *   FDAS_ALGO_FFT  overlap-save FFTs; in FDAS_BF16 the spectrum, the FFT'd
+ *                  bank and every inter-pass exchange are rounded to bf16.
+ *   FDAS_ALGO_MMA  FDAS_BF16 only.  The spectrum and the taps h_z[j] are rounded to bf16 once
+ *                  (RNE) and the sum over the <= 2 m_max + 1 taps runs on the tensor cores with
+ *                  fp32 accumulation ("bf16 storage / fp32 accumulate", north_star).  Needs
+ *                  m_max <= 255.
+ * Errors: INVALID_ARG (NULL, unknown value), UNSUPPORTED (FDAS_ALGO_MMA on a plan that is not
+ * FDAS_BF16 or whose taps do not fit).  fdas_get_algorithm reports the algorithm fdas_convolve
+ * will run (FDAS_ALGO_FFT or FDAS_ALGO_MMA, never AUTO).
+ */
+int fdas_set_algorithm(fdas_plan_t *p, int algorithm);
+int fdas_get_algorithm(const fdas_plan_t *p, int *algorithm);
 
 /* Frees the plan and its device memory (synchronises the device first).  NULL is OK. */
 int fdas_plan_destroy(fdas_plan_t *p);
@@ -177,6 +201,13 @@ int fdas_search_host(fdas_plan_t *p, const void *spectrum_host, float threshold,
  */
 int fdas_templates_host(const fdas_plan_t *p, void *dst_host, size_t bytes);
 int fdas_taps_host(const fdas_plan_t *p, void *dst_host, size_t bytes);
+/*
+ * FDAS_BF16 plans only: the bf16 taps the tensor-core path multiplies with (PAPER.md:105
+ * "converted to bfloat16"), un-permuted from its tap-matrix image: [K][2*m_max+1][2] uint16
+ * bit patterns (re, im), j = -m_max..m_max.  `bytes` = K*(2*m_max+1)*4.  Synchronises.
+ * Errors: UNSUPPORTED when the plan has no tap matrix.
+ */
+int fdas_tapmatrix_host(const fdas_plan_t *p, void *dst_host, size_t bytes);
 
 /* Number of kernels this plan has launched so far (template build + convolve + peaks). */
 int fdas_launch_count(const fdas_plan_t *p, int64_t *count);

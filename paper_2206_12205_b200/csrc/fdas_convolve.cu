@@ -425,6 +425,7 @@ int launch_prec(fdas_plan *p, const ConvParams &cp, int batch, int groups, cudaS
 
 int fdas_launch_convolve(fdas_plan *p, const void *spectra, void *planes, int batch, cudaStream_t st)
 {
+    if (fdas_uses_mma(p)) return fdas_launch_convolve_mma(p, spectra, planes, batch, st);
     ConvParams cp;
     cp.spectra = spectra;
     cp.planes = planes;

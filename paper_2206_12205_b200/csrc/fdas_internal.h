@@ -22,6 +22,14 @@ struct fdas_plan {
     double2 *taps;     // [K][2*m_max+1] fp64 taps h_z[j], zero padded
     void *twiddle;     // [S] complex of the compute type: exp(+2 pi i j / S)
     int built;
+    // tensor-core path of the bf16 variant (fdas_mma.cu): tap matrix image and |z| tables
+    int algo;          // fdas_algorithm_t requested by the caller
+    int tc_supported;  // the MMA kernel can run this shape
+    int tc_groups, tc_nzg, tc_NT, tc_KS, tc_full_chunks;
+    void *tc_bmat;     // [groups][2 KS][NT][8] bf16
+    size_t tc_bmat_bytes;
+    int2 *tc_ktab;     // [groups][nzg] plane rows of (+|z|, -|z|), -1 where absent
+    int2 *tc_kref;     // [groups][nzg] (template whose taps fill the columns, its sign)
     // host-buffer entry points: lazily allocated device staging
     void *stage_spectrum, *stage_plane;
     fdas_peak_t *stage_peaks;
@@ -65,5 +73,14 @@ __host__ __device__ static inline size_t fdas_bank_offset(int k, int f, int T, i
 // implemented in fdas_templates.cu / fdas_convolve.cu / fdas_peaks.cu
 int fdas_launch_build_templates(fdas_plan *p, cudaStream_t st);
 int fdas_launch_convolve(fdas_plan *p, const void *spectra, void *planes, int batch, cudaStream_t st);
+// fdas_mma.cu: host-side grouping (plan creation), tap matrix build, the tcgen05 convolution
+int fdas_mma_plan(fdas_plan *p);
+int fdas_launch_build_tapmatrix(fdas_plan *p, cudaStream_t st);
+int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, int batch, cudaStream_t st);
+// true when fdas_convolve runs the tensor-core kernel for this plan
+static inline int fdas_uses_mma(const fdas_plan *p)
+{
+    return p->precision == FDAS_BF16 && p->tc_supported && p->algo != FDAS_ALGO_FFT;
+}
 int fdas_launch_peaks(fdas_plan *p, const void *plane, float thr, fdas_peak_t *peaks, int capacity,
                       int *count, cudaStream_t st);

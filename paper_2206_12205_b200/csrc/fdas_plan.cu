@@ -14,6 +14,9 @@ static void free_device_members(fdas_plan *p)
     cudaFree(p->bank);
     cudaFree(p->taps);
     cudaFree(p->twiddle);
+    cudaFree(p->tc_bmat);
+    cudaFree(p->tc_ktab);
+    cudaFree(p->tc_kref);
     cudaFree(p->stage_spectrum);
     cudaFree(p->stage_plane);
     cudaFree(p->stage_peaks);
@@ -74,7 +77,31 @@ extern "C" int fdas_plan_create(fdas_plan_t **out, int64_t N, double zmax, doubl
         cudaGetLastError();
         return e == cudaErrorMemoryAllocation ? FDAS_ERR_ALLOC : FDAS_ERR_CUDA;
     }
+    const int rc = fdas_mma_plan(p);
+    if (rc != FDAS_OK) {
+        free_device_members(p);
+        delete p;
+        cudaGetLastError();
+        return rc;
+    }
     *out = p;
+    return FDAS_OK;
+}
+
+extern "C" int fdas_set_algorithm(fdas_plan_t *p, int algorithm)
+{
+    if (!p) return FDAS_ERR_INVALID_ARG;
+    if (algorithm != FDAS_ALGO_AUTO && algorithm != FDAS_ALGO_FFT && algorithm != FDAS_ALGO_MMA)
+        return FDAS_ERR_INVALID_ARG;
+    if (algorithm == FDAS_ALGO_MMA && !(p->precision == FDAS_BF16 && p->tc_supported)) return FDAS_ERR_UNSUPPORTED;
+    p->algo = algorithm;
+    return FDAS_OK;
+}
+
+extern "C" int fdas_get_algorithm(const fdas_plan_t *p, int *algorithm)
+{
+    if (!p || !algorithm) return FDAS_ERR_INVALID_ARG;
+    *algorithm = fdas_uses_mma(p) ? FDAS_ALGO_MMA : FDAS_ALGO_FFT;
     return FDAS_OK;
 }
 
@@ -116,6 +143,7 @@ extern "C" int fdas_build_templates(fdas_plan_t *p, void *stream)
 {
     if (!p) return FDAS_ERR_INVALID_ARG;
     int rc = fdas_launch_build_templates(p, (cudaStream_t)stream);
+    if (rc == FDAS_OK) rc = fdas_launch_build_tapmatrix(p, (cudaStream_t)stream);
     if (rc == FDAS_OK) p->built = 1;
     return rc;
 }
@@ -236,6 +264,49 @@ extern "C" int fdas_taps_host(const fdas_plan_t *p, void *dst_host, size_t bytes
     fdas_plan *q = const_cast<fdas_plan *>(p);
     FDAS_CUDA_TRY(q, cudaDeviceSynchronize());
     FDAS_CUDA_TRY(q, cudaMemcpy(dst_host, p->taps, bytes, cudaMemcpyDeviceToHost));
+    return FDAS_OK;
+}
+
+extern "C" int fdas_tapmatrix_host(const fdas_plan_t *p, void *dst_host, size_t bytes)
+{
+    if (!p || !dst_host) return FDAS_ERR_INVALID_ARG;
+    if (!p->built) return FDAS_ERR_NOT_BUILT;
+    if (!(p->precision == FDAS_BF16 && p->tc_supported)) return FDAS_ERR_UNSUPPORTED;
+    const int ntap = 2 * p->m_max + 1;
+    if (bytes != (size_t)p->K * ntap * 2 * sizeof(uint16_t)) return FDAS_ERR_INVALID_ARG;
+    fdas_plan *q = const_cast<fdas_plan *>(p);
+    const size_t n_tab = (size_t)p->tc_groups * p->tc_nzg;
+    std::vector<uint16_t> img;
+    std::vector<int2> tab;
+    try {
+        img.resize(p->tc_bmat_bytes / 2);
+        tab.resize(n_tab);
+    } catch (...) {
+        return FDAS_ERR_ALLOC;
+    }
+    FDAS_CUDA_TRY(q, cudaDeviceSynchronize());
+    FDAS_CUDA_TRY(q, cudaMemcpy(img.data(), p->tc_bmat, p->tc_bmat_bytes, cudaMemcpyDeviceToHost));
+    FDAS_CUDA_TRY(q, cudaMemcpy(tab.data(), p->tc_ktab, n_tab * sizeof(int2), cudaMemcpyDeviceToHost));
+    // image [g][q][n][e] (kappa = 8 q + e, j = m_max - kappa; n = 2 zi + {re, im} of h_{+|z|})
+    // -> natural [K][2 m_max + 1][re, im] with the conjugate for the -|z| rows
+    uint16_t *dst = (uint16_t *)dst_host;
+    for (int g = 0; g < p->tc_groups; ++g)
+        for (int zi = 0; zi < p->tc_nzg; ++zi) {
+            const int2 kk = tab[(size_t)g * p->tc_nzg + zi];
+            for (int j = -p->m_max; j <= p->m_max; ++j) {
+                const int kappa = p->m_max - j;
+                const size_t base = (((size_t)g * 2 * p->tc_KS + kappa / 8) * p->tc_NT + 2 * zi) * 8 + kappa % 8;
+                const uint16_t re = img[base], im = img[base + 8];
+                if (kk.x >= 0) {
+                    dst[((size_t)kk.x * ntap + (j + p->m_max)) * 2 + 0] = re;
+                    dst[((size_t)kk.x * ntap + (j + p->m_max)) * 2 + 1] = im;
+                }
+                if (kk.y >= 0 && kk.y != kk.x) {
+                    dst[((size_t)kk.y * ntap + (j + p->m_max)) * 2 + 0] = re;
+                    dst[((size_t)kk.y * ntap + (j + p->m_max)) * 2 + 1] = (uint16_t)(im ^ 0x8000u);
+                }
+            }
+        }
     return FDAS_OK;
 }
 

@@ -16,12 +16,15 @@ LIB_PATH = os.environ.get("FDAS_LIBRARY", os.path.join(_HERE, "libfdas.so"))   #
 FDAS_F64, FDAS_F32, FDAS_BF16 = 0, 1, 2
 FDAS_OK, FDAS_ERR_INVALID_ARG, FDAS_ERR_ALLOC, FDAS_ERR_CUDA, FDAS_ERR_NOT_BUILT, FDAS_ERR_UNSUPPORTED = range(6)
 PRECISIONS = {"f64": FDAS_F64, "f32": FDAS_F32, "bf16": FDAS_BF16}
+FDAS_ALGO_AUTO, FDAS_ALGO_FFT, FDAS_ALGO_MMA = 0, 1, 2
+ALGORITHMS = {"auto": FDAS_ALGO_AUTO, "fft": FDAS_ALGO_FFT, "mma": FDAS_ALGO_MMA}
 
 EXPORTS = [
     "fdas_plan_create", "fdas_plan_destroy", "fdas_plan_info", "fdas_z_of_index",
     "fdas_build_templates", "fdas_convolve", "fdas_convolve_batched", "fdas_peaks",
     "fdas_convolve_host", "fdas_search_host", "fdas_templates_host", "fdas_taps_host",
     "fdas_launch_count", "fdas_status_string", "fdas_last_cuda_error",
+    "fdas_set_algorithm", "fdas_get_algorithm", "fdas_tapmatrix_host",
 ]
 
 
@@ -66,6 +69,9 @@ def lib() -> ctypes.CDLL:
     L.fdas_search_host.argtypes = [vp, vp, ctypes.c_float, vp, i, ctypes.POINTER(i), vp]
     L.fdas_templates_host.argtypes = [vp, vp, ctypes.c_size_t]
     L.fdas_taps_host.argtypes = [vp, vp, ctypes.c_size_t]
+    L.fdas_tapmatrix_host.argtypes = [vp, vp, ctypes.c_size_t]
+    L.fdas_set_algorithm.argtypes = [vp, i]
+    L.fdas_get_algorithm.argtypes = [vp, ctypes.POINTER(i)]
     L.fdas_launch_count.argtypes = [vp, ctypes.POINTER(i64)]
     L.fdas_status_string.argtypes = [i]
     L.fdas_status_string.restype = ctypes.c_char_p
@@ -147,6 +153,20 @@ def fdas_taps_host(h, dst_ptr, nbytes):
     return lib().fdas_taps_host(h, ctypes.c_void_p(dst_ptr), int(nbytes))
 
 
+def fdas_tapmatrix_host(h, dst_ptr, nbytes):
+    return lib().fdas_tapmatrix_host(h, ctypes.c_void_p(dst_ptr), int(nbytes))
+
+
+def fdas_set_algorithm(h, algorithm):
+    return lib().fdas_set_algorithm(h, int(algorithm))
+
+
+def fdas_get_algorithm(h):
+    a = ctypes.c_int(-1)
+    rc = lib().fdas_get_algorithm(h, ctypes.byref(a))
+    return rc, a.value
+
+
 def fdas_launch_count(h):
     n = ctypes.c_int64()
     rc = lib().fdas_launch_count(h, ctypes.byref(n))
@@ -167,7 +187,7 @@ class Plan:
     torch's; all arithmetic is the library's)."""
 
     def __init__(self, N: int, zmax: float, dz: float, seglen: int, precision="f32", build: bool = True,
-                 stream: int = 0):
+                 stream: int = 0, algorithm="auto"):
         prec = PRECISIONS[precision] if isinstance(precision, str) else int(precision)
         rc, self._h = fdas_plan_create(N, zmax, dz, seglen, prec)
         if rc:
@@ -176,6 +196,9 @@ class Plan:
         rc, self.info = fdas_plan_info(self._h)
         self._check(rc, "fdas_plan_info")
         self.precision = prec
+        algo = ALGORITHMS[algorithm] if isinstance(algorithm, str) else int(algorithm)
+        if algo != FDAS_ALGO_AUTO:
+            self._check(fdas_set_algorithm(self._h, algo), "fdas_set_algorithm")
         if build:
             self.build_templates(stream)
 
@@ -270,6 +293,19 @@ class Plan:
         out = np.empty((self.K, 2 * m + 1), dtype=np.complex128)
         self._check(fdas_taps_host(self._h, out.ctypes.data, out.nbytes), "fdas_taps_host")
         return out
+
+    def tapmatrix(self):
+        """bf16 plans: the taps the tensor-core path uses, uint16 bit patterns [K, 2*m_max+1, 2]."""
+        import numpy as np
+        m = int(self.info.halfwidth_max)
+        out = np.empty((self.K, 2 * m + 1, 2), dtype=np.uint16)
+        self._check(fdas_tapmatrix_host(self._h, out.ctypes.data, out.nbytes), "fdas_tapmatrix_host")
+        return out
+
+    def algorithm(self) -> str:
+        rc, a = fdas_get_algorithm(self._h)
+        self._check(rc, "fdas_get_algorithm")
+        return {FDAS_ALGO_FFT: "fft", FDAS_ALGO_MMA: "mma"}[a]
 
     def launch_count(self) -> int:
         return fdas_launch_count(self._h)[1]
