@@ -5,11 +5,12 @@
     python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
 
 A step = one pass of the whole hot path over one
-spectrum of BASELINE.json config 3 (N = 2^23 samples, 97 templates, segment 2048): the fused
-convolve kernel (segment load, forward FFT, template multiply, inverse FFT, power, store) and
-the peak pass, both through the C ABI of libfdas.  Headline variant: bf16 storage / fp32
-accumulate (the north_star target); the fp32 variant is timed in the same run for the
-bf16-over-fp32 speedup.  Prints ONE JSON line (rank 0).
+spectrum of BASELINE.json config 3 (N = 2^23 samples, 97 templates, segment 2048) through the
+C ABI of libfdas: fdas_search = the convolution (spectrum load, template filter bank, |.|^2,
+plane store) and the threshold / local-maximum peak pass.  Headline variant: bf16 storage /
+fp32 accumulate (the north_star target; tensor-core kernel with the threshold test fused into
+its epilogue); the fp32 variant (overlap-save FFT kernel + peak kernel) and the FFT form of the
+bf16 variant are timed in the same run.  Prints ONE JSON line (rank 0).
 
 N > 1: the path shards by independent series (no data-path collective):
 every rank convolves its own config-3-shaped series -> weak scaling.
@@ -202,17 +203,20 @@ def main():
     peaks_pin = torch.empty(PEAK_CAPACITY * 3, dtype=torch.int32).pin_memory()
     sampler = None
 
-    for prec in ("f32", "bf16"):          # headline (bf16) last so the clock sample covers it
-        plan = fdas.Plan(w.N, ZMAX, DZ, SEGLEN, prec, stream=sptr)
+    for prec in ("f32", "bf16_fft", "bf16"):          # headline (bf16) last so the clock sample covers it
+        plan = fdas.Plan(w.N, ZMAX, DZ, SEGLEN, prec.split("_")[0], stream=sptr,
+                         algorithm="fft" if prec.endswith("_fft") else "auto")
         K, M, S, V = plan.K, plan.M, plan.S, int(plan.info.valid_per_seg)
         plane = torch.empty((K, M), dtype=torch.float32, device="cuda")
         h = plan._h
 
         def step():
-            rc = fdas.fdas_convolve(h, x_dev.data_ptr(), plane.data_ptr(), sptr)
-            rc |= fdas.fdas_peaks(h, plane.data_ptr(), THRESH, peaks_dev.data_ptr(), PEAK_CAPACITY,
+            rc = fdas.fdas_search(h, x_dev.data_ptr(), plane.data_ptr(), THRESH, peaks_dev.data_ptr(), PEAK_CAPACITY,
                                   count_dev.data_ptr(), sptr)
             assert rc == 0
+
+        def convolve_only():
+            assert fdas.fdas_convolve(h, x_dev.data_ptr(), plane.data_ptr(), sptr) == 0
 
         with torch.cuda.stream(stream):
             for _ in range(args.warmup):
@@ -224,24 +228,29 @@ def main():
             if prec == "bf16" and rank == 0:
                 sampler = ClockSampler(local)
             l0 = plan.launch_count()
-            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True),
-                   torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-            for a, b, c in ev:
+            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+                  for _ in range(args.steps)]
+            for a, c in ev:                         # the timed region: K steps of the whole hot path
                 flush.zero_()                       # L2 flush between timed iterations (untimed)
                 a.record(stream)
-                rc = fdas.fdas_convolve(h, x_dev.data_ptr(), plane.data_ptr(), sptr)
-                b.record(stream)
-                rc |= fdas.fdas_peaks(h, plane.data_ptr(), THRESH, peaks_dev.data_ptr(), PEAK_CAPACITY,
-                                      count_dev.data_ptr(), sptr)
+                step()
                 c.record(stream)
-                assert rc == 0
             stream.synchronize()
             torch.cuda.synchronize()
             launches = plan.launch_count() - l0
             if world > 1:
                 dist.barrier()
-        conv_ms = [a.elapsed_time(b) for a, b, c in ev]
-        step_ms = [a.elapsed_time(c) for a, b, c in ev]
+            # the dominant kernel alone (roofline): fdas_convolve, same stream, same flush
+            evk = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+                   for _ in range(args.steps)]
+            for a, b in evk:
+                flush.zero_()
+                a.record(stream)
+                convolve_only()
+                b.record(stream)
+            stream.synchronize()
+        conv_ms = [a.elapsed_time(b) for a, b in evk]
+        step_ms = [a.elapsed_time(c) for a, c in ev]
         total_ms = sharding.max_over_ranks(float(sum(step_ms)), device="cuda")
         n_found = int(count_dev.item())
 
@@ -270,6 +279,7 @@ def main():
 
     r = results["bf16"]
     rf = results["f32"]
+    rb = results["bf16_fft"]
     K, M, S, V = r["K"], r["M"], r["S"], r["V"]
     points = K * M
     value = world * points / (r["step_ms"] * 1e-3)
@@ -279,6 +289,14 @@ def main():
     flops = nominal_flops(K, M, S, V)
     sm_max = float(peaks_json.get("sm_max_mhz", 1965.0))
     alu_peak = 148 * 128 * 2 * sm_max * 1e6 / 1e12       # TFLOP/s fp32 FMA, DESIGN.md section 7
+    # tensor-core work the MMA kernel issues: per 128-bin tile 2 parts x KS K-steps of
+    # a 128 x NT x 16 MMA, NT = 16*ceil(2*49/16) = 112, KS = ceil(129/16) = 9
+    nz = (K + 1) // 2
+    NT = -(-2 * nz // 16) * 16
+    KS = -(-(2 * (int(math.ceil(ZMAX / 2)) + 16) + 1) // 16)
+    mma_flops = (-(-M // 128)) * 2 * KS * 2 * 128 * NT * 16
+    tensor_peak = float(peaks_json.get("bf16_tflops", 1590.0))
+    tensor_src = "measured (MEASURED_PEAKS.json bf16_tflops, burst)" if "bf16_tflops" in peaks_json else "fallback 1.59 PFLOP/s"
     traffic = None
     tp = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tp):
@@ -293,8 +311,10 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": r["step_ms"], "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": WORKLOAD, "storage": "bf16 (spectrum on load, bank, FFT staging); fp32 accumulate; fp32 plane",
-                   "step": "fdas_convolve + fdas_peaks (threshold %.1f)" % THRESH, "sharding": "independent series per rank",
+        "config": {"workload": WORKLOAD,
+                   "storage": "bf16 spectrum and taps (RNE), fp32 accumulate on the tensor cores (tcgen05), fp32 plane",
+                   "step": "fdas_search = convolve + threshold/local-max peaks (threshold %.1f)" % THRESH,
+                   "sharding": "independent series per rank",
                    "l2": "256 MB buffer written between timed steps; plane 1.63 GB per step >> 126 MB L2",
                    "noise_only": bool(args.noise_only)},
         "clocks": {"sm_mhz": clocks["sm_mhz"], "sm_max_mhz": clocks["sm_max_mhz"], "reasons": clocks["reasons"]},
@@ -302,14 +322,19 @@ def main():
                 "h2d_bytes_per_step": int(M * 8), "d2h_bytes_per_step": int(4 + 12 * min(r["n_e2e"], PEAK_CAPACITY)),
                 "api": "fdas_search_host (pinned host spectrum in, peak list out)", "ms_per_step": r["e2e_s"] * 1e3},
         "gpu_launches": int(r["launches"]),
-        "roofline": {"bound": "hbm", "kernel": "fdas_convolve_kernel<TraitsBF16,2048>", "achieved": achieved,
+        "roofline": {"bound": "hbm", "kernel": "fdas_mma_convolve_kernel<7> (fdas_convolve, bf16)", "achieved": achieved,
                      "peak": peak_gbs, "unit": "GB/s", "frac": achieved / peak_gbs, "traffic": traffic,
                      "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
                      "kernel_ms": r["conv_ms"], "kernel_ms_min": r["conv_ms_min"],
                      "frac_of_nominal_8TBs": achieved / 8000.0},
-        "roofline_alu": {"bound": "alu", "achieved": flops / (r["conv_ms"] * 1e-3) / 1e12, "peak": alu_peak,
-                         "unit": "TFLOP/s", "frac": flops / (r["conv_ms"] * 1e-3) / 1e12 / alu_peak,
-                         "flops_per_launch": flops, "count": "nominal 5 N log2 N (SURVEY.md 8(d))"},
+        "roofline_tensor": {"bound": "tensor", "kernel": "fdas_mma_convolve_kernel<7>", "achieved": mma_flops / (r["conv_ms"] * 1e-3) / 1e12,
+                            "peak": tensor_peak, "unit": "TFLOP/s", "frac": mma_flops / (r["conv_ms"] * 1e-3) / 1e12 / tensor_peak,
+                            "flops_per_launch": mma_flops, "peak_source": tensor_src,
+                            "count": "issued dense MMA flops: tiles x 2 parts x 9 K-steps x 2*128*112*16 (padding included)"},
+        "roofline_alu_fp32": {"bound": "alu", "kernel": "fdas_convolve_kernel<TraitsF32,2048>",
+                              "achieved": flops / (rf["conv_ms"] * 1e-3) / 1e12, "peak": alu_peak,
+                              "unit": "TFLOP/s", "frac": flops / (rf["conv_ms"] * 1e-3) / 1e12 / alu_peak,
+                              "flops_per_launch": flops, "count": "nominal 5 N log2 N (SURVEY.md 8(d))"},
         "cpu_baseline": cpu,
         "precisions": {
             "bf16": {"convolve_ms": r["conv_ms"], "step_ms": r["step_ms"], "points_per_s": points / (r["step_ms"] * 1e-3),
@@ -317,7 +342,13 @@ def main():
             "f32": {"convolve_ms": rf["conv_ms"], "step_ms": rf["step_ms"], "points_per_s": points / (rf["step_ms"] * 1e-3),
                     "convolve_points_per_s": points / (rf["conv_ms"] * 1e-3),
                     "hbm_gbs": alg_bytes / (rf["conv_ms"] * 1e-3) / 1e9, "peaks_found": rf["n_found"]},
+            "bf16_fft": {"convolve_ms": rb["conv_ms"], "step_ms": rb["step_ms"],
+                         "points_per_s": points / (rb["step_ms"] * 1e-3),
+                         "convolve_points_per_s": points / (rb["conv_ms"] * 1e-3),
+                         "hbm_gbs": alg_bytes / (rb["conv_ms"] * 1e-3) / 1e9, "peaks_found": rb["n_found"],
+                         "note": "FDAS_ALGO_FFT: the overlap-save FFT kernel with bf16 storage"},
             "bf16_over_fp32_speedup": rf["conv_ms"] / r["conv_ms"],
+            "bf16_over_fp32_speedup_whole_step": rf["step_ms"] / r["step_ms"],
             "paper_bf16_over_fp32_speedup": "~1.6x on 'NVIDIA Ampere' (PAPER.md:15; context, not the target)",
         },
     }

@@ -180,12 +180,24 @@ int fdas_peaks(fdas_plan_t *p, const void *plane_dev, float threshold, fdas_peak
                int capacity, int *count_dev, void *stream);
 
 /*
+ * fdas_search -- fdas_convolve followed by fdas_peaks in one call: the same plane in plane_dev
+ * and the same peak set.  Where the convolution runs on the tensor-core
+ * path the threshold test is fused into its epilogue: the kernel flags the (rare) cells above
+ * `threshold` while it stores them and a small second kernel applies the local-maximum rule to
+ * those cells only, so the plane is never read back from HBM.  Other plans run the two kernels
+ * of fdas_convolve and fdas_peaks.  Arguments, ownership and the snprintf convention for
+ * count_dev are those of fdas_convolve and fdas_peaks.  Asynchronous on `stream`.
+ */
+int fdas_search(fdas_plan_t *p, const void *spectrum_dev, void *plane_dev, float threshold,
+                fdas_peak_t *peaks_dev, int capacity, int *count_dev, void *stream);
+
+/*
  * Host-buffer forms (end-to-end path): copy the spectrum host->device, run fdas_convolve
  * (and fdas_peaks), copy the result device->host, on `stream`, then synchronise the stream.
  * Device staging buffers are owned by the plan and allocated on first use.  Pinned host
  * memory makes the copies asynchronous and fast; pageable memory also works.
  *   fdas_convolve_host   plane_host receives [K][M]
- *   fdas_search_host     convolve + peaks; the plane stays on the device; peaks_host
+ *   fdas_search_host     fdas_search; the plane stays on the device; peaks_host
  *                        receives min(count, capacity) records and *count_host the total.
  */
 int fdas_convolve_host(fdas_plan_t *p, const void *spectrum_host, void *plane_host, void *stream);

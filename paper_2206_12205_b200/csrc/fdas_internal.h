@@ -30,6 +30,11 @@ struct fdas_plan {
     size_t tc_bmat_bytes;
     int2 *tc_ktab;     // [groups][nzg] plane rows of (+|z|, -|z|), -1 where absent
     int2 *tc_kref;     // [groups][nzg] (template whose taps fill the columns, its sign)
+    // fused search (fdas_search): coarse candidates flagged by the convolve epilogue
+    fdas_peak_t *cand;     // [cand_capacity] (z_index = first |z| table entry of the chunk, r, chunk maximum)
+    int *cand_ctr;         // two counters used alternately: call n appends to [n & 1] and clears [(n + 1) & 1]
+    int cand_capacity;
+    unsigned search_calls;
     // host-buffer entry points: lazily allocated device staging
     void *stage_spectrum, *stage_plane;
     fdas_peak_t *stage_peaks;
@@ -61,6 +66,17 @@ __host__ __device__ static inline size_t fdas_bank_offset(int k, int f, int T, i
     return (((size_t)k * (FDAS_PTS / VC) + a / VC) * T + t) * VC + a % VC;
 }
 
+// What the convolve epilogue needs to flag candidates for fdas_search (enabled = 0: plain convolve).
+struct fdas_search_args {
+    int enabled;
+    float thr;
+    fdas_peak_t *cand;
+    int *cand_count;       // appended to by this launch
+    int *cand_count_next;  // cleared by this launch for the next call
+    int cand_capacity;
+    int *count_out;        // caller's peak counter, cleared by this launch
+};
+
 #define FDAS_CUDA_TRY(p, call)                                  \
     do {                                                        \
         cudaError_t e__ = (call);                               \
@@ -76,7 +92,11 @@ int fdas_launch_convolve(fdas_plan *p, const void *spectra, void *planes, int ba
 // fdas_mma.cu: host-side grouping (plan creation), tap matrix build, the tcgen05 convolution
 int fdas_mma_plan(fdas_plan *p);
 int fdas_launch_build_tapmatrix(fdas_plan *p, cudaStream_t st);
-int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, int batch, cudaStream_t st);
+int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, int batch, cudaStream_t st,
+                             const fdas_search_args *search = nullptr);
+// fdas_peaks.cu: turns the candidates of a fused search into the peak list (same rule as fdas_peaks)
+int fdas_launch_resolve(fdas_plan *p, const void *plane, const fdas_search_args &sa, fdas_peak_t *peaks, int capacity,
+                        cudaStream_t st);
 // true when fdas_convolve runs the tensor-core kernel for this plan
 static inline int fdas_uses_mma(const fdas_plan *p)
 {

@@ -62,6 +62,7 @@ struct TcParams {
     int NT;                  // UMMA N: columns per part (multiple of 16, <= 128) = 16 NCH
     int nzg;                 // |z| values per group
     int full_chunks;         // 16-column chunks whose 8 |z| entries all have both plane rows
+    fdas_search_args search; // fused threshold pass (fdas_search); enabled = 0 for plain fdas_convolve
 };
 
 // ---- PTX wrappers ---------------------------------------------------------------------
@@ -209,9 +210,12 @@ constexpr uint32_t TC_NO_ROW = 0xFFFFFFFFu;   // row-offset table: this |z| has 
 // stores.  v[0..15] = (Ure, Vre) pairs, v[16..31] = (Uim, Vim) pairs of this thread's output bin;
 // o4[0..3] = row offsets (+|z|, -|z|) of two |z| each, in plane elements.
 // FAST: the tile lies inside the plane and every entry has both rows -> straight-line code.
+// Returns the largest power this thread stored (0 if none): the fused search flags the chunk
+// when it exceeds the threshold (fdas_search).
 template <bool FAST>
-__device__ __forceinline__ void epilogue_chunk(const uint32_t *v, const uint4 *o4, float *out, bool ok)
+__device__ __forceinline__ float epilogue_chunk(const uint32_t *v, const uint4 *o4, float *out, bool ok)
 {
+    float mx = 0.f;
 #pragma unroll
     for (int e2 = 0; e2 < 4; ++e2) {
         const uint4 o = o4[e2];
@@ -223,19 +227,40 @@ __device__ __forceinline__ void epilogue_chunk(const uint32_t *v, const uint4 *o
             const float uim = __uint_as_float(v[16 + 2 * e]), vim = __uint_as_float(v[16 + 2 * e + 1]);
             if (FAST) {
                 const float a = ure - vim, b = uim + vre, c = ure + vim, d = uim - vre;
-                st_cs_at(out, offp, a * a + b * b);
-                st_cs_at(out, offm, c * c + d * d);
+                const float pp = a * a + b * b, pm = c * c + d * d;
+                st_cs_at(out, offp, pp);
+                st_cs_at(out, offm, pm);
+                mx = fmaxf(mx, fmaxf(pp, pm));
             } else {
                 if (offp != TC_NO_ROW && ok) {
                     const float a = ure - vim, b = uim + vre;
-                    st_cs_at(out, offp, a * a + b * b);
+                    const float pp = a * a + b * b;
+                    st_cs_at(out, offp, pp);
+                    mx = fmaxf(mx, pp);
                 }
                 if (offm != TC_NO_ROW && ok) {
                     const float c = ure + vim, d = uim - vre;
-                    st_cs_at(out, offm, c * c + d * d);
+                    const float pm = c * c + d * d;
+                    st_cs_at(out, offm, pm);
+                    mx = fmaxf(mx, pm);
                 }
             }
         }
+    }
+    return mx;
+}
+
+// fused search: "some power of bin r in the 8 |z| entries starting at table entry zi0 exceeds thr"
+__device__ __noinline__ void flag_candidate(fdas_peak_t *cand, int *cand_count, int cand_capacity, int zi0, int r,
+                                            float mx)
+{
+    const int slot = atomicAdd(cand_count, 1);
+    if (slot < cand_capacity) {
+        fdas_peak_t rec;
+        rec.z_index = zi0;
+        rec.r = r;
+        rec.power = mx;
+        cand[slot] = rec;
     }
 }
 
@@ -244,7 +269,8 @@ __device__ __forceinline__ void epilogue_chunk(const uint32_t *v, const uint4 *o
 // the TMEM stage is handed back to the MMA issuer as soon as the last load has landed.
 template <int NCH, int HALF>
 __device__ __forceinline__ void epilogue_tile(uint32_t taddr, const uint4 *otab4, float *out, bool inside, bool ok,
-                                              int full_chunks, uint32_t empty_bar, int lane)
+                                              int full_chunks, uint32_t empty_bar, int lane,
+                                              const fdas_search_args &sa, float thr, int zi_group0, long long col)
 {
     constexpr int NMY = (NCH - HALF + 1) / 2;
     constexpr uint32_t NT = 16 * NCH;
@@ -263,8 +289,11 @@ __device__ __forceinline__ void epilogue_tile(uint32_t taddr, const uint4 *otab4
 #ifdef FDAS_MMA_DEBUG_NOSTORE
         ok = false; inside = false;
 #endif
-        if (inside && c < full_chunks) epilogue_chunk<true>(v[i & 1], otab4 + 4 * c, out, true);
-        else epilogue_chunk<false>(v[i & 1], otab4 + 4 * c, out, ok);
+        float mx;
+        if (inside && c < full_chunks) mx = epilogue_chunk<true>(v[i & 1], otab4 + 4 * c, out, true);
+        else mx = epilogue_chunk<false>(v[i & 1], otab4 + 4 * c, out, ok);
+        if (mx > thr)   // thr = +inf unless fdas_search
+            flag_candidate(sa.cand, sa.cand_count, sa.cand_capacity, zi_group0 + 8 * c, (int)col, mx);
     }
     if (NMY == 0) {
         tc_fence_before();
@@ -304,6 +333,10 @@ __global__ void __launch_bounds__(TC_THREADS, 1) fdas_mma_convolve_kernel(const 
         }
         fence_proxy_async();   // the tap matrix is read by the tensor core (async proxy)
     }
+    if (threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0 && p.search.enabled) {
+        *p.search.cand_count_next = 0;   // the other counter: nobody appends to it during this launch
+        *p.search.count_out = 0;         // written by the resolve kernel that follows in stream order
+    }
     if (threadIdx.x == 0) {
         for (int s = 0; s < 2; ++s) {
             mbar_init(z_full + 8 * s, TC_LOAD_THREADS);
@@ -323,6 +356,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1) fdas_mma_convolve_kernel(const 
         // =========================== epilogue ===========================
         const int q = warp & 3, half = warp >> 2;
         const uint4 *otab4 = reinterpret_cast<const uint4 *>(otab);
+        const float thr = p.search.enabled ? p.search.thr : __int_as_float(0x7f800000);
+        const int zi_group0 = grp * p.nzg;
         uint32_t t = 0;
         for (long long it = blockIdx.x; it < n_items; it += gridDim.x) {
             const long long ser = it / p.n_blocks;
@@ -339,9 +374,11 @@ __global__ void __launch_bounds__(TC_THREADS, 1) fdas_mma_convolve_kernel(const 
                 mbar_wait(t_full + 8 * stage, use & 1);
                 tc_fence_after();
                 if (half == 0)
-                    epilogue_tile<NCH, 0>(taddr, otab4, out, inside, col < p.M, p.full_chunks, t_empty + 8 * stage, lane);
+                    epilogue_tile<NCH, 0>(taddr, otab4, out, inside, col < p.M, p.full_chunks, t_empty + 8 * stage, lane,
+                                          p.search, thr, zi_group0, col);
                 else
-                    epilogue_tile<NCH, 1>(taddr, otab4, out, inside, col < p.M, p.full_chunks, t_empty + 8 * stage, lane);
+                    epilogue_tile<NCH, 1>(taddr, otab4, out, inside, col < p.M, p.full_chunks, t_empty + 8 * stage, lane,
+                                          p.search, thr, zi_group0, col);
             }
         }
     } else if (warp == TC_MMA_WARP) {
@@ -562,7 +599,8 @@ static int launch_mma(fdas_plan *p, const TcParams &tp, unsigned gx, size_t smem
     return FDAS_OK;
 }
 
-int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, int batch, cudaStream_t st)
+int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, int batch, cudaStream_t st,
+                             const fdas_search_args *search)
 {
     if (p->precision != FDAS_BF16 || !p->tc_supported) return FDAS_ERR_UNSUPPORTED;
     // outputs per work item: the largest of 1024..128 that fits shared memory and leaves at
@@ -591,6 +629,8 @@ int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, in
     tp.NT = p->tc_NT;
     tp.nzg = p->tc_nzg;
     tp.full_chunks = p->tc_full_chunks;
+    if (search) tp.search = *search;
+    else tp.search = fdas_search_args{0, 0.f, nullptr, nullptr, nullptr, 0, nullptr};
     const long long items = (long long)batch * tp.n_blocks;
     const unsigned gx = (unsigned)(items < sms_per_group ? items : sms_per_group);
     switch (p->tc_NT / 16) {

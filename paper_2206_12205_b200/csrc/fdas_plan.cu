@@ -17,6 +17,8 @@ static void free_device_members(fdas_plan *p)
     cudaFree(p->tc_bmat);
     cudaFree(p->tc_ktab);
     cudaFree(p->tc_kref);
+    cudaFree(p->cand);
+    cudaFree(p->cand_ctr);
     cudaFree(p->stage_spectrum);
     cudaFree(p->stage_plane);
     cudaFree(p->stage_peaks);
@@ -171,6 +173,47 @@ extern "C" int fdas_peaks(fdas_plan_t *p, const void *plane_dev, float threshold
                              (cudaStream_t)stream);
 }
 
+// fdas_search: convolve + peaks.  On the tensor-core path the convolve epilogue flags the
+// (rare) chunks holding a power above the threshold and a small second kernel applies the
+// peak rule to those cells only, so the plane is not read back from HBM.
+static int search_on_device(fdas_plan *p, const void *spectrum_dev, void *plane_dev, float threshold,
+                            fdas_peak_t *peaks_dev, int capacity, int *count_dev, cudaStream_t st)
+{
+    if (!fdas_uses_mma(p)) {
+        int rc = fdas_launch_convolve(p, spectrum_dev, plane_dev, 1, st);
+        if (rc) return rc;
+        return fdas_launch_peaks(p, plane_dev, threshold, peaks_dev, capacity, count_dev, st);
+    }
+    if (!p->cand) {
+        p->cand_capacity = 1 << 18;
+        FDAS_CUDA_TRY(p, cudaMalloc((void **)&p->cand, sizeof(fdas_peak_t) * (size_t)p->cand_capacity));
+        FDAS_CUDA_TRY(p, cudaMalloc((void **)&p->cand_ctr, 2 * sizeof(int)));
+        FDAS_CUDA_TRY(p, cudaMemsetAsync(p->cand_ctr, 0, 2 * sizeof(int), st));
+    }
+    fdas_search_args sa;
+    sa.enabled = 1;
+    sa.thr = threshold;
+    sa.cand = p->cand;
+    sa.cand_count = p->cand_ctr + (p->search_calls & 1);
+    sa.cand_count_next = p->cand_ctr + ((p->search_calls + 1) & 1);
+    sa.cand_capacity = p->cand_capacity;
+    sa.count_out = count_dev;
+    p->search_calls += 1;
+    int rc = fdas_launch_convolve_mma(p, spectrum_dev, plane_dev, 1, st, &sa);
+    if (rc) return rc;
+    return fdas_launch_resolve(p, plane_dev, sa, peaks_dev, capacity, st);
+}
+
+extern "C" int fdas_search(fdas_plan_t *p, const void *spectrum_dev, void *plane_dev, float threshold,
+                           fdas_peak_t *peaks_dev, int capacity, int *count_dev, void *stream)
+{
+    if (!p || !spectrum_dev || !plane_dev || !count_dev || capacity < 0 || (capacity > 0 && !peaks_dev))
+        return FDAS_ERR_INVALID_ARG;
+    if (!p->built) return FDAS_ERR_NOT_BUILT;
+    return search_on_device(p, spectrum_dev, plane_dev, threshold, peaks_dev, capacity, count_dev,
+                            (cudaStream_t)stream);
+}
+
 static int ensure_staging(fdas_plan *p, bool want_plane, int peaks_capacity)
 {
     const size_t spec_bytes = (size_t)p->M * (p->precision == FDAS_F64 ? 16 : 8);
@@ -217,9 +260,8 @@ extern "C" int fdas_search_host(fdas_plan_t *p, const void *spectrum_host, float
     if (rc) return rc;
     const size_t spec_bytes = (size_t)p->M * (p->precision == FDAS_F64 ? 16 : 8);
     FDAS_CUDA_TRY(p, cudaMemcpyAsync(p->stage_spectrum, spectrum_host, spec_bytes, cudaMemcpyHostToDevice, st));
-    rc = fdas_launch_convolve(p, p->stage_spectrum, p->stage_plane, 1, st);
-    if (rc) return rc;
-    rc = fdas_launch_peaks(p, p->stage_plane, threshold, p->stage_peaks, capacity, p->stage_count, st);
+    rc = search_on_device(p, p->stage_spectrum, p->stage_plane, threshold, p->stage_peaks, capacity,
+                          p->stage_count, st);
     if (rc) return rc;
     FDAS_CUDA_TRY(p, cudaMemcpyAsync(count_host, p->stage_count, sizeof(int), cudaMemcpyDeviceToHost, st));
     FDAS_CUDA_TRY(p, cudaStreamSynchronize(st));

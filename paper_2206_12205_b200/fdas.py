@@ -24,7 +24,7 @@ EXPORTS = [
     "fdas_build_templates", "fdas_convolve", "fdas_convolve_batched", "fdas_peaks",
     "fdas_convolve_host", "fdas_search_host", "fdas_templates_host", "fdas_taps_host",
     "fdas_launch_count", "fdas_status_string", "fdas_last_cuda_error",
-    "fdas_set_algorithm", "fdas_get_algorithm", "fdas_tapmatrix_host",
+    "fdas_set_algorithm", "fdas_get_algorithm", "fdas_tapmatrix_host", "fdas_search",
 ]
 
 
@@ -65,6 +65,7 @@ def lib() -> ctypes.CDLL:
     L.fdas_convolve.argtypes = [vp, vp, vp, vp]
     L.fdas_convolve_batched.argtypes = [vp, vp, vp, i, vp]
     L.fdas_peaks.argtypes = [vp, vp, ctypes.c_float, vp, i, vp, vp]
+    L.fdas_search.argtypes = [vp, vp, vp, ctypes.c_float, vp, i, vp, vp]
     L.fdas_convolve_host.argtypes = [vp, vp, vp, vp]
     L.fdas_search_host.argtypes = [vp, vp, ctypes.c_float, vp, i, ctypes.POINTER(i), vp]
     L.fdas_templates_host.argtypes = [vp, vp, ctypes.c_size_t]
@@ -130,6 +131,12 @@ def fdas_convolve_batched(h, spectra_ptr, planes_ptr, batch, stream=0):
 def fdas_peaks(h, plane_ptr, threshold, peaks_ptr, capacity, count_ptr, stream=0):
     return lib().fdas_peaks(h, ctypes.c_void_p(plane_ptr), float(threshold), ctypes.c_void_p(peaks_ptr),
                             int(capacity), ctypes.c_void_p(count_ptr), ctypes.c_void_p(stream))
+
+
+def fdas_search(h, spectrum_ptr, plane_ptr, threshold, peaks_ptr, capacity, count_ptr, stream=0):
+    return lib().fdas_search(h, ctypes.c_void_p(spectrum_ptr), ctypes.c_void_p(plane_ptr), float(threshold),
+                             ctypes.c_void_p(peaks_ptr), int(capacity), ctypes.c_void_p(count_ptr),
+                             ctypes.c_void_p(stream))
 
 
 def fdas_convolve_host(h, spectrum_host_ptr, plane_host_ptr, stream=0):
@@ -263,6 +270,29 @@ class Plan:
         rec["r"] = raw[:, 1]
         rec["power"] = raw[:, 2].copy().view(np.float32)
         return n, rec
+
+    def search(self, spectrum, threshold: float, plane=None, capacity: int = 1 << 16, stream: Optional[int] = None):
+        """fdas_search: returns (plane, total_count, records)."""
+        import numpy as np
+        import torch
+        assert spectrum.is_cuda and spectrum.is_contiguous() and spectrum.dtype == self.spectrum_dtype()
+        assert tuple(spectrum.shape) == (self.M,)
+        if plane is None:
+            plane = torch.empty((self.K, self.M), dtype=self.plane_dtype(), device=spectrum.device)
+        if stream is None:
+            stream = torch.cuda.current_stream().cuda_stream
+        buf = torch.empty(max(capacity, 1) * 3, dtype=torch.int32, device=plane.device)
+        cnt = torch.zeros(1, dtype=torch.int32, device=plane.device)
+        self._check(fdas_search(self._h, spectrum.data_ptr(), plane.data_ptr(), threshold,
+                                buf.data_ptr() if capacity else 0, capacity, cnt.data_ptr(), stream), "fdas_search")
+        n = int(cnt.item())
+        w = min(n, capacity)
+        raw = buf[: 3 * w].cpu().numpy().reshape(w, 3)
+        rec = np.zeros(w, dtype=[("z_index", np.int32), ("r", np.int32), ("power", np.float32)])
+        rec["z_index"] = raw[:, 0]
+        rec["r"] = raw[:, 1]
+        rec["power"] = raw[:, 2].copy().view(np.float32)
+        return plane, n, rec
 
     def convolve_host(self, spectrum_host, plane_host, stream: int = 0):
         """numpy or pinned torch CPU buffers; copies are inside the call."""

@@ -62,6 +62,9 @@ def test_unsupported_and_null_handling(F):
     assert F.fdas_build_templates(None) == F.FDAS_ERR_INVALID_ARG
     assert F.fdas_convolve(None, 0, 0) == F.FDAS_ERR_INVALID_ARG
     assert F.fdas_plan_info(None)[0] == F.FDAS_ERR_INVALID_ARG
+    assert F.fdas_set_algorithm(None, F.FDAS_ALGO_MMA) == F.FDAS_ERR_INVALID_ARG
+    assert F.fdas_get_algorithm(None)[0] == F.FDAS_ERR_INVALID_ARG
+    assert F.fdas_tapmatrix_host(None, 0, 0) == F.FDAS_ERR_INVALID_ARG
 
 
 def test_no_cpu_fallback_without_a_device(F):

@@ -31,10 +31,10 @@ def F():
     return fdas
 
 
-def gpu_plane(F, w, precision, spectrum=None):
+def gpu_plane(F, w, precision, spectrum=None, algorithm="auto"):
     import torch
     X = w.spectrum if spectrum is None else spectrum
-    plan = F.Plan(w.N, w.zmax, w.dz, w.seglen, precision)
+    plan = F.Plan(w.N, w.zmax, w.dz, w.seglen, precision, algorithm=algorithm)
     dt = np.complex128 if precision == "f64" else np.complex64
     x = torch.from_numpy(np.ascontiguousarray(X.astype(dt))).cuda()
     P = plan.convolve(x)
@@ -52,6 +52,32 @@ def check_fp32(got, exp, p_peak=None):
     if p_peak is None:
         p_peak = float(exp.max())
     tol = 1e-4 * p_peak + 1e-4
+    err = np.abs(got.astype(np.float64) - exp)
+    assert err.max() <= tol, f"max |dP| {err.max():.3e} > {tol:.3e}"
+    return err.max(), tol
+
+
+def bf16_input_plane(w, r0=0, r1=None):
+    """What FDAS_ALGO_MMA computes, by the oracle: spectrum and taps rounded once to bf16 (RNE,
+    DESIGN.md reading A12), then the plain fp64 direct sum (oracle.convolve_row)."""
+    X = w.spectrum
+    Xb = bf16_rne(X.real).astype(np.float64) + 1j * bf16_rne(X.imag).astype(np.float64)
+    rows = []
+    for z in z_values(w.zmax, w.dz):
+        h = oracle.template_taps(float(z))
+        hb = bf16_rne(h.real.astype(np.float32)).astype(np.float64) + \
+            1j * bf16_rne(h.imag.astype(np.float32)).astype(np.float64)
+        rows.append(oracle.convolve_row(Xb, hb, r0, r1))
+    return np.stack(rows)
+
+
+def check_mma(got, exp, p_peak=None):
+    """fp32 accumulation of <= 2 (2 m_max + 1) <= 466 exact bf16 x bf16 products per component:
+    |dY| <~ n eps |Y|-scale with eps = 2^-24, so |dP| <= 1e-5 P_peak + 1e-5 leaves > 10x margin
+    (DESIGN.md section 7); a wrong tap, sign or index shows up at the 1e-2 .. 1 level."""
+    if p_peak is None:
+        p_peak = float(exp.max())
+    tol = 1e-5 * p_peak + 1e-5
     err = np.abs(got.astype(np.float64) - exp)
     assert err.max() <= tol, f"max |dP| {err.max():.3e} > {tol:.3e}"
     return err.max(), tol
@@ -134,10 +160,12 @@ def test_config1_fp32(F, c1):
     assert z_values(20.0, 2.0)[k] == 20.0 and r == 10000      # injected tone (z=+20, r0=10000.25)
 
 
-def test_config1_bf16_rules(F, c1):
+@pytest.mark.parametrize("algo", ["mma", "fft"])
+def test_config1_bf16_rules(F, c1, algo):
     w, exp = c1
     planf, Pf = gpu_plane(F, w, "f32")
-    _, Pb = gpu_plane(F, w, "bf16")
+    planb, Pb = gpu_plane(F, w, "bf16", algorithm=algo)
+    assert planb.algorithm() == algo
     n, rec = planf.peaks(Pf, THRESH)
     assert n >= 1
     mean_rel, worst = check_bf16_rules(Pb.cpu().numpy(), Pf.cpu().numpy().astype(np.float64),
@@ -171,10 +199,11 @@ def test_config2_fp32_full_plane(F, c2):
     print(f"config2 fp32 max |dP| {err:.3e} (tol {tol:.3e})")
 
 
-def test_config2_bf16_rules(F, c2):
+@pytest.mark.parametrize("algo", ["mma", "fft"])
+def test_config2_bf16_rules(F, c2, algo):
     w, _ = c2
     planf, Pf = gpu_plane(F, w, "f32")
-    _, Pb = gpu_plane(F, w, "bf16")
+    _, Pb = gpu_plane(F, w, "bf16", algorithm=algo)
     n, rec = planf.peaks(Pf, THRESH)
     assert n >= 8
     mean_rel, worst = check_bf16_rules(Pb.cpu().numpy(), Pf.cpu().numpy().astype(np.float64),
@@ -204,20 +233,28 @@ def test_config3_full_size_sampled_windows(F):
     for s in starts:
         exp = oracle.power_plane(w.spectrum, w.zmax, w.dz, s, s + 4096)
         check_fp32(Pf[:, s:s + 4096].cpu().numpy(), exp, p_peak)
-    # bf16 against fp32 at full size
-    _, Pb = gpu_plane(F, w, "bf16")
+    # bf16 against fp32 at full size, in the launch configuration bench.py times (auto = mma), and the FFT form
     n, rec = planf.peaks(Pf, THRESH)
     assert n >= 64
-    rel_mean = float(((Pb - Pf).abs() / Pf).mean().item())
-    assert rel_mean <= 0.02
-    Pb_h = Pb.cpu().numpy()
-    worst = 0.0
-    for k, r, pw in rec:
-        best = max(Pb_h[kk, r] for kk in (k - 1, k, k + 1) if 0 <= kk < 97)
-        worst = max(worst, abs(best - pw) / pw)
-    assert worst <= 0.03
-    print(f"config3: {n} peaks, bf16 mean rel {rel_mean:.4f}, worst peak {worst:.4f}")
-    del Pb, Pf
+    for algo in ("auto", "fft"):
+        planb, Pb = gpu_plane(F, w, "bf16", algorithm=algo)
+        assert planb.algorithm() == ("mma" if algo == "auto" else "fft")
+        rel_mean = float(((Pb - Pf).abs() / Pf).mean().item())
+        assert rel_mean <= 0.02
+        Pb_h = Pb.cpu().numpy()
+        worst = 0.0
+        for k, r, pw in rec:
+            best = max(Pb_h[kk, r] for kk in (k - 1, k, k + 1) if 0 <= kk < 97)
+            worst = max(worst, abs(best - pw) / pw)
+        assert worst <= 0.03
+        print(f"config3 bf16/{planb.algorithm()}: {n} peaks, mean rel {rel_mean:.4f}, worst peak {worst:.4f}")
+        if algo == "auto":
+            # tensor-core path element by element: oracle direct sum over the SAME bf16-rounded inputs
+            for s0 in starts[:6]:
+                exp_b = bf16_input_plane(w, s0, s0 + 4096)
+                check_mma(Pb[:, s0:s0 + 4096].cpu().numpy(), exp_b, p_peak)
+        del Pb
+    del Pf
     torch.cuda.empty_cache()
 
 
@@ -331,6 +368,106 @@ def test_zero_drift_row_is_the_power_spectrum(F):
     assert np.abs(row - (X.real ** 2 + X.imag ** 2)).max() < 1e-12 * row.max()
 
 
+# ------------------------------------------------------------------ tensor-core (MMA) path of the bf16 variant
+def test_mma_config1_element_by_element(F):
+    w = workloads.config1()
+    plan, P = gpu_plane(F, w, "bf16")
+    assert plan.algorithm() == "mma"                    # AUTO picks the tensor-core path for bf16
+    err, tol = check_mma(P.cpu().numpy(), bf16_input_plane(w))
+    print(f"config1 mma vs bf16-input oracle: max |dP| {err:.3e} (tol {tol:.3e})")
+    got = P.cpu().numpy()
+    k, r = np.unravel_index(np.argmax(got), got.shape)
+    assert (k, r) == (20, 10000)                        # injected tone (z=+20, r0=10000.25)
+
+
+@pytest.mark.parametrize("N,zmax,dz,S", [
+    (2 * 5000, 5.0, 2.0, 1024),        # asymmetric grid z = -5..3 (no +-z pairs), M not a multiple of 128
+    (2 * 70001, 200.0, 2.0, 4096),     # K = 201 -> two template groups; odd M
+    (2 * 1501, 8.0, 2.0, 256),         # tiny: a few tiles, last one ragged
+    (2 * 33000, 7.5, 2.5, 1024),       # fractional z step
+    (2 * 4099, 96.0, 2.0, 2048),       # bench bank on a short, odd spectrum
+])
+def test_mma_ragged_odd_and_grouped(F, N, zmax, dz, S):
+    w = workloads.noise_only(N, seed=S + 11, zmax=zmax, dz=dz, seglen=S)
+    plan, P = gpu_plane(F, w, "bf16", algorithm="mma")
+    got = P.cpu().numpy()
+    exp = bf16_input_plane(w)
+    assert got.shape == exp.shape
+    check_mma(got, exp)
+    # and the FFT form of the bf16 variant obeys the bf16 rule on the same input
+    _, Pfft = gpu_plane(F, w, "bf16", algorithm="fft")
+    _, Pf = gpu_plane(F, w, "f32")
+    assert float(((Pfft - Pf).abs() / Pf).mean().item()) <= 0.02
+    assert float(((P - Pf).abs() / Pf).mean().item()) <= 0.02
+
+
+def test_mma_tap_matrix_is_the_rounded_oracle_taps(F):
+    # PAPER.md:105 "converted to bfloat16": RNE once from fp64; Table 1 statistics
+    for zmax, dz, S in ((96.0, 2.0, 2048), (5.0, 2.0, 1024)):
+        plan = F.Plan(1 << 16, zmax, dz, S, "bf16")
+        tm = plan.tapmatrix()
+        mm = int(plan.info.halfwidth_max)
+        rels = []
+        for k, z in enumerate(plan.z_values()):
+            h = oracle.template_taps(z)
+            m = (len(h) - 1) // 2
+            got = (tm[k].astype(np.uint32) << 16).view(np.float32)
+            assert np.all(got[: mm - m] == 0) and np.all(got[mm + m + 1:] == 0)
+            g = got[mm - m: mm + m + 1]
+            for part, e64 in ((0, h.real), (1, h.imag)):
+                big = np.abs(e64) > 1e-12                  # (z = 0: off-centre taps are quadrature noise)
+                if not big.any():
+                    continue
+                e = bf16_rne(e64.astype(np.float32))
+                assert np.mean(g[big, part] == e[big]) > 0.999      # double-rounding ties only
+                rel = (g[big, part].astype(np.float64) - e64[big]) / e64[big]
+                assert np.abs(rel).max() <= 2.0 ** -8 * 1.0001
+                rels.append(rel)
+        rels = np.concatenate(rels) * 100.0
+        assert abs(rels.mean()) < 0.02 and 0.13 < rels.std() < 0.19    # paper: mean ~ -0.001 %, sigma 0.153 %
+
+
+def test_mma_deterministic_batched_and_algorithm_switch(F):
+    import torch
+    w = workloads.noise_only(1 << 18, seed=5, zmax=96.0, dz=2.0, seglen=2048)
+    plan = F.Plan(w.N, w.zmax, w.dz, w.seglen, "bf16")
+    x = torch.from_numpy(w.spectrum).cuda()
+    P1 = plan.convolve(x)
+    P2 = plan.convolve(x)
+    assert torch.equal(P1, P2)                                       # bit-reproducible
+    xb = torch.stack([x, torch.roll(x, 17), x])
+    Pb = plan.convolve(xb)
+    assert torch.equal(Pb[0], P1) and torch.equal(Pb[2], P1)
+    # switching the algorithm on a live plan
+    assert F.fdas_set_algorithm(plan._h, F.FDAS_ALGO_FFT) == 0 and plan.algorithm() == "fft"
+    Pfft = plan.convolve(x)
+    assert not torch.equal(Pfft, P1)
+    assert float(((Pfft - P1).abs() / P1).mean().item()) < 0.03
+    assert F.fdas_set_algorithm(plan._h, F.FDAS_ALGO_AUTO) == 0 and plan.algorithm() == "mma"
+    assert F.fdas_set_algorithm(plan._h, 7) == F.FDAS_ERR_INVALID_ARG
+    planf = F.Plan(w.N, w.zmax, w.dz, w.seglen, "f32")
+    assert planf.algorithm() == "fft"
+    assert F.fdas_set_algorithm(planf._h, F.FDAS_ALGO_MMA) == F.FDAS_ERR_UNSUPPORTED
+    assert F.fdas_tapmatrix_host(planf._h, 0, 0) == F.FDAS_ERR_INVALID_ARG
+
+
+def test_mma_zero_input_and_shift_invariance(F):
+    import torch
+    w = workloads.config2()
+    plan = F.Plan(w.N, w.zmax, w.dz, w.seglen, "bf16")
+    x = torch.from_numpy(w.spectrum).cuda()
+    P0 = plan.convolve(torch.zeros_like(x))
+    assert float(P0.abs().max().item()) == 0.0
+    P1 = plan.convolve(x)
+    d = 333
+    xs = torch.zeros_like(x)
+    xs[d:] = x[:-d]
+    P3 = plan.convolve(xs)
+    a = P1[:, 1000:200000]
+    b = P3[:, 1000 + d:200000 + d]
+    assert float((a - b).abs().max().item()) <= 1e-5 * float(a.max().item()) + 1e-5   # P8: no tile seams
+
+
 # ------------------------------------------------------------------ peaks
 def test_peaks_match_oracle_rule_on_gpu_plane(F):
     import torch
@@ -349,6 +486,52 @@ def test_peaks_match_oracle_rule_on_gpu_plane(F):
     assert n2 == n and len(rec2) == 5
     n3, rec3 = plan.peaks(P, 12.0, capacity=0)
     assert n3 == n and len(rec3) == 0
+
+
+@pytest.mark.parametrize("prec", ["bf16", "f32"])
+def test_fused_search_equals_convolve_then_peaks(F, prec):
+    # fdas_search (threshold test fused into the tensor-core epilogue for bf16) returns the plane of
+    # fdas_convolve and the peak set of fdas_peaks; a candidate-buffer overflow falls back to a full scan
+    import torch
+    w = workloads.config2()
+    plan = F.Plan(w.N, w.zmax, w.dz, w.seglen, prec)
+    x = torch.from_numpy(w.spectrum).cuda()
+    P = plan.convolve(x)
+    for thr in (THRESH, 12.0, 6.0):
+        n_ref, rec_ref = plan.peaks(P, thr, capacity=1 << 20)
+        P2, n, rec = plan.search(x, thr, capacity=1 << 20)
+        assert torch.equal(P2, P)
+        assert n == n_ref == len(rec)
+        assert sorted(map(tuple, rec.tolist())) == sorted(map(tuple, rec_ref.tolist()))
+    # repeated calls alternate the two candidate counters
+    for _ in range(3):
+        _, n, rec = plan.search(x, THRESH)
+        assert n == plan.peaks(P, THRESH)[0]
+    # overflow of the candidate buffer (threshold inside the noise) -> same answer through the full scan
+    w2 = workloads.noise_only(1 << 19, seed=9, zmax=96.0, dz=2.0, seglen=2048)
+    plan2 = F.Plan(w2.N, w2.zmax, w2.dz, w2.seglen, prec)
+    x2 = torch.from_numpy(w2.spectrum).cuda()
+    P2 = plan2.convolve(x2)
+    n_ref, rec_ref = plan2.peaks(P2, 2.0, capacity=1 << 22)
+    _, n, rec = plan2.search(x2, 2.0, capacity=1 << 22)
+    assert n == n_ref and n > (1 << 18) // 4
+    assert sorted(map(tuple, rec.tolist())) == sorted(map(tuple, rec_ref.tolist()))
+    # snprintf convention
+    _, n3, rec3 = plan2.search(x2, 2.0, capacity=7)
+    assert n3 == n_ref and len(rec3) == 7
+
+
+def test_fused_search_asymmetric_grid_and_groups(F):
+    import torch
+    for N, zmax, dz, S in ((2 * 50001, 5.0, 2.0, 1024), (2 * 70001, 200.0, 2.0, 4096)):
+        w = workloads.noise_only(N, seed=21, zmax=zmax, dz=dz, seglen=S)
+        plan = F.Plan(w.N, zmax, dz, S, "bf16")
+        x = torch.from_numpy(w.spectrum).cuda()
+        P = plan.convolve(x)
+        n_ref, rec_ref = plan.peaks(P, 7.0, capacity=1 << 20)
+        P2, n, rec = plan.search(x, 7.0, capacity=1 << 20)
+        assert torch.equal(P2, P) and n == n_ref and n > 10
+        assert sorted(map(tuple, rec.tolist())) == sorted(map(tuple, rec_ref.tolist()))
 
 
 def test_peaks_hand_built_planes(F):
