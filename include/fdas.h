@@ -59,8 +59,12 @@ typedef enum {
 typedef enum {
     FDAS_ALGO_AUTO = 0, /* default: FDAS_ALGO_MMA where it applies (FDAS_BF16), else FDAS_ALGO_FFT */
     FDAS_ALGO_FFT = 1,  /* overlap-save FFTs on the fp32/fp64 ALUs, all precisions */
-    FDAS_ALGO_MMA = 2   /* FDAS_BF16 only: the same linear convolution as a bf16 x bf16 -> fp32
+    FDAS_ALGO_MMA = 2,  /* FDAS_BF16 only: the same linear convolution as a bf16 x bf16 -> fp32
                            tensor-core contraction over the taps (tcgen05), no FFT            */
+    FDAS_ALGO_MMA_SCALAR = 3 /* FDAS_ALGO_MMA with the plane written by per-thread stores instead of
+                           shared-memory staging + bulk copies: the form FDAS_ALGO_MMA falls back
+                           to when M % 4 != 0.  Same arithmetic, bit-identical plane; selectable
+                           so that tests and profiles can compare the two store paths.      */
 } fdas_algorithm_t;
 
 typedef enum {
@@ -122,7 +126,7 @@ int fdas_plan_create(fdas_plan_t **out, int64_t N, double zmax, double dz, int s
  *                  m_max <= 255.
  * Errors: INVALID_ARG (NULL, unknown value), UNSUPPORTED (FDAS_ALGO_MMA on a plan that is not
  * FDAS_BF16 or whose taps do not fit).  fdas_get_algorithm reports the algorithm fdas_convolve
- * will run (FDAS_ALGO_FFT or FDAS_ALGO_MMA, never AUTO).
+ * will run (FDAS_ALGO_FFT, FDAS_ALGO_MMA or FDAS_ALGO_MMA_SCALAR, never AUTO).
  */
 int fdas_set_algorithm(fdas_plan_t *p, int algorithm);
 int fdas_get_algorithm(const fdas_plan_t *p, int *algorithm);

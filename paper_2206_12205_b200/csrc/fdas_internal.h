@@ -26,6 +26,7 @@ struct fdas_plan {
     int algo;          // fdas_algorithm_t requested by the caller
     int tc_supported;  // the MMA kernel can run this shape
     int tc_groups, tc_nzg, tc_NT, tc_KS, tc_full_chunks;
+    int tc_force_scalar_stores;   // testing: run the generic (scalar-store) tensor-core kernel
     void *tc_bmat;     // [groups][2 KS][NT][8] bf16
     size_t tc_bmat_bytes;
     int2 *tc_ktab;     // [groups][nzg] plane rows of (+|z|, -|z|), -1 where absent
@@ -66,6 +67,12 @@ __host__ __device__ static inline size_t fdas_bank_offset(int k, int f, int T, i
     return (((size_t)k * (FDAS_PTS / VC) + a / VC) * T + t) * VC + a % VC;
 }
 
+// Column order of the tensor-core tap matrix (fdas_mma.cu): entry pair p = n/4 holds
+// (hre_2p, hre_2p+1, him_2p, him_2p+1).
+__host__ __device__ static inline int fdas_tc_entry_of_column(int n) { return 2 * (n >> 2) + (n & 1); }
+__host__ __device__ static inline int fdas_tc_column_is_imag(int n) { return (n >> 1) & 1; }
+__host__ __device__ static inline int fdas_tc_column_of_entry(int zi, int imag) { return 4 * (zi >> 1) + (zi & 1) + 2 * imag; }
+
 // What the convolve epilogue needs to flag candidates for fdas_search (enabled = 0: plain convolve).
 struct fdas_search_args {
     int enabled;
@@ -75,6 +82,7 @@ struct fdas_search_args {
     int *cand_count_next;  // cleared by this launch for the next call
     int cand_capacity;
     int *count_out;        // caller's peak counter, cleared by this launch
+    int cand_span;         // |z| table entries one candidate covers (set by the convolve launch)
 };
 
 #define FDAS_CUDA_TRY(p, call)                                  \
@@ -93,7 +101,7 @@ int fdas_launch_convolve(fdas_plan *p, const void *spectra, void *planes, int ba
 int fdas_mma_plan(fdas_plan *p);
 int fdas_launch_build_tapmatrix(fdas_plan *p, cudaStream_t st);
 int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, int batch, cudaStream_t st,
-                             const fdas_search_args *search = nullptr);
+                             fdas_search_args *search = nullptr);
 // fdas_peaks.cu: turns the candidates of a fused search into the peak list (same rule as fdas_peaks)
 int fdas_launch_resolve(fdas_plan *p, const void *plane, const fdas_search_args &sa, fdas_peak_t *peaks, int capacity,
                         cudaStream_t st);

@@ -11,7 +11,10 @@
 //
 //      D[r][n] = sum_kappa T[r][kappa] * B[n][kappa]
 //      T[r][kappa] = X_part[r - M0 + kappa]      (Toeplitz matrix of the spectrum, part = re | im)
-//      B[n][kappa] = hre_|z|[M0 - kappa] (n even) or him_|z|[M0 - kappa] (n odd)
+//      B[n][kappa] = hre_|z|[M0 - kappa] or him_|z|[M0 - kappa]; the columns of two consecutive
+//                    |z| entries e, e+1 are ordered (hre_e, hre_e+1, him_e, him_e+1) so that
+//                    the accumulators of an entry pair sit in adjacent registers (packed
+//                    fp32x2 arithmetic in the epilogue)
 //
 // The Toeplitz matrix is never materialised per tile: shared memory holds Z[i] = the eight
 // consecutive bf16 samples X_part[g0 + i .. g0 + i + 7] as one 16-byte row, and a K-major,
@@ -26,10 +29,20 @@
 // and Uim/Vim in the SAME TMEM lane, so the epilogue thread of lane r forms both powers
 // without any exchange and a warp stores 32 consecutive bins of one plane row (128 bytes).
 //
-// One persistent CTA per SM, warp-specialised:
+// One persistent CTA per SM, warp-specialised.  Two kernels share the loader and the MMA issuer:
+//
+// fdas_mma_bulk_kernel (M % 4 == 0, the normal case)
+//   warps 0-15  epilogue: tcgen05.ld -> packed |.|^2 -> shared-memory staging rows of 128 bins;
+//               one thread per plane row then pushes its 512-byte row segment to HBM with a 1-D
+//               bulk copy (cp.async.bulk.global.shared::cta).  Measured on B200: 128-byte scalar
+//               row segments cap the plane write at ~4.9 TB/s, 512-byte bulk segments reach
+//               6.3 TB/s.
+//   warp  16    one thread issues tcgen05.mma and tcgen05.commit
+//   warps 17-20 loader: spectrum block -> bf16 (RNE, reading A12) -> Z rows
+//
+// fdas_mma_convolve_kernel (any M: bulk copies need 16-byte aligned rows)
 //   warps 0-7   epilogue: tcgen05.ld -> |.|^2 -> st.global.cs (TMEM double-buffered)
-//   warp  8     one thread issues tcgen05.mma and tcgen05.commit
-//   warps 9-12  loader: spectrum block -> bf16 (RNE, reading A12) -> Z rows
+//   warp  8     MMA issuer;  warps 9-12 loader
 #include <cuda_bf16.h>
 #include <math.h>
 #include <stdlib.h>
@@ -207,7 +220,8 @@ __device__ __forceinline__ void st_cs_at(const float *base, uint32_t off, float 
 constexpr uint32_t TC_NO_ROW = 0xFFFFFFFFu;   // row-offset table: this |z| has no such plane row
 
 // |.|^2 of Y_{+|z|} and Y_{-|z|} for the eight |z| of one 16-column chunk (file header) and the
-// stores.  v[0..15] = (Ure, Vre) pairs, v[16..31] = (Uim, Vim) pairs of this thread's output bin;
+// stores.  v[0..15] = (Ure_e, Ure_e+1, Vre_e, Vre_e+1) per entry pair, v[16..31] likewise for
+// Uim, Vim, of this thread's output bin;
 // o4[0..3] = row offsets (+|z|, -|z|) of two |z| each, in plane elements.
 // FAST: the tile lies inside the plane and every entry has both rows -> straight-line code.
 // Returns the largest power this thread stored (0 if none): the fused search flags the chunk
@@ -221,26 +235,25 @@ __device__ __forceinline__ float epilogue_chunk(const uint32_t *v, const uint4 *
         const uint4 o = o4[e2];
 #pragma unroll
         for (int s = 0; s < 2; ++s) {
-            const int e = 2 * e2 + s;
             const uint32_t offp = s ? o.z : o.x, offm = s ? o.w : o.y;
-            const float ure = __uint_as_float(v[2 * e]), vre = __uint_as_float(v[2 * e + 1]);
-            const float uim = __uint_as_float(v[16 + 2 * e]), vim = __uint_as_float(v[16 + 2 * e + 1]);
+            const float ure = __uint_as_float(v[4 * e2 + s]), vre = __uint_as_float(v[4 * e2 + 2 + s]);
+            const float uim = __uint_as_float(v[16 + 4 * e2 + s]), vim = __uint_as_float(v[16 + 4 * e2 + 2 + s]);
             if (FAST) {
                 const float a = ure - vim, b = uim + vre, c = ure + vim, d = uim - vre;
-                const float pp = a * a + b * b, pm = c * c + d * d;
+                const float pp = __fmaf_rn(b, b, __fmul_rn(a, a)), pm = __fmaf_rn(d, d, __fmul_rn(c, c));   // as the bulk kernel
                 st_cs_at(out, offp, pp);
                 st_cs_at(out, offm, pm);
                 mx = fmaxf(mx, fmaxf(pp, pm));
             } else {
                 if (offp != TC_NO_ROW && ok) {
                     const float a = ure - vim, b = uim + vre;
-                    const float pp = a * a + b * b;
+                    const float pp = __fmaf_rn(b, b, __fmul_rn(a, a));
                     st_cs_at(out, offp, pp);
                     mx = fmaxf(mx, pp);
                 }
                 if (offm != TC_NO_ROW && ok) {
                     const float c = ure + vim, d = uim - vre;
-                    const float pm = c * c + d * d;
+                    const float pm = __fmaf_rn(d, d, __fmul_rn(c, c));
                     st_cs_at(out, offm, pm);
                     mx = fmaxf(mx, pm);
                 }
@@ -299,6 +312,57 @@ __device__ __forceinline__ void epilogue_tile(uint32_t taddr, const uint4 *otab4
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(empty_bar);
+    }
+}
+
+// The loader warps of both kernels: per work item, the spectrum block -> bf16 (round to nearest
+// even, reading A12) -> the Z rows (file header) of buffer n & 1.
+__device__ __forceinline__ void spectrum_loader(const TcParams &p, unsigned char *smem, uint32_t off_xs,
+                                                uint32_t xs_part_bytes, uint32_t xn, uint32_t off_z, uint32_t z_buf_bytes,
+                                                uint32_t z_part_bytes, uint32_t zr, uint32_t z_full, uint32_t z_empty,
+                                                int lt, long long n_items)
+{
+    uint32_t *xs_re = reinterpret_cast<uint32_t *>(smem + off_xs);
+    uint32_t *xs_im = reinterpret_cast<uint32_t *>(smem + off_xs + xs_part_bytes);
+    uint32_t n = 0;
+    for (long long it = blockIdx.x; it < n_items; it += gridDim.x, ++n) {
+        const uint32_t buf = n & 1, zuse = n >> 1;
+        const long long ser = it / p.n_blocks;
+        const long long g0 = (it % p.n_blocks) * p.R - p.M0;   // sample index of xs[0]
+        const float2 *__restrict__ X = p.spectra + (size_t)ser * p.M;
+        // phase A: spectrum block -> bf16 (round-to-nearest-even), re and im planes
+        for (uint32_t pi = lt; pi < xn / 2; pi += TC_LOAD_THREADS) {
+            const long long g = g0 + 2 * (long long)pi;
+            float2 a = make_float2(0.f, 0.f), b = make_float2(0.f, 0.f);
+            if (g >= 0 && g < p.M) a = __ldg(X + g);
+            if (g + 1 >= 0 && g + 1 < p.M) b = __ldg(X + g + 1);
+            xs_re[pi] = pack_bf16(a.x, b.x);
+            xs_im[pi] = pack_bf16(a.y, b.y);
+        }
+        named_bar_sync(1, TC_LOAD_THREADS);
+        mbar_wait<64>(z_empty + 8 * buf, (zuse & 1) ^ 1);
+        // phase B: Z row i = samples i .. i+7 (16 bytes), for both parts
+        unsigned char *zb = smem + off_z + buf * z_buf_bytes;
+        for (uint32_t row = lt; row < zr; row += TC_LOAD_THREADS) {
+#pragma unroll
+            for (int part = 0; part < 2; ++part) {
+                const uint32_t *w = (part ? xs_im : xs_re) + (row >> 1);
+                uint4 o;
+                if (row & 1) {
+                    const uint32_t w0 = w[0], w1 = w[1], w2 = w[2], w3 = w[3], w4 = w[4];
+                    o.x = __byte_perm(w0, w1, 0x5432);
+                    o.y = __byte_perm(w1, w2, 0x5432);
+                    o.z = __byte_perm(w2, w3, 0x5432);
+                    o.w = __byte_perm(w3, w4, 0x5432);
+                } else {
+                    o = make_uint4(w[0], w[1], w[2], w[3]);
+                }
+                *reinterpret_cast<uint4 *>(zb + part * z_part_bytes + (size_t)row * 16) = o;
+            }
+        }
+        fence_proxy_async();   // generic-proxy writes of Z -> visible to tcgen05.mma
+        mbar_arrive(z_full + 8 * buf);
+        named_bar_sync(1, TC_LOAD_THREADS);   // xs is rewritten by the next item
     }
 }
 
@@ -423,49 +487,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1) fdas_mma_convolve_kernel(const 
         }
     } else {
         // =========================== loader ===========================
-        const int lt = threadIdx.x - TC_LOAD_WARP0 * 32;
-        uint32_t *xs_re = reinterpret_cast<uint32_t *>(smem + L.off_xs);
-        uint32_t *xs_im = reinterpret_cast<uint32_t *>(smem + L.off_xs + L.xs_part_bytes);
-        uint32_t n = 0;
-        for (long long it = blockIdx.x; it < n_items; it += gridDim.x, ++n) {
-            const uint32_t buf = n & 1, zuse = n >> 1;
-            const long long ser = it / p.n_blocks;
-            const long long g0 = (it % p.n_blocks) * p.R - p.M0;   // sample index of xs[0]
-            const float2 *__restrict__ X = p.spectra + (size_t)ser * p.M;
-            // phase A: spectrum block -> bf16 (round-to-nearest-even), re and im planes
-            for (uint32_t pi = lt; pi < L.xn / 2; pi += TC_LOAD_THREADS) {
-                const long long g = g0 + 2 * (long long)pi;
-                float2 a = make_float2(0.f, 0.f), b = make_float2(0.f, 0.f);
-                if (g >= 0 && g < p.M) a = __ldg(X + g);
-                if (g + 1 >= 0 && g + 1 < p.M) b = __ldg(X + g + 1);
-                xs_re[pi] = pack_bf16(a.x, b.x);
-                xs_im[pi] = pack_bf16(a.y, b.y);
-            }
-            named_bar_sync(1, TC_LOAD_THREADS);
-            mbar_wait<64>(z_empty + 8 * buf, (zuse & 1) ^ 1);
-            // phase B: Z row i = samples i .. i+7 (16 bytes), for both parts
-            unsigned char *zb = smem + L.off_z + buf * L.z_buf_bytes;
-            for (uint32_t row = lt; row < L.zr; row += TC_LOAD_THREADS) {
-#pragma unroll
-                for (int part = 0; part < 2; ++part) {
-                    const uint32_t *w = (part ? xs_im : xs_re) + (row >> 1);
-                    uint4 o;
-                    if (row & 1) {
-                        const uint32_t w0 = w[0], w1 = w[1], w2 = w[2], w3 = w[3], w4 = w[4];
-                        o.x = __byte_perm(w0, w1, 0x5432);
-                        o.y = __byte_perm(w1, w2, 0x5432);
-                        o.z = __byte_perm(w2, w3, 0x5432);
-                        o.w = __byte_perm(w3, w4, 0x5432);
-                    } else {
-                        o = make_uint4(w[0], w[1], w[2], w[3]);
-                    }
-                    *reinterpret_cast<uint4 *>(zb + part * L.z_part_bytes + (size_t)row * 16) = o;
-                }
-            }
-            fence_proxy_async();   // generic-proxy writes of Z -> visible to tcgen05.mma
-            mbar_arrive(z_full + 8 * buf);
-            named_bar_sync(1, TC_LOAD_THREADS);   // xs is rewritten by the next item
-        }
+        spectrum_loader(p, smem, L.off_xs, L.xs_part_bytes, L.xn, L.off_z, L.z_buf_bytes, L.z_part_bytes, L.zr, z_full,
+                        z_empty, threadIdx.x - TC_LOAD_WARP0 * 32, n_items);
     }
 
     tc_fence_before();
@@ -477,9 +500,299 @@ __global__ void __launch_bounds__(TC_THREADS, 1) fdas_mma_convolve_kernel(const 
     }
 }
 
+// =====================================================================================
+// fdas_mma_bulk_kernel: the same loader and MMA issuer; the epilogue stages the powers in
+// shared memory and writes the plane with bulk copies.
+// =====================================================================================
+constexpr int TB_EPI_WARPS = 16;        // 4 TMEM lane quarters x 4 column groups
+constexpr int TB_MMA_WARP = 16;
+constexpr int TB_LOAD_WARP0 = 17;
+constexpr int TB_THREADS = 32 * (TB_EPI_WARPS + 1 + TC_LOAD_WARPS);   // 672
+constexpr int TB_CGROUPS = 4;           // column groups: NCH entry pairs (4 NCH columns per part) each
+constexpr int TB_MAX_SLOTS = 32;        // staging rows per column group = 4 NCH <= 32
+
+// shared-memory carve-up of the bulk kernel.  ROWB = bytes of one staging row (one plane row
+// segment pushed out by one bulk copy): 128 bins x 4 B.
+struct TbSmem {
+    uint32_t b_bytes, zr, z_part_bytes, z_buf_bytes, xn, xs_part_bytes, slots, stage_cg_bytes;
+    uint32_t off_z, off_xs, off_stage, off_rowtab, off_bars, off_holder, total;
+    __host__ __device__ TbSmem(int R, int KS, int NT, int rowb)
+    {
+        const uint32_t TP = 16u * KS;
+        b_bytes = 2u * KS * NT * 16u;
+        zr = R + TP - 8;
+        z_part_bytes = zr * 16u;
+        z_buf_bytes = 2u * z_part_bytes;
+        xn = R + TP;
+        xs_part_bytes = xn * 2u;
+        slots = (uint32_t)NT / 4u;                 // 4 NCH
+        stage_cg_bytes = slots * (uint32_t)rowb;   // one buffer of one column group
+        off_z = b_bytes;
+        off_xs = off_z + 2u * z_buf_bytes;
+        off_stage = (off_xs + 2u * xs_part_bytes + 127u) & ~127u;
+        off_rowtab = off_stage + 2u * TB_CGROUPS * stage_cg_bytes;
+        off_bars = (off_rowtab + 4u * TB_CGROUPS * TB_MAX_SLOTS + 15u) & ~15u;
+        off_holder = off_bars + 8u * 8u;
+        total = off_holder + 16u;
+    }
+};
+
+// TMEM -> registers, this warp's 32 lanes x N consecutive columns (N a multiple of 4, <= 32)
+template <int N>
+__device__ __forceinline__ void tmem_ld_cols(uint32_t taddr, uint32_t *v)
+{
+    if constexpr (N >= 16) {
+        asm volatile(
+            "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+            : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+              "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+            : "r"(taddr)
+            : "memory");
+        tmem_ld_cols<N - 16>(taddr + 16, v + 16);
+    } else if constexpr (N >= 8) {
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                     : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+                     : "r"(taddr)
+                     : "memory");
+        tmem_ld_cols<N - 8>(taddr + 8, v + 8);
+    } else if constexpr (N >= 4) {
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
+                     : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3])
+                     : "r"(taddr)
+                     : "memory");
+        tmem_ld_cols<N - 4>(taddr + 4, v + 4);
+    }
+}
+// tcgen05.wait::ld, then pin every loaded register behind it (an empty asm the compiler cannot
+// hoist a use across)
+template <int N>
+__device__ __forceinline__ void tmem_ld_fence(uint32_t *v)
+{
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+    for (int i = 0; i < N; ++i) asm volatile("" : "+r"(v[i]));
+}
+
+// packed fp32x2 arithmetic (FADD2 / FMUL2 / FFMA2 on sm_100a)
+__device__ __forceinline__ unsigned long long f2_pack(uint32_t lo, uint32_t hi)
+{
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(lo), "r"(hi));
+    return r;
+}
+__device__ __forceinline__ void f2_unpack(unsigned long long v, float &lo, float &hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ unsigned long long f2_add(unsigned long long a, unsigned long long b)
+{
+    unsigned long long r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ unsigned long long f2_sub(unsigned long long a, unsigned long long b)
+{
+    unsigned long long r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ unsigned long long f2_mul(unsigned long long a, unsigned long long b)
+{
+    unsigned long long r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ unsigned long long f2_fma(unsigned long long a, unsigned long long b, unsigned long long c)
+{
+    unsigned long long r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+
+__device__ __forceinline__ void bulk_store(void *gdst, uint32_t ssrc, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(ssrc), "r"(bytes)
+                 : "memory");
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+}
+__device__ __forceinline__ void bulk_wait_read_all() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+
+template <int NCH>
+__global__ void __launch_bounds__(TB_THREADS, 1) fdas_mma_bulk_kernel(const TcParams p)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    constexpr int NT = 16 * NCH;
+    constexpr int NC = 4 * NCH;            // columns per part per column group = staging rows (slots)
+    constexpr uint32_t ROWB = TC_TILE * 4; // bytes of one staging row
+    const TbSmem L(p.R, p.KS, NT, ROWB);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int grp = blockIdx.y;
+    const long long n_items = (long long)p.batch * p.n_blocks;
+
+    const uint32_t s_base = smem_u32(smem);
+    const uint32_t bars = s_base + L.off_bars;
+    const uint32_t z_full = bars, z_empty = bars + 16, t_full = bars + 32, t_empty = bars + 48;
+    uint32_t *holder = reinterpret_cast<uint32_t *>(smem + L.off_holder);
+    int *rowtab = reinterpret_cast<int *>(smem + L.off_rowtab);   // [TB_CGROUPS][TB_MAX_SLOTS] plane row or -1
+
+    // ---- one-time setup: tap matrix image and staging-row table -> shared memory, barriers, TMEM
+    {
+        const uint4 *src = p.bmat + (size_t)grp * (L.b_bytes / 16);
+        uint4 *dst = reinterpret_cast<uint4 *>(smem);
+        for (uint32_t i = threadIdx.x; i < L.b_bytes / 16; i += TB_THREADS) dst[i] = __ldg(src + i);
+        // slot 4 pr + 2 s + sign of column group cg <-> |z| entry 2 (cg NCH + pr) + s, sign: 0 = +|z|, 1 = -|z|
+        for (int i = threadIdx.x; i < TB_CGROUPS * TB_MAX_SLOTS; i += TB_THREADS) {
+            const int cg = i / TB_MAX_SLOTS, slot = i % TB_MAX_SLOTS;
+            const int el = 2 * (cg * NCH + (slot >> 2)) + ((slot >> 1) & 1);
+            int row = -1;
+            if (slot < NC && el < p.nzg) {
+                const int2 kk = p.ktab[(size_t)grp * p.nzg + el];
+                row = (slot & 1) ? (kk.y == kk.x ? -1 : kk.y) : kk.x;   // z = 0 names its row twice
+            }
+            rowtab[i] = row;
+        }
+        fence_proxy_async();
+    }
+    if (threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0 && p.search.enabled) {
+        *p.search.cand_count_next = 0;
+        *p.search.count_out = 0;
+    }
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < 2; ++s) {
+            mbar_init(z_full + 8 * s, TC_LOAD_THREADS);
+            mbar_init(z_empty + 8 * s, 1);
+            mbar_init(t_full + 8 * s, 1);
+            mbar_init(t_empty + 8 * s, TB_EPI_WARPS);
+        }
+        fence_barrier_init();
+    }
+    if (warp == TB_MMA_WARP) tmem_alloc(smem_u32(holder), TC_TMEM_COLS);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *holder;
+
+    if (warp < TB_EPI_WARPS) {
+        // =========================== epilogue ===========================
+        const int q = warp & 3, cg = warp >> 2;
+        const int lt = q * 32 + lane;                       // bin inside the tile = TMEM lane
+        const float thr = p.search.enabled ? p.search.thr : __int_as_float(0x7f800000);
+        const int zi_cg0 = grp * p.nzg + 2 * cg * NCH;      // first |z| table entry of this column group
+        // staging row (slot) this thread pushes out: the NC slots are dealt round-robin to the four
+        // warps of the column group (a warp issues its bulk copies one lane at a time)
+        const int my_slot = 4 * lane + q;
+        const int my_row = my_slot < NC ? rowtab[cg * TB_MAX_SLOTS + my_slot] : -1;
+        unsigned char *const stage_cg = smem + L.off_stage + (size_t)cg * 2 * L.stage_cg_bytes;
+        uint32_t t = 0;
+        for (long long it = blockIdx.x; it < n_items; it += gridDim.x) {
+            const long long ser = it / p.n_blocks;
+            const long long blk0 = (it % p.n_blocks) * p.R;
+            const long long left = p.M - blk0;
+            const int n_tiles = (int)((left < p.R ? left : p.R) + TC_TILE - 1) / TC_TILE;
+            for (int tile = 0; tile < n_tiles; ++tile, ++t) {
+                const uint32_t stage = t & 1, use = t >> 1;
+                const long long col0 = blk0 + tile * TC_TILE;
+                const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + stage * TC_STAGE_COLS + cg * NC;
+                uint32_t v[2 * NC];
+                mbar_wait(t_full + 8 * stage, use & 1);
+                tc_fence_after();
+                tmem_ld_cols<NC>(taddr, v);
+                tmem_ld_cols<NC>(taddr + NT, v + NC);
+                tmem_ld_fence<2 * NC>(v);
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(t_empty + 8 * stage);
+                // staging buffer `stage` of this column group was handed to the bulk copies two tiles
+                // ago; the thread that issued them waited for their shared-memory reads before the
+                // previous tile's barrier, so it is free
+                float *const sb = reinterpret_cast<float *>(stage_cg + stage * L.stage_cg_bytes) + lt;
+                float mx = 0.f;
+#pragma unroll
+                for (int pr = 0; pr < NCH; ++pr) {
+                    const unsigned long long ure = f2_pack(v[4 * pr], v[4 * pr + 1]), vre = f2_pack(v[4 * pr + 2], v[4 * pr + 3]);
+                    const unsigned long long uim = f2_pack(v[NC + 4 * pr], v[NC + 4 * pr + 1]);
+                    const unsigned long long vim = f2_pack(v[NC + 4 * pr + 2], v[NC + 4 * pr + 3]);
+                    const unsigned long long a = f2_sub(ure, vim), b = f2_add(uim, vre);
+                    const unsigned long long c = f2_add(ure, vim), d = f2_sub(uim, vre);
+                    const unsigned long long pp = f2_fma(b, b, f2_mul(a, a)), pm = f2_fma(d, d, f2_mul(c, c));
+                    float pp0, pp1, pm0, pm1;
+                    f2_unpack(pp, pp0, pp1);
+                    f2_unpack(pm, pm0, pm1);
+                    sb[(4 * pr + 0) * TC_TILE] = pp0;
+                    sb[(4 * pr + 1) * TC_TILE] = pm0;
+                    sb[(4 * pr + 2) * TC_TILE] = pp1;
+                    sb[(4 * pr + 3) * TC_TILE] = pm1;
+                    // padded columns give exactly zero; a sign whose row is not in the plane (asymmetric
+                    // grids) can only add a candidate, which the resolve kernel then rejects
+                    mx = fmaxf(mx, fmaxf(fmaxf(pp0, pm0), fmaxf(pp1, pm1)));
+                }
+                if (my_row >= 0) bulk_wait_read_all();     // the other buffer's copies (previous tile) have read it
+                fence_proxy_async();                       // staging writes -> visible to the bulk copy engine
+                named_bar_sync(2 + cg, 128);
+                if (my_row >= 0) {
+                    const long long rest = p.M - col0;     // > 0
+                    const uint32_t bytes = rest >= TC_TILE ? ROWB : (uint32_t)rest * 4u;
+                    float *dst = p.planes + ((size_t)ser * p.K + my_row) * p.M + col0;
+                    bulk_store(dst, smem_u32(stage_cg + stage * L.stage_cg_bytes + (size_t)my_slot * ROWB), bytes);
+                }
+                if (mx > thr && col0 + lt < p.M && 2 * cg * NCH < p.nzg)
+                    flag_candidate(p.search.cand, p.search.cand_count, p.search.cand_capacity, zi_cg0, (int)(col0 + lt), mx);
+            }
+        }
+        if (my_row >= 0) bulk_wait_all();
+    } else if (warp == TB_MMA_WARP) {
+        // =========================== MMA issuer ===========================
+        if (lane == 0) {
+            const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(NT >> 3) << 17) |
+                                   ((uint32_t)(TC_TILE >> 4) << 24);
+            const uint32_t b_addr = s_base;
+            const uint32_t b_lbo = (uint32_t)NT * 16u;
+            uint32_t n = 0, t = 0;
+            for (long long it = blockIdx.x; it < n_items; it += gridDim.x, ++n) {
+                const uint32_t buf = n & 1, zuse = n >> 1;
+                const long long blk0 = (it % p.n_blocks) * p.R;
+                const long long left = p.M - blk0;
+                const int n_tiles = (int)((left < p.R ? left : p.R) + TC_TILE - 1) / TC_TILE;
+                mbar_wait(z_full + 8 * buf, zuse & 1);
+                tc_fence_after();
+                const uint32_t z_addr = s_base + L.off_z + buf * L.z_buf_bytes;
+                for (int tile = 0; tile < n_tiles; ++tile, ++t) {
+                    const uint32_t stage = t & 1, use = t >> 1;
+                    mbar_wait(t_empty + 8 * stage, (use & 1) ^ 1);
+                    tc_fence_after();
+                    for (int part = 0; part < 2; ++part) {
+                        const uint32_t d = tmem_base + stage * TC_STAGE_COLS + part * NT;
+                        const uint32_t a0 = z_addr + part * L.z_part_bytes + (uint32_t)(tile * TC_TILE) * 16u;
+                        for (int ks = 0; ks < p.KS; ++ks) {
+                            const uint64_t ad = smem_desc(a0 + ks * 256u, 128u, 128u);
+                            const uint64_t bd = smem_desc(b_addr + ks * 2u * b_lbo, b_lbo, 128u);
+                            umma_bf16(d, ad, bd, idesc, ks > 0);
+                        }
+                    }
+                    umma_commit(t_full + 8 * stage);
+                }
+                umma_commit(z_empty + 8 * buf);
+            }
+        }
+    } else {
+        // =========================== loader ===========================
+        spectrum_loader(p, smem, L.off_xs, L.xs_part_bytes, L.xn, L.off_z, L.z_buf_bytes, L.z_part_bytes, L.zr, z_full,
+                        z_empty, threadIdx.x - TB_LOAD_WARP0 * 32, n_items);
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == TB_MMA_WARP) {
+        __syncwarp();
+        tc_fence_after();
+        tmem_dealloc(tmem_base, TC_TMEM_COLS);
+    }
+}
+
 // ---- tap matrix builder -----------------------------------------------------------------
-// bmat[g][q][n][e], kappa = 8 q + e, j = M0 - kappa: bf16(RNE, once from fp64) of the real
-// (n even) or imaginary (n odd) part of h_{+|z|}[j] for |z| index g*nzg + n/2; zero padding.
+// bmat[g][q][n][e], kappa = 8 q + e, j = M0 - kappa: bf16(RNE, once from fp64) of h_{+|z|}[j] for
+// |z| index zi = g*nzg + 2 (n/4) + (n & 1), real part if (n & 2) == 0 else imaginary; zero padding.
 // kref[g][zi] = (template whose fp64 taps are read, +1 if its z >= 0 else -1): h_{+|z|} = conj(h_{-|z|}).
 __global__ void fdas_tapmatrix_kernel(__nv_bfloat16 *bmat, const double2 *__restrict__ taps, const int2 *__restrict__ kref,
                                       int groups, int nzg, int NT, int KS, int m_max)
@@ -491,13 +804,13 @@ __global__ void fdas_tapmatrix_kernel(__nv_bfloat16 *bmat, const double2 *__rest
         const int qq = (int)((idx / 8 / NT) % (2 * KS));
         const int g = (int)(idx / 8 / NT / (2 * KS));
         const int j = m_max - (8 * qq + e);
-        const int zi = n >> 1;
+        const int zi = fdas_tc_entry_of_column(n);
         double v = 0.0;
         if (j >= -m_max && zi < nzg) {
             const int2 kr = kref[(size_t)g * nzg + zi];
             if (kr.x >= 0) {
                 const double2 h = taps[(size_t)kr.x * (2 * m_max + 1) + (m_max + j)];
-                v = (n & 1) ? (double)kr.y * h.y : h.x;
+                v = fdas_tc_column_is_imag(n) ? (double)kr.y * h.y : h.x;
             }
         }
         bmat[idx] = __double2bfloat16(v);
@@ -585,35 +898,50 @@ int fdas_launch_build_tapmatrix(fdas_plan *p, cudaStream_t st)
 }
 
 template <int NCH>
-static int launch_mma(fdas_plan *p, const TcParams &tp, unsigned gx, size_t smem_bytes, cudaStream_t st)
+static int launch_mma(fdas_plan *p, const TcParams &tp, unsigned gx, size_t smem_bytes, bool bulk, cudaStream_t st)
 {
-    auto kern = fdas_mma_convolve_kernel<NCH>;
-    static size_t attr_bytes = 0;
-    if (smem_bytes > attr_bytes) {
-        FDAS_CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
-        attr_bytes = smem_bytes;
+    if (bulk) {
+        auto kern = fdas_mma_bulk_kernel<NCH>;
+        static size_t attr_bytes = 0;
+        if (smem_bytes > attr_bytes) {
+            FDAS_CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
+            attr_bytes = smem_bytes;
+        }
+        kern<<<dim3(gx, p->tc_groups), TB_THREADS, smem_bytes, st>>>(tp);
+    } else {
+        auto kern = fdas_mma_convolve_kernel<NCH>;
+        static size_t attr_bytes = 0;
+        if (smem_bytes > attr_bytes) {
+            FDAS_CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
+            attr_bytes = smem_bytes;
+        }
+        kern<<<dim3(gx, p->tc_groups), TC_THREADS, smem_bytes, st>>>(tp);
     }
-    kern<<<dim3(gx, p->tc_groups), TC_THREADS, smem_bytes, st>>>(tp);
     FDAS_CUDA_TRY(p, cudaGetLastError());
     p->launches += 1;
     return FDAS_OK;
 }
 
 int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, int batch, cudaStream_t st,
-                             const fdas_search_args *search)
+                             fdas_search_args *search)
 {
     if (p->precision != FDAS_BF16 || !p->tc_supported) return FDAS_ERR_UNSUPPORTED;
+    // bulk copies need every plane row segment 16-byte aligned: M % 4 == 0 (the caller's plane is 16-byte aligned)
+    const bool bulk = (p->M % 4 == 0) && ((reinterpret_cast<uintptr_t>(planes) & 15u) == 0) && !p->tc_force_scalar_stores;
+    const uint32_t smem_cap = 227u * 1024u;
+    auto smem_total = [&](int R) -> uint32_t {
+        return bulk ? TbSmem(R, p->tc_KS, p->tc_NT, TC_TILE * 4).total : TcSmem(R, p->tc_KS, p->tc_NT).total;
+    };
     // outputs per work item: the largest of 1024..128 that fits shared memory and leaves at
     // least two items per CTA
     const int sms_per_group = p->num_sms / p->tc_groups > 0 ? p->num_sms / p->tc_groups : 1;
     int R = 1024;
     for (;; R >>= 1) {
-        const TcSmem L(R, p->tc_KS, p->tc_NT);
         const long long items = (long long)batch * ((p->M + R - 1) / R);
-        if (R == 128 || (L.total <= 227u * 1024u && items >= 2LL * sms_per_group)) break;
+        if (R == 128 || (smem_total(R) <= smem_cap && items >= 2LL * sms_per_group)) break;
     }
-    const TcSmem L(R, p->tc_KS, p->tc_NT);
-    if (L.total > 227u * 1024u) return FDAS_ERR_UNSUPPORTED;
+    const uint32_t total = smem_total(R);
+    if (total > smem_cap) return FDAS_ERR_UNSUPPORTED;
     TcParams tp;
     tp.spectra = static_cast<const float2 *>(spectra);
     tp.planes = static_cast<float *>(planes);
@@ -629,19 +957,23 @@ int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, in
     tp.NT = p->tc_NT;
     tp.nzg = p->tc_nzg;
     tp.full_chunks = p->tc_full_chunks;
-    if (search) tp.search = *search;
-    else tp.search = fdas_search_args{0, 0.f, nullptr, nullptr, nullptr, 0, nullptr};
+    if (search) {
+        search->cand_span = bulk ? p->tc_NT / 8 : 8;   // |z| entries per column group (2 NCH) / per 16-column chunk
+        tp.search = *search;
+    } else {
+        tp.search = fdas_search_args{0, 0.f, nullptr, nullptr, nullptr, 0, nullptr, 8};
+    }
     const long long items = (long long)batch * tp.n_blocks;
     const unsigned gx = (unsigned)(items < sms_per_group ? items : sms_per_group);
     switch (p->tc_NT / 16) {
-    case 1: return launch_mma<1>(p, tp, gx, L.total, st);
-    case 2: return launch_mma<2>(p, tp, gx, L.total, st);
-    case 3: return launch_mma<3>(p, tp, gx, L.total, st);
-    case 4: return launch_mma<4>(p, tp, gx, L.total, st);
-    case 5: return launch_mma<5>(p, tp, gx, L.total, st);
-    case 6: return launch_mma<6>(p, tp, gx, L.total, st);
-    case 7: return launch_mma<7>(p, tp, gx, L.total, st);
-    case 8: return launch_mma<8>(p, tp, gx, L.total, st);
+    case 1: return launch_mma<1>(p, tp, gx, total, bulk, st);
+    case 2: return launch_mma<2>(p, tp, gx, total, bulk, st);
+    case 3: return launch_mma<3>(p, tp, gx, total, bulk, st);
+    case 4: return launch_mma<4>(p, tp, gx, total, bulk, st);
+    case 5: return launch_mma<5>(p, tp, gx, total, bulk, st);
+    case 6: return launch_mma<6>(p, tp, gx, total, bulk, st);
+    case 7: return launch_mma<7>(p, tp, gx, total, bulk, st);
+    case 8: return launch_mma<8>(p, tp, gx, total, bulk, st);
     default: return FDAS_ERR_UNSUPPORTED;
     }
 }

@@ -73,22 +73,23 @@ fdas_peaks_kernel(const PT *__restrict__ P, int K, long long M, float thr, fdas_
 }
 
 // fdas_search, second kernel.  The convolve epilogue flagged (zi0, r): "one of the powers of bin
-// r in |z| table entries zi0 .. zi0+7 exceeds the threshold".  Each thread takes one (entry,
+// r in |z| table entries zi0 .. zi0+span-1 exceeds the threshold".  Each thread takes one (entry,
 // sign) of one candidate, reads that cell from the plane just written and applies the peak rule.
 // If the candidate buffer overflowed, the whole plane is scanned instead (same result).
 template <typename PT, typename VT, int NE>
 __global__ void __launch_bounds__(256)
 fdas_resolve_kernel(const PT *__restrict__ P, int K, long long M, float thr, const fdas_peak_t *__restrict__ cand,
-                    const int *__restrict__ cand_count, int cand_capacity, const int2 *__restrict__ ktab, int nzg,
-                    fdas_peak_t *peaks, int capacity, int *count)
+                    const int *__restrict__ cand_count, int cand_capacity, int span, const int2 *__restrict__ ktab,
+                    int nzg, fdas_peak_t *peaks, int capacity, int *count)
 {
     const int n = *cand_count;
     const long long stride = (long long)gridDim.x * blockDim.x;
     const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (n <= cand_capacity) {
-        for (long long i = tid; i < 16LL * n; i += stride) {
-            const fdas_peak_t c = cand[i >> 4];
-            const int zi = c.z_index + (int)((i & 15) >> 1);
+        const int cells = 2 * span;
+        for (long long i = tid; i < (long long)cells * n; i += stride) {
+            const fdas_peak_t c = cand[i / cells];
+            const int zi = c.z_index + (int)((i % cells) >> 1);
             if (zi >= (c.z_index / nzg + 1) * nzg) continue;      // past the end of this template group
             const int2 kk = ktab[zi];
             const int k = (i & 1) ? kk.y : kk.x;
@@ -111,7 +112,7 @@ int fdas_launch_resolve(fdas_plan *p, const void *plane, const fdas_search_args 
 {
     const int grid = p->num_sms * 2;
     fdas_resolve_kernel<float, float4, 4><<<grid, 256, 0, st>>>((const float *)plane, p->K, p->M, sa.thr, sa.cand,
-                                                               sa.cand_count, sa.cand_capacity, p->tc_ktab, p->tc_nzg,
+                                                               sa.cand_count, sa.cand_capacity, sa.cand_span, p->tc_ktab, p->tc_nzg,
                                                                peaks, capacity, sa.count_out);
     FDAS_CUDA_TRY(p, cudaGetLastError());
     p->launches += 1;

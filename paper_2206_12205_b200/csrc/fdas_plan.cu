@@ -93,17 +93,21 @@ extern "C" int fdas_plan_create(fdas_plan_t **out, int64_t N, double zmax, doubl
 extern "C" int fdas_set_algorithm(fdas_plan_t *p, int algorithm)
 {
     if (!p) return FDAS_ERR_INVALID_ARG;
-    if (algorithm != FDAS_ALGO_AUTO && algorithm != FDAS_ALGO_FFT && algorithm != FDAS_ALGO_MMA)
+    if (algorithm != FDAS_ALGO_AUTO && algorithm != FDAS_ALGO_FFT && algorithm != FDAS_ALGO_MMA &&
+        algorithm != FDAS_ALGO_MMA_SCALAR)
         return FDAS_ERR_INVALID_ARG;
-    if (algorithm == FDAS_ALGO_MMA && !(p->precision == FDAS_BF16 && p->tc_supported)) return FDAS_ERR_UNSUPPORTED;
-    p->algo = algorithm;
+    const bool mma = algorithm == FDAS_ALGO_MMA || algorithm == FDAS_ALGO_MMA_SCALAR;
+    if (mma && !(p->precision == FDAS_BF16 && p->tc_supported)) return FDAS_ERR_UNSUPPORTED;
+    p->algo = mma ? FDAS_ALGO_MMA : algorithm;
+    p->tc_force_scalar_stores = algorithm == FDAS_ALGO_MMA_SCALAR;
     return FDAS_OK;
 }
 
 extern "C" int fdas_get_algorithm(const fdas_plan_t *p, int *algorithm)
 {
     if (!p || !algorithm) return FDAS_ERR_INVALID_ARG;
-    *algorithm = fdas_uses_mma(p) ? FDAS_ALGO_MMA : FDAS_ALGO_FFT;
+    *algorithm = fdas_uses_mma(p) ? ((p->tc_force_scalar_stores || p->M % 4 != 0) ? FDAS_ALGO_MMA_SCALAR : FDAS_ALGO_MMA)
+                                  : FDAS_ALGO_FFT;
     return FDAS_OK;
 }
 
@@ -198,8 +202,9 @@ static int search_on_device(fdas_plan *p, const void *spectrum_dev, void *plane_
     sa.cand_count_next = p->cand_ctr + ((p->search_calls + 1) & 1);
     sa.cand_capacity = p->cand_capacity;
     sa.count_out = count_dev;
+    sa.cand_span = 8;   // overwritten by the convolve launch
     p->search_calls += 1;
-    int rc = fdas_launch_convolve_mma(p, spectrum_dev, plane_dev, 1, st, &sa);
+    int rc = fdas_launch_convolve_mma(p, spectrum_dev, plane_dev, 1, st, &sa);   // sets sa.cand_span
     if (rc) return rc;
     return fdas_launch_resolve(p, plane_dev, sa, peaks_dev, capacity, st);
 }
@@ -329,7 +334,7 @@ extern "C" int fdas_tapmatrix_host(const fdas_plan_t *p, void *dst_host, size_t 
     FDAS_CUDA_TRY(q, cudaDeviceSynchronize());
     FDAS_CUDA_TRY(q, cudaMemcpy(img.data(), p->tc_bmat, p->tc_bmat_bytes, cudaMemcpyDeviceToHost));
     FDAS_CUDA_TRY(q, cudaMemcpy(tab.data(), p->tc_ktab, n_tab * sizeof(int2), cudaMemcpyDeviceToHost));
-    // image [g][q][n][e] (kappa = 8 q + e, j = m_max - kappa; n = 2 zi + {re, im} of h_{+|z|})
+    // image [g][q][n][e] (kappa = 8 q + e, j = m_max - kappa; column n of (zi, re | im): fdas_tc_column_of_entry)
     // -> natural [K][2 m_max + 1][re, im] with the conjugate for the -|z| rows
     uint16_t *dst = (uint16_t *)dst_host;
     for (int g = 0; g < p->tc_groups; ++g)
@@ -337,8 +342,9 @@ extern "C" int fdas_tapmatrix_host(const fdas_plan_t *p, void *dst_host, size_t 
             const int2 kk = tab[(size_t)g * p->tc_nzg + zi];
             for (int j = -p->m_max; j <= p->m_max; ++j) {
                 const int kappa = p->m_max - j;
-                const size_t base = (((size_t)g * 2 * p->tc_KS + kappa / 8) * p->tc_NT + 2 * zi) * 8 + kappa % 8;
-                const uint16_t re = img[base], im = img[base + 8];
+                const size_t chunk = ((size_t)g * 2 * p->tc_KS + kappa / 8) * p->tc_NT;
+                const uint16_t re = img[(chunk + fdas_tc_column_of_entry(zi, 0)) * 8 + kappa % 8];
+                const uint16_t im = img[(chunk + fdas_tc_column_of_entry(zi, 1)) * 8 + kappa % 8];
                 if (kk.x >= 0) {
                     dst[((size_t)kk.x * ntap + (j + p->m_max)) * 2 + 0] = re;
                     dst[((size_t)kk.x * ntap + (j + p->m_max)) * 2 + 1] = im;

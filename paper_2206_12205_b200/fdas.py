@@ -16,8 +16,9 @@ LIB_PATH = os.environ.get("FDAS_LIBRARY", os.path.join(_HERE, "libfdas.so"))   #
 FDAS_F64, FDAS_F32, FDAS_BF16 = 0, 1, 2
 FDAS_OK, FDAS_ERR_INVALID_ARG, FDAS_ERR_ALLOC, FDAS_ERR_CUDA, FDAS_ERR_NOT_BUILT, FDAS_ERR_UNSUPPORTED = range(6)
 PRECISIONS = {"f64": FDAS_F64, "f32": FDAS_F32, "bf16": FDAS_BF16}
-FDAS_ALGO_AUTO, FDAS_ALGO_FFT, FDAS_ALGO_MMA = 0, 1, 2
-ALGORITHMS = {"auto": FDAS_ALGO_AUTO, "fft": FDAS_ALGO_FFT, "mma": FDAS_ALGO_MMA}
+FDAS_ALGO_AUTO, FDAS_ALGO_FFT, FDAS_ALGO_MMA, FDAS_ALGO_MMA_SCALAR = 0, 1, 2, 3
+ALGORITHMS = {"auto": FDAS_ALGO_AUTO, "fft": FDAS_ALGO_FFT, "mma": FDAS_ALGO_MMA,
+              "mma_scalar": FDAS_ALGO_MMA_SCALAR}
 
 EXPORTS = [
     "fdas_plan_create", "fdas_plan_destroy", "fdas_plan_info", "fdas_z_of_index",
@@ -335,7 +336,7 @@ class Plan:
     def algorithm(self) -> str:
         rc, a = fdas_get_algorithm(self._h)
         self._check(rc, "fdas_get_algorithm")
-        return {FDAS_ALGO_FFT: "fft", FDAS_ALGO_MMA: "mma"}[a]
+        return {FDAS_ALGO_FFT: "fft", FDAS_ALGO_MMA: "mma", FDAS_ALGO_MMA_SCALAR: "mma_scalar"}[a]
 
     def launch_count(self) -> int:
         return fdas_launch_count(self._h)[1]

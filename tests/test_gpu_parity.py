@@ -386,14 +386,26 @@ def test_mma_config1_element_by_element(F):
     (2 * 1501, 8.0, 2.0, 256),         # tiny: a few tiles, last one ragged
     (2 * 33000, 7.5, 2.5, 1024),       # fractional z step
     (2 * 4099, 96.0, 2.0, 2048),       # bench bank on a short, odd spectrum
+    # M % 4 == 0: the bulk-copy kernel (staged 512-byte row segments), ragged last tile
+    (2 * 5004, 5.0, 2.0, 1024),        # asymmetric grid, every entry has one plane row only
+    (2 * 70004, 200.0, 2.0, 4096),     # two template groups, 15 K-steps
+    (2 * 1500, 8.0, 2.0, 256),         # tiny
+    (2 * 4100, 96.0, 2.0, 2048),       # bench bank, last tile of 4 bins
+    (2 * 16384, 30.0, 2.0, 512),       # M a multiple of the tile; few |z| entries (empty column groups)
 ])
 def test_mma_ragged_odd_and_grouped(F, N, zmax, dz, S):
+    import torch
     w = workloads.noise_only(N, seed=S + 11, zmax=zmax, dz=dz, seglen=S)
     plan, P = gpu_plane(F, w, "bf16", algorithm="mma")
+    assert plan.algorithm() == ("mma" if (N // 2) % 4 == 0 else "mma_scalar")
     got = P.cpu().numpy()
     exp = bf16_input_plane(w)
     assert got.shape == exp.shape
     check_mma(got, exp)
+    # the two store paths of the tensor-core kernel hold the same bits
+    plans, Ps = gpu_plane(F, w, "bf16", algorithm="mma_scalar")
+    assert plans.algorithm() == "mma_scalar"
+    assert torch.equal(P, Ps)
     # and the FFT form of the bf16 variant obeys the bf16 rule on the same input
     _, Pfft = gpu_plane(F, w, "bf16", algorithm="fft")
     _, Pf = gpu_plane(F, w, "f32")
