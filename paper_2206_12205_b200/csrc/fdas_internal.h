@@ -31,6 +31,11 @@ struct fdas_plan {
     size_t tc_bmat_bytes;
     int2 *tc_ktab;     // [groups][nzg] plane rows of (+|z|, -|z|), -1 where absent
     int2 *tc_kref;     // [groups][nzg] (template whose taps fill the columns, its sign)
+    int4 *tc_ranges;   // [groups][4] plane-row runs of the bulk kernel's staging rows
+    int tc_bulk_ok;    // those runs are contiguous (always, for the grids fdas_plan_create builds)
+    void *tc_maps;     // host: cached tensor maps of the last plane buffer (fdas_mma.cu)
+    const void *tc_maps_plane;
+    int tc_maps_batch;
     // fused search (fdas_search): coarse candidates flagged by the convolve epilogue
     fdas_peak_t *cand;     // [cand_capacity] (z_index = first |z| table entry of the chunk, r, chunk maximum)
     int *cand_ctr;         // two counters used alternately: call n appends to [n & 1] and clears [(n + 1) & 1]

@@ -43,6 +43,7 @@
 // fdas_mma_convolve_kernel (any M: bulk copies need 16-byte aligned rows)
 //   warps 0-7   epilogue: tcgen05.ld -> |.|^2 -> st.global.cs (TMEM double-buffered)
 //   warp  8     MMA issuer;  warps 9-12 loader
+#include <cuda.h>        // CUtensorMap (types only; the encoder is fetched through cudaGetDriverEntryPoint)
 #include <cuda_bf16.h>
 #include <math.h>
 #include <stdlib.h>
@@ -66,6 +67,7 @@ struct TcParams {
     float *planes;           // [batch][K][M]
     const uint4 *bmat;       // [groups][2 KS][NT] rows of 8 bf16 (the shared-memory image)
     const int2 *ktab;        // [groups][nzg]: plane rows of (+|z|, -|z|), -1 where absent
+    const int4 *ranges;      // bulk kernel: [groups][4 column groups] (row0_n, cnt_n, row0_p, cnt_p), see fdas_mma_plan
     long long M;
     int K, batch;
     int R;                   // outputs per work item (multiple of 128)
@@ -214,7 +216,11 @@ __device__ __forceinline__ void st_cs_at(const float *base, uint32_t off, float 
 {
     unsigned long long addr;
     asm("mad.wide.u32 %0, %1, 4, %2;" : "=l"(addr) : "r"(off), "l"(base));
+#ifdef FDAS_MMA_ST_DEFAULT
+    asm volatile("st.global.f32 [%0], %1;" ::"l"(addr), "f"(v) : "memory");
+#else
     asm volatile("st.global.cs.f32 [%0], %1;" ::"l"(addr), "f"(v) : "memory");
+#endif
 }
 
 constexpr uint32_t TC_NO_ROW = 0xFFFFFFFFu;   // row-offset table: this |z| has no such plane row
@@ -315,8 +321,112 @@ __device__ __forceinline__ void epilogue_tile(uint32_t taddr, const uint4 *otab4
     }
 }
 
+// One lane of a converged warp (elect.sync), as a predicate value
+__device__ __forceinline__ uint32_t elect_one()
+{
+    uint32_t pred;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "elect.sync _|p, 0xffffffff;\n\t"
+        "selp.b32 %0, 1, 0, p;\n\t}"
+        : "=r"(pred));
+    return pred;
+}
+// umma_bf16 issued by the elected lane only; every lane of the warp executes the surrounding code,
+// so the descriptors stay in uniform registers and MMAs issue back to back
+__device__ __forceinline__ void umma_bf16_elected(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc,
+                                                  uint32_t accumulate, uint32_t elected)
+{
+    asm volatile(
+        "{\n\t.reg .pred p, q;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "setp.ne.b32 q, %5, 0;\n\t"
+        "@q tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+        ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate), "r"(elected)
+        : "memory");
+}
+__device__ __forceinline__ void umma_commit_elected(uint32_t bar, uint32_t elected)
+{
+    asm volatile(
+        "{\n\t.reg .pred q;\n\t"
+        "setp.ne.b32 q, %1, 0;\n\t"
+        "@q tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n\t}"
+        ::"r"(bar), "r"(elected)
+        : "memory");
+}
+
+// The MMA warp of both kernels.  Per tile 2 KS MMAs (K steps outermost, so consecutive MMAs
+// alternate between the re and im accumulators), then a commit that signals the epilogue.
+template <int NT>
+__device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, uint32_t off_z, uint32_t z_buf_bytes,
+                                           uint32_t z_part_bytes, uint32_t z_full, uint32_t z_empty, uint32_t t_full,
+                                           uint32_t t_empty, uint32_t tmem_base, long long n_items)
+{
+    // instruction descriptor (cute::UMMA::InstrDescriptor): fp32 accumulate, bf16 A and B, both K-major,
+    // N = NT, M = 128
+    constexpr uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(NT >> 3) << 17) |
+                               ((uint32_t)(TC_TILE >> 4) << 24);
+    constexpr uint32_t b_lbo = (uint32_t)NT * 16u;   // next 8-tap chunk of the tap matrix
+    const uint32_t elected = elect_one();
+    const uint64_t b_desc0 = smem_desc(s_base, b_lbo, 128u);
+    uint32_t n = 0, t = 0;
+    for (long long it = blockIdx.x; it < n_items; it += gridDim.x, ++n) {
+        const uint32_t buf = n & 1, zuse = n >> 1;
+        const long long blk0 = (it % p.n_blocks) * p.R;
+        const long long left = p.M - blk0;
+        const int n_tiles = (int)((left < p.R ? left : p.R) + TC_TILE - 1) / TC_TILE;
+        mbar_wait(z_full + 8 * buf, zuse & 1);
+        tc_fence_after();
+        const uint32_t z_addr = s_base + off_z + buf * z_buf_bytes;
+        for (int tile = 0; tile < n_tiles; ++tile, ++t) {
+            const uint32_t stage = t & 1, use = t >> 1;
+            mbar_wait(t_empty + 8 * stage, (use & 1) ^ 1);
+            tc_fence_after();
+            const uint32_t d_re = tmem_base + stage * TC_STAGE_COLS, d_im = d_re + NT;
+            // descriptors advance by adding to their 14-bit address field (units of 16 bytes; shared
+            // memory is < 256 KB, so no carry leaves the field)
+            uint64_t a_re = smem_desc(z_addr + (uint32_t)(tile * TC_TILE) * 16u, 128u, 128u);
+            uint64_t a_im = smem_desc(z_addr + z_part_bytes + (uint32_t)(tile * TC_TILE) * 16u, 128u, 128u);
+            uint64_t bd = b_desc0;
+#pragma unroll 3
+            for (int ks = 0; ks < p.KS; ++ks) {
+                umma_bf16_elected(d_re, a_re, bd, idesc, ks > 0, elected);
+                umma_bf16_elected(d_im, a_im, bd, idesc, ks > 0, elected);
+                a_re += 256u >> 4;
+                a_im += 256u >> 4;
+                bd += (2u * b_lbo) >> 4;
+            }
+            umma_commit_elected(t_full + 8 * stage, elected);
+        }
+        umma_commit_elected(z_empty + 8 * buf, elected);
+    }
+}
+
 // The loader warps of both kernels: per work item, the spectrum block -> bf16 (round to nearest
-// even, reading A12) -> the Z rows (file header) of buffer n & 1.
+// even, reading A12) -> the Z rows (file header) of buffer n & 1.  The global loads of
+// item n+1 are issued before the wait for buffer n and stay in registers across it, so that
+// their latency hides behind the tensor core working on the previous items.
+constexpr int TC_LD_ITERS = 6;   // sample pairs per loader thread: (R + 16 KS) / 2 / 128 <= (1024 + 512) / 256
+
+__device__ __forceinline__ void loader_fetch(const TcParams &p, long long it, uint32_t xn, int lt, float2 (&a)[TC_LD_ITERS],
+                                             float2 (&b)[TC_LD_ITERS])
+{
+    const long long ser = it / p.n_blocks;
+    const long long g0 = (it % p.n_blocks) * p.R - p.M0;   // sample index of xs[0]
+    const float2 *__restrict__ X = p.spectra + (size_t)ser * p.M;
+#pragma unroll
+    for (int i = 0; i < TC_LD_ITERS; ++i) {
+        const uint32_t pi = lt + i * TC_LOAD_THREADS;
+        const long long g = g0 + 2 * (long long)pi;
+        a[i] = make_float2(0.f, 0.f);
+        b[i] = make_float2(0.f, 0.f);
+        if (pi < xn / 2) {
+            if (g >= 0 && g < p.M) a[i] = __ldg(X + g);
+            if (g + 1 >= 0 && g + 1 < p.M) b[i] = __ldg(X + g + 1);
+        }
+    }
+}
+
 __device__ __forceinline__ void spectrum_loader(const TcParams &p, unsigned char *smem, uint32_t off_xs,
                                                 uint32_t xs_part_bytes, uint32_t xn, uint32_t off_z, uint32_t z_buf_bytes,
                                                 uint32_t z_part_bytes, uint32_t zr, uint32_t z_full, uint32_t z_empty,
@@ -324,22 +434,22 @@ __device__ __forceinline__ void spectrum_loader(const TcParams &p, unsigned char
 {
     uint32_t *xs_re = reinterpret_cast<uint32_t *>(smem + off_xs);
     uint32_t *xs_im = reinterpret_cast<uint32_t *>(smem + off_xs + xs_part_bytes);
+    float2 a[TC_LD_ITERS], b[TC_LD_ITERS];
     uint32_t n = 0;
+    if ((long long)blockIdx.x < n_items) loader_fetch(p, blockIdx.x, xn, lt, a, b);
     for (long long it = blockIdx.x; it < n_items; it += gridDim.x, ++n) {
         const uint32_t buf = n & 1, zuse = n >> 1;
-        const long long ser = it / p.n_blocks;
-        const long long g0 = (it % p.n_blocks) * p.R - p.M0;   // sample index of xs[0]
-        const float2 *__restrict__ X = p.spectra + (size_t)ser * p.M;
         // phase A: spectrum block -> bf16 (round-to-nearest-even), re and im planes
-        for (uint32_t pi = lt; pi < xn / 2; pi += TC_LOAD_THREADS) {
-            const long long g = g0 + 2 * (long long)pi;
-            float2 a = make_float2(0.f, 0.f), b = make_float2(0.f, 0.f);
-            if (g >= 0 && g < p.M) a = __ldg(X + g);
-            if (g + 1 >= 0 && g + 1 < p.M) b = __ldg(X + g + 1);
-            xs_re[pi] = pack_bf16(a.x, b.x);
-            xs_im[pi] = pack_bf16(a.y, b.y);
+#pragma unroll
+        for (int i = 0; i < TC_LD_ITERS; ++i) {
+            const uint32_t pi = lt + i * TC_LOAD_THREADS;
+            if (pi < xn / 2) {
+                xs_re[pi] = pack_bf16(a[i].x, b[i].x);
+                xs_im[pi] = pack_bf16(a[i].y, b[i].y);
+            }
         }
         named_bar_sync(1, TC_LOAD_THREADS);
+        if (it + gridDim.x < n_items) loader_fetch(p, it + gridDim.x, xn, lt, a, b);
         mbar_wait<64>(z_empty + 8 * buf, (zuse & 1) ^ 1);
         // phase B: Z row i = samples i .. i+7 (16 bytes), for both parts
         unsigned char *zb = smem + off_z + buf * z_buf_bytes;
@@ -447,44 +557,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1) fdas_mma_convolve_kernel(const 
         }
     } else if (warp == TC_MMA_WARP) {
         // =========================== MMA issuer ===========================
-        if (lane == 0) {
-            // instruction descriptor (cute::UMMA::InstrDescriptor): fp32 accumulate, bf16 A and B,
-            // both K-major, N = NT, M = 128
-            const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(NT >> 3) << 17) |
-                                   ((uint32_t)(TC_TILE >> 4) << 24);
-            const uint32_t b_addr = s_base;
-            const uint32_t b_lbo = (uint32_t)NT * 16u;   // next 8-tap chunk of the tap matrix
-            uint32_t n = 0, t = 0;
-            for (long long it = blockIdx.x; it < n_items; it += gridDim.x, ++n) {
-                const uint32_t buf = n & 1, zuse = n >> 1;
-                const long long blk0 = (it % p.n_blocks) * p.R;
-                const long long left = p.M - blk0;
-                const int n_tiles = (int)((left < p.R ? left : p.R) + TC_TILE - 1) / TC_TILE;
-                mbar_wait(z_full + 8 * buf, zuse & 1);
-                tc_fence_after();
-                const uint32_t z_addr = s_base + L.off_z + buf * L.z_buf_bytes;
-                for (int tile = 0; tile < n_tiles; ++tile, ++t) {
-                    const uint32_t stage = t & 1, use = t >> 1;
-                    mbar_wait(t_empty + 8 * stage, (use & 1) ^ 1);
-                    tc_fence_after();
-                    for (int part = 0; part < 2; ++part) {
-                        const uint32_t d = tmem_base + stage * TC_STAGE_COLS + part * NT;
-                        const uint32_t a0 = z_addr + part * L.z_part_bytes + (uint32_t)(tile * TC_TILE) * 16u;
-                        for (int ks = 0; ks < p.KS; ++ks) {
-                            const uint64_t ad = smem_desc(a0 + ks * 256u, 128u, 128u);
-                            const uint64_t bd = smem_desc(b_addr + ks * 2u * b_lbo, b_lbo, 128u);
-#ifndef FDAS_MMA_DEBUG_NOMMA
-                            umma_bf16(d, ad, bd, idesc, ks > 0);
-#else
-                            (void)ad; (void)bd; (void)d;
-#endif
-                        }
-                    }
-                    umma_commit(t_full + 8 * stage);
-                }
-                umma_commit(z_empty + 8 * buf);
-            }
-        }
+        mma_issuer<NT>(p, s_base, L.off_z, L.z_buf_bytes, L.z_part_bytes, z_full, z_empty, t_full, t_empty,
+                       __shfl_sync(0xffffffffu, tmem_base, 0), n_items);
     } else {
         // =========================== loader ===========================
         spectrum_loader(p, smem, L.off_xs, L.xs_part_bytes, L.xn, L.off_z, L.z_buf_bytes, L.z_part_bytes, L.zr, z_full,
@@ -509,13 +583,16 @@ constexpr int TB_MMA_WARP = 16;
 constexpr int TB_LOAD_WARP0 = 17;
 constexpr int TB_THREADS = 32 * (TB_EPI_WARPS + 1 + TC_LOAD_WARPS);   // 672
 constexpr int TB_CGROUPS = 4;           // column groups: NCH entry pairs (4 NCH columns per part) each
-constexpr int TB_MAX_SLOTS = 32;        // staging rows per column group = 4 NCH <= 32
+constexpr int TB_BOXES = 4;             // tensor maps with box heights 8, 4, 2, 1 rows
+struct TbMaps {
+    CUtensorMap m[TB_BOXES];            // the planes as a [batch*K][M] fp32 matrix, box = (8 >> i) rows x 128 bins
+};
 
 // shared-memory carve-up of the bulk kernel.  ROWB = bytes of one staging row (one plane row
 // segment pushed out by one bulk copy): 128 bins x 4 B.
 struct TbSmem {
     uint32_t b_bytes, zr, z_part_bytes, z_buf_bytes, xn, xs_part_bytes, slots, stage_cg_bytes;
-    uint32_t off_z, off_xs, off_stage, off_rowtab, off_bars, off_holder, total;
+    uint32_t off_z, off_xs, off_stage, off_bars, off_holder, total;
     __host__ __device__ TbSmem(int R, int KS, int NT, int rowb)
     {
         const uint32_t TP = 16u * KS;
@@ -530,8 +607,7 @@ struct TbSmem {
         off_z = b_bytes;
         off_xs = off_z + 2u * z_buf_bytes;
         off_stage = (off_xs + 2u * xs_part_bytes + 127u) & ~127u;
-        off_rowtab = off_stage + 2u * TB_CGROUPS * stage_cg_bytes;
-        off_bars = (off_rowtab + 4u * TB_CGROUPS * TB_MAX_SLOTS + 15u) & ~15u;
+        off_bars = (off_stage + 2u * TB_CGROUPS * stage_cg_bytes + 15u) & ~15u;
         off_holder = off_bars + 8u * 8u;
         total = off_holder + 16u;
     }
@@ -609,17 +685,33 @@ __device__ __forceinline__ unsigned long long f2_fma(unsigned long long a, unsig
     return r;
 }
 
-__device__ __forceinline__ void bulk_store(void *gdst, uint32_t ssrc, uint32_t bytes)
+// smem box [h][128] floats (dense rows) -> plane rows row..row+h-1, bins col..col+127 (clipped at M)
+__device__ __forceinline__ void tensor_store(const CUtensorMap *map, uint32_t ssrc, int col, int row)
 {
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(ssrc), "r"(bytes)
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];" ::"l"(map), "r"(col),
+                 "r"(row), "r"(ssrc)
                  : "memory");
-    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
 }
+// a run of cnt staging rows starting at shared address ssrc -> plane rows row.. as boxes of 8, 4, 2, 1 rows
+__device__ __forceinline__ void store_rows(const TbMaps &maps, uint32_t ssrc, int col, int row, int cnt, uint32_t rowb)
+{
+    int done = 0;
+#pragma unroll
+    for (int b = 0; b < TB_BOXES; ++b) {
+        const int h = 8 >> b;
+        while (cnt - done >= h) {
+            tensor_store(&maps.m[b], ssrc + (uint32_t)done * rowb, col, row + done);
+            done += h;
+        }
+    }
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_read_all() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 
 template <int NCH>
-__global__ void __launch_bounds__(TB_THREADS, 1) fdas_mma_bulk_kernel(const TcParams p)
+__global__ void __launch_bounds__(TB_THREADS, 1)
+fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int NT = 16 * NCH;
@@ -634,24 +726,12 @@ __global__ void __launch_bounds__(TB_THREADS, 1) fdas_mma_bulk_kernel(const TcPa
     const uint32_t bars = s_base + L.off_bars;
     const uint32_t z_full = bars, z_empty = bars + 16, t_full = bars + 32, t_empty = bars + 48;
     uint32_t *holder = reinterpret_cast<uint32_t *>(smem + L.off_holder);
-    int *rowtab = reinterpret_cast<int *>(smem + L.off_rowtab);   // [TB_CGROUPS][TB_MAX_SLOTS] plane row or -1
 
-    // ---- one-time setup: tap matrix image and staging-row table -> shared memory, barriers, TMEM
+    // ---- one-time setup: tap matrix image -> shared memory, barriers, TMEM
     {
         const uint4 *src = p.bmat + (size_t)grp * (L.b_bytes / 16);
         uint4 *dst = reinterpret_cast<uint4 *>(smem);
         for (uint32_t i = threadIdx.x; i < L.b_bytes / 16; i += TB_THREADS) dst[i] = __ldg(src + i);
-        // slot 4 pr + 2 s + sign of column group cg <-> |z| entry 2 (cg NCH + pr) + s, sign: 0 = +|z|, 1 = -|z|
-        for (int i = threadIdx.x; i < TB_CGROUPS * TB_MAX_SLOTS; i += TB_THREADS) {
-            const int cg = i / TB_MAX_SLOTS, slot = i % TB_MAX_SLOTS;
-            const int el = 2 * (cg * NCH + (slot >> 2)) + ((slot >> 1) & 1);
-            int row = -1;
-            if (slot < NC && el < p.nzg) {
-                const int2 kk = p.ktab[(size_t)grp * p.nzg + el];
-                row = (slot & 1) ? (kk.y == kk.x ? -1 : kk.y) : kk.x;   // z = 0 names its row twice
-            }
-            rowtab[i] = row;
-        }
         fence_proxy_async();
     }
     if (threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0 && p.search.enabled) {
@@ -663,7 +743,7 @@ __global__ void __launch_bounds__(TB_THREADS, 1) fdas_mma_bulk_kernel(const TcPa
             mbar_init(z_full + 8 * s, TC_LOAD_THREADS);
             mbar_init(z_empty + 8 * s, 1);
             mbar_init(t_full + 8 * s, 1);
-            mbar_init(t_empty + 8 * s, TB_EPI_WARPS);
+            mbar_init(t_empty + 8 * s, TB_EPI_WARPS / 2);   // the warp set that owns stage s
         }
         fence_barrier_init();
     }
@@ -675,15 +755,19 @@ __global__ void __launch_bounds__(TB_THREADS, 1) fdas_mma_bulk_kernel(const TcPa
 
     if (warp < TB_EPI_WARPS) {
         // =========================== epilogue ===========================
-        const int q = warp & 3, cg = warp >> 2;
+        // Two warp sets take alternate tiles (set = TMEM stage), so that one set's chain
+        // TMEM load -> powers -> staging -> fence -> barrier -> store issue overlaps the other's.
+        // Inside a set, warp (q, half) owns TMEM lane quarter q and column groups 2 half, 2 half + 1.
+        const int q = warp & 3, half = (warp >> 2) & 1, set = warp >> 3;
         const int lt = q * 32 + lane;                       // bin inside the tile = TMEM lane
         const float thr = p.search.enabled ? p.search.thr : __int_as_float(0x7f800000);
-        const int zi_cg0 = grp * p.nzg + 2 * cg * NCH;      // first |z| table entry of this column group
-        // staging row (slot) this thread pushes out: the NC slots are dealt round-robin to the four
-        // warps of the column group (a warp issues its bulk copies one lane at a time)
-        const int my_slot = 4 * lane + q;
-        const int my_row = my_slot < NC ? rowtab[cg * TB_MAX_SLOTS + my_slot] : -1;
-        unsigned char *const stage_cg = smem + L.off_stage + (size_t)cg * 2 * L.stage_cg_bytes;
+        // Staging rows of a column group (NC = 4 NCH rows of 128 bins): the -|z| rows of its entries
+        // el = 0, 1, .. in rows el, the +|z| rows in rows NC-1-el, so that each block is a run of
+        // consecutive plane rows in ascending order (ranges[]: row0_n, cnt_n / row0_p, cnt_p) and
+        // leaves as a few tensor-map boxes issued by one thread of the four warps sharing it.
+        const bool issuer = q == 0 && lane == 0;
+        const int bar_id = 2 + 2 * set + half;              // the 128 threads (set, half)
+        const uint32_t stage = set;
         uint32_t t = 0;
         for (long long it = blockIdx.x; it < n_items; it += gridDim.x) {
             const long long ser = it / p.n_blocks;
@@ -691,90 +775,78 @@ __global__ void __launch_bounds__(TB_THREADS, 1) fdas_mma_bulk_kernel(const TcPa
             const long long left = p.M - blk0;
             const int n_tiles = (int)((left < p.R ? left : p.R) + TC_TILE - 1) / TC_TILE;
             for (int tile = 0; tile < n_tiles; ++tile, ++t) {
-                const uint32_t stage = t & 1, use = t >> 1;
+                if ((t & 1) != stage) continue;
+                const uint32_t use = t >> 1;
                 const long long col0 = blk0 + tile * TC_TILE;
-                const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + stage * TC_STAGE_COLS + cg * NC;
-                uint32_t v[2 * NC];
+                const uint32_t taddr0 = tmem_base + ((uint32_t)(q * 32) << 16) + stage * TC_STAGE_COLS;
+                // this set's staging buffers last fed the stores of tile t-2: their shared-memory reads are over
+                if (issuer) bulk_wait_read_all();
                 mbar_wait(t_full + 8 * stage, use & 1);
                 tc_fence_after();
-                tmem_ld_cols<NC>(taddr, v);
-                tmem_ld_cols<NC>(taddr + NT, v + NC);
-                tmem_ld_fence<2 * NC>(v);
+                named_bar_sync(bar_id, 128);
+#ifdef FDAS_MMA_DEBUG_NOEPI
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(t_empty + 8 * stage);
-                // staging buffer `stage` of this column group was handed to the bulk copies two tiles
-                // ago; the thread that issued them waited for their shared-memory reads before the
-                // previous tile's barrier, so it is free
-                float *const sb = reinterpret_cast<float *>(stage_cg + stage * L.stage_cg_bytes) + lt;
-                float mx = 0.f;
+                continue;
+#endif
 #pragma unroll
-                for (int pr = 0; pr < NCH; ++pr) {
-                    const unsigned long long ure = f2_pack(v[4 * pr], v[4 * pr + 1]), vre = f2_pack(v[4 * pr + 2], v[4 * pr + 3]);
-                    const unsigned long long uim = f2_pack(v[NC + 4 * pr], v[NC + 4 * pr + 1]);
-                    const unsigned long long vim = f2_pack(v[NC + 4 * pr + 2], v[NC + 4 * pr + 3]);
-                    const unsigned long long a = f2_sub(ure, vim), b = f2_add(uim, vre);
-                    const unsigned long long c = f2_add(ure, vim), d = f2_sub(uim, vre);
-                    const unsigned long long pp = f2_fma(b, b, f2_mul(a, a)), pm = f2_fma(d, d, f2_mul(c, c));
-                    float pp0, pp1, pm0, pm1;
-                    f2_unpack(pp, pp0, pp1);
-                    f2_unpack(pm, pm0, pm1);
-                    sb[(4 * pr + 0) * TC_TILE] = pp0;
-                    sb[(4 * pr + 1) * TC_TILE] = pm0;
-                    sb[(4 * pr + 2) * TC_TILE] = pp1;
-                    sb[(4 * pr + 3) * TC_TILE] = pm1;
-                    // padded columns give exactly zero; a sign whose row is not in the plane (asymmetric
-                    // grids) can only add a candidate, which the resolve kernel then rejects
-                    mx = fmaxf(mx, fmaxf(fmaxf(pp0, pm0), fmaxf(pp1, pm1)));
+                for (int pass = 0; pass < 2; ++pass) {
+                    const int cg = 2 * half + pass;
+                    const int4 rg = p.ranges[grp * TB_CGROUPS + cg];
+                    uint32_t v[2 * NC];
+                    tmem_ld_cols<NC>(taddr0 + cg * NC, v);
+                    tmem_ld_cols<NC>(taddr0 + NT + cg * NC, v + NC);
+                    tmem_ld_fence<2 * NC>(v);
+                    if (pass == 1) {                        // both column groups are in registers: hand the stage back
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(t_empty + 8 * stage);
+                    }
+                    unsigned char *const stage_buf = smem + L.off_stage + (size_t)(2 * cg + stage) * L.stage_cg_bytes;
+                    float *const sb = reinterpret_cast<float *>(stage_buf) + lt;
+                    float mx = 0.f;
+#pragma unroll
+                    for (int pr = 0; pr < NCH; ++pr) {
+                        const unsigned long long ure = f2_pack(v[4 * pr], v[4 * pr + 1]), vre = f2_pack(v[4 * pr + 2], v[4 * pr + 3]);
+                        const unsigned long long uim = f2_pack(v[NC + 4 * pr], v[NC + 4 * pr + 1]);
+                        const unsigned long long vim = f2_pack(v[NC + 4 * pr + 2], v[NC + 4 * pr + 3]);
+                        const unsigned long long a = f2_sub(ure, vim), b = f2_add(uim, vre);
+                        const unsigned long long c = f2_add(ure, vim), d = f2_sub(uim, vre);
+                        const unsigned long long pp = f2_fma(b, b, f2_mul(a, a)), pm = f2_fma(d, d, f2_mul(c, c));
+                        float pp0, pp1, pm0, pm1;
+                        f2_unpack(pp, pp0, pp1);
+                        f2_unpack(pm, pm0, pm1);
+                        sb[(2 * pr) * TC_TILE] = pm0;
+                        sb[(2 * pr + 1) * TC_TILE] = pm1;
+                        sb[(NC - 1 - 2 * pr) * TC_TILE] = pp0;
+                        sb[(NC - 2 - 2 * pr) * TC_TILE] = pp1;
+                        // padded columns give exactly zero; a sign whose row is not in the plane (asymmetric
+                        // grids) can only add a candidate, which the resolve kernel then rejects
+                        mx = fmaxf(mx, fmaxf(fmaxf(pp0, pm0), fmaxf(pp1, pm1)));
+                    }
+                    fence_proxy_async();                    // staging writes -> visible to the bulk copy engine
+                    named_bar_sync(bar_id, 128);
+                    if (issuer) {
+                        const uint32_t sst = smem_u32(stage_buf);
+                        const int row_s = (int)ser * p.K;
+#ifndef FDAS_MMA_DEBUG_NOSTORE
+                        store_rows(maps, sst, (int)col0, row_s + rg.x, rg.y, ROWB);
+                        store_rows(maps, sst + (uint32_t)(NC - rg.w) * ROWB, (int)col0, row_s + rg.z, rg.w, ROWB);
+                        bulk_commit();
+#endif
+                    }
+                    if (mx > thr && col0 + lt < p.M && 2 * cg * NCH < p.nzg)
+                        flag_candidate(p.search.cand, p.search.cand_count, p.search.cand_capacity,
+                                       grp * p.nzg + 2 * cg * NCH, (int)(col0 + lt), mx);
                 }
-                if (my_row >= 0) bulk_wait_read_all();     // the other buffer's copies (previous tile) have read it
-                fence_proxy_async();                       // staging writes -> visible to the bulk copy engine
-                named_bar_sync(2 + cg, 128);
-                if (my_row >= 0) {
-                    const long long rest = p.M - col0;     // > 0
-                    const uint32_t bytes = rest >= TC_TILE ? ROWB : (uint32_t)rest * 4u;
-                    float *dst = p.planes + ((size_t)ser * p.K + my_row) * p.M + col0;
-                    bulk_store(dst, smem_u32(stage_cg + stage * L.stage_cg_bytes + (size_t)my_slot * ROWB), bytes);
-                }
-                if (mx > thr && col0 + lt < p.M && 2 * cg * NCH < p.nzg)
-                    flag_candidate(p.search.cand, p.search.cand_count, p.search.cand_capacity, zi_cg0, (int)(col0 + lt), mx);
             }
         }
-        if (my_row >= 0) bulk_wait_all();
+        if (issuer) bulk_wait_all();
     } else if (warp == TB_MMA_WARP) {
         // =========================== MMA issuer ===========================
-        if (lane == 0) {
-            const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(NT >> 3) << 17) |
-                                   ((uint32_t)(TC_TILE >> 4) << 24);
-            const uint32_t b_addr = s_base;
-            const uint32_t b_lbo = (uint32_t)NT * 16u;
-            uint32_t n = 0, t = 0;
-            for (long long it = blockIdx.x; it < n_items; it += gridDim.x, ++n) {
-                const uint32_t buf = n & 1, zuse = n >> 1;
-                const long long blk0 = (it % p.n_blocks) * p.R;
-                const long long left = p.M - blk0;
-                const int n_tiles = (int)((left < p.R ? left : p.R) + TC_TILE - 1) / TC_TILE;
-                mbar_wait(z_full + 8 * buf, zuse & 1);
-                tc_fence_after();
-                const uint32_t z_addr = s_base + L.off_z + buf * L.z_buf_bytes;
-                for (int tile = 0; tile < n_tiles; ++tile, ++t) {
-                    const uint32_t stage = t & 1, use = t >> 1;
-                    mbar_wait(t_empty + 8 * stage, (use & 1) ^ 1);
-                    tc_fence_after();
-                    for (int part = 0; part < 2; ++part) {
-                        const uint32_t d = tmem_base + stage * TC_STAGE_COLS + part * NT;
-                        const uint32_t a0 = z_addr + part * L.z_part_bytes + (uint32_t)(tile * TC_TILE) * 16u;
-                        for (int ks = 0; ks < p.KS; ++ks) {
-                            const uint64_t ad = smem_desc(a0 + ks * 256u, 128u, 128u);
-                            const uint64_t bd = smem_desc(b_addr + ks * 2u * b_lbo, b_lbo, 128u);
-                            umma_bf16(d, ad, bd, idesc, ks > 0);
-                        }
-                    }
-                    umma_commit(t_full + 8 * stage);
-                }
-                umma_commit(z_empty + 8 * buf);
-            }
-        }
+        mma_issuer<NT>(p, s_base, L.off_z, L.z_buf_bytes, L.z_part_bytes, z_full, z_empty, t_full, t_empty,
+                       __shfl_sync(0xffffffffu, tmem_base, 0), n_items);
     } else {
         // =========================== loader ===========================
         spectrum_loader(p, smem, L.off_xs, L.xs_part_bytes, L.xn, L.off_z, L.z_buf_bytes, L.z_part_bytes, L.zr, z_full,
@@ -856,9 +928,11 @@ int fdas_mma_plan(fdas_plan *p)
             tab[i] = make_int2(kp, kn);   // z = 0: both entries name the same row (equal values, V = 0)
             ref[i] = make_int2(kp, 1);
         } else {
-            const bool neg = (-p->zmax + (double)i * p->dz) < 0.0;
-            tab[i] = neg ? make_int2(-1, (int)i) : make_int2((int)i, -1);
-            ref[i] = make_int2((int)i, neg ? -1 : 1);
+            // no mirror pairs: every template is listed as the "-|z|" row of an entry whose columns
+            // hold conj(h_z) (the -|z| row conjugates them again), so that the rows of consecutive
+            // entries are consecutive plane rows
+            tab[i] = make_int2(-1, (int)i);
+            ref[i] = make_int2((int)i, -1);
         }
     }
     // leading 16-column chunks (8 |z| each) in which every entry has both plane rows, in every group
@@ -868,20 +942,56 @@ int fdas_mma_plan(fdas_plan *p)
         while (lead < nzg && tab[(size_t)g * nzg + lead].x >= 0 && tab[(size_t)g * nzg + lead].y >= 0) ++lead;
         if (lead / 8 < p->tc_full_chunks) p->tc_full_chunks = lead / 8;
     }
+    // bulk kernel (fdas_mma_bulk_kernel): per (group, column group of 2 NCH entries) the runs of
+    // consecutive plane rows its staging rows map to: -|z| rows of entries el = 0.. ascending,
+    // +|z| rows ascending with el descending; a mirror entry (z = 0) keeps its -|z| listing only.
+    const int EPC = NT / 8;   // entries per column group = 2 NCH
+    int4 *rng = (int4 *)malloc((size_t)groups * 4 * sizeof(int4));
+    if (!rng) {
+        free(tab);
+        free(ref);
+        return FDAS_ERR_ALLOC;
+    }
+    p->tc_bulk_ok = 1;
+    for (int g = 0; g < groups; ++g)
+        for (int cg = 0; cg < 4; ++cg) {
+            int4 r = make_int4(0, 0, 0, 0);
+            int x0 = -1;
+            for (int el = 0; el < EPC; ++el) {
+                const int e = cg * EPC + el;
+                const int2 t = e < nzg ? tab[(size_t)g * nzg + e] : make_int2(-1, -1);
+                if (t.y >= 0) {
+                    if (r.y == 0) r.x = t.y;
+                    if (el != r.y || t.y != r.x + r.y) p->tc_bulk_ok = 0;
+                    r.y += 1;
+                }
+                if (t.x >= 0 && t.x != t.y) {
+                    if (r.w == 0) x0 = t.x;
+                    if (el != r.w || t.x != x0 - r.w) p->tc_bulk_ok = 0;
+                    r.w += 1;
+                }
+            }
+            r.z = r.w > 0 ? x0 - (r.w - 1) : 0;
+            rng[g * 4 + cg] = r;
+        }
     p->tc_bmat_bytes = (size_t)groups * 2 * KS * NT * 16;
     cudaError_t e;
     if ((e = cudaMalloc(&p->tc_bmat, p->tc_bmat_bytes)) != cudaSuccess ||
         (e = cudaMalloc((void **)&p->tc_ktab, n_tab * sizeof(int2))) != cudaSuccess ||
         (e = cudaMalloc((void **)&p->tc_kref, n_tab * sizeof(int2))) != cudaSuccess ||
         (e = cudaMemcpy(p->tc_ktab, tab, n_tab * sizeof(int2), cudaMemcpyHostToDevice)) != cudaSuccess ||
-        (e = cudaMemcpy(p->tc_kref, ref, n_tab * sizeof(int2), cudaMemcpyHostToDevice)) != cudaSuccess) {
+        (e = cudaMemcpy(p->tc_kref, ref, n_tab * sizeof(int2), cudaMemcpyHostToDevice)) != cudaSuccess ||
+        (e = cudaMalloc((void **)&p->tc_ranges, (size_t)groups * 4 * sizeof(int4))) != cudaSuccess ||
+        (e = cudaMemcpy(p->tc_ranges, rng, (size_t)groups * 4 * sizeof(int4), cudaMemcpyHostToDevice)) != cudaSuccess) {
         free(tab);
         free(ref);
+        free(rng);
         p->last_err = e;
         return e == cudaErrorMemoryAllocation ? FDAS_ERR_ALLOC : FDAS_ERR_CUDA;
     }
     free(tab);
     free(ref);
+    free(rng);
     return FDAS_OK;
 }
 
@@ -897,17 +1007,61 @@ int fdas_launch_build_tapmatrix(fdas_plan *p, cudaStream_t st)
     return FDAS_OK;
 }
 
-template <int NCH>
-static int launch_mma(fdas_plan *p, const TcParams &tp, unsigned gx, size_t smem_bytes, bool bulk, cudaStream_t st)
+// The planes as a rank-2 fp32 tensor [batch*K rows][M bins] with boxes of 8, 4, 2, 1 rows x 128
+// bins, for the bulk kernel's stores.  Encoded on the host (cuTensorMapEncodeTiled, fetched through
+// the runtime so that libfdas does not link libcuda) and cached for the last plane buffer.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static int plane_maps(fdas_plan *p, void *planes, int batch, const TbMaps **out)
 {
-    if (bulk) {
+    static EncodeTiledFn encode = nullptr;
+    if (!encode) {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        FDAS_CUDA_TRY(p, cudaGetDriverEntryPointByVersion("cuTensorMapEncodeTiled", &fn, 12000, cudaEnableDefault, &qres));
+        if (!fn || qres != cudaDriverEntryPointSuccess) return FDAS_ERR_UNSUPPORTED;
+        encode = (EncodeTiledFn)fn;
+    }
+    if (!p->tc_maps) {
+        p->tc_maps = aligned_alloc(64, sizeof(TbMaps));
+        if (!p->tc_maps) return FDAS_ERR_ALLOC;
+        p->tc_maps_plane = nullptr;
+    }
+    TbMaps *maps = static_cast<TbMaps *>(p->tc_maps);
+    if (p->tc_maps_plane != planes || p->tc_maps_batch != batch) {
+        const cuuint64_t dims[2] = {(cuuint64_t)p->M, (cuuint64_t)batch * (cuuint64_t)p->K};
+        const cuuint64_t strides[1] = {(cuuint64_t)p->M * sizeof(float)};
+        const cuuint32_t estr[2] = {1, 1};
+        for (int b = 0; b < TB_BOXES; ++b) {
+            const cuuint32_t box[2] = {(cuuint32_t)TC_TILE, (cuuint32_t)(8 >> b)};
+            const CUresult r = encode(&maps->m[b], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, planes, dims, strides, box, estr,
+                                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                      CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r != CUDA_SUCCESS) {
+                p->tc_maps_plane = nullptr;
+                return FDAS_ERR_UNSUPPORTED;
+            }
+        }
+        p->tc_maps_plane = planes;
+        p->tc_maps_batch = batch;
+    }
+    *out = maps;
+    return FDAS_OK;
+}
+
+template <int NCH>
+static int launch_mma(fdas_plan *p, const TcParams &tp, unsigned gx, size_t smem_bytes, const TbMaps *maps, cudaStream_t st)
+{
+    if (maps) {
         auto kern = fdas_mma_bulk_kernel<NCH>;
         static size_t attr_bytes = 0;
         if (smem_bytes > attr_bytes) {
             FDAS_CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
             attr_bytes = smem_bytes;
         }
-        kern<<<dim3(gx, p->tc_groups), TB_THREADS, smem_bytes, st>>>(tp);
+        kern<<<dim3(gx, p->tc_groups), TB_THREADS, smem_bytes, st>>>(tp, *maps);
     } else {
         auto kern = fdas_mma_convolve_kernel<NCH>;
         static size_t attr_bytes = 0;
@@ -926,8 +1080,14 @@ int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, in
                              fdas_search_args *search)
 {
     if (p->precision != FDAS_BF16 || !p->tc_supported) return FDAS_ERR_UNSUPPORTED;
-    // bulk copies need every plane row segment 16-byte aligned: M % 4 == 0 (the caller's plane is 16-byte aligned)
-    const bool bulk = (p->M % 4 == 0) && ((reinterpret_cast<uintptr_t>(planes) & 15u) == 0) && !p->tc_force_scalar_stores;
+    // tensor-map stores need 16-byte aligned plane rows: M % 4 == 0 and a 16-byte aligned plane
+    bool bulk = (p->M % 4 == 0) && ((reinterpret_cast<uintptr_t>(planes) & 15u) == 0) && !p->tc_force_scalar_stores &&
+                p->tc_bulk_ok && (long long)batch * p->K < 0x7FFFFFFFLL;
+    const TbMaps *maps = nullptr;
+    if (bulk && plane_maps(p, planes, batch, &maps) != FDAS_OK) {   // no encoder in this driver: scalar stores
+        bulk = false;
+        maps = nullptr;
+    }
     const uint32_t smem_cap = 227u * 1024u;
     auto smem_total = [&](int R) -> uint32_t {
         return bulk ? TbSmem(R, p->tc_KS, p->tc_NT, TC_TILE * 4).total : TcSmem(R, p->tc_KS, p->tc_NT).total;
@@ -947,6 +1107,7 @@ int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, in
     tp.planes = static_cast<float *>(planes);
     tp.bmat = static_cast<const uint4 *>(p->tc_bmat);
     tp.ktab = p->tc_ktab;
+    tp.ranges = p->tc_ranges;
     tp.M = p->M;
     tp.K = p->K;
     tp.batch = batch;
@@ -966,14 +1127,14 @@ int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, in
     const long long items = (long long)batch * tp.n_blocks;
     const unsigned gx = (unsigned)(items < sms_per_group ? items : sms_per_group);
     switch (p->tc_NT / 16) {
-    case 1: return launch_mma<1>(p, tp, gx, total, bulk, st);
-    case 2: return launch_mma<2>(p, tp, gx, total, bulk, st);
-    case 3: return launch_mma<3>(p, tp, gx, total, bulk, st);
-    case 4: return launch_mma<4>(p, tp, gx, total, bulk, st);
-    case 5: return launch_mma<5>(p, tp, gx, total, bulk, st);
-    case 6: return launch_mma<6>(p, tp, gx, total, bulk, st);
-    case 7: return launch_mma<7>(p, tp, gx, total, bulk, st);
-    case 8: return launch_mma<8>(p, tp, gx, total, bulk, st);
+    case 1: return launch_mma<1>(p, tp, gx, total, maps, st);
+    case 2: return launch_mma<2>(p, tp, gx, total, maps, st);
+    case 3: return launch_mma<3>(p, tp, gx, total, maps, st);
+    case 4: return launch_mma<4>(p, tp, gx, total, maps, st);
+    case 5: return launch_mma<5>(p, tp, gx, total, maps, st);
+    case 6: return launch_mma<6>(p, tp, gx, total, maps, st);
+    case 7: return launch_mma<7>(p, tp, gx, total, maps, st);
+    case 8: return launch_mma<8>(p, tp, gx, total, maps, st);
     default: return FDAS_ERR_UNSUPPORTED;
     }
 }

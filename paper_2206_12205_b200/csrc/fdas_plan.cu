@@ -17,6 +17,8 @@ static void free_device_members(fdas_plan *p)
     cudaFree(p->tc_bmat);
     cudaFree(p->tc_ktab);
     cudaFree(p->tc_kref);
+    cudaFree(p->tc_ranges);
+    free(p->tc_maps);
     cudaFree(p->cand);
     cudaFree(p->cand_ctr);
     cudaFree(p->stage_spectrum);
