@@ -322,12 +322,12 @@ def main():
                 "h2d_bytes_per_step": int(M * 8), "d2h_bytes_per_step": int(4 + 12 * min(r["n_e2e"], PEAK_CAPACITY)),
                 "api": "fdas_search_host (pinned host spectrum in, peak list out)", "ms_per_step": r["e2e_s"] * 1e3},
         "gpu_launches": int(r["launches"]),
-        "roofline": {"bound": "hbm", "kernel": "fdas_mma_convolve_kernel<7> (fdas_convolve, bf16)", "achieved": achieved,
+        "roofline": {"bound": "hbm", "kernel": "fdas_mma_bulk_kernel<7> (fdas_convolve, bf16)", "achieved": achieved,
                      "peak": peak_gbs, "unit": "GB/s", "frac": achieved / peak_gbs, "traffic": traffic,
                      "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
                      "kernel_ms": r["conv_ms"], "kernel_ms_min": r["conv_ms_min"],
                      "frac_of_nominal_8TBs": achieved / 8000.0},
-        "roofline_tensor": {"bound": "tensor", "kernel": "fdas_mma_convolve_kernel<7>", "achieved": mma_flops / (r["conv_ms"] * 1e-3) / 1e12,
+        "roofline_tensor": {"bound": "tensor", "kernel": "fdas_mma_bulk_kernel<7>", "achieved": mma_flops / (r["conv_ms"] * 1e-3) / 1e12,
                             "peak": tensor_peak, "unit": "TFLOP/s", "frac": mma_flops / (r["conv_ms"] * 1e-3) / 1e12 / tensor_peak,
                             "flops_per_launch": mma_flops, "peak_source": tensor_src,
                             "count": "issued dense MMA flops: tiles x 2 parts x 9 K-steps x 2*128*112*16 (padding included)"},
