@@ -8,6 +8,7 @@
 // Points of the length-S transforms held per thread, and the derived kernel geometry
 // (DESIGN.md section 5):  S = 16 * 16 * R3,  T = S/16 threads per segment.
 #define FDAS_PTS 16
+#define FDAS_TC_MAX_BOXES 8   // distinct plane-row run lengths the tensor-core kernel's box stores can serve
 
 struct fdas_plan {
     // problem shape
@@ -31,7 +32,9 @@ struct fdas_plan {
     size_t tc_bmat_bytes;
     int2 *tc_ktab;     // [groups][nzg] plane rows of (+|z|, -|z|), -1 where absent
     int2 *tc_kref;     // [groups][nzg] (template whose taps fill the columns, its sign)
-    int4 *tc_ranges;   // [groups][4] plane-row runs of the bulk kernel's staging rows
+    int4 *tc_ranges;   // [groups][4] plane-row runs of the bulk kernel's staging rows (row0_n, cnt_n, row0_p, cnt_p;
+                       // each cnt carries the index of its tensor-map box in bits 16+)
+    int tc_box_heights[FDAS_TC_MAX_BOXES], tc_n_boxes;   // distinct run lengths = box heights of the tensor maps
     int tc_bulk_ok;    // those runs are contiguous (always, for the grids fdas_plan_create builds)
     void *tc_maps;     // host: cached tensor maps of the last plane buffer (fdas_mma.cu)
     const void *tc_maps_plane;

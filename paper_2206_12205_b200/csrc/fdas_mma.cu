@@ -32,17 +32,19 @@
 // One persistent CTA per SM, warp-specialised.  Two kernels share the loader and the MMA issuer:
 //
 // fdas_mma_bulk_kernel (M % 4 == 0, the normal case)
-//   warps 0-15  epilogue: tcgen05.ld -> packed |.|^2 -> shared-memory staging rows of 128 bins;
-//               one thread per plane row then pushes its 512-byte row segment to HBM with a 1-D
-//               bulk copy (cp.async.bulk.global.shared::cta).  Measured on B200: 128-byte scalar
-//               row segments cap the plane write at ~4.9 TB/s, 512-byte bulk segments reach
-//               6.3 TB/s.
+//   warps 0-15  epilogue, two sets taking alternate tiles: tcgen05.ld -> packed |.|^2, the powers
+//               of the whole tile held in registers and the TMEM stage handed back at once, so
+//               the MMAs never wait for the store path; then registers -> shared-memory staging
+//               rows of 128 bins -> one tensor-map box store (cp.async.bulk.tensor.2d) per run of
+//               consecutive plane rows.  Measured on B200: plane rows
+//               written as 128-byte segments cap at ~4.5 TB/s, 256..1024-byte segments reach
+//               5.8-6.0 TB/s, a linear fill 7.1 TB/s.
 //   warp  16    one thread issues tcgen05.mma and tcgen05.commit
-//   warps 17-20 loader: spectrum block -> bf16 (RNE, reading A12) -> Z rows
+//   warps 17-19 loader: spectrum block -> bf16 (RNE, reading A12) -> Z rows
 //
 // fdas_mma_convolve_kernel (any M: bulk copies need 16-byte aligned rows)
 //   warps 0-7   epilogue: tcgen05.ld -> |.|^2 -> st.global.cs (TMEM double-buffered)
-//   warp  8     MMA issuer;  warps 9-12 loader
+//   warp  8     MMA issuer;  warps 9-11 loader
 #include <cuda.h>        // CUtensorMap (types only; the encoder is fetched through cudaGetDriverEntryPoint)
 #include <cuda_bf16.h>
 #include <math.h>
@@ -55,9 +57,9 @@ constexpr int TC_TILE = 128;            // outputs per MMA tile = UMMA M = TMEM 
 constexpr int TC_EPI_WARPS = 8;
 constexpr int TC_MMA_WARP = 8;
 constexpr int TC_LOAD_WARP0 = 9;
-constexpr int TC_LOAD_WARPS = 4;
+constexpr int TC_LOAD_WARPS = 3;       // 16 + 1 + 3 = 20 warps: registers are granted per 4 warps, 20 warps leave 96 per thread
 constexpr int TC_LOAD_THREADS = 32 * TC_LOAD_WARPS;
-constexpr int TC_THREADS = 32 * (TC_EPI_WARPS + 1 + TC_LOAD_WARPS);   // 416
+constexpr int TC_THREADS = 32 * (TC_EPI_WARPS + 1 + TC_LOAD_WARPS);   // 384
 constexpr int TC_TMEM_COLS = 512;       // whole TMEM: 2 stages x (re | im) x NT <= 128 columns
 constexpr int TC_STAGE_COLS = 256;
 constexpr long long TC_SPIN_LIMIT = 1LL << 26;   // a stuck pipeline traps instead of hanging the GPU
@@ -79,6 +81,17 @@ struct TcParams {
     int full_chunks;         // 16-column chunks whose 8 |z| entries all have both plane rows
     fdas_search_args search; // fused threshold pass (fdas_search); enabled = 0 for plain fdas_convolve
 };
+
+#ifdef FDAS_MMA_TRACE   // tuning builds only: clock64 time line of CTA 0 (warp, tile, event)
+__device__ long long g_trace[24][64][16];
+#define TR(tile_idx, ev)                                                                              \
+    do {                                                                                              \
+        if (blockIdx.x == 0 && (threadIdx.x & 31) == 0 && (tile_idx) >= 64u && (tile_idx) < 128u)     \
+            g_trace[threadIdx.x >> 5][(tile_idx) - 64u][ev] = clock64();                              \
+    } while (0)
+#else
+#define TR(tile_idx, ev)
+#endif
 
 // ---- PTX wrappers ---------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -375,13 +388,17 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
         const long long blk0 = (it % p.n_blocks) * p.R;
         const long long left = p.M - blk0;
         const int n_tiles = (int)((left < p.R ? left : p.R) + TC_TILE - 1) / TC_TILE;
+        TR(t, 3);
         mbar_wait(z_full + 8 * buf, zuse & 1);
         tc_fence_after();
+        TR(t, 4);
         const uint32_t z_addr = s_base + off_z + buf * z_buf_bytes;
         for (int tile = 0; tile < n_tiles; ++tile, ++t) {
             const uint32_t stage = t & 1, use = t >> 1;
+            TR(t, 0);
             mbar_wait(t_empty + 8 * stage, (use & 1) ^ 1);
             tc_fence_after();
+            TR(t, 1);
             const uint32_t d_re = tmem_base + stage * TC_STAGE_COLS, d_im = d_re + NT;
             // descriptors advance by adding to their 14-bit address field (units of 16 bytes; shared
             // memory is < 256 KB, so no carry leaves the field)
@@ -397,6 +414,7 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
                 bd += (2u * b_lbo) >> 4;
             }
             umma_commit_elected(t_full + 8 * stage, elected);
+            TR(t, 2);
         }
         umma_commit_elected(z_empty + 8 * buf, elected);
     }
@@ -406,7 +424,7 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
 // even, reading A12) -> the Z rows (file header) of buffer n & 1.  The global loads of
 // item n+1 are issued before the wait for buffer n and stay in registers across it, so that
 // their latency hides behind the tensor core working on the previous items.
-constexpr int TC_LD_ITERS = 6;   // sample pairs per loader thread: (R + 16 KS) / 2 / 128 <= (1024 + 512) / 256
+constexpr int TC_LD_ITERS = 8;   // sample pairs per loader thread: (R + 16 KS) / 2 / 96 <= (1024 + 512) / 192
 
 __device__ __forceinline__ void loader_fetch(const TcParams &p, long long it, uint32_t xn, int lt, float2 (&a)[TC_LD_ITERS],
                                              float2 (&b)[TC_LD_ITERS])
@@ -581,11 +599,11 @@ __global__ void __launch_bounds__(TC_THREADS, 1) fdas_mma_convolve_kernel(const 
 constexpr int TB_EPI_WARPS = 16;        // 4 TMEM lane quarters x 4 column groups
 constexpr int TB_MMA_WARP = 16;
 constexpr int TB_LOAD_WARP0 = 17;
-constexpr int TB_THREADS = 32 * (TB_EPI_WARPS + 1 + TC_LOAD_WARPS);   // 672
+constexpr int TB_THREADS = 32 * (TB_EPI_WARPS + 1 + TC_LOAD_WARPS);   // 640
 constexpr int TB_CGROUPS = 4;           // column groups: NCH entry pairs (4 NCH columns per part) each
-constexpr int TB_BOXES = 4;             // tensor maps with box heights 8, 4, 2, 1 rows
+constexpr int TB_BOXES = FDAS_TC_MAX_BOXES;   // tensor maps, one per distinct run length (plan->tc_box_heights)
 struct TbMaps {
-    CUtensorMap m[TB_BOXES];            // the planes as a [batch*K][M] fp32 matrix, box = (8 >> i) rows x 128 bins
+    CUtensorMap m[TB_BOXES];            // the planes as a [batch*K][M] fp32 matrix, box = tc_box_heights[i] rows x 128 bins
 };
 
 // shared-memory carve-up of the bulk kernel.  ROWB = bytes of one staging row (one plane row
@@ -692,21 +710,9 @@ __device__ __forceinline__ void tensor_store(const CUtensorMap *map, uint32_t ss
                  "r"(row), "r"(ssrc)
                  : "memory");
 }
-// a run of cnt staging rows starting at shared address ssrc -> plane rows row.. as boxes of 8, 4, 2, 1 rows
-__device__ __forceinline__ void store_rows(const TbMaps &maps, uint32_t ssrc, int col, int row, int cnt, uint32_t rowb)
-{
-    int done = 0;
-#pragma unroll
-    for (int b = 0; b < TB_BOXES; ++b) {
-        const int h = 8 >> b;
-        while (cnt - done >= h) {
-            tensor_store(&maps.m[b], ssrc + (uint32_t)done * rowb, col, row + done);
-            done += h;
-        }
-    }
-}
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void bulk_wait_read_all() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 
 template <int NCH>
@@ -764,10 +770,16 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
         // Staging rows of a column group (NC = 4 NCH rows of 128 bins): the -|z| rows of its entries
         // el = 0, 1, .. in rows el, the +|z| rows in rows NC-1-el, so that each block is a run of
         // consecutive plane rows in ascending order (ranges[]: row0_n, cnt_n / row0_p, cnt_p) and
-        // leaves as a few tensor-map boxes issued by one thread of the four warps sharing it.
-        const bool issuer = q == 0 && lane == 0;
+        // leaves as ONE tensor-map box (ranges[]: the run length selects a map whose box has exactly
+        // that many rows).  Two of the four warps sharing a staging block issue one box each: a
+        // UTMASTG costs its issuing warp ~220 cycles (measured), which must not serialise.
+        const bool issuer = q < 2 && lane == 0;
         const int bar_id = 2 + 2 * set + half;              // the 128 threads (set, half)
         const uint32_t stage = set;
+        // the row runs of this warp's two column groups, read once: nothing inside the tile loop may touch
+        // global memory (a load behind the saturated write stream stalls its warp, and with it the barrier
+        // of its staging block, for thousands of cycles)
+        const int4 rg2[2] = {p.ranges[grp * TB_CGROUPS + 2 * half], p.ranges[grp * TB_CGROUPS + 2 * half + 1]};
         uint32_t t = 0;
         for (long long it = blockIdx.x; it < n_items; it += gridDim.x) {
             const long long ser = it / p.n_blocks;
@@ -779,66 +791,110 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
                 const uint32_t use = t >> 1;
                 const long long col0 = blk0 + tile * TC_TILE;
                 const uint32_t taddr0 = tmem_base + ((uint32_t)(q * 32) << 16) + stage * TC_STAGE_COLS;
-                // this set's staging buffers last fed the stores of tile t-2: their shared-memory reads are over
-                if (issuer) bulk_wait_read_all();
+                TR(t, 0);
                 mbar_wait(t_full + 8 * stage, use & 1);
                 tc_fence_after();
-                named_bar_sync(bar_id, 128);
+                TR(t, 1);
 #ifdef FDAS_MMA_DEBUG_NOEPI
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(t_empty + 8 * stage);
                 continue;
 #endif
+                // ---- TMEM -> powers in registers, for both column groups, then hand the stage back at once:
+                // the MMA of tile t+2 never waits for the store path (shared-memory staging, TMA backlog)
+                float pw[2][NC];   // per column group: (pm0, pm1, pp0, pp1) of each entry pair
+                float mx2[2];
 #pragma unroll
                 for (int pass = 0; pass < 2; ++pass) {
                     const int cg = 2 * half + pass;
-                    const int4 rg = p.ranges[grp * TB_CGROUPS + cg];
-                    uint32_t v[2 * NC];
-                    tmem_ld_cols<NC>(taddr0 + cg * NC, v);
-                    tmem_ld_cols<NC>(taddr0 + NT + cg * NC, v + NC);
-                    tmem_ld_fence<2 * NC>(v);
-                    if (pass == 1) {                        // both column groups are in registers: hand the stage back
-                        tc_fence_before();
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive(t_empty + 8 * stage);
-                    }
-                    unsigned char *const stage_buf = smem + L.off_stage + (size_t)(2 * cg + stage) * L.stage_cg_bytes;
-                    float *const sb = reinterpret_cast<float *>(stage_buf) + lt;
                     float mx = 0.f;
 #pragma unroll
-                    for (int pr = 0; pr < NCH; ++pr) {
-                        const unsigned long long ure = f2_pack(v[4 * pr], v[4 * pr + 1]), vre = f2_pack(v[4 * pr + 2], v[4 * pr + 3]);
-                        const unsigned long long uim = f2_pack(v[NC + 4 * pr], v[NC + 4 * pr + 1]);
-                        const unsigned long long vim = f2_pack(v[NC + 4 * pr + 2], v[NC + 4 * pr + 3]);
-                        const unsigned long long a = f2_sub(ure, vim), b = f2_add(uim, vre);
-                        const unsigned long long c = f2_add(ure, vim), d = f2_sub(uim, vre);
-                        const unsigned long long pp = f2_fma(b, b, f2_mul(a, a)), pm = f2_fma(d, d, f2_mul(c, c));
-                        float pp0, pp1, pm0, pm1;
-                        f2_unpack(pp, pp0, pp1);
-                        f2_unpack(pm, pm0, pm1);
-                        sb[(2 * pr) * TC_TILE] = pm0;
-                        sb[(2 * pr + 1) * TC_TILE] = pm1;
-                        sb[(NC - 1 - 2 * pr) * TC_TILE] = pp0;
-                        sb[(NC - 2 - 2 * pr) * TC_TILE] = pp1;
-                        // padded columns give exactly zero; a sign whose row is not in the plane (asymmetric
-                        // grids) can only add a candidate, which the resolve kernel then rejects
-                        mx = fmaxf(mx, fmaxf(fmaxf(pp0, pm0), fmaxf(pp1, pm1)));
+                    for (int pr0 = 0; pr0 < NCH; pr0 += 4) {
+                        constexpr int dummy = 0;
+                        (void)dummy;
+                        const int npr = NCH - pr0 < 4 ? NCH - pr0 : 4;   // entry pairs in this chunk (compile time after unrolling)
+                        uint32_t v[32];
+                        if (npr == 4) {
+                            tmem_ld_cols<16>(taddr0 + cg * NC + 4 * pr0, v);
+                            tmem_ld_cols<16>(taddr0 + NT + cg * NC + 4 * pr0, v + 16);
+                        } else if (npr == 3) {
+                            tmem_ld_cols<12>(taddr0 + cg * NC + 4 * pr0, v);
+                            tmem_ld_cols<12>(taddr0 + NT + cg * NC + 4 * pr0, v + 16);
+                        } else if (npr == 2) {
+                            tmem_ld_cols<8>(taddr0 + cg * NC + 4 * pr0, v);
+                            tmem_ld_cols<8>(taddr0 + NT + cg * NC + 4 * pr0, v + 16);
+                        } else {
+                            tmem_ld_cols<4>(taddr0 + cg * NC + 4 * pr0, v);
+                            tmem_ld_cols<4>(taddr0 + NT + cg * NC + 4 * pr0, v + 16);
+                        }
+                        tmem_ld_fence<32>(v);
+                        if (pass == 1 && pr0 + 4 >= NCH) {           // last load of this tile has landed
+                            tc_fence_before();
+                            __syncwarp();
+                            if (lane == 0) mbar_arrive(t_empty + 8 * stage);
+                        }
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            if (i >= npr) continue;
+                            const int pr = pr0 + i;
+                            const unsigned long long ure = f2_pack(v[4 * i], v[4 * i + 1]), vre = f2_pack(v[4 * i + 2], v[4 * i + 3]);
+                            const unsigned long long uim = f2_pack(v[16 + 4 * i], v[16 + 4 * i + 1]);
+                            const unsigned long long vim = f2_pack(v[16 + 4 * i + 2], v[16 + 4 * i + 3]);
+                            const unsigned long long a = f2_sub(ure, vim), b = f2_add(uim, vre);
+                            const unsigned long long c = f2_add(ure, vim), d = f2_sub(uim, vre);
+                            const unsigned long long pp = f2_fma(b, b, f2_mul(a, a)), pm = f2_fma(d, d, f2_mul(c, c));
+                            f2_unpack(pm, pw[pass][4 * pr], pw[pass][4 * pr + 1]);
+                            f2_unpack(pp, pw[pass][4 * pr + 2], pw[pass][4 * pr + 3]);
+                            // padded columns give exactly zero; a sign whose row is not in the plane (asymmetric
+                            // grids) can only add a candidate, which the resolve kernel then rejects
+                            mx = fmaxf(mx, fmaxf(fmaxf(pw[pass][4 * pr], pw[pass][4 * pr + 1]),
+                                                 fmaxf(pw[pass][4 * pr + 2], pw[pass][4 * pr + 3])));
+                        }
                     }
+                    mx2[pass] = mx;
+                }
+                TR(t, 2);
+                // ---- registers -> staging rows -> one tensor-map box per run
+#pragma unroll
+                for (int pass = 0; pass < 2; ++pass) {
+                    const int cg = 2 * half + pass;
+                    const int4 rg = rg2[pass];
+                    // staging block (cg, stage) last fed this issuer's store of two commits ago (tile t-2, same
+                    // pass): at most the newest group may still be reading shared memory
+                    if (issuer) bulk_wait_read<1>();
+                    TR(t, 3 + 5 * pass);
+                    named_bar_sync(bar_id, 128);
+                    TR(t, 4 + 5 * pass);
+                    unsigned char *const stage_buf = smem + L.off_stage + (size_t)(2 * cg + stage) * L.stage_cg_bytes;
+                    float *const sb = reinterpret_cast<float *>(stage_buf) + lt;
+#pragma unroll
+                    for (int pr = 0; pr < NCH; ++pr) {
+                        sb[(2 * pr) * TC_TILE] = pw[pass][4 * pr];
+                        sb[(2 * pr + 1) * TC_TILE] = pw[pass][4 * pr + 1];
+                        sb[(NC - 1 - 2 * pr) * TC_TILE] = pw[pass][4 * pr + 2];
+                        sb[(NC - 2 - 2 * pr) * TC_TILE] = pw[pass][4 * pr + 3];
+                    }
+                    TR(t, 5 + 5 * pass);
                     fence_proxy_async();                    // staging writes -> visible to the bulk copy engine
                     named_bar_sync(bar_id, 128);
+                    TR(t, 6 + 5 * pass);
                     if (issuer) {
                         const uint32_t sst = smem_u32(stage_buf);
                         const int row_s = (int)ser * p.K;
 #ifndef FDAS_MMA_DEBUG_NOSTORE
-                        store_rows(maps, sst, (int)col0, row_s + rg.x, rg.y, ROWB);
-                        store_rows(maps, sst + (uint32_t)(NC - rg.w) * ROWB, (int)col0, row_s + rg.z, rg.w, ROWB);
-                        bulk_commit();
+                        // one box per run: warp q = 0 pushes the -|z| rows, warp q = 1 the +|z| rows
+                        const int cnt = (q ? rg.w : rg.y) & 0xFFFF, box = (q ? rg.w : rg.y) >> 16;
+                        if (cnt > 0)
+                            tensor_store(&maps.m[box], sst + (q ? (uint32_t)(NC - cnt) * ROWB : 0u), (int)col0,
+                                         row_s + (q ? rg.z : rg.x));
 #endif
+                        bulk_commit();                      // one group per pass, empty or not: bulk_wait_read<1> counts them
                     }
-                    if (mx > thr && col0 + lt < p.M && 2 * cg * NCH < p.nzg)
+                    TR(t, 7 + 5 * pass);
+                    if (mx2[pass] > thr && col0 + lt < p.M && 2 * cg * NCH < p.nzg)
                         flag_candidate(p.search.cand, p.search.cand_count, p.search.cand_capacity,
-                                       grp * p.nzg + 2 * cg * NCH, (int)(col0 + lt), mx);
+                                       grp * p.nzg + 2 * cg * NCH, (int)(col0 + lt), mx2[pass]);
                 }
             }
         }
@@ -890,6 +946,13 @@ __global__ void fdas_tapmatrix_kernel(__nv_bfloat16 *bmat, const double2 *__rest
 }
 
 }  // namespace
+
+#ifdef FDAS_MMA_TRACE
+extern "C" int fdas_debug_trace(void *dst_host)
+{
+    return (int)cudaMemcpyFromSymbol(dst_host, g_trace, sizeof(g_trace));
+}
+#endif
 
 // Host: the |z| grouping.  Templates z_k = -zmax + k dz pair up as (k, K-1-k) when zmax is a
 // multiple of dz; otherwise every template stands alone.
@@ -953,6 +1016,7 @@ int fdas_mma_plan(fdas_plan *p)
         return FDAS_ERR_ALLOC;
     }
     p->tc_bulk_ok = 1;
+    p->tc_n_boxes = 0;
     for (int g = 0; g < groups; ++g)
         for (int cg = 0; cg < 4; ++cg) {
             int4 r = make_int4(0, 0, 0, 0);
@@ -972,6 +1036,20 @@ int fdas_mma_plan(fdas_plan *p)
                 }
             }
             r.z = r.w > 0 ? x0 - (r.w - 1) : 0;
+            // the run length picks the tensor map whose box has exactly that many rows (index in bits 16+)
+            for (int *cnt : {&r.y, &r.w}) {
+                if (*cnt == 0) continue;
+                int b = 0;
+                while (b < p->tc_n_boxes && p->tc_box_heights[b] != *cnt) ++b;
+                if (b == p->tc_n_boxes) {
+                    if (b == FDAS_TC_MAX_BOXES) {
+                        p->tc_bulk_ok = 0;
+                        continue;
+                    }
+                    p->tc_box_heights[p->tc_n_boxes++] = *cnt;
+                }
+                *cnt |= b << 16;
+            }
             rng[g * 4 + cg] = r;
         }
     p->tc_bmat_bytes = (size_t)groups * 2 * KS * NT * 16;
@@ -1007,8 +1085,8 @@ int fdas_launch_build_tapmatrix(fdas_plan *p, cudaStream_t st)
     return FDAS_OK;
 }
 
-// The planes as a rank-2 fp32 tensor [batch*K rows][M bins] with boxes of 8, 4, 2, 1 rows x 128
-// bins, for the bulk kernel's stores.  Encoded on the host (cuTensorMapEncodeTiled, fetched through
+// The planes as a rank-2 fp32 tensor [batch*K rows][M bins] with one box shape per distinct run
+// length (tc_box_heights[] rows x 128 bins), for the bulk kernel's stores.  Encoded on the host (cuTensorMapEncodeTiled, fetched through
 // the runtime so that libfdas does not link libcuda) and cached for the last plane buffer.
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
@@ -1034,8 +1112,8 @@ static int plane_maps(fdas_plan *p, void *planes, int batch, const TbMaps **out)
         const cuuint64_t dims[2] = {(cuuint64_t)p->M, (cuuint64_t)batch * (cuuint64_t)p->K};
         const cuuint64_t strides[1] = {(cuuint64_t)p->M * sizeof(float)};
         const cuuint32_t estr[2] = {1, 1};
-        for (int b = 0; b < TB_BOXES; ++b) {
-            const cuuint32_t box[2] = {(cuuint32_t)TC_TILE, (cuuint32_t)(8 >> b)};
+        for (int b = 0; b < p->tc_n_boxes; ++b) {
+            const cuuint32_t box[2] = {(cuuint32_t)TC_TILE, (cuuint32_t)p->tc_box_heights[b]};
             const CUresult r = encode(&maps->m[b], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, planes, dims, strides, box, estr,
                                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                       CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
@@ -1100,6 +1178,9 @@ int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, in
         const long long items = (long long)batch * ((p->M + R - 1) / R);
         if (R == 128 || (smem_total(R) <= smem_cap && items >= 2LL * sms_per_group)) break;
     }
+#ifdef FDAS_MMA_TUNE
+    if (getenv("FDAS_TC_R")) R = atoi(getenv("FDAS_TC_R"));
+#endif
     const uint32_t total = smem_total(R);
     if (total > smem_cap) return FDAS_ERR_UNSUPPORTED;
     TcParams tp;
