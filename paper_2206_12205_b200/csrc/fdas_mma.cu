@@ -373,7 +373,7 @@ __device__ __forceinline__ void umma_commit_elected(uint32_t bar, uint32_t elect
 template <int NT>
 __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, uint32_t off_z, uint32_t z_buf_bytes,
                                            uint32_t z_part_bytes, uint32_t z_full, uint32_t z_empty, uint32_t t_full,
-                                           uint32_t t_empty, uint32_t tmem_base, long long n_items)
+                                           uint32_t t_empty, uint32_t tmem_base, uint32_t n_items)
 {
     // instruction descriptor (cute::UMMA::InstrDescriptor): fp32 accumulate, bf16 A and B, both K-major,
     // N = NT, M = 128
@@ -383,9 +383,9 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
     const uint32_t elected = elect_one();
     const uint64_t b_desc0 = smem_desc(s_base, b_lbo, 128u);
     uint32_t n = 0, t = 0;
-    for (long long it = blockIdx.x; it < n_items; it += gridDim.x, ++n) {
+    for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x, ++n) {
         const uint32_t buf = n & 1, zuse = n >> 1;
-        const long long blk0 = (it % p.n_blocks) * p.R;
+        const long long blk0 = (long long)(it % (uint32_t)p.n_blocks) * p.R;
         const long long left = p.M - blk0;
         const int n_tiles = (int)((left < p.R ? left : p.R) + TC_TILE - 1) / TC_TILE;
         TR(t, 3);
@@ -426,11 +426,11 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
 // their latency hides behind the tensor core working on the previous items.
 constexpr int TC_LD_ITERS = 8;   // sample pairs per loader thread: (R + 16 KS) / 2 / 96 <= (1024 + 512) / 192
 
-__device__ __forceinline__ void loader_fetch(const TcParams &p, long long it, uint32_t xn, int lt, float2 (&a)[TC_LD_ITERS],
+__device__ __forceinline__ void loader_fetch(const TcParams &p, uint32_t it, uint32_t xn, int lt, float2 (&a)[TC_LD_ITERS],
                                              float2 (&b)[TC_LD_ITERS])
 {
-    const long long ser = it / p.n_blocks;
-    const long long g0 = (it % p.n_blocks) * p.R - p.M0;   // sample index of xs[0]
+    const long long ser = it / (uint32_t)p.n_blocks;   // 32-bit division: items < 2^31 (checked by the launcher)
+    const long long g0 = (long long)(it % (uint32_t)p.n_blocks) * p.R - p.M0;   // sample index of xs[0]
     const float2 *__restrict__ X = p.spectra + (size_t)ser * p.M;
 #pragma unroll
     for (int i = 0; i < TC_LD_ITERS; ++i) {
@@ -448,14 +448,14 @@ __device__ __forceinline__ void loader_fetch(const TcParams &p, long long it, ui
 __device__ __forceinline__ void spectrum_loader(const TcParams &p, unsigned char *smem, uint32_t off_xs,
                                                 uint32_t xs_part_bytes, uint32_t xn, uint32_t off_z, uint32_t z_buf_bytes,
                                                 uint32_t z_part_bytes, uint32_t zr, uint32_t z_full, uint32_t z_empty,
-                                                int lt, long long n_items)
+                                                int lt, uint32_t n_items)
 {
     uint32_t *xs_re = reinterpret_cast<uint32_t *>(smem + off_xs);
     uint32_t *xs_im = reinterpret_cast<uint32_t *>(smem + off_xs + xs_part_bytes);
     float2 a[TC_LD_ITERS], b[TC_LD_ITERS];
     uint32_t n = 0;
-    if ((long long)blockIdx.x < n_items) loader_fetch(p, blockIdx.x, xn, lt, a, b);
-    for (long long it = blockIdx.x; it < n_items; it += gridDim.x, ++n) {
+    if (blockIdx.x < n_items) loader_fetch(p, blockIdx.x, xn, lt, a, b);
+    for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x, ++n) {
         const uint32_t buf = n & 1, zuse = n >> 1;
         // phase A: spectrum block -> bf16 (round-to-nearest-even), re and im planes
 #pragma unroll
@@ -502,7 +502,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) fdas_mma_convolve_kernel(const 
     const TcSmem L(p.R, p.KS, NT);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int grp = blockIdx.y;
-    const long long n_items = (long long)p.batch * p.n_blocks;
+    const uint32_t n_items = (uint32_t)p.batch * (uint32_t)p.n_blocks;
 
     const uint32_t s_base = smem_u32(smem);
     const uint32_t bars = s_base + L.off_bars;
@@ -551,9 +551,9 @@ __global__ void __launch_bounds__(TC_THREADS, 1) fdas_mma_convolve_kernel(const 
         const float thr = p.search.enabled ? p.search.thr : __int_as_float(0x7f800000);
         const int zi_group0 = grp * p.nzg;
         uint32_t t = 0;
-        for (long long it = blockIdx.x; it < n_items; it += gridDim.x) {
-            const long long ser = it / p.n_blocks;
-            const long long blk0 = (it % p.n_blocks) * p.R;
+        for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
+            const long long ser = it / (uint32_t)p.n_blocks;   // 32-bit division: items < 2^31 (checked by the launcher)
+            const long long blk0 = (long long)(it % (uint32_t)p.n_blocks) * p.R;
             const long long left = p.M - blk0;
             const int n_tiles = (int)((left < p.R ? left : p.R) + TC_TILE - 1) / TC_TILE;
             for (int tile = 0; tile < n_tiles; ++tile, ++t) {
@@ -726,7 +726,7 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
     const TbSmem L(p.R, p.KS, NT, ROWB);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int grp = blockIdx.y;
-    const long long n_items = (long long)p.batch * p.n_blocks;
+    const uint32_t n_items = (uint32_t)p.batch * (uint32_t)p.n_blocks;
 
     const uint32_t s_base = smem_u32(smem);
     const uint32_t bars = s_base + L.off_bars;
@@ -781,9 +781,9 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
         // of its staging block, for thousands of cycles)
         const int4 rg2[2] = {p.ranges[grp * TB_CGROUPS + 2 * half], p.ranges[grp * TB_CGROUPS + 2 * half + 1]};
         uint32_t t = 0;
-        for (long long it = blockIdx.x; it < n_items; it += gridDim.x) {
-            const long long ser = it / p.n_blocks;
-            const long long blk0 = (it % p.n_blocks) * p.R;
+        for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
+            const long long ser = it / (uint32_t)p.n_blocks;   // 32-bit division: items < 2^31 (checked by the launcher)
+            const long long blk0 = (long long)(it % (uint32_t)p.n_blocks) * p.R;
             const long long left = p.M - blk0;
             const int n_tiles = (int)((left < p.R ? left : p.R) + TC_TILE - 1) / TC_TILE;
             for (int tile = 0; tile < n_tiles; ++tile, ++t) {
@@ -1206,6 +1206,7 @@ int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, in
         tp.search = fdas_search_args{0, 0.f, nullptr, nullptr, nullptr, 0, nullptr, 8};
     }
     const long long items = (long long)batch * tp.n_blocks;
+    if (items >= 0x7FFFFFFFLL) return FDAS_ERR_UNSUPPORTED;   // the kernels count work items in 32 bits
     const unsigned gx = (unsigned)(items < sms_per_group ? items : sms_per_group);
     switch (p->tc_NT / 16) {
     case 1: return launch_mma<1>(p, tp, gx, total, maps, st);
