@@ -67,6 +67,14 @@ typedef enum {
                            so that tests and profiles can compare the two store paths.      */
 } fdas_algorithm_t;
 
+/* Element type of the power plane written by fdas_convolve (fdas_set_plane_format). */
+typedef enum {
+    FDAS_PLANE_F32 = 0, /* default: float (double in FDAS_F64)                                   */
+    FDAS_PLANE_BF16 = 1 /* bfloat16 bit patterns (uint16): the paper's bfloat16 pipeline keeps the
+                           f-fdot plane in bfloat16 and widens it afterwards by the "quick cast"
+                           (PAPER.md:91-93); halves the dominant HBM stream of the path        */
+} fdas_plane_format_t;
+
 typedef enum {
     FDAS_OK = 0,
     FDAS_ERR_INVALID_ARG = 1, /* NULL pointer, bad size, illegal parameter combination   */
@@ -93,7 +101,7 @@ typedef struct {
     int32_t precision;       /* fdas_precision_t                                         */
     int64_t n_segments;      /* ceil(M / V)                                              */
     int64_t plane_row_pitch; /* elements between plane rows (= M: rows are contiguous)   */
-    size_t plane_elem_bytes; /* 4 (float) or 8 (double, FDAS_F64)                        */
+    size_t plane_elem_bytes; /* 4 (float), 8 (double, FDAS_F64) or 2 (FDAS_PLANE_BF16)           */
     size_t spectrum_elem_bytes; /* 8 (complex64) or 16 (complex128, FDAS_F64)            */
     size_t bank_bytes;       /* device bytes of the template bank                        */
 } fdas_info_t;
@@ -130,6 +138,31 @@ int fdas_plan_create(fdas_plan_t **out, int64_t N, double zmax, double dz, int s
  */
 int fdas_set_algorithm(fdas_plan_t *p, int algorithm);
 int fdas_get_algorithm(const fdas_plan_t *p, int *algorithm);
+
+/*
+ * fdas_set_plane_format -- choose the element type of the plane (section 3.1).
+ *   FDAS_PLANE_BF16  FDAS_BF16 plans on the tensor-core algorithm only.  Every power is computed
+ *                    in fp32 exactly as for FDAS_PLANE_F32 and rounded once, to nearest even, to
+ *                    bfloat16; plane_dev of fdas_convolve / fdas_convolve_batched / fdas_search /
+ *                    fdas_peaks and plane_host of fdas_convolve_host are then [K][M] uint16 bit
+ *                    patterns (fdas_info_t.plane_elem_bytes = 2).  fdas_peaks and fdas_search
+ *                    apply the peak rule to the stored (rounded) values; rounding creates ties,
+ *                    which the rule's ordering resolves (one peak per plateau).
+ * Errors: INVALID_ARG (NULL, unknown value), UNSUPPORTED (bf16 plane on a plan that does not run
+ * the tensor-core kernels; fdas_set_algorithm(FDAS_ALGO_FFT) while the plane format is bf16).
+ */
+int fdas_set_plane_format(fdas_plan_t *p, int format);
+int fdas_get_plane_format(const fdas_plan_t *p, int *format);
+
+/*
+ * fdas_quick_cast -- the paper's widening of a bf16-stored plane ("copying the two
+ * bytes of data for each bfloat16 number into the corresponding positions of an all zero
+ * single-precision output array").  plane_bf16_dev: batch*K*M uint16; plane_f32_dev: batch*K*M
+ * float, fully overwritten: word i = (uint32) bits[i] << 16, bit-exact.  The two buffers must not
+ * overlap.  Works for any plan (only K and M are used).  Asynchronous on `stream`.
+ * Errors: INVALID_ARG (NULL, batch < 1), CUDA.
+ */
+int fdas_quick_cast(fdas_plan_t *p, const void *plane_bf16_dev, void *plane_f32_dev, int batch, void *stream);
 
 /* Frees the plan and its device memory (synchronises the device first).  NULL is OK. */
 int fdas_plan_destroy(fdas_plan_t *p);

@@ -38,7 +38,9 @@ struct fdas_plan {
     int tc_bulk_ok;    // those runs are contiguous (always, for the grids fdas_plan_create builds)
     void *tc_maps;     // host: cached tensor maps of the last plane buffer (fdas_mma.cu)
     const void *tc_maps_plane;
-    int tc_maps_batch;
+    int tc_maps_batch, tc_maps_elem;
+    // NEXT-1: the plane is stored as bf16 bit patterns (fdas_set_plane_format)
+    int plane_bf16;
     // fused search (fdas_search): coarse candidates flagged by the convolve epilogue
     fdas_peak_t *cand;     // [cand_capacity] (z_index = first |z| table entry of the chunk, r, chunk maximum)
     int *cand_ctr;         // two counters used alternately: call n appends to [n & 1] and clears [(n + 1) & 1]
@@ -58,6 +60,11 @@ struct fdas_plan {
 static inline size_t fdas_storage_scalar_bytes(int precision)
 {
     return precision == FDAS_F64 ? 8 : (precision == FDAS_F32 ? 4 : 2);
+}
+
+static inline size_t fdas_plane_elem_bytes(const fdas_plan *p)
+{
+    return p->precision == FDAS_F64 ? 8 : (p->plane_bf16 ? 2 : 4);
 }
 
 // complexes of the storage type per 16-byte vector: 1 (fp64), 2 (fp32), 4 (bf16)
@@ -120,3 +127,5 @@ static inline int fdas_uses_mma(const fdas_plan *p)
 }
 int fdas_launch_peaks(fdas_plan *p, const void *plane, float thr, fdas_peak_t *peaks, int capacity,
                       int *count, cudaStream_t st);
+// fdas_cast.cu: the paper's quick cast of a bf16-stored plane
+int fdas_launch_quick_cast(fdas_plan *p, const void *src_bf16, void *dst_f32, long long n, cudaStream_t st);

@@ -66,7 +66,7 @@ constexpr long long TC_SPIN_LIMIT = 1LL << 26;   // a stuck pipeline traps inste
 
 struct TcParams {
     const float2 *spectra;   // [batch][M] complex64
-    float *planes;           // [batch][K][M]
+    void *planes;            // [batch][K][M] float, or bf16 bit patterns when the plan stores a bf16 plane
     const uint4 *bmat;       // [groups][2 KS][NT] rows of 8 bf16 (the shared-memory image)
     const int2 *ktab;        // [groups][nzg]: plane rows of (+|z|, -|z|), -1 where absent
     const int4 *ranges;      // bulk kernel: [groups][4 column groups] (row0_n, cnt_n, row0_p, cnt_p), see fdas_mma_plan
@@ -224,16 +224,26 @@ struct TcSmem {
     }
 };
 
-// streaming store of v at base + off (plane elements): one IMAD.WIDE for the address
-__device__ __forceinline__ void st_cs_at(const float *base, uint32_t off, float v)
+// streaming store of v at base + off (plane elements): one IMAD.WIDE for the address.  OT = float, or
+// __nv_bfloat16 for the bf16-stored plane of PAPER.md:91 (the power rounded once, RNE).
+template <typename OT>
+__device__ __forceinline__ void st_cs_at(const OT *base, uint32_t off, float v)
 {
     unsigned long long addr;
-    asm("mad.wide.u32 %0, %1, 4, %2;" : "=l"(addr) : "r"(off), "l"(base));
-#ifdef FDAS_MMA_ST_DEFAULT
-    asm volatile("st.global.f32 [%0], %1;" ::"l"(addr), "f"(v) : "memory");
-#else
-    asm volatile("st.global.cs.f32 [%0], %1;" ::"l"(addr), "f"(v) : "memory");
-#endif
+    if constexpr (sizeof(OT) == 4) {
+        asm("mad.wide.u32 %0, %1, 4, %2;" : "=l"(addr) : "r"(off), "l"(base));
+        asm volatile("st.global.cs.f32 [%0], %1;" ::"l"(addr), "f"(v) : "memory");
+    } else {
+        asm("mad.wide.u32 %0, %1, 2, %2;" : "=l"(addr) : "r"(off), "l"(base));
+        asm volatile("st.global.cs.u16 [%0], %1;" ::"l"(addr), "h"(__bfloat16_as_ushort(__float2bfloat16_rn(v))) : "memory");
+    }
+}
+// the value a plane of element type OT holds for the fp32 power v (what fdas_peaks will read back)
+template <typename OT>
+__device__ __forceinline__ float stored_value(float v)
+{
+    if constexpr (sizeof(OT) == 4) return v;
+    else return __bfloat162float(__float2bfloat16_rn(v));
 }
 
 constexpr uint32_t TC_NO_ROW = 0xFFFFFFFFu;   // row-offset table: this |z| has no such plane row
@@ -245,8 +255,8 @@ constexpr uint32_t TC_NO_ROW = 0xFFFFFFFFu;   // row-offset table: this |z| has 
 // FAST: the tile lies inside the plane and every entry has both rows -> straight-line code.
 // Returns the largest power this thread stored (0 if none): the fused search flags the chunk
 // when it exceeds the threshold (fdas_search).
-template <bool FAST>
-__device__ __forceinline__ float epilogue_chunk(const uint32_t *v, const uint4 *o4, float *out, bool ok)
+template <bool FAST, typename OT>
+__device__ __forceinline__ float epilogue_chunk(const uint32_t *v, const uint4 *o4, OT *out, bool ok)
 {
     float mx = 0.f;
 #pragma unroll
@@ -299,8 +309,8 @@ __device__ __noinline__ void flag_candidate(fdas_peak_t *cand, int *cand_count, 
 // One tile for one epilogue warp: chunks HALF, HALF+2, ... of the NCH 16-column chunks.  The
 // TMEM load of the next chunk is in flight while the current one is squared and stored, and
 // the TMEM stage is handed back to the MMA issuer as soon as the last load has landed.
-template <int NCH, int HALF>
-__device__ __forceinline__ void epilogue_tile(uint32_t taddr, const uint4 *otab4, float *out, bool inside, bool ok,
+template <int NCH, int HALF, typename OT>
+__device__ __forceinline__ void epilogue_tile(uint32_t taddr, const uint4 *otab4, OT *out, bool inside, bool ok,
                                               int full_chunks, uint32_t empty_bar, int lane,
                                               const fdas_search_args &sa, float thr, int zi_group0, long long col)
 {
@@ -322,8 +332,9 @@ __device__ __forceinline__ void epilogue_tile(uint32_t taddr, const uint4 *otab4
         ok = false; inside = false;
 #endif
         float mx;
-        if (inside && c < full_chunks) mx = epilogue_chunk<true>(v[i & 1], otab4 + 4 * c, out, true);
-        else mx = epilogue_chunk<false>(v[i & 1], otab4 + 4 * c, out, ok);
+        if (inside && c < full_chunks) mx = epilogue_chunk<true, OT>(v[i & 1], otab4 + 4 * c, out, true);
+        else mx = epilogue_chunk<false, OT>(v[i & 1], otab4 + 4 * c, out, ok);
+        mx = stored_value<OT>(mx);   // rounding is monotone: the largest stored value
         if (mx > thr)   // thr = +inf unless fdas_search
             flag_candidate(sa.cand, sa.cand_count, sa.cand_capacity, zi_group0 + 8 * c, (int)col, mx);
     }
@@ -494,7 +505,7 @@ __device__ __forceinline__ void spectrum_loader(const TcParams &p, unsigned char
     }
 }
 
-template <int NCH>
+template <int NCH, typename OT>
 __global__ void __launch_bounds__(TC_THREADS, 1) fdas_mma_convolve_kernel(const TcParams p)
 {
     extern __shared__ __align__(128) unsigned char smem[];
@@ -560,16 +571,16 @@ __global__ void __launch_bounds__(TC_THREADS, 1) fdas_mma_convolve_kernel(const 
                 const uint32_t stage = t & 1, use = t >> 1;
                 const long long col0 = blk0 + tile * TC_TILE;
                 const long long col = col0 + q * 32 + lane;
-                float *const out = p.planes + (size_t)ser * p.K * p.M + col;
+                OT *const out = static_cast<OT *>(p.planes) + (size_t)ser * p.K * p.M + col;
                 const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + stage * TC_STAGE_COLS;
                 const bool inside = col0 + TC_TILE <= p.M;
                 mbar_wait(t_full + 8 * stage, use & 1);
                 tc_fence_after();
                 if (half == 0)
-                    epilogue_tile<NCH, 0>(taddr, otab4, out, inside, col < p.M, p.full_chunks, t_empty + 8 * stage, lane,
+                    epilogue_tile<NCH, 0, OT>(taddr, otab4, out, inside, col < p.M, p.full_chunks, t_empty + 8 * stage, lane,
                                           p.search, thr, zi_group0, col);
                 else
-                    epilogue_tile<NCH, 1>(taddr, otab4, out, inside, col < p.M, p.full_chunks, t_empty + 8 * stage, lane,
+                    epilogue_tile<NCH, 1, OT>(taddr, otab4, out, inside, col < p.M, p.full_chunks, t_empty + 8 * stage, lane,
                                           p.search, thr, zi_group0, col);
             }
         }
@@ -715,14 +726,14 @@ template <int N>
 __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 
-template <int NCH>
+template <int NCH, typename OT>
 __global__ void __launch_bounds__(TB_THREADS, 1)
 fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int NT = 16 * NCH;
     constexpr int NC = 4 * NCH;            // columns per part per column group = staging rows (slots)
-    constexpr uint32_t ROWB = TC_TILE * 4; // bytes of one staging row
+    constexpr uint32_t ROWB = TC_TILE * sizeof(OT);   // bytes of one staging row
     const TbSmem L(p.R, p.KS, NT, ROWB);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int grp = blockIdx.y;
@@ -852,7 +863,7 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
                                                  fmaxf(pw[pass][4 * pr + 2], pw[pass][4 * pr + 3])));
                         }
                     }
-                    mx2[pass] = mx;
+                    mx2[pass] = stored_value<OT>(mx);   // rounding is monotone: the largest stored value
                 }
                 TR(t, 2);
                 // ---- registers -> staging rows -> one tensor-map box per run
@@ -867,13 +878,13 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
                     named_bar_sync(bar_id, 128);
                     TR(t, 4 + 5 * pass);
                     unsigned char *const stage_buf = smem + L.off_stage + (size_t)(2 * cg + stage) * L.stage_cg_bytes;
-                    float *const sb = reinterpret_cast<float *>(stage_buf) + lt;
+                    OT *const sb = reinterpret_cast<OT *>(stage_buf) + lt;
 #pragma unroll
                     for (int pr = 0; pr < NCH; ++pr) {
-                        sb[(2 * pr) * TC_TILE] = pw[pass][4 * pr];
-                        sb[(2 * pr + 1) * TC_TILE] = pw[pass][4 * pr + 1];
-                        sb[(NC - 1 - 2 * pr) * TC_TILE] = pw[pass][4 * pr + 2];
-                        sb[(NC - 2 - 2 * pr) * TC_TILE] = pw[pass][4 * pr + 3];
+                        sb[(2 * pr) * TC_TILE] = (OT)pw[pass][4 * pr];           // float -> bf16: round to nearest even
+                        sb[(2 * pr + 1) * TC_TILE] = (OT)pw[pass][4 * pr + 1];
+                        sb[(NC - 1 - 2 * pr) * TC_TILE] = (OT)pw[pass][4 * pr + 2];
+                        sb[(NC - 2 - 2 * pr) * TC_TILE] = (OT)pw[pass][4 * pr + 3];
                     }
                     TR(t, 5 + 5 * pass);
                     fence_proxy_async();                    // staging writes -> visible to the bulk copy engine
@@ -1108,13 +1119,14 @@ static int plane_maps(fdas_plan *p, void *planes, int batch, const TbMaps **out)
         p->tc_maps_plane = nullptr;
     }
     TbMaps *maps = static_cast<TbMaps *>(p->tc_maps);
-    if (p->tc_maps_plane != planes || p->tc_maps_batch != batch) {
+    const size_t esz = p->plane_bf16 ? 2 : 4;
+    if (p->tc_maps_plane != planes || p->tc_maps_batch != batch || p->tc_maps_elem != (int)esz) {
         const cuuint64_t dims[2] = {(cuuint64_t)p->M, (cuuint64_t)batch * (cuuint64_t)p->K};
-        const cuuint64_t strides[1] = {(cuuint64_t)p->M * sizeof(float)};
+        const cuuint64_t strides[1] = {(cuuint64_t)p->M * esz};
         const cuuint32_t estr[2] = {1, 1};
         for (int b = 0; b < p->tc_n_boxes; ++b) {
             const cuuint32_t box[2] = {(cuuint32_t)TC_TILE, (cuuint32_t)p->tc_box_heights[b]};
-            const CUresult r = encode(&maps->m[b], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, planes, dims, strides, box, estr,
+            const CUresult r = encode(&maps->m[b], p->plane_bf16 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, planes, dims, strides, box, estr,
                                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                       CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
             if (r != CUDA_SUCCESS) {
@@ -1124,16 +1136,17 @@ static int plane_maps(fdas_plan *p, void *planes, int batch, const TbMaps **out)
         }
         p->tc_maps_plane = planes;
         p->tc_maps_batch = batch;
+        p->tc_maps_elem = (int)esz;
     }
     *out = maps;
     return FDAS_OK;
 }
 
-template <int NCH>
+template <int NCH, typename OT>
 static int launch_mma(fdas_plan *p, const TcParams &tp, unsigned gx, size_t smem_bytes, const TbMaps *maps, cudaStream_t st)
 {
     if (maps) {
-        auto kern = fdas_mma_bulk_kernel<NCH>;
+        auto kern = fdas_mma_bulk_kernel<NCH, OT>;
         static size_t attr_bytes = 0;
         if (smem_bytes > attr_bytes) {
             FDAS_CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
@@ -1141,7 +1154,7 @@ static int launch_mma(fdas_plan *p, const TcParams &tp, unsigned gx, size_t smem
         }
         kern<<<dim3(gx, p->tc_groups), TB_THREADS, smem_bytes, st>>>(tp, *maps);
     } else {
-        auto kern = fdas_mma_convolve_kernel<NCH>;
+        auto kern = fdas_mma_convolve_kernel<NCH, OT>;
         static size_t attr_bytes = 0;
         if (smem_bytes > attr_bytes) {
             FDAS_CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
@@ -1158,8 +1171,9 @@ int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, in
                              fdas_search_args *search)
 {
     if (p->precision != FDAS_BF16 || !p->tc_supported) return FDAS_ERR_UNSUPPORTED;
-    // tensor-map stores need 16-byte aligned plane rows: M % 4 == 0 and a 16-byte aligned plane
-    bool bulk = (p->M % 4 == 0) && ((reinterpret_cast<uintptr_t>(planes) & 15u) == 0) && !p->tc_force_scalar_stores &&
+    // tensor-map stores need 16-byte aligned plane rows: M % 4 == 0 (% 8 for a bf16 plane) and a 16-byte aligned plane
+    const uint32_t esz = p->plane_bf16 ? 2u : 4u;
+    bool bulk = ((p->M * esz) % 16 == 0) && ((reinterpret_cast<uintptr_t>(planes) & 15u) == 0) && !p->tc_force_scalar_stores &&
                 p->tc_bulk_ok && (long long)batch * p->K < 0x7FFFFFFFLL;
     const TbMaps *maps = nullptr;
     if (bulk && plane_maps(p, planes, batch, &maps) != FDAS_OK) {   // no encoder in this driver: scalar stores
@@ -1168,7 +1182,7 @@ int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, in
     }
     const uint32_t smem_cap = 227u * 1024u;
     auto smem_total = [&](int R) -> uint32_t {
-        return bulk ? TbSmem(R, p->tc_KS, p->tc_NT, TC_TILE * 4).total : TcSmem(R, p->tc_KS, p->tc_NT).total;
+        return bulk ? TbSmem(R, p->tc_KS, p->tc_NT, TC_TILE * esz).total : TcSmem(R, p->tc_KS, p->tc_NT).total;
     };
     // outputs per work item: the largest of 1024..128 that fits shared memory and leaves at
     // least two items per CTA
@@ -1185,7 +1199,7 @@ int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, in
     if (total > smem_cap) return FDAS_ERR_UNSUPPORTED;
     TcParams tp;
     tp.spectra = static_cast<const float2 *>(spectra);
-    tp.planes = static_cast<float *>(planes);
+    tp.planes = planes;
     tp.bmat = static_cast<const uint4 *>(p->tc_bmat);
     tp.ktab = p->tc_ktab;
     tp.ranges = p->tc_ranges;
@@ -1209,14 +1223,14 @@ int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, in
     if (items >= 0x7FFFFFFFLL) return FDAS_ERR_UNSUPPORTED;   // the kernels count work items in 32 bits
     const unsigned gx = (unsigned)(items < sms_per_group ? items : sms_per_group);
     switch (p->tc_NT / 16) {
-    case 1: return launch_mma<1>(p, tp, gx, total, maps, st);
-    case 2: return launch_mma<2>(p, tp, gx, total, maps, st);
-    case 3: return launch_mma<3>(p, tp, gx, total, maps, st);
-    case 4: return launch_mma<4>(p, tp, gx, total, maps, st);
-    case 5: return launch_mma<5>(p, tp, gx, total, maps, st);
-    case 6: return launch_mma<6>(p, tp, gx, total, maps, st);
-    case 7: return launch_mma<7>(p, tp, gx, total, maps, st);
-    case 8: return launch_mma<8>(p, tp, gx, total, maps, st);
+    case 1: return p->plane_bf16 ? launch_mma<1, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<1, float>(p, tp, gx, total, maps, st);
+    case 2: return p->plane_bf16 ? launch_mma<2, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<2, float>(p, tp, gx, total, maps, st);
+    case 3: return p->plane_bf16 ? launch_mma<3, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<3, float>(p, tp, gx, total, maps, st);
+    case 4: return p->plane_bf16 ? launch_mma<4, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<4, float>(p, tp, gx, total, maps, st);
+    case 5: return p->plane_bf16 ? launch_mma<5, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<5, float>(p, tp, gx, total, maps, st);
+    case 6: return p->plane_bf16 ? launch_mma<6, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<6, float>(p, tp, gx, total, maps, st);
+    case 7: return p->plane_bf16 ? launch_mma<7, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<7, float>(p, tp, gx, total, maps, st);
+    case 8: return p->plane_bf16 ? launch_mma<8, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<8, float>(p, tp, gx, total, maps, st);
     default: return FDAS_ERR_UNSUPPORTED;
     }
 }

@@ -8,11 +8,26 @@
 
 namespace {
 
+// Plane element types: double (FDAS_F64), float, and bf16 bit patterns (the bf16-stored plane of
+// PAPER.md:91; its value is the fp32 number with those 16 bits on top -- the "quick cast").
+struct bf16raw {
+    unsigned short bits;
+};
+template <typename PT> struct elem {
+    using cmp = PT;
+    static __device__ __forceinline__ cmp val(PT x) { return x; }
+};
+template <> struct elem<bf16raw> {
+    using cmp = float;
+    static __device__ __forceinline__ cmp val(bf16raw x) { return __uint_as_float((unsigned)x.bits << 16); }
+};
+
 template <typename PT>
-__device__ __forceinline__ void test_cell(const PT *__restrict__ P, int K, long long M, int k, long long r, PT v,
-                                          float thr, fdas_peak_t *peaks, int capacity, int *count)
+__device__ __forceinline__ void test_cell(const PT *__restrict__ P, int K, long long M, int k, long long r,
+                                          typename elem<PT>::cmp v, float thr, fdas_peak_t *peaks, int capacity, int *count)
 {
-    if (!(v > (PT)thr)) return;
+    using CT = typename elem<PT>::cmp;
+    if (!(v > (CT)thr)) return;
     bool ok = true;
 #pragma unroll
     for (int dk = -1; dk <= 1; ++dk) {
@@ -22,7 +37,7 @@ __device__ __forceinline__ void test_cell(const PT *__restrict__ P, int K, long 
             const int kk = k + dk;
             const long long rr = r + dr;
             if (kk < 0 || kk >= K || rr < 0 || rr >= M) continue;
-            const PT n = P[(size_t)kk * M + rr];
+            const CT n = elem<PT>::val(P[(size_t)kk * M + rr]);
             const bool precedes = (dk < 0) || (dk == 0 && dr < 0);
             ok = ok && (precedes ? (v > n) : (v >= n));
         }
@@ -53,21 +68,22 @@ fdas_peaks_kernel(const PT *__restrict__ P, int K, long long M, float thr, fdas_
         for (long long q = tid; q < nv; q += stride) {
             union { VT v; PT e[NE]; } u;
             u.v = __ldcs(PV + q);   // 128-bit streaming load
-            PT m = u.e[0];
+            using CT = typename elem<PT>::cmp;
+            CT m = elem<PT>::val(u.e[0]);
 #pragma unroll
-            for (int c = 1; c < NE; ++c) m = max(m, u.e[c]);
-            if (m > (PT)thr) {
+            for (int c = 1; c < NE; ++c) m = max(m, elem<PT>::val(u.e[c]));
+            if (m > (CT)thr) {
                 const long long e0 = q * NE;
                 const int k = (int)(e0 / M);
                 const long long r = e0 - (long long)k * M;
 #pragma unroll
-                for (int c = 0; c < NE; ++c) test_cell<PT>(P, K, M, k, r + c, u.e[c], thr, peaks, capacity, count);
+                for (int c = 0; c < NE; ++c) test_cell<PT>(P, K, M, k, r + c, elem<PT>::val(u.e[c]), thr, peaks, capacity, count);
             }
         }
     } else {
         for (long long e = tid; e < total; e += stride) {
             const int k = (int)(e / M);
-            test_cell<PT>(P, K, M, k, e - (long long)k * M, P[e], thr, peaks, capacity, count);
+            test_cell<PT>(P, K, M, k, e - (long long)k * M, elem<PT>::val(P[e]), thr, peaks, capacity, count);
         }
     }
 }
@@ -94,14 +110,14 @@ fdas_resolve_kernel(const PT *__restrict__ P, int K, long long M, float thr, con
             const int2 kk = ktab[zi];
             const int k = (i & 1) ? kk.y : kk.x;
             if (k < 0 || ((i & 1) && kk.y == kk.x)) continue;      // no such row / z = 0 listed twice
-            test_cell<PT>(P, K, M, k, c.r, P[(size_t)k * M + c.r], thr, peaks, capacity, count);
+            test_cell<PT>(P, K, M, k, c.r, elem<PT>::val(P[(size_t)k * M + c.r]), thr, peaks, capacity, count);
         }
         return;
     }
     const long long total = (long long)K * M;
     for (long long e = tid; e < total; e += stride) {
         const int k = (int)(e / M);
-        test_cell<PT>(P, K, M, k, e - (long long)k * M, P[e], thr, peaks, capacity, count);
+        test_cell<PT>(P, K, M, k, e - (long long)k * M, elem<PT>::val(P[e]), thr, peaks, capacity, count);
     }
 }
 
@@ -111,9 +127,14 @@ int fdas_launch_resolve(fdas_plan *p, const void *plane, const fdas_search_args 
                         cudaStream_t st)
 {
     const int grid = p->num_sms * 2;
-    fdas_resolve_kernel<float, float4, 4><<<grid, 256, 0, st>>>((const float *)plane, p->K, p->M, sa.thr, sa.cand,
-                                                               sa.cand_count, sa.cand_capacity, sa.cand_span, p->tc_ktab, p->tc_nzg,
-                                                               peaks, capacity, sa.count_out);
+    if (p->plane_bf16)
+        fdas_resolve_kernel<bf16raw, uint4, 8><<<grid, 256, 0, st>>>((const bf16raw *)plane, p->K, p->M, sa.thr, sa.cand,
+                                                                     sa.cand_count, sa.cand_capacity, sa.cand_span, p->tc_ktab,
+                                                                     p->tc_nzg, peaks, capacity, sa.count_out);
+    else
+        fdas_resolve_kernel<float, float4, 4><<<grid, 256, 0, st>>>((const float *)plane, p->K, p->M, sa.thr, sa.cand,
+                                                                   sa.cand_count, sa.cand_capacity, sa.cand_span, p->tc_ktab,
+                                                                   p->tc_nzg, peaks, capacity, sa.count_out);
     FDAS_CUDA_TRY(p, cudaGetLastError());
     p->launches += 1;
     return FDAS_OK;
@@ -129,6 +150,8 @@ int fdas_launch_peaks(fdas_plan *p, const void *plane, float thr, fdas_peak_t *p
     const int grid = (int)(want < cap ? (want > 0 ? want : 1) : cap);
     if (p->precision == FDAS_F64)
         fdas_peaks_kernel<double, double2, 2><<<grid, 256, 0, st>>>((const double *)plane, p->K, p->M, thr, peaks, capacity, count);
+    else if (p->plane_bf16)
+        fdas_peaks_kernel<bf16raw, uint4, 8><<<grid, 256, 0, st>>>((const bf16raw *)plane, p->K, p->M, thr, peaks, capacity, count);
     else
         fdas_peaks_kernel<float, float4, 4><<<grid, 256, 0, st>>>((const float *)plane, p->K, p->M, thr, peaks, capacity, count);
     FDAS_CUDA_TRY(p, cudaGetLastError());

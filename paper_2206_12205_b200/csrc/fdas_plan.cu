@@ -100,6 +100,7 @@ extern "C" int fdas_set_algorithm(fdas_plan_t *p, int algorithm)
         return FDAS_ERR_INVALID_ARG;
     const bool mma = algorithm == FDAS_ALGO_MMA || algorithm == FDAS_ALGO_MMA_SCALAR;
     if (mma && !(p->precision == FDAS_BF16 && p->tc_supported)) return FDAS_ERR_UNSUPPORTED;
+    if (algorithm == FDAS_ALGO_FFT && p->plane_bf16) return FDAS_ERR_UNSUPPORTED;   // only the tensor-core kernels write a bf16 plane
     p->algo = mma ? FDAS_ALGO_MMA : algorithm;
     p->tc_force_scalar_stores = algorithm == FDAS_ALGO_MMA_SCALAR;
     return FDAS_OK;
@@ -108,9 +109,36 @@ extern "C" int fdas_set_algorithm(fdas_plan_t *p, int algorithm)
 extern "C" int fdas_get_algorithm(const fdas_plan_t *p, int *algorithm)
 {
     if (!p || !algorithm) return FDAS_ERR_INVALID_ARG;
-    *algorithm = fdas_uses_mma(p) ? ((p->tc_force_scalar_stores || p->M % 4 != 0) ? FDAS_ALGO_MMA_SCALAR : FDAS_ALGO_MMA)
+    *algorithm = fdas_uses_mma(p) ? ((p->tc_force_scalar_stores || (p->M * fdas_plane_elem_bytes(p)) % 16 != 0) ? FDAS_ALGO_MMA_SCALAR : FDAS_ALGO_MMA)
                                   : FDAS_ALGO_FFT;
     return FDAS_OK;
+}
+
+extern "C" int fdas_set_plane_format(fdas_plan_t *p, int format)
+{
+    if (!p) return FDAS_ERR_INVALID_ARG;
+    if (format != FDAS_PLANE_F32 && format != FDAS_PLANE_BF16) return FDAS_ERR_INVALID_ARG;
+    // a bf16 plane is written by the tensor-core kernels only
+    if (format == FDAS_PLANE_BF16 && !fdas_uses_mma(p)) return FDAS_ERR_UNSUPPORTED;
+    if (p->plane_bf16 != (format == FDAS_PLANE_BF16)) {   // the host-path staging plane has the old element size
+        cudaFree(p->stage_plane);
+        p->stage_plane = NULL;
+    }
+    p->plane_bf16 = format == FDAS_PLANE_BF16;
+    return FDAS_OK;
+}
+
+extern "C" int fdas_get_plane_format(const fdas_plan_t *p, int *format)
+{
+    if (!p || !format) return FDAS_ERR_INVALID_ARG;
+    *format = p->plane_bf16 ? FDAS_PLANE_BF16 : FDAS_PLANE_F32;
+    return FDAS_OK;
+}
+
+extern "C" int fdas_quick_cast(fdas_plan_t *p, const void *plane_bf16_dev, void *plane_f32_dev, int batch, void *stream)
+{
+    if (!p || !plane_bf16_dev || !plane_f32_dev || batch < 1) return FDAS_ERR_INVALID_ARG;
+    return fdas_launch_quick_cast(p, plane_bf16_dev, plane_f32_dev, (long long)batch * p->K * p->M, (cudaStream_t)stream);
 }
 
 extern "C" int fdas_plan_destroy(fdas_plan_t *p)
@@ -134,7 +162,7 @@ extern "C" int fdas_plan_info(const fdas_plan_t *p, fdas_info_t *info)
     info->precision = p->precision;
     info->n_segments = p->n_seg;
     info->plane_row_pitch = p->M;
-    info->plane_elem_bytes = p->precision == FDAS_F64 ? 8 : 4;
+    info->plane_elem_bytes = fdas_plane_elem_bytes(p);
     info->spectrum_elem_bytes = p->precision == FDAS_F64 ? 16 : 8;
     info->bank_bytes = p->bank_bytes;
     return FDAS_OK;
@@ -224,7 +252,7 @@ extern "C" int fdas_search(fdas_plan_t *p, const void *spectrum_dev, void *plane
 static int ensure_staging(fdas_plan *p, bool want_plane, int peaks_capacity)
 {
     const size_t spec_bytes = (size_t)p->M * (p->precision == FDAS_F64 ? 16 : 8);
-    const size_t plane_bytes = (size_t)p->K * p->M * (p->precision == FDAS_F64 ? 8 : 4);
+    const size_t plane_bytes = (size_t)p->K * p->M * fdas_plane_elem_bytes(p);
     if (!p->stage_spectrum) FDAS_CUDA_TRY(p, cudaMalloc(&p->stage_spectrum, spec_bytes));
     if (want_plane && !p->stage_plane) FDAS_CUDA_TRY(p, cudaMalloc(&p->stage_plane, plane_bytes));
     if (!p->stage_count) FDAS_CUDA_TRY(p, cudaMalloc((void **)&p->stage_count, sizeof(int)));
@@ -247,7 +275,7 @@ extern "C" int fdas_convolve_host(fdas_plan_t *p, const void *spectrum_host, voi
     int rc = ensure_staging(p, true, 0);
     if (rc) return rc;
     const size_t spec_bytes = (size_t)p->M * (p->precision == FDAS_F64 ? 16 : 8);
-    const size_t plane_bytes = (size_t)p->K * p->M * (p->precision == FDAS_F64 ? 8 : 4);
+    const size_t plane_bytes = (size_t)p->K * p->M * fdas_plane_elem_bytes(p);
     FDAS_CUDA_TRY(p, cudaMemcpyAsync(p->stage_spectrum, spectrum_host, spec_bytes, cudaMemcpyHostToDevice, st));
     rc = fdas_launch_convolve(p, p->stage_spectrum, p->stage_plane, 1, st);
     if (rc) return rc;

@@ -19,6 +19,8 @@ PRECISIONS = {"f64": FDAS_F64, "f32": FDAS_F32, "bf16": FDAS_BF16}
 FDAS_ALGO_AUTO, FDAS_ALGO_FFT, FDAS_ALGO_MMA, FDAS_ALGO_MMA_SCALAR = 0, 1, 2, 3
 ALGORITHMS = {"auto": FDAS_ALGO_AUTO, "fft": FDAS_ALGO_FFT, "mma": FDAS_ALGO_MMA,
               "mma_scalar": FDAS_ALGO_MMA_SCALAR}
+FDAS_PLANE_F32, FDAS_PLANE_BF16 = 0, 1
+PLANE_FORMATS = {"f32": FDAS_PLANE_F32, "bf16": FDAS_PLANE_BF16}
 
 EXPORTS = [
     "fdas_plan_create", "fdas_plan_destroy", "fdas_plan_info", "fdas_z_of_index",
@@ -26,6 +28,7 @@ EXPORTS = [
     "fdas_convolve_host", "fdas_search_host", "fdas_templates_host", "fdas_taps_host",
     "fdas_launch_count", "fdas_status_string", "fdas_last_cuda_error",
     "fdas_set_algorithm", "fdas_get_algorithm", "fdas_tapmatrix_host", "fdas_search",
+    "fdas_set_plane_format", "fdas_get_plane_format", "fdas_quick_cast",
 ]
 
 
@@ -75,6 +78,9 @@ def lib() -> ctypes.CDLL:
     L.fdas_set_algorithm.argtypes = [vp, i]
     L.fdas_get_algorithm.argtypes = [vp, ctypes.POINTER(i)]
     L.fdas_launch_count.argtypes = [vp, ctypes.POINTER(i64)]
+    L.fdas_set_plane_format.argtypes = [vp, i]
+    L.fdas_get_plane_format.argtypes = [vp, ctypes.POINTER(i)]
+    L.fdas_quick_cast.argtypes = [vp, vp, vp, i, vp]
     L.fdas_status_string.argtypes = [i]
     L.fdas_status_string.restype = ctypes.c_char_p
     L.fdas_last_cuda_error.argtypes = [vp]
@@ -175,6 +181,20 @@ def fdas_get_algorithm(h):
     return rc, a.value
 
 
+def fdas_set_plane_format(h, fmt):
+    return lib().fdas_set_plane_format(h, int(fmt))
+
+
+def fdas_get_plane_format(h):
+    out = ctypes.c_int(0)
+    rc = lib().fdas_get_plane_format(h, ctypes.byref(out))
+    return rc, out.value
+
+
+def fdas_quick_cast(h, plane_bf16_ptr, plane_f32_ptr, batch=1, stream=0):
+    return lib().fdas_quick_cast(h, plane_bf16_ptr, plane_f32_ptr, int(batch), stream)
+
+
 def fdas_launch_count(h):
     n = ctypes.c_int64()
     rc = lib().fdas_launch_count(h, ctypes.byref(n))
@@ -195,7 +215,7 @@ class Plan:
     torch's; all arithmetic is the library's)."""
 
     def __init__(self, N: int, zmax: float, dz: float, seglen: int, precision="f32", build: bool = True,
-                 stream: int = 0, algorithm="auto"):
+                 stream: int = 0, algorithm="auto", plane="f32"):
         prec = PRECISIONS[precision] if isinstance(precision, str) else int(precision)
         rc, self._h = fdas_plan_create(N, zmax, dz, seglen, prec)
         if rc:
@@ -207,6 +227,11 @@ class Plan:
         algo = ALGORITHMS[algorithm] if isinstance(algorithm, str) else int(algorithm)
         if algo != FDAS_ALGO_AUTO:
             self._check(fdas_set_algorithm(self._h, algo), "fdas_set_algorithm")
+        self.plane_format = PLANE_FORMATS[plane] if isinstance(plane, str) else int(plane)
+        if self.plane_format != FDAS_PLANE_F32:
+            self._check(fdas_set_plane_format(self._h, self.plane_format), "fdas_set_plane_format")
+            rc, self.info = fdas_plan_info(self._h)
+            self._check(rc, "fdas_plan_info")
         if build:
             self.build_templates(stream)
 
@@ -227,7 +252,23 @@ class Plan:
 
     def plane_dtype(self):
         import torch
+        if self.plane_format == FDAS_PLANE_BF16:
+            return torch.bfloat16          # the library writes bf16 bit patterns; torch reads them as bfloat16
         return torch.float64 if self.precision == FDAS_F64 else torch.float32
+
+    def quick_cast(self, plane_bf16, out=None, stream: Optional[int] = None):
+        """fdas_quick_cast: bf16-stored plane(s) -> float32 by byte placement."""
+        import torch
+        assert plane_bf16.is_cuda and plane_bf16.is_contiguous() and plane_bf16.dtype == torch.bfloat16
+        assert tuple(plane_bf16.shape[-2:]) == (self.K, self.M)
+        batch = 1 if plane_bf16.dim() == 2 else plane_bf16.shape[0]
+        if out is None:
+            out = torch.empty(plane_bf16.shape, dtype=torch.float32, device=plane_bf16.device)
+        assert out.is_cuda and out.is_contiguous() and out.dtype == torch.float32 and out.shape == plane_bf16.shape
+        if stream is None:
+            stream = torch.cuda.current_stream().cuda_stream
+        self._check(fdas_quick_cast(self._h, plane_bf16.data_ptr(), out.data_ptr(), batch, stream), "fdas_quick_cast")
+        return out
 
     def spectrum_dtype(self):
         import torch
