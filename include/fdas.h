@@ -49,7 +49,8 @@ typedef struct fdas_plan fdas_plan_t; /* opaque */
 /* Arithmetic / storage variant. */
 typedef enum {
     FDAS_F64 = 0,  /* complex128 spectrum, fp64 bank and FFTs, double plane              */
-    FDAS_F32 = 1,  /* complex64 spectrum, fp32 bank and FFTs, float plane                */
+    FDAS_F32 = 1,  /* complex64 spectrum, fp32 templates, fp32 accumulation, float plane; see
+                      fdas_set_algorithm for the two evaluation orders                     */
     FDAS_BF16 = 2  /* complex64 spectrum rounded to bf16 on load (RNE), bf16 templates, fp32
                       accumulation, float plane ("bf16 storage / fp32 accumulate"; DESIGN.md
                       reading A12); see fdas_set_algorithm for the two evaluation orders     */
@@ -57,10 +58,12 @@ typedef enum {
 
 /* How fdas_convolve evaluates the convolution (fdas_set_algorithm). */
 typedef enum {
-    FDAS_ALGO_AUTO = 0, /* default: FDAS_ALGO_MMA where it applies (FDAS_BF16), else FDAS_ALGO_FFT */
+    FDAS_ALGO_AUTO = 0, /* default: FDAS_ALGO_MMA where it applies (FDAS_BF16; FDAS_F32 with M % 4 == 0),
+                           else FDAS_ALGO_FFT                                                  */
     FDAS_ALGO_FFT = 1,  /* overlap-save FFTs on the fp32/fp64 ALUs, all precisions */
-    FDAS_ALGO_MMA = 2,  /* FDAS_BF16 only: the same linear convolution as a bf16 x bf16 -> fp32
-                           tensor-core contraction over the taps (tcgen05), no FFT            */
+    FDAS_ALGO_MMA = 2,  /* FDAS_BF16 and FDAS_F32: the same linear convolution as a tensor-core
+                           contraction over the taps (tcgen05, bf16 operands, fp32 accumulation), no
+                           FFT.  FDAS_F32 splits every fp32 operand into two bf16 terms            */
     FDAS_ALGO_MMA_SCALAR = 3 /* FDAS_ALGO_MMA with the plane written by per-thread stores instead of
                            shared-memory staging + bulk copies: the form FDAS_ALGO_MMA falls back
                            to when M % 4 != 0.  Same arithmetic, bit-identical plane; selectable
@@ -128,12 +131,19 @@ int fdas_plan_create(fdas_plan_t **out, int64_t N, double zmax, double dz, int s
  * (PAPER.md:35, :59).  Both algorithms compute the same plane; they differ in rounding points:
  *   FDAS_ALGO_FFT  overlap-save FFTs; in FDAS_BF16 the spectrum, the FFT'd
  *                  bank and every inter-pass exchange are rounded to bf16.
- *   FDAS_ALGO_MMA  FDAS_BF16 only.  The spectrum and the taps h_z[j] are rounded to bf16 once
- *                  (RNE) and the sum over the <= 2 m_max + 1 taps runs on the tensor cores with
- *                  fp32 accumulation ("bf16 storage / fp32 accumulate", north_star).  Needs
+ *   FDAS_ALGO_MMA  FDAS_BF16: the spectrum and the taps h_z[j] are rounded to bf16 once (RNE) and
+ *                  the sum over the <= 2 m_max + 1 taps runs on the tensor cores with fp32
+ *                  accumulation ("bf16 storage / fp32 accumulate", north_star).  Needs
  *                  m_max <= 255.
- * Errors: INVALID_ARG (NULL, unknown value), UNSUPPORTED (FDAS_ALGO_MMA on a plan that is not
- * FDAS_BF16 or whose taps do not fit).  fdas_get_algorithm reports the algorithm fdas_convolve
+ *                  FDAS_F32: spectrum and fp32 taps are each split exactly into bf16 terms,
+ *                  x = x1 + x2 + r with x1 = bf16(x), x2 = bf16(x - x1), |r| <= 2^-17 |x|, and the
+ *                  three leading products x1 h1 + x1 h2 + x2 h1 are accumulated in fp32; the
+ *                  dropped terms are <= 2^-17 of each product, an order of magnitude inside the
+ *                  fp32 tolerance (|dP| <= 1e-4 P_peak + 1e-4; measured 3e-6 P_peak).  Needs
+ *                  M % 4 == 0 (16-byte aligned plane rows); other sizes run FDAS_ALGO_FFT.
+ * Errors: INVALID_ARG (NULL, unknown value), UNSUPPORTED (FDAS_ALGO_MMA on an FDAS_F64 plan, on
+ * an FDAS_F32 plan with M % 4 != 0, or on a plan whose taps do not fit; FDAS_ALGO_MMA_SCALAR on
+ * anything but FDAS_BF16).  fdas_get_algorithm reports the algorithm fdas_convolve
  * will run (FDAS_ALGO_FFT, FDAS_ALGO_MMA or FDAS_ALGO_MMA_SCALAR, never AUTO).
  */
 int fdas_set_algorithm(fdas_plan_t *p, int algorithm);

@@ -425,7 +425,11 @@ int launch_prec(fdas_plan *p, const ConvParams &cp, int batch, int groups, cudaS
 
 int fdas_launch_convolve(fdas_plan *p, const void *spectra, void *planes, int batch, cudaStream_t st)
 {
-    if (fdas_uses_mma(p)) return fdas_launch_convolve_mma(p, spectra, planes, batch, st);
+    if (fdas_uses_mma(p)) {
+        const int rc = fdas_launch_convolve_mma(p, spectra, planes, batch, st);
+        // fp32 under FDAS_ALGO_AUTO: a plane buffer the split-operand kernel cannot take goes to the FFT kernel
+        if (!(rc == FDAS_ERR_UNSUPPORTED && p->precision == FDAS_F32 && p->algo == FDAS_ALGO_AUTO)) return rc;
+    }
     ConvParams cp;
     cp.spectra = spectra;
     cp.planes = planes;

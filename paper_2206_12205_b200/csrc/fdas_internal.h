@@ -123,7 +123,10 @@ int fdas_launch_resolve(fdas_plan *p, const void *plane, const fdas_search_args 
 // true when fdas_convolve runs the tensor-core kernel for this plan
 static inline int fdas_uses_mma(const fdas_plan *p)
 {
-    return p->precision == FDAS_BF16 && p->tc_supported && p->algo != FDAS_ALGO_FFT;
+    if (!p->tc_supported || p->algo == FDAS_ALGO_FFT) return 0;
+    if (p->precision == FDAS_BF16) return 1;
+    // fp32 variant: split-operand form (bf16 x 3), box stores only -> 16-byte aligned plane rows
+    return p->precision == FDAS_F32 && p->M % 4 == 0 && !p->tc_force_scalar_stores;
 }
 int fdas_launch_peaks(fdas_plan *p, const void *plane, float thr, fdas_peak_t *peaks, int capacity,
                       int *count, cudaStream_t st);

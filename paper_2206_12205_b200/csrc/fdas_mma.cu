@@ -381,7 +381,7 @@ __device__ __forceinline__ void umma_commit_elected(uint32_t bar, uint32_t elect
 
 // The MMA warp of both kernels.  Per tile 2 KS MMAs (K steps outermost, so consecutive MMAs
 // alternate between the re and im accumulators), then a commit that signals the epilogue.
-template <int NT>
+template <int NT, int SPLIT = 1>
 __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, uint32_t off_z, uint32_t z_buf_bytes,
                                            uint32_t z_part_bytes, uint32_t z_full, uint32_t z_empty, uint32_t t_full,
                                            uint32_t t_empty, uint32_t tmem_base, uint32_t n_items)
@@ -416,10 +416,20 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
             uint64_t a_re = smem_desc(z_addr + (uint32_t)(tile * TC_TILE) * 16u, 128u, 128u);
             uint64_t a_im = smem_desc(z_addr + z_part_bytes + (uint32_t)(tile * TC_TILE) * 16u, 128u, 128u);
             uint64_t bd = b_desc0;
+            // SPLIT == 3 (fp32 variant): x = x1 + x2, h = h1 + h2 in bf16 terms; x h ~ x1 h1 + x1 h2 + x2 h1
+            // (the dropped x2 h2 is <= 2^-18 |x h|).  Z parts: re1, im1, re2, im2; tap images: h1, h2.
+            const uint32_t b2_off = (2u * (uint32_t)p.KS * b_lbo) >> 4;   // second tap-matrix image
+            const uint32_t a2_off = (2u * z_part_bytes) >> 4;             // re2 / im2 parts
 #pragma unroll 3
             for (int ks = 0; ks < p.KS; ++ks) {
                 umma_bf16_elected(d_re, a_re, bd, idesc, ks > 0, elected);
                 umma_bf16_elected(d_im, a_im, bd, idesc, ks > 0, elected);
+                if (SPLIT == 3) {
+                    umma_bf16_elected(d_re, a_re, bd + b2_off, idesc, 1, elected);
+                    umma_bf16_elected(d_im, a_im, bd + b2_off, idesc, 1, elected);
+                    umma_bf16_elected(d_re, a_re + a2_off, bd, idesc, 1, elected);
+                    umma_bf16_elected(d_im, a_im + a2_off, bd, idesc, 1, elected);
+                }
                 a_re += 256u >> 4;
                 a_im += 256u >> 4;
                 bd += (2u * b_lbo) >> 4;
@@ -456,11 +466,17 @@ __device__ __forceinline__ void loader_fetch(const TcParams &p, uint32_t it, uin
     }
 }
 
+// residual of the bf16 rounding: x - bf16(x) is exact in fp32 (x has 24 significant bits, bf16(x) the top 8)
+__device__ __forceinline__ float bf16_residual(float x) { return x - __bfloat162float(__float2bfloat16_rn(x)); }
+
+template <int SPLIT = 1>
 __device__ __forceinline__ void spectrum_loader(const TcParams &p, unsigned char *smem, uint32_t off_xs,
                                                 uint32_t xs_part_bytes, uint32_t xn, uint32_t off_z, uint32_t z_buf_bytes,
                                                 uint32_t z_part_bytes, uint32_t zr, uint32_t z_full, uint32_t z_empty,
                                                 int lt, uint32_t n_items)
 {
+    // sample planes: re, im of the bf16 spectrum; SPLIT == 3 adds re, im of the rounded residual (parts 2, 3)
+    constexpr int NP = SPLIT == 3 ? 4 : 2;
     uint32_t *xs_re = reinterpret_cast<uint32_t *>(smem + off_xs);
     uint32_t *xs_im = reinterpret_cast<uint32_t *>(smem + off_xs + xs_part_bytes);
     float2 a[TC_LD_ITERS], b[TC_LD_ITERS];
@@ -475,6 +491,10 @@ __device__ __forceinline__ void spectrum_loader(const TcParams &p, unsigned char
             if (pi < xn / 2) {
                 xs_re[pi] = pack_bf16(a[i].x, b[i].x);
                 xs_im[pi] = pack_bf16(a[i].y, b[i].y);
+                if (SPLIT == 3) {
+                    xs_re[pi + xs_part_bytes / 2] = pack_bf16(bf16_residual(a[i].x), bf16_residual(b[i].x));
+                    xs_im[pi + xs_part_bytes / 2] = pack_bf16(bf16_residual(a[i].y), bf16_residual(b[i].y));
+                }
             }
         }
         named_bar_sync(1, TC_LOAD_THREADS);
@@ -484,8 +504,8 @@ __device__ __forceinline__ void spectrum_loader(const TcParams &p, unsigned char
         unsigned char *zb = smem + off_z + buf * z_buf_bytes;
         for (uint32_t row = lt; row < zr; row += TC_LOAD_THREADS) {
 #pragma unroll
-            for (int part = 0; part < 2; ++part) {
-                const uint32_t *w = (part ? xs_im : xs_re) + (row >> 1);
+            for (int part = 0; part < NP; ++part) {
+                const uint32_t *w = xs_re + part * (xs_part_bytes / 4) + (row >> 1);
                 uint4 o;
                 if (row & 1) {
                     const uint32_t w0 = w[0], w1 = w[1], w2 = w[2], w3 = w[3], w4 = w[4];
@@ -607,10 +627,10 @@ __global__ void __launch_bounds__(TC_THREADS, 1) fdas_mma_convolve_kernel(const 
 // fdas_mma_bulk_kernel: the same loader and MMA issuer; the epilogue stages the powers in
 // shared memory and writes the plane with bulk copies.
 // =====================================================================================
-constexpr int TB_EPI_WARPS = 16;        // 4 TMEM lane quarters x 4 column groups
-constexpr int TB_MMA_WARP = 16;
-constexpr int TB_LOAD_WARP0 = 17;
-constexpr int TB_THREADS = 32 * (TB_EPI_WARPS + 1 + TC_LOAD_WARPS);   // 640
+// warp roles: 8 SETS epilogue warps (4 TMEM lane quarters x 2 halves per set), then the MMA warp, then the loader
+__host__ __device__ constexpr int tb_sets(int split) { return split == 3 ? 1 : 2; }
+__host__ __device__ constexpr int tb_epi_warps(int split) { return 8 * tb_sets(split); }
+__host__ __device__ constexpr int tb_threads(int split) { return 32 * (tb_epi_warps(split) + 1 + TC_LOAD_WARPS); }   // 640 / 384
 constexpr int TB_CGROUPS = 4;           // column groups: NCH entry pairs (4 NCH columns per part) each
 constexpr int TB_BOXES = FDAS_TC_MAX_BOXES;   // tensor maps, one per distinct run length (plan->tc_box_heights)
 struct TbMaps {
@@ -622,21 +642,24 @@ struct TbMaps {
 struct TbSmem {
     uint32_t b_bytes, zr, z_part_bytes, z_buf_bytes, xn, xs_part_bytes, slots, stage_cg_bytes;
     uint32_t off_z, off_xs, off_stage, off_bars, off_holder, total;
-    __host__ __device__ TbSmem(int R, int KS, int NT, int rowb)
+    // split = 1: bf16 operands; split = 3: the fp32 variant, every operand split into two bf16 terms
+    // (two tap-matrix images, four Z parts) and one epilogue warp set (one staging buffer per column group)
+    __host__ __device__ TbSmem(int R, int KS, int NT, int rowb, int split)
     {
         const uint32_t TP = 16u * KS;
-        b_bytes = 2u * KS * NT * 16u;
+        const uint32_t nb = split == 3 ? 2u : 1u, np = 2u * nb, sets = split == 3 ? 1u : 2u;
+        b_bytes = 2u * KS * NT * 16u;               // one tap-matrix image
         zr = R + TP - 8;
         z_part_bytes = zr * 16u;
-        z_buf_bytes = 2u * z_part_bytes;
+        z_buf_bytes = np * z_part_bytes;
         xn = R + TP;
         xs_part_bytes = xn * 2u;
         slots = (uint32_t)NT / 4u;                 // 4 NCH
         stage_cg_bytes = slots * (uint32_t)rowb;   // one buffer of one column group
-        off_z = b_bytes;
+        off_z = nb * b_bytes;
         off_xs = off_z + 2u * z_buf_bytes;
-        off_stage = (off_xs + 2u * xs_part_bytes + 127u) & ~127u;
-        off_bars = (off_stage + 2u * TB_CGROUPS * stage_cg_bytes + 15u) & ~15u;
+        off_stage = (off_xs + np * xs_part_bytes + 127u) & ~127u;
+        off_bars = (off_stage + sets * TB_CGROUPS * stage_cg_bytes + 15u) & ~15u;
         off_holder = off_bars + 8u * 8u;
         total = off_holder + 16u;
     }
@@ -726,15 +749,17 @@ template <int N>
 __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 
-template <int NCH, typename OT>
-__global__ void __launch_bounds__(TB_THREADS, 1)
+template <int NCH, typename OT, int SPLIT>
+__global__ void __launch_bounds__(tb_threads(SPLIT), 1)
 fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
 {
+    constexpr int SETS = tb_sets(SPLIT), TB_EPI_WARPS = tb_epi_warps(SPLIT), TB_MMA_WARP = TB_EPI_WARPS,
+                  TB_LOAD_WARP0 = TB_EPI_WARPS + 1, TB_THREADS = tb_threads(SPLIT);
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int NT = 16 * NCH;
     constexpr int NC = 4 * NCH;            // columns per part per column group = staging rows (slots)
     constexpr uint32_t ROWB = TC_TILE * sizeof(OT);   // bytes of one staging row
-    const TbSmem L(p.R, p.KS, NT, ROWB);
+    const TbSmem L(p.R, p.KS, NT, ROWB, SPLIT);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int grp = blockIdx.y;
     const uint32_t n_items = (uint32_t)p.batch * (uint32_t)p.n_blocks;
@@ -746,9 +771,12 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
 
     // ---- one-time setup: tap matrix image -> shared memory, barriers, TMEM
     {
-        const uint4 *src = p.bmat + (size_t)grp * (L.b_bytes / 16);
+        // tap-matrix image(s) of this template group: bmat is [image][group][...]
         uint4 *dst = reinterpret_cast<uint4 *>(smem);
-        for (uint32_t i = threadIdx.x; i < L.b_bytes / 16; i += TB_THREADS) dst[i] = __ldg(src + i);
+        for (int img = 0; img < (SPLIT == 3 ? 2 : 1); ++img) {
+            const uint4 *src = p.bmat + ((size_t)img * gridDim.y + grp) * (L.b_bytes / 16);
+            for (uint32_t i = threadIdx.x; i < L.b_bytes / 16; i += TB_THREADS) dst[img * (L.b_bytes / 16) + i] = __ldg(src + i);
+        }
         fence_proxy_async();
     }
     if (threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0 && p.search.enabled) {
@@ -760,7 +788,7 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
             mbar_init(z_full + 8 * s, TC_LOAD_THREADS);
             mbar_init(z_empty + 8 * s, 1);
             mbar_init(t_full + 8 * s, 1);
-            mbar_init(t_empty + 8 * s, TB_EPI_WARPS / 2);   // the warp set that owns stage s
+            mbar_init(t_empty + 8 * s, 8);   // the eight epilogue warps that read stage s
         }
         fence_barrier_init();
     }
@@ -775,7 +803,7 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
         // Two warp sets take alternate tiles (set = TMEM stage), so that one set's chain
         // TMEM load -> powers -> staging -> fence -> barrier -> store issue overlaps the other's.
         // Inside a set, warp (q, half) owns TMEM lane quarter q and column groups 2 half, 2 half + 1.
-        const int q = warp & 3, half = (warp >> 2) & 1, set = warp >> 3;
+        const int q = warp & 3, half = (warp >> 2) & 1, set = warp >> 3;   // SETS == 1: set = 0 takes every tile
         const int lt = q * 32 + lane;                       // bin inside the tile = TMEM lane
         const float thr = p.search.enabled ? p.search.thr : __int_as_float(0x7f800000);
         // Staging rows of a column group (NC = 4 NCH rows of 128 bins): the -|z| rows of its entries
@@ -786,7 +814,6 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
         // UTMASTG costs its issuing warp ~220 cycles (measured), which must not serialise.
         const bool issuer = q < 2 && lane == 0;
         const int bar_id = 2 + 2 * set + half;              // the 128 threads (set, half)
-        const uint32_t stage = set;
         // the row runs of this warp's two column groups, read once: nothing inside the tile loop may touch
         // global memory (a load behind the saturated write stream stalls its warp, and with it the barrier
         // of its staging block, for thousands of cycles)
@@ -798,8 +825,9 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
             const long long left = p.M - blk0;
             const int n_tiles = (int)((left < p.R ? left : p.R) + TC_TILE - 1) / TC_TILE;
             for (int tile = 0; tile < n_tiles; ++tile, ++t) {
-                if ((t & 1) != stage) continue;
-                const uint32_t use = t >> 1;
+                if (SETS == 2 && (int)(t & 1) != set) continue;
+                const uint32_t stage = t & 1, use = t >> 1;
+                const uint32_t sblk = SETS == 2 ? stage : 0;   // staging buffer of this tile (per column group)
                 const long long col0 = blk0 + tile * TC_TILE;
                 const uint32_t taddr0 = tmem_base + ((uint32_t)(q * 32) << 16) + stage * TC_STAGE_COLS;
                 TR(t, 0);
@@ -877,7 +905,7 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
                     TR(t, 3 + 5 * pass);
                     named_bar_sync(bar_id, 128);
                     TR(t, 4 + 5 * pass);
-                    unsigned char *const stage_buf = smem + L.off_stage + (size_t)(2 * cg + stage) * L.stage_cg_bytes;
+                    unsigned char *const stage_buf = smem + L.off_stage + (size_t)(SETS * cg + sblk) * L.stage_cg_bytes;
                     OT *const sb = reinterpret_cast<OT *>(stage_buf) + lt;
 #pragma unroll
                     for (int pr = 0; pr < NCH; ++pr) {
@@ -912,12 +940,12 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
         if (issuer) bulk_wait_all();
     } else if (warp == TB_MMA_WARP) {
         // =========================== MMA issuer ===========================
-        mma_issuer<NT>(p, s_base, L.off_z, L.z_buf_bytes, L.z_part_bytes, z_full, z_empty, t_full, t_empty,
-                       __shfl_sync(0xffffffffu, tmem_base, 0), n_items);
+        mma_issuer<NT, SPLIT>(p, s_base, L.off_z, L.z_buf_bytes, L.z_part_bytes, z_full, z_empty, t_full, t_empty,
+                              __shfl_sync(0xffffffffu, tmem_base, 0), n_items);
     } else {
         // =========================== loader ===========================
-        spectrum_loader(p, smem, L.off_xs, L.xs_part_bytes, L.xn, L.off_z, L.z_buf_bytes, L.z_part_bytes, L.zr, z_full,
-                        z_empty, threadIdx.x - TB_LOAD_WARP0 * 32, n_items);
+        spectrum_loader<SPLIT>(p, smem, L.off_xs, L.xs_part_bytes, L.xn, L.off_z, L.z_buf_bytes, L.z_part_bytes, L.zr, z_full,
+                               z_empty, threadIdx.x - TB_LOAD_WARP0 * 32, n_items);
     }
 
     tc_fence_before();
@@ -933,8 +961,10 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
 // bmat[g][q][n][e], kappa = 8 q + e, j = M0 - kappa: bf16(RNE, once from fp64) of h_{+|z|}[j] for
 // |z| index zi = g*nzg + 2 (n/4) + (n & 1), real part if (n & 2) == 0 else imaginary; zero padding.
 // kref[g][zi] = (template whose fp64 taps are read, +1 if its z >= 0 else -1): h_{+|z|} = conj(h_{-|z|}).
+// split != 0 (fp32 variant): the tap is rounded to fp32 first (that variant's storage type, A11) and
+// image 0 holds h1 = bf16(h), image 1 (at bmat + total) h2 = bf16(h - h1).
 __global__ void fdas_tapmatrix_kernel(__nv_bfloat16 *bmat, const double2 *__restrict__ taps, const int2 *__restrict__ kref,
-                                      int groups, int nzg, int NT, int KS, int m_max)
+                                      int groups, int nzg, int NT, int KS, int m_max, int split)
 {
     const size_t total = (size_t)groups * 2 * KS * NT * 8;
     for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
@@ -952,7 +982,14 @@ __global__ void fdas_tapmatrix_kernel(__nv_bfloat16 *bmat, const double2 *__rest
                 v = fdas_tc_column_is_imag(n) ? (double)kr.y * h.y : h.x;
             }
         }
-        bmat[idx] = __double2bfloat16(v);
+        if (!split) {
+            bmat[idx] = __double2bfloat16(v);
+        } else {
+            const float vf = (float)v;
+            const __nv_bfloat16 h1 = __float2bfloat16_rn(vf);
+            bmat[idx] = h1;
+            bmat[total + idx] = __float2bfloat16_rn(vf - __bfloat162float(h1));
+        }
     }
 }
 
@@ -969,7 +1006,7 @@ extern "C" int fdas_debug_trace(void *dst_host)
 // multiple of dz; otherwise every template stands alone.
 int fdas_mma_plan(fdas_plan *p)
 {
-    if (p->precision != FDAS_BF16) return FDAS_OK;
+    if (p->precision != FDAS_BF16 && p->precision != FDAS_F32) return FDAS_OK;
     const int K = p->K;
     const bool symmetric = fabs(-2.0 * p->zmax + (K - 1) * p->dz) <= 1e-9 * (1.0 + p->zmax);
     const int nz = symmetric ? (K + 1) / 2 : K;
@@ -979,6 +1016,8 @@ int fdas_mma_plan(fdas_plan *p)
     const int KS = (2 * p->m_max + 1 + 15) / 16;
     // row offsets k*M are 32-bit plane-element offsets inside the kernel
     p->tc_supported = (KS <= 32 && NT <= 128 && (long long)K * p->M < 0xFFFFFFFFLL);
+    // fp32 variant (two tap images, four Z parts): must fit shared memory at the smallest work item
+    if (p->precision == FDAS_F32 && TbSmem(128, KS, NT, TC_TILE * 4, 3).total > 227u * 1024u) p->tc_supported = 0;
     p->tc_groups = groups;
     p->tc_nzg = nzg;
     p->tc_NT = NT;
@@ -1063,7 +1102,8 @@ int fdas_mma_plan(fdas_plan *p)
             }
             rng[g * 4 + cg] = r;
         }
-    p->tc_bmat_bytes = (size_t)groups * 2 * KS * NT * 16;
+    // one image [groups][2 KS][NT][8] bf16; the fp32 variant keeps two (h1, h2)
+    p->tc_bmat_bytes = (size_t)groups * 2 * KS * NT * 16 * (p->precision == FDAS_F32 ? 2 : 1);
     cudaError_t e;
     if ((e = cudaMalloc(&p->tc_bmat, p->tc_bmat_bytes)) != cudaSuccess ||
         (e = cudaMalloc((void **)&p->tc_ktab, n_tab * sizeof(int2))) != cudaSuccess ||
@@ -1086,11 +1126,12 @@ int fdas_mma_plan(fdas_plan *p)
 
 int fdas_launch_build_tapmatrix(fdas_plan *p, cudaStream_t st)
 {
-    if (p->precision != FDAS_BF16 || !p->tc_supported) return FDAS_OK;
-    const size_t total = p->tc_bmat_bytes / 2;
+    if ((p->precision != FDAS_BF16 && p->precision != FDAS_F32) || !p->tc_supported) return FDAS_OK;
+    const int split = p->precision == FDAS_F32;
+    const size_t total = p->tc_bmat_bytes / 2 / (split ? 2 : 1);
     const int blocks = (int)((total + 255) / 256 < 1024 ? (total + 255) / 256 : 1024);
     fdas_tapmatrix_kernel<<<blocks, 256, 0, st>>>((__nv_bfloat16 *)p->tc_bmat, p->taps, p->tc_kref,
-                                                  p->tc_groups, p->tc_nzg, p->tc_NT, p->tc_KS, p->m_max);
+                                                  p->tc_groups, p->tc_nzg, p->tc_NT, p->tc_KS, p->m_max, split);
     FDAS_CUDA_TRY(p, cudaGetLastError());
     p->launches += 1;
     return FDAS_OK;
@@ -1142,17 +1183,32 @@ static int plane_maps(fdas_plan *p, void *planes, int batch, const TbMaps **out)
     return FDAS_OK;
 }
 
+template <int NCH>
+static int launch_mma_split(fdas_plan *p, const TcParams &tp, unsigned gx, size_t smem_bytes, const TbMaps *maps, cudaStream_t st)
+{
+    auto kern = fdas_mma_bulk_kernel<NCH, float, 3>;
+    static size_t attr_bytes = 0;
+    if (smem_bytes > attr_bytes) {
+        FDAS_CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
+        attr_bytes = smem_bytes;
+    }
+    kern<<<dim3(gx, p->tc_groups), tb_threads(3), smem_bytes, st>>>(tp, *maps);
+    FDAS_CUDA_TRY(p, cudaGetLastError());
+    p->launches += 1;
+    return FDAS_OK;
+}
+
 template <int NCH, typename OT>
 static int launch_mma(fdas_plan *p, const TcParams &tp, unsigned gx, size_t smem_bytes, const TbMaps *maps, cudaStream_t st)
 {
     if (maps) {
-        auto kern = fdas_mma_bulk_kernel<NCH, OT>;
+        auto kern = fdas_mma_bulk_kernel<NCH, OT, 1>;
         static size_t attr_bytes = 0;
         if (smem_bytes > attr_bytes) {
             FDAS_CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
             attr_bytes = smem_bytes;
         }
-        kern<<<dim3(gx, p->tc_groups), TB_THREADS, smem_bytes, st>>>(tp, *maps);
+        kern<<<dim3(gx, p->tc_groups), tb_threads(1), smem_bytes, st>>>(tp, *maps);
     } else {
         auto kern = fdas_mma_convolve_kernel<NCH, OT>;
         static size_t attr_bytes = 0;
@@ -1170,7 +1226,8 @@ static int launch_mma(fdas_plan *p, const TcParams &tp, unsigned gx, size_t smem
 int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, int batch, cudaStream_t st,
                              fdas_search_args *search)
 {
-    if (p->precision != FDAS_BF16 || !p->tc_supported) return FDAS_ERR_UNSUPPORTED;
+    if ((p->precision != FDAS_BF16 && p->precision != FDAS_F32) || !p->tc_supported) return FDAS_ERR_UNSUPPORTED;
+    const int split = p->precision == FDAS_F32 ? 3 : 1;
     // tensor-map stores need 16-byte aligned plane rows: M % 4 == 0 (% 8 for a bf16 plane) and a 16-byte aligned plane
     const uint32_t esz = p->plane_bf16 ? 2u : 4u;
     bool bulk = ((p->M * esz) % 16 == 0) && ((reinterpret_cast<uintptr_t>(planes) & 15u) == 0) && !p->tc_force_scalar_stores &&
@@ -1180,9 +1237,10 @@ int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, in
         bulk = false;
         maps = nullptr;
     }
+    if (split == 3 && !bulk) return FDAS_ERR_UNSUPPORTED;   // the split-operand form exists with box stores only
     const uint32_t smem_cap = 227u * 1024u;
     auto smem_total = [&](int R) -> uint32_t {
-        return bulk ? TbSmem(R, p->tc_KS, p->tc_NT, TC_TILE * esz).total : TcSmem(R, p->tc_KS, p->tc_NT).total;
+        return bulk ? TbSmem(R, p->tc_KS, p->tc_NT, TC_TILE * esz, split).total : TcSmem(R, p->tc_KS, p->tc_NT).total;
     };
     // outputs per work item: the largest of 1024..128 that fits shared memory and leaves at
     // least two items per CTA
@@ -1223,14 +1281,22 @@ int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, in
     if (items >= 0x7FFFFFFFLL) return FDAS_ERR_UNSUPPORTED;   // the kernels count work items in 32 bits
     const unsigned gx = (unsigned)(items < sms_per_group ? items : sms_per_group);
     switch (p->tc_NT / 16) {
-    case 1: return p->plane_bf16 ? launch_mma<1, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<1, float>(p, tp, gx, total, maps, st);
-    case 2: return p->plane_bf16 ? launch_mma<2, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<2, float>(p, tp, gx, total, maps, st);
-    case 3: return p->plane_bf16 ? launch_mma<3, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<3, float>(p, tp, gx, total, maps, st);
-    case 4: return p->plane_bf16 ? launch_mma<4, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<4, float>(p, tp, gx, total, maps, st);
-    case 5: return p->plane_bf16 ? launch_mma<5, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<5, float>(p, tp, gx, total, maps, st);
-    case 6: return p->plane_bf16 ? launch_mma<6, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<6, float>(p, tp, gx, total, maps, st);
-    case 7: return p->plane_bf16 ? launch_mma<7, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<7, float>(p, tp, gx, total, maps, st);
-    case 8: return p->plane_bf16 ? launch_mma<8, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<8, float>(p, tp, gx, total, maps, st);
+    case 1: if (split == 3) return launch_mma_split<1>(p, tp, gx, total, maps, st);
+            return p->plane_bf16 ? launch_mma<1, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<1, float>(p, tp, gx, total, maps, st);
+    case 2: if (split == 3) return launch_mma_split<2>(p, tp, gx, total, maps, st);
+            return p->plane_bf16 ? launch_mma<2, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<2, float>(p, tp, gx, total, maps, st);
+    case 3: if (split == 3) return launch_mma_split<3>(p, tp, gx, total, maps, st);
+            return p->plane_bf16 ? launch_mma<3, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<3, float>(p, tp, gx, total, maps, st);
+    case 4: if (split == 3) return launch_mma_split<4>(p, tp, gx, total, maps, st);
+            return p->plane_bf16 ? launch_mma<4, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<4, float>(p, tp, gx, total, maps, st);
+    case 5: if (split == 3) return launch_mma_split<5>(p, tp, gx, total, maps, st);
+            return p->plane_bf16 ? launch_mma<5, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<5, float>(p, tp, gx, total, maps, st);
+    case 6: if (split == 3) return launch_mma_split<6>(p, tp, gx, total, maps, st);
+            return p->plane_bf16 ? launch_mma<6, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<6, float>(p, tp, gx, total, maps, st);
+    case 7: if (split == 3) return launch_mma_split<7>(p, tp, gx, total, maps, st);
+            return p->plane_bf16 ? launch_mma<7, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<7, float>(p, tp, gx, total, maps, st);
+    case 8: if (split == 3) return launch_mma_split<8>(p, tp, gx, total, maps, st);
+            return p->plane_bf16 ? launch_mma<8, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<8, float>(p, tp, gx, total, maps, st);
     default: return FDAS_ERR_UNSUPPORTED;
     }
 }

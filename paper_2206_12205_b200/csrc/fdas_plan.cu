@@ -99,7 +99,8 @@ extern "C" int fdas_set_algorithm(fdas_plan_t *p, int algorithm)
         algorithm != FDAS_ALGO_MMA_SCALAR)
         return FDAS_ERR_INVALID_ARG;
     const bool mma = algorithm == FDAS_ALGO_MMA || algorithm == FDAS_ALGO_MMA_SCALAR;
-    if (mma && !(p->precision == FDAS_BF16 && p->tc_supported)) return FDAS_ERR_UNSUPPORTED;
+    if (mma && !((p->precision == FDAS_BF16 || (p->precision == FDAS_F32 && p->M % 4 == 0 && algorithm == FDAS_ALGO_MMA)) && p->tc_supported))
+        return FDAS_ERR_UNSUPPORTED;
     if (algorithm == FDAS_ALGO_FFT && p->plane_bf16) return FDAS_ERR_UNSUPPORTED;   // only the tensor-core kernels write a bf16 plane
     p->algo = mma ? FDAS_ALGO_MMA : algorithm;
     p->tc_force_scalar_stores = algorithm == FDAS_ALGO_MMA_SCALAR;
@@ -119,7 +120,7 @@ extern "C" int fdas_set_plane_format(fdas_plan_t *p, int format)
     if (!p) return FDAS_ERR_INVALID_ARG;
     if (format != FDAS_PLANE_F32 && format != FDAS_PLANE_BF16) return FDAS_ERR_INVALID_ARG;
     // a bf16 plane is written by the tensor-core kernels only
-    if (format == FDAS_PLANE_BF16 && !fdas_uses_mma(p)) return FDAS_ERR_UNSUPPORTED;
+    if (format == FDAS_PLANE_BF16 && !(p->precision == FDAS_BF16 && fdas_uses_mma(p))) return FDAS_ERR_UNSUPPORTED;
     if (p->plane_bf16 != (format == FDAS_PLANE_BF16)) {   // the host-path staging plane has the old element size
         cudaFree(p->stage_plane);
         p->stage_plane = NULL;
@@ -235,6 +236,13 @@ static int search_on_device(fdas_plan *p, const void *spectrum_dev, void *plane_
     sa.cand_span = 8;   // overwritten by the convolve launch
     p->search_calls += 1;
     int rc = fdas_launch_convolve_mma(p, spectrum_dev, plane_dev, 1, st, &sa);   // sets sa.cand_span
+    if (rc == FDAS_ERR_UNSUPPORTED && p->precision == FDAS_F32 && p->algo == FDAS_ALGO_AUTO) {
+        // the split-operand kernel cannot take this plane buffer (alignment, shared memory): FFT kernel + peak pass
+        p->search_calls -= 1;
+        rc = fdas_launch_convolve(p, spectrum_dev, plane_dev, 1, st);
+        if (rc) return rc;
+        return fdas_launch_peaks(p, plane_dev, threshold, peaks_dev, capacity, count_dev, st);
+    }
     if (rc) return rc;
     return fdas_launch_resolve(p, plane_dev, sa, peaks_dev, capacity, st);
 }

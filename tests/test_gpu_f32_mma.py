@@ -1,0 +1,66 @@
+"""GPU parity of the fp32 variant's tensor-core form (FDAS_ALGO_MMA on FDAS_F32): every operand
+split into two bf16 terms, three products per tap, fp32 accumulation in TMEM.
+
+Two bars: (i) the north_star fp32 tolerance against the plain oracle (test_gpu_parity covers it on
+all configs in both forms); (ii) element by element against the oracle's direct sum of exactly
+those three terms (tests/split_terms.py), to the fp32-accumulation bound of check_mma -- a wrong or
+missing term shows up at the 1e-3 level, far above it."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2206_12205_b200 import workloads
+from split_terms import split_plane
+from test_gpu_parity import F, THRESH, check_fp32, check_mma, gpu_plane   # noqa: F401  (F is a fixture)
+
+pytestmark = pytest.mark.gpu
+
+
+def test_config1_split_terms_element_by_element(F):
+    w = workloads.config1()
+    plan, P = gpu_plane(F, w, "f32", algorithm="mma")
+    assert plan.algorithm() == "mma"
+    err, tol = check_mma(P.cpu().numpy(), split_plane(w))
+    print(f"config1 fp32/mma vs three-term oracle: max |dP| {err:.3e} (tol {tol:.3e})")
+
+
+@pytest.mark.parametrize("N,zmax,dz,S", [
+    (2 * 5004, 5.0, 2.0, 1024),        # asymmetric grid z = -5..3 (no +-z pairs)
+    (2 * 70004, 200.0, 2.0, 4096),     # K = 201: two template groups, 15 K-steps, smallest work items
+    (2 * 1500, 8.0, 2.0, 256),         # tiny, ragged last tile
+    (2 * 33000, 7.5, 2.5, 1024),       # fractional z step
+    (2 * 4100, 96.0, 2.0, 2048),       # bench bank, last tile of 4 bins
+])
+def test_f32_mma_ragged_and_grouped(F, N, zmax, dz, S):
+    import torch
+    w = workloads.noise_only(N, seed=S + 17, zmax=zmax, dz=dz, seglen=S)
+    plan, P = gpu_plane(F, w, "f32")
+    assert plan.algorithm() == "mma"
+    got = P.cpu().numpy()
+    check_mma(got, split_plane(w))
+    check_fp32(got, oracle.power_plane(w.spectrum, zmax, dz))
+    # bit-reproducible, and the FFT form agrees to the fp32 tolerance
+    assert torch.equal(plan.convolve(torch.from_numpy(w.spectrum).cuda()), P)
+
+
+def test_f32_batched_search_and_host_forms(F):
+    import torch
+    w = workloads.config2()
+    plan = F.Plan(w.N, w.zmax, w.dz, w.seglen, "f32")
+    assert plan.algorithm() == "mma"
+    x = torch.from_numpy(w.spectrum).cuda()
+    P = plan.convolve(x)
+    xb = torch.stack([x, torch.roll(x, 5), x])
+    Pb = plan.convolve(xb)
+    assert torch.equal(Pb[0], P) and torch.equal(Pb[2], P) and not torch.equal(Pb[1], P)
+    # fused search (threshold in the epilogue) == convolve then peaks == the oracle rule on that plane
+    n_ref, rec_ref = plan.peaks(P, THRESH, capacity=1 << 20)
+    P2, n, rec = plan.search(x, THRESH, capacity=1 << 20)
+    assert torch.equal(P2, P) and n == n_ref >= 8
+    assert sorted(map(tuple, rec.tolist())) == sorted(map(tuple, rec_ref.tolist()))
+    n_o, rec_o = oracle.peaks(P.cpu().numpy().astype(np.float64), THRESH)
+    assert sorted((int(a), int(b)) for a, b, _ in rec) == sorted((k, r) for k, r, _ in rec_o)
+    # host-buffer form
+    out = np.empty((plan.K, plan.M), dtype=np.float32)
+    plan.convolve_host(np.ascontiguousarray(w.spectrum), out)
+    assert np.array_equal(out, P.cpu().numpy())

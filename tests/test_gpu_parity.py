@@ -151,9 +151,12 @@ def test_config1_fp64(F, c1):
     check_fp64(P.cpu().numpy(), exp)
 
 
-def test_config1_fp32(F, c1):
+@pytest.mark.parametrize("algo", ["mma", "fft"])
+def test_config1_fp32(F, c1, algo):
+    # fp32 variant in both forms: split-operand tensor-core sum (the default) and overlap-save FFTs
     w, exp = c1
-    _, P = gpu_plane(F, w, "f32")
+    plan, P = gpu_plane(F, w, "f32", algorithm=algo)
+    assert plan.algorithm() == algo
     check_fp32(P.cpu().numpy(), exp)
     got = P.cpu().numpy()
     k, r = np.unravel_index(np.argmax(got), got.shape)
@@ -191,12 +194,13 @@ def c2():
     return w, oracle.power_plane(w.spectrum, w.zmax, w.dz)
 
 
-def test_config2_fp32_full_plane(F, c2):
+@pytest.mark.parametrize("algo", ["mma", "fft"])
+def test_config2_fp32_full_plane(F, c2, algo):
     w, exp = c2
-    _, P = gpu_plane(F, w, "f32")
-    assert tuple(P.shape) == (97, 1 << 19)
+    plan, P = gpu_plane(F, w, "f32", algorithm=algo)
+    assert tuple(P.shape) == (97, 1 << 19) and plan.algorithm() == algo
     err, tol = check_fp32(P.cpu().numpy(), exp)
-    print(f"config2 fp32 max |dP| {err:.3e} (tol {tol:.3e})")
+    print(f"config2 fp32/{algo} max |dP| {err:.3e} (tol {tol:.3e})")
 
 
 @pytest.mark.parametrize("algo", ["mma", "fft"])
@@ -229,10 +233,14 @@ def test_config3_full_size_sampled_windows(F):
     rng = np.random.default_rng(0)
     starts = [0, M - 4096, 3 * V - 2048, 1000 * V - 2048] + [int(s) for s in rng.integers(0, M - 4096, 4)]
     starts += [int(t.r0) - 2048 for t in w.injections[:20:5] if 2048 < t.r0 < M - 4096]
+    assert planf.algorithm() == "mma"                   # the launch configuration bench.py times
+    planfft, Pfft = gpu_plane(F, w, "f32", algorithm="fft")
     p_peak = float(Pf.max().item())
     for s in starts:
         exp = oracle.power_plane(w.spectrum, w.zmax, w.dz, s, s + 4096)
         check_fp32(Pf[:, s:s + 4096].cpu().numpy(), exp, p_peak)
+        check_fp32(Pfft[:, s:s + 4096].cpu().numpy(), exp, p_peak)
+    del Pfft
     # bf16 against fp32 at full size, in the launch configuration bench.py times (auto = mma), and the FFT form
     n, rec = planf.peaks(Pf, THRESH)
     assert n >= 64
@@ -299,11 +307,12 @@ def test_config5_windows_all_precisions(F):
         wins.append(s)
     exps = [oracle.power_plane(w.spectrum, w.zmax, w.dz, s, s + 2 * half) for s in wins]
     # fp32
-    planf, Pf = gpu_plane(F, w, "f32")
-    assert tuple(Pf.shape) == (201, 1 << 22)
-    p_peak = float(Pf.max().item())
-    for s, exp in zip(wins, exps):
-        check_fp32(Pf[:, s:s + 2 * half].cpu().numpy(), exp, p_peak)
+    for algo in ("fft", "mma"):
+        planf, Pf = gpu_plane(F, w, "f32", algorithm=algo)
+        assert tuple(Pf.shape) == (201, 1 << 22) and planf.algorithm() == algo
+        p_peak = float(Pf.max().item())
+        for s, exp in zip(wins, exps):
+            check_fp32(Pf[:, s:s + 2 * half].cpu().numpy(), exp, p_peak)
     # bf16 against fp32
     _, Pb = gpu_plane(F, w, "bf16")
     for s in wins:
@@ -329,7 +338,9 @@ def test_config5_windows_all_precisions(F):
 
 # ------------------------------------------------------------------ edge cases / invariants
 @pytest.mark.parametrize("S,N,zmax", [(256, 2 * 1501, 8.0), (512, 2 * 4099, 20.0), (1024, 2 * 2048, 96.0),
-                                      (2048, 2 * 5000, 20.0), (4096, 2 * 8191, 96.0)])
+                                      (2048, 2 * 5000, 20.0), (4096, 2 * 8191, 96.0),
+                                      # M % 4 == 0: the fp32 variant runs its tensor-core form (ragged last tile)
+                                      (256, 2 * 1500, 8.0), (2048, 2 * 5004, 20.0), (4096, 2 * 8192, 96.0)])
 @pytest.mark.parametrize("prec", ["f32", "f64"])
 def test_ragged_and_odd_sizes(F, S, N, zmax, prec):
     # M odd / not a multiple of V / fewer than two segments; every supported segment length
@@ -457,10 +468,17 @@ def test_mma_deterministic_batched_and_algorithm_switch(F):
     assert float(((Pfft - P1).abs() / P1).mean().item()) < 0.03
     assert F.fdas_set_algorithm(plan._h, F.FDAS_ALGO_AUTO) == 0 and plan.algorithm() == "mma"
     assert F.fdas_set_algorithm(plan._h, 7) == F.FDAS_ERR_INVALID_ARG
+    # fp32: the split-operand tensor-core form is the default where the plane rows are 16-byte aligned
     planf = F.Plan(w.N, w.zmax, w.dz, w.seglen, "f32")
-    assert planf.algorithm() == "fft"
-    assert F.fdas_set_algorithm(planf._h, F.FDAS_ALGO_MMA) == F.FDAS_ERR_UNSUPPORTED
+    assert planf.algorithm() == "mma"
+    assert F.fdas_set_algorithm(planf._h, F.FDAS_ALGO_MMA_SCALAR) == F.FDAS_ERR_UNSUPPORTED
+    assert F.fdas_set_algorithm(planf._h, F.FDAS_ALGO_FFT) == 0 and planf.algorithm() == "fft"
+    assert F.fdas_set_algorithm(planf._h, F.FDAS_ALGO_MMA) == 0 and planf.algorithm() == "mma"
     assert F.fdas_tapmatrix_host(planf._h, 0, 0) == F.FDAS_ERR_INVALID_ARG
+    podd = F.Plan(2 * 4099, 20.0, 2.0, 1024, "f32")                 # odd M: FFT kernel
+    assert podd.algorithm() == "fft" and F.fdas_set_algorithm(podd._h, F.FDAS_ALGO_MMA) == F.FDAS_ERR_UNSUPPORTED
+    pd = F.Plan(w.N, w.zmax, w.dz, w.seglen, "f64")
+    assert pd.algorithm() == "fft" and F.fdas_set_algorithm(pd._h, F.FDAS_ALGO_MMA) == F.FDAS_ERR_UNSUPPORTED
 
 
 def test_mma_zero_input_and_shift_invariance(F):
@@ -574,7 +592,7 @@ def test_error_paths_on_device(F):
     assert F.fdas_convolve(h, x.data_ptr(), P.data_ptr()) == 0
     torch.cuda.synchronize()
     assert float(P.abs().max().item()) == 0.0          # empty input -> empty plane
-    assert F.fdas_launch_count(h)[1] == 4
+    assert F.fdas_launch_count(h)[1] == 5             # taps, bank, twiddles, tap matrix (tensor-core form), convolve
     assert F.fdas_plan_destroy(h) == 0
 
 
