@@ -8,9 +8,11 @@ A step = one pass of the whole hot path over
 spectrum of BASELINE.json config 3 (N = 2^23 samples, 97 templates, segment 2048) through the
 C ABI of libfdas: fdas_search = the convolution (spectrum load, template filter bank, |.|^2,
 plane store) and the threshold / local-maximum peak pass.  Headline variant: bf16 storage /
-fp32 accumulate (the north_star target; tensor-core kernel with the threshold test fused into
-its epilogue); the fp32 variant (overlap-save FFT kernel + peak kernel) and the FFT form of the
-bf16 variant are timed in the same run.  Prints ONE JSON line (rank 0).
+fp32 accumulate with a float plane (the north_star target; tensor-core kernel with the threshold
+test fused into its epilogue).  Timed in the same run and reported under "precisions": the fp32
+variant in its tensor-core form (split operands) and its overlap-save FFT form, the FFT form of
+the bf16 variant, and the bf16-stored plane with the paper's quick cast.  Prints ONE JSON line
+(rank 0).
 
 N > 1: the path shards by independent series (no data-path collective):
 every rank convolves its own config-3-shaped series -> weak scaling.
@@ -203,11 +205,13 @@ def main():
     peaks_pin = torch.empty(PEAK_CAPACITY * 3, dtype=torch.int32).pin_memory()
     sampler = None
 
-    for prec in ("f32", "bf16_fft", "bf16"):          # headline (bf16) last so the clock sample covers it
-        plan = fdas.Plan(w.N, ZMAX, DZ, SEGLEN, prec.split("_")[0], stream=sptr,
-                         algorithm="fft" if prec.endswith("_fft") else "auto")
+    # (name, precision, algorithm, plane format); headline (bf16, float plane) last so the clock sample covers it
+    variants = (("f32_fft", "f32", "fft", "f32"), ("f32", "f32", "auto", "f32"), ("bf16_fft", "bf16", "fft", "f32"),
+                ("bf16_plane16", "bf16", "auto", "bf16"), ("bf16", "bf16", "auto", "f32"))
+    for prec, pname, algo, pfmt in variants:
+        plan = fdas.Plan(w.N, ZMAX, DZ, SEGLEN, pname, stream=sptr, algorithm=algo, plane=pfmt)
         K, M, S, V = plan.K, plan.M, plan.S, int(plan.info.valid_per_seg)
-        plane = torch.empty((K, M), dtype=torch.float32, device="cuda")
+        plane = torch.empty((K, M), dtype=plan.plane_dtype(), device="cuda")
         h = plan._h
 
         def step():
@@ -249,6 +253,18 @@ def main():
                 convolve_only()
                 b.record(stream)
             stream.synchronize()
+            cast_ms = None
+            if pfmt == "bf16":                       # the paper's quick cast of the bf16-stored plane
+                wide = torch.empty((K, M), dtype=torch.float32, device="cuda")
+                evc = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(5)]
+                for a, b in evc:
+                    flush.zero_()
+                    a.record(stream)
+                    plan.quick_cast(plane, wide, stream=sptr)
+                    b.record(stream)
+                stream.synchronize()
+                cast_ms = float(np.mean([a.elapsed_time(b) for a, b in evc]))
+                del wide
         conv_ms = [a.elapsed_time(b) for a, b in evk]
         step_ms = [a.elapsed_time(c) for a, c in ev]
         total_ms = sharding.max_over_ranks(float(sum(step_ms)), device="cuda")
@@ -267,7 +283,7 @@ def main():
         e2e_s = sharding.max_over_ranks(e2e_s, device="cuda")
         results[prec] = dict(K=K, M=M, S=S, V=V, conv_ms=float(np.mean(conv_ms)), conv_ms_min=float(np.min(conv_ms)),
                              step_ms=total_ms / args.steps, launches=launches, n_found=n_found,
-                             e2e_s=e2e_s, n_e2e=n_e2e)
+                             e2e_s=e2e_s, n_e2e=n_e2e, cast_ms=cast_ms, algorithm=plan.algorithm())
         del plane
         plan.close()
 
@@ -279,7 +295,9 @@ def main():
 
     r = results["bf16"]
     rf = results["f32"]
+    rff = results["f32_fft"]
     rb = results["bf16_fft"]
+    rp = results["bf16_plane16"]
     K, M, S, V = r["K"], r["M"], r["S"], r["V"]
     points = K * M
     value = world * points / (r["step_ms"] * 1e-3)
@@ -322,33 +340,54 @@ def main():
                 "h2d_bytes_per_step": int(M * 8), "d2h_bytes_per_step": int(4 + 12 * min(r["n_e2e"], PEAK_CAPACITY)),
                 "api": "fdas_search_host (pinned host spectrum in, peak list out)", "ms_per_step": r["e2e_s"] * 1e3},
         "gpu_launches": int(r["launches"]),
-        "roofline": {"bound": "hbm", "kernel": "fdas_mma_bulk_kernel<7> (fdas_convolve, bf16)", "achieved": achieved,
+        "roofline": {"bound": "hbm", "kernel": "fdas_mma_bulk_kernel<7, float, 1> (fdas_convolve, bf16)", "achieved": achieved,
                      "peak": peak_gbs, "unit": "GB/s", "frac": achieved / peak_gbs, "traffic": traffic,
                      "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
                      "kernel_ms": r["conv_ms"], "kernel_ms_min": r["conv_ms_min"],
                      "frac_of_nominal_8TBs": achieved / 8000.0},
-        "roofline_tensor": {"bound": "tensor", "kernel": "fdas_mma_bulk_kernel<7>", "achieved": mma_flops / (r["conv_ms"] * 1e-3) / 1e12,
+        "roofline_tensor": {"bound": "tensor", "kernel": "fdas_mma_bulk_kernel<7, float, 1>", "achieved": mma_flops / (r["conv_ms"] * 1e-3) / 1e12,
                             "peak": tensor_peak, "unit": "TFLOP/s", "frac": mma_flops / (r["conv_ms"] * 1e-3) / 1e12 / tensor_peak,
                             "flops_per_launch": mma_flops, "peak_source": tensor_src,
                             "count": "issued dense MMA flops: tiles x 2 parts x 9 K-steps x 2*128*112*16 (padding included)"},
-        "roofline_alu_fp32": {"bound": "alu", "kernel": "fdas_convolve_kernel<TraitsF32,2048>",
-                              "achieved": flops / (rf["conv_ms"] * 1e-3) / 1e12, "peak": alu_peak,
-                              "unit": "TFLOP/s", "frac": flops / (rf["conv_ms"] * 1e-3) / 1e12 / alu_peak,
-                              "flops_per_launch": flops, "count": "nominal 5 N log2 N (SURVEY.md 8(d))"},
+        "roofline_tensor_fp32": {"bound": "tensor", "kernel": "fdas_mma_bulk_kernel<7,float,3> (fdas_convolve, fp32 variant: bf16 x 3 split operands)",
+                                 "achieved": 3 * mma_flops / (rf["conv_ms"] * 1e-3) / 1e12, "peak": tensor_peak, "unit": "TFLOP/s",
+                                 "frac": 3 * mma_flops / (rf["conv_ms"] * 1e-3) / 1e12 / tensor_peak, "flops_per_launch": 3 * mma_flops,
+                                 "peak_source": tensor_src, "count": "issued dense MMA flops: 3 products per tap"},
+        "roofline_alu_fp32_fft": {"bound": "alu", "kernel": "fdas_convolve_kernel<TraitsF32,2048>",
+                                  "achieved": flops / (rff["conv_ms"] * 1e-3) / 1e12, "peak": alu_peak,
+                                  "unit": "TFLOP/s", "frac": flops / (rff["conv_ms"] * 1e-3) / 1e12 / alu_peak,
+                                  "flops_per_launch": flops, "count": "nominal 5 N log2 N (SURVEY.md 8(d))"},
         "cpu_baseline": cpu,
         "precisions": {
-            "bf16": {"convolve_ms": r["conv_ms"], "step_ms": r["step_ms"], "points_per_s": points / (r["step_ms"] * 1e-3),
+            "bf16": {"algorithm": r["algorithm"], "convolve_ms": r["conv_ms"], "step_ms": r["step_ms"],
+                     "points_per_s": points / (r["step_ms"] * 1e-3),
                      "convolve_points_per_s": points / (r["conv_ms"] * 1e-3), "hbm_gbs": achieved, "peaks_found": r["n_found"]},
-            "f32": {"convolve_ms": rf["conv_ms"], "step_ms": rf["step_ms"], "points_per_s": points / (rf["step_ms"] * 1e-3),
+            "f32": {"algorithm": rf["algorithm"], "convolve_ms": rf["conv_ms"], "step_ms": rf["step_ms"],
+                    "points_per_s": points / (rf["step_ms"] * 1e-3),
                     "convolve_points_per_s": points / (rf["conv_ms"] * 1e-3),
-                    "hbm_gbs": alg_bytes / (rf["conv_ms"] * 1e-3) / 1e9, "peaks_found": rf["n_found"]},
-            "bf16_fft": {"convolve_ms": rb["conv_ms"], "step_ms": rb["step_ms"],
+                    "hbm_gbs": alg_bytes / (rf["conv_ms"] * 1e-3) / 1e9, "peaks_found": rf["n_found"],
+                    "note": "FDAS_ALGO_MMA on FDAS_F32: operands split into two bf16 terms, three products per tap"},
+            "f32_fft": {"algorithm": rff["algorithm"], "convolve_ms": rff["conv_ms"], "step_ms": rff["step_ms"],
+                        "points_per_s": points / (rff["step_ms"] * 1e-3),
+                        "convolve_points_per_s": points / (rff["conv_ms"] * 1e-3),
+                        "hbm_gbs": alg_bytes / (rff["conv_ms"] * 1e-3) / 1e9, "peaks_found": rff["n_found"],
+                        "note": "FDAS_ALGO_FFT: the overlap-save FFT kernel (PAPER.md:65-67) + separate peak pass"},
+            "bf16_fft": {"algorithm": rb["algorithm"], "convolve_ms": rb["conv_ms"], "step_ms": rb["step_ms"],
                          "points_per_s": points / (rb["step_ms"] * 1e-3),
                          "convolve_points_per_s": points / (rb["conv_ms"] * 1e-3),
                          "hbm_gbs": alg_bytes / (rb["conv_ms"] * 1e-3) / 1e9, "peaks_found": rb["n_found"],
                          "note": "FDAS_ALGO_FFT: the overlap-save FFT kernel with bf16 storage"},
+            "bf16_plane16": {"algorithm": rp["algorithm"], "convolve_ms": rp["conv_ms"], "step_ms": rp["step_ms"],
+                             "quick_cast_ms": rp["cast_ms"], "points_per_s": points / (rp["step_ms"] * 1e-3),
+                             "convolve_points_per_s": points / (rp["conv_ms"] * 1e-3),
+                             "hbm_gbs": algorithmic_bytes(K, M, S, V, plane_elem=2) / (rp["conv_ms"] * 1e-3) / 1e9,
+                             "quick_cast_hbm_gbs": None if not rp["cast_ms"] else 6.0 * points / (rp["cast_ms"] * 1e-3) / 1e9,
+                             "peaks_found": rp["n_found"],
+                             "note": "NEXT-1: bf16-stored plane (PAPER.md:91-93) + fdas_quick_cast timed separately"},
             "bf16_over_fp32_speedup": rf["conv_ms"] / r["conv_ms"],
             "bf16_over_fp32_speedup_whole_step": rf["step_ms"] / r["step_ms"],
+            "bf16_over_fp32_fft_speedup": rff["conv_ms"] / r["conv_ms"],
+            "bf16_fft_over_fp32_fft_speedup": rff["conv_ms"] / rb["conv_ms"],
             "paper_bf16_over_fp32_speedup": "~1.6x on 'NVIDIA Ampere' (PAPER.md:15; context, not the target)",
         },
     }
