@@ -190,6 +190,17 @@ def config5() -> Workload:
     return Workload("config5", N, 200.0, 2.0, 4096, spectrum_of(x), inj, seed)
 
 
+def harmonic_train(N: int, seed: int, r0: float, z: float, power: float, rel_amplitudes, zmax: float = 20.0,
+                   dz: float = 2.0, seglen: int = 1024, noise: bool = True) -> Workload:
+    """One pulse train whose harmonic h = 1.. has amplitude rel_amplitudes[h-1] (relative to the
+    fundamental of coherent power ``power``) and sits at (h r0, h z): input of the harmonic-sum tests."""
+    rng = np.random.default_rng(seed)
+    x = _noise(rng, N) if noise else np.zeros(N, dtype=np.float32)
+    inj = Injection(float(r0), float(z), float(power), 0.0)
+    _add_tone(x, r0, z, power, 0.0, harmonics=[(h + 1, float(a)) for h, a in enumerate(rel_amplitudes)])
+    return Workload("harmonic_train", N, zmax, dz, seglen, spectrum_of(x), [inj], seed)
+
+
 def noise_only(N: int, seed: int, zmax: float = 96.0, dz: float = 2.0, seglen: int = 2048) -> Workload:
     """White-noise series of any length (throughput runs and the chi^2_2 invariant)."""
     rng = np.random.default_rng(seed)
