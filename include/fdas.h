@@ -174,6 +174,23 @@ int fdas_get_plane_format(const fdas_plan_t *p, int *format);
  */
 int fdas_quick_cast(fdas_plan_t *p, const void *plane_bf16_dev, void *plane_f32_dev, int batch, void *stream);
 
+/*
+ * fdas_harmonic_sum -- gather the power of the harmonics of every cell ("diminishing
+ * harmonics at integer multiples of both f and fdot.  The summed height (power) of the peak and
+ * harmonics is typically used to calculate the signal-to-noise ratio").  Plain
+ * definition (reading A23):
+ *      S[k][r] = sum_{h=1..n_harmonics} P[k0 + h (k - k0)][h r],    k0 = (K-1)/2, the row of z = 0,
+ * terms whose row or bin falls outside the plane are skipped.
+ *   plane_dev  [K][M] in the plan's plane format (float, double for FDAS_F64, bf16 bits)
+ *   sum_dev    [K][M] float (double for FDAS_F64), fully overwritten; must not overlap plane_dev
+ *   n_harmonics 1..32 (1 copies / widens the plane)
+ * The result is a plane like any other: fdas_peaks accepts it when the plan's plane format is
+ * float.  Asynchronous on `stream`.
+ * Errors: INVALID_ARG (NULL, n_harmonics out of range), UNSUPPORTED (z = 0 is not a row of the
+ * template grid, i.e. zmax is not a multiple of dz: harmonics would fall between rows), CUDA.
+ */
+int fdas_harmonic_sum(fdas_plan_t *p, const void *plane_dev, void *sum_dev, int n_harmonics, void *stream);
+
 /* Frees the plan and its device memory (synchronises the device first).  NULL is OK. */
 int fdas_plan_destroy(fdas_plan_t *p);
 

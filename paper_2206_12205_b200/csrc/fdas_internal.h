@@ -130,5 +130,7 @@ static inline int fdas_uses_mma(const fdas_plan *p)
 }
 int fdas_launch_peaks(fdas_plan *p, const void *plane, float thr, fdas_peak_t *peaks, int capacity,
                       int *count, cudaStream_t st);
+// fdas_harmonic.cu: S_H[k][r] = sum_h P[k0 + h (k - k0)][h r]
+int fdas_launch_harmonic_sum(fdas_plan *p, const void *plane, void *sum, int n_harmonics, int k0, cudaStream_t st);
 // fdas_cast.cu: the paper's quick cast of a bf16-stored plane
 int fdas_launch_quick_cast(fdas_plan *p, const void *src_bf16, void *dst_f32, long long n, cudaStream_t st);

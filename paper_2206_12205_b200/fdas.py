@@ -28,7 +28,7 @@ EXPORTS = [
     "fdas_convolve_host", "fdas_search_host", "fdas_templates_host", "fdas_taps_host",
     "fdas_launch_count", "fdas_status_string", "fdas_last_cuda_error",
     "fdas_set_algorithm", "fdas_get_algorithm", "fdas_tapmatrix_host", "fdas_search",
-    "fdas_set_plane_format", "fdas_get_plane_format", "fdas_quick_cast",
+    "fdas_set_plane_format", "fdas_get_plane_format", "fdas_quick_cast", "fdas_harmonic_sum",
 ]
 
 
@@ -81,6 +81,7 @@ def lib() -> ctypes.CDLL:
     L.fdas_set_plane_format.argtypes = [vp, i]
     L.fdas_get_plane_format.argtypes = [vp, ctypes.POINTER(i)]
     L.fdas_quick_cast.argtypes = [vp, vp, vp, i, vp]
+    L.fdas_harmonic_sum.argtypes = [vp, vp, vp, i, vp]
     L.fdas_status_string.argtypes = [i]
     L.fdas_status_string.restype = ctypes.c_char_p
     L.fdas_last_cuda_error.argtypes = [vp]
@@ -195,6 +196,10 @@ def fdas_quick_cast(h, plane_bf16_ptr, plane_f32_ptr, batch=1, stream=0):
     return lib().fdas_quick_cast(h, plane_bf16_ptr, plane_f32_ptr, int(batch), stream)
 
 
+def fdas_harmonic_sum(h, plane_ptr, sum_ptr, n_harmonics, stream=0):
+    return lib().fdas_harmonic_sum(h, plane_ptr, sum_ptr, int(n_harmonics), stream)
+
+
 def fdas_launch_count(h):
     n = ctypes.c_int64()
     rc = lib().fdas_launch_count(h, ctypes.byref(n))
@@ -255,6 +260,20 @@ class Plan:
         if self.plane_format == FDAS_PLANE_BF16:
             return torch.bfloat16          # the library writes bf16 bit patterns; torch reads them as bfloat16
         return torch.float64 if self.precision == FDAS_F64 else torch.float32
+
+    def harmonic_sum(self, plane, n_harmonics: int, out=None, stream: Optional[int] = None):
+        """fdas_harmonic_sum: S[k][r] = sum_h P[k0 + h (k - k0)][h r]."""
+        import torch
+        assert plane.is_cuda and plane.is_contiguous() and tuple(plane.shape) == (self.K, self.M)
+        assert plane.dtype == self.plane_dtype()
+        odt = torch.float64 if self.precision == FDAS_F64 else torch.float32
+        if out is None:
+            out = torch.empty((self.K, self.M), dtype=odt, device=plane.device)
+        assert out.is_cuda and out.is_contiguous() and out.dtype == odt and tuple(out.shape) == (self.K, self.M)
+        if stream is None:
+            stream = torch.cuda.current_stream().cuda_stream
+        self._check(fdas_harmonic_sum(self._h, plane.data_ptr(), out.data_ptr(), n_harmonics, stream), "fdas_harmonic_sum")
+        return out
 
     def quick_cast(self, plane_bf16, out=None, stream: Optional[int] = None):
         """fdas_quick_cast: bf16-stored plane(s) -> float32 by byte placement."""
