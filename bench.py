@@ -56,6 +56,13 @@ def algorithmic_bytes(K, M, S, V, plane_elem=4, spec_elem=8):
     return K * M * plane_elem + n_seg * S * spec_elem
 
 
+def hsum_bytes(K, M, H, elem=4):
+    """Elements the harmonic sum must read (rows k0 + h (k - k0) in range, bins h r < M) plus the plane it writes."""
+    k0 = (K - 1) // 2
+    reads = sum((2 * (k0 // h) + 1) * (-(-M // h)) for h in range(1, H + 1))
+    return elem * (reads + K * M)
+
+
 def nominal_flops(K, M, S, V):
     """per segment 5 S log2 S (forward) + K (6S + 5 S log2 S + 3V)."""
     n_seg = -(-M // V)
@@ -265,6 +272,18 @@ def main():
                 stream.synchronize()
                 cast_ms = float(np.mean([a.elapsed_time(b) for a, b in evc]))
                 del wide
+            hsum_ms = None
+            if prec == "bf16":                       # NEXT-3: harmonic sum (4 harmonics) of the headline plane
+                hs = torch.empty((K, M), dtype=torch.float32, device="cuda")
+                evh = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(5)]
+                for a, b in evh:
+                    flush.zero_()
+                    a.record(stream)
+                    plan.harmonic_sum(plane, 4, hs, stream=sptr)
+                    b.record(stream)
+                stream.synchronize()
+                hsum_ms = float(np.mean([a.elapsed_time(b) for a, b in evh]))
+                del hs
         conv_ms = [a.elapsed_time(b) for a, b in evk]
         step_ms = [a.elapsed_time(c) for a, c in ev]
         total_ms = sharding.max_over_ranks(float(sum(step_ms)), device="cuda")
@@ -283,7 +302,7 @@ def main():
         e2e_s = sharding.max_over_ranks(e2e_s, device="cuda")
         results[prec] = dict(K=K, M=M, S=S, V=V, conv_ms=float(np.mean(conv_ms)), conv_ms_min=float(np.min(conv_ms)),
                              step_ms=total_ms / args.steps, launches=launches, n_found=n_found,
-                             e2e_s=e2e_s, n_e2e=n_e2e, cast_ms=cast_ms, algorithm=plan.algorithm())
+                             e2e_s=e2e_s, n_e2e=n_e2e, cast_ms=cast_ms, hsum_ms=hsum_ms, algorithm=plan.algorithm())
         del plane
         plan.close()
 
@@ -384,6 +403,9 @@ def main():
                              "quick_cast_hbm_gbs": None if not rp["cast_ms"] else 6.0 * points / (rp["cast_ms"] * 1e-3) / 1e9,
                              "peaks_found": rp["n_found"],
                              "note": "NEXT-1: bf16-stored plane (PAPER.md:91-93) + fdas_quick_cast timed separately"},
+            "harmonic_sum_4": {"ms": r["hsum_ms"],
+                               "algorithmic_gbs": None if not r["hsum_ms"] else hsum_bytes(K, M, 4) / (r["hsum_ms"] * 1e-3) / 1e9,
+                               "note": "NEXT-3: fdas_harmonic_sum, 4 harmonics, on the headline float plane; bytes = elements read + plane written"},
             "bf16_over_fp32_speedup": rf["conv_ms"] / r["conv_ms"],
             "bf16_over_fp32_speedup_whole_step": rf["step_ms"] / r["step_ms"],
             "bf16_over_fp32_fft_speedup": rff["conv_ms"] / r["conv_ms"],
