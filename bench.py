@@ -347,7 +347,7 @@ def main():
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": r["step_ms"], "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
         "config": {"workload": WORKLOAD,
                    "storage": "bf16 spectrum and taps (RNE), fp32 accumulate on the tensor cores (tcgen05), fp32 plane",
                    "step": "fdas_search = convolve + threshold/local-max peaks (threshold %.1f)" % THRESH,
