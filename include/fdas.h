@@ -191,6 +191,22 @@ int fdas_quick_cast(fdas_plan_t *p, const void *plane_bf16_dev, void *plane_f32_
  */
 int fdas_harmonic_sum(fdas_plan_t *p, const void *plane_dev, void *sum_dev, int n_harmonics, void *stream);
 
+/*
+ * fdas_band_max -- the paper's own peak selection (section 4.3, Table 3): the
+ * plane is split into harmonic bands derived from the fundamental frequency f and "the n-th
+ * harmonic is taken to be the highest point in the n-th band".  Band 0 (fundamental) holds the
+ * bins 0 <= r <= 1.5 f, band n >= 1 the bins (n + 0.5) f < r <= (n + 1.5) f (upper bound
+ * inclusive, Table 3's caption), over all K rows.
+ *   plane_dev  [K][M] in the plan's plane format
+ *   f_bin      fundamental frequency in Fourier bins (f T), > 0
+ *   n_bands    1..32
+ *   out_dev    n_bands records (z_index, r, power); among equal maxima the first in (k, r) order;
+ *              (-1, -1, 0) for a band that lies beyond the plane
+ * Asynchronous on `stream`; scratch memory is owned by the plan (allocated on first use).
+ * Errors: INVALID_ARG, CUDA.
+ */
+int fdas_band_max(fdas_plan_t *p, const void *plane_dev, double f_bin, int n_bands, fdas_peak_t *out_dev, void *stream);
+
 /* Frees the plan and its device memory (synchronises the device first).  NULL is OK. */
 int fdas_plan_destroy(fdas_plan_t *p);
 

@@ -8,6 +8,7 @@
 // Points of the length-S transforms held per thread, and the derived kernel geometry
 // (DESIGN.md section 5):  S = 16 * 16 * R3,  T = S/16 threads per segment.
 #define FDAS_PTS 16
+#define FDAS_MAX_BANDS 32     // harmonic bands one fdas_band_max call can take
 #define FDAS_TC_MAX_BOXES 8   // distinct plane-row run lengths the tensor-core kernel's box stores can serve
 
 struct fdas_plan {
@@ -51,6 +52,9 @@ struct fdas_plan {
     fdas_peak_t *stage_peaks;
     int *stage_count;
     int stage_peaks_capacity;
+    // fdas_band_max: per-block partial maxima
+    void *band_scratch;
+    size_t band_scratch_bytes;
     // bookkeeping
     int device, num_sms;
     cudaError_t last_err;
@@ -132,5 +136,7 @@ int fdas_launch_peaks(fdas_plan *p, const void *plane, float thr, fdas_peak_t *p
                       int *count, cudaStream_t st);
 // fdas_harmonic.cu: S_H[k][r] = sum_h P[k0 + h (k - k0)][h r]
 int fdas_launch_harmonic_sum(fdas_plan *p, const void *plane, void *sum, int n_harmonics, int k0, cudaStream_t st);
+// fdas_bands.cu: Table 3 band maxima
+int fdas_launch_band_max(fdas_plan *p, const void *plane, double f_bin, int n_bands, fdas_peak_t *out, cudaStream_t st);
 // fdas_cast.cu: the paper's quick cast of a bf16-stored plane
 int fdas_launch_quick_cast(fdas_plan *p, const void *src_bf16, void *dst_f32, long long n, cudaStream_t st);

@@ -14,6 +14,7 @@ static void free_device_members(fdas_plan *p)
     cudaFree(p->bank);
     cudaFree(p->taps);
     cudaFree(p->twiddle);
+    cudaFree(p->band_scratch);
     cudaFree(p->tc_bmat);
     cudaFree(p->tc_ktab);
     cudaFree(p->tc_kref);
@@ -149,6 +150,13 @@ extern "C" int fdas_harmonic_sum(fdas_plan_t *p, const void *plane_dev, void *su
     const int k0 = (p->K - 1) / 2;
     if (fabs(-p->zmax + k0 * p->dz) > 1e-9 * (1.0 + p->zmax)) return FDAS_ERR_UNSUPPORTED;
     return fdas_launch_harmonic_sum(p, plane_dev, sum_dev, n_harmonics, k0, (cudaStream_t)stream);
+}
+
+extern "C" int fdas_band_max(fdas_plan_t *p, const void *plane_dev, double f_bin, int n_bands, fdas_peak_t *out_dev, void *stream)
+{
+    if (!p || !plane_dev || !out_dev || n_bands < 1 || n_bands > FDAS_MAX_BANDS || !(f_bin > 0.0) || !(f_bin < 1e15))
+        return FDAS_ERR_INVALID_ARG;
+    return fdas_launch_band_max(p, plane_dev, f_bin, n_bands, out_dev, (cudaStream_t)stream);
 }
 
 extern "C" int fdas_plan_destroy(fdas_plan_t *p)

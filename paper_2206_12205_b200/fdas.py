@@ -28,7 +28,7 @@ EXPORTS = [
     "fdas_convolve_host", "fdas_search_host", "fdas_templates_host", "fdas_taps_host",
     "fdas_launch_count", "fdas_status_string", "fdas_last_cuda_error",
     "fdas_set_algorithm", "fdas_get_algorithm", "fdas_tapmatrix_host", "fdas_search",
-    "fdas_set_plane_format", "fdas_get_plane_format", "fdas_quick_cast", "fdas_harmonic_sum",
+    "fdas_set_plane_format", "fdas_get_plane_format", "fdas_quick_cast", "fdas_harmonic_sum", "fdas_band_max",
 ]
 
 
@@ -82,6 +82,7 @@ def lib() -> ctypes.CDLL:
     L.fdas_get_plane_format.argtypes = [vp, ctypes.POINTER(i)]
     L.fdas_quick_cast.argtypes = [vp, vp, vp, i, vp]
     L.fdas_harmonic_sum.argtypes = [vp, vp, vp, i, vp]
+    L.fdas_band_max.argtypes = [vp, vp, dbl, i, vp, vp]
     L.fdas_status_string.argtypes = [i]
     L.fdas_status_string.restype = ctypes.c_char_p
     L.fdas_last_cuda_error.argtypes = [vp]
@@ -200,6 +201,10 @@ def fdas_harmonic_sum(h, plane_ptr, sum_ptr, n_harmonics, stream=0):
     return lib().fdas_harmonic_sum(h, plane_ptr, sum_ptr, int(n_harmonics), stream)
 
 
+def fdas_band_max(h, plane_ptr, f_bin, n_bands, out_ptr, stream=0):
+    return lib().fdas_band_max(h, plane_ptr, float(f_bin), int(n_bands), out_ptr, stream)
+
+
 def fdas_launch_count(h):
     n = ctypes.c_int64()
     rc = lib().fdas_launch_count(h, ctypes.byref(n))
@@ -274,6 +279,18 @@ class Plan:
             stream = torch.cuda.current_stream().cuda_stream
         self._check(fdas_harmonic_sum(self._h, plane.data_ptr(), out.data_ptr(), n_harmonics, stream), "fdas_harmonic_sum")
         return out
+
+    def band_max(self, plane, f_bin: float, n_bands: int, stream: Optional[int] = None):
+        """fdas_band_max (Table 3): list of (z_index, r, power), one per harmonic band."""
+        import numpy as np
+        import torch
+        assert plane.is_cuda and plane.is_contiguous() and tuple(plane.shape) == (self.K, self.M)
+        if stream is None:
+            stream = torch.cuda.current_stream().cuda_stream
+        buf = torch.empty(3 * n_bands, dtype=torch.int32, device=plane.device)
+        self._check(fdas_band_max(self._h, plane.data_ptr(), f_bin, n_bands, buf.data_ptr(), stream), "fdas_band_max")
+        raw = buf.cpu().numpy().reshape(n_bands, 3)
+        return [(int(a), int(b), float(np.int32(c).view(np.float32))) for a, b, c in raw]
 
     def quick_cast(self, plane_bf16, out=None, stream: Optional[int] = None):
         """fdas_quick_cast: bf16-stored plane(s) -> float32 by byte placement."""
