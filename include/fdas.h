@@ -285,6 +285,21 @@ int fdas_search_host(fdas_plan_t *p, const void *spectrum_host, float threshold,
                      fdas_peak_t *peaks_host, int capacity, int *count_host, void *stream);
 
 /*
+ * fdas_search_host_batched -- survey form of fdas_search_host for many independent series sharing
+ * one plan (BASELINE.json config 4; PAPER.md:295-297 times 256-run batches): series i+1 is copied
+ * host->device on an internal copy stream while series i is searched on `stream`; the plane never
+ * leaves the device (one plane buffer is reused), only the peak lists come back.
+ *   spectra_host  [n_series][M] interleaved complex (pinned memory makes the overlap real)
+ *   peaks_host    [n_series][capacity] records; for series i the first min(counts_host[i], capacity)
+ *                 are valid (the whole slot of `capacity` records is copied: keep capacity modest)
+ *   counts_host   [n_series] total number of peaks found per series (snprintf convention)
+ * Per series the peak SET equals that of fdas_search_host.  Synchronises `stream` before returning.
+ * Errors: INVALID_ARG (NULL, n_series < 1, capacity < 0), NOT_BUILT, ALLOC, CUDA.
+ */
+int fdas_search_host_batched(fdas_plan_t *p, const void *spectra_host, int n_series, float threshold,
+                             fdas_peak_t *peaks_host, int capacity, int *counts_host, void *stream);
+
+/*
  * Debug / test access to the bank: copies H_z[f] in NATURAL order, [K][S] interleaved
  * complex of the storage type (double2 / float2 / 2 x bf16 bit patterns), to host memory.
  * `bytes` must equal K*S*2*sizeof(storage scalar).  Synchronises.

@@ -52,6 +52,13 @@ struct fdas_plan {
     fdas_peak_t *stage_peaks;
     int *stage_count;
     int stage_peaks_capacity;
+    // fdas_search_host_batched: copy stream, events and double-buffered staging of the host pipeline
+    cudaStream_t pipe_stream;
+    cudaEvent_t pipe_ev[3][2];     // [h2d done | search done | d2h done][buffer]
+    void *pipe_spec[2];
+    fdas_peak_t *pipe_peaks[2];
+    int *pipe_count[2];
+    int pipe_capacity, pipe_ready;
     // fdas_band_max: per-block partial maxima
     void *band_scratch;
     size_t band_scratch_bytes;

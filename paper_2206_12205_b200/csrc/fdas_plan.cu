@@ -15,6 +15,16 @@ static void free_device_members(fdas_plan *p)
     cudaFree(p->taps);
     cudaFree(p->twiddle);
     cudaFree(p->band_scratch);
+    if (p->pipe_ready) {
+        cudaStreamDestroy(p->pipe_stream);
+        for (int e = 0; e < 3; ++e)
+            for (int b = 0; b < 2; ++b) cudaEventDestroy(p->pipe_ev[e][b]);
+    }
+    for (int b = 0; b < 2; ++b) {
+        cudaFree(p->pipe_spec[b]);
+        cudaFree(p->pipe_peaks[b]);
+        cudaFree(p->pipe_count[b]);
+    }
     cudaFree(p->tc_bmat);
     cudaFree(p->tc_ktab);
     cudaFree(p->tc_kref);
@@ -331,6 +341,68 @@ extern "C" int fdas_search_host(fdas_plan_t *p, const void *spectrum_host, float
                                          cudaMemcpyDeviceToHost, st));
         FDAS_CUDA_TRY(p, cudaStreamSynchronize(st));
     }
+    return FDAS_OK;
+}
+
+// Survey form of the host path: series i+1 crosses PCIe while series i is searched.
+//   copy stream:    [wait search(i-1)] H2D spectrum(i+1)            [wait search(i)] D2H count(i), peaks(i)
+//   caller stream:  [wait H2D(i)] [wait D2H(i-2)] fdas_search(i)
+extern "C" int fdas_search_host_batched(fdas_plan_t *p, const void *spectra_host, int n_series, float threshold,
+                                        fdas_peak_t *peaks_host, int capacity, int *counts_host, void *stream)
+{
+    if (!p || !spectra_host || !counts_host || n_series < 1 || capacity < 0 || (capacity > 0 && !peaks_host))
+        return FDAS_ERR_INVALID_ARG;
+    if (!p->built) return FDAS_ERR_NOT_BUILT;
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = ensure_staging(p, true, 0);
+    if (rc) return rc;
+    const size_t spec_bytes = (size_t)p->M * (p->precision == FDAS_F64 ? 16 : 8);
+    if (!p->pipe_ready) {
+        FDAS_CUDA_TRY(p, cudaStreamCreateWithFlags(&p->pipe_stream, cudaStreamNonBlocking));
+        for (int e = 0; e < 3; ++e)
+            for (int b = 0; b < 2; ++b) FDAS_CUDA_TRY(p, cudaEventCreateWithFlags(&p->pipe_ev[e][b], cudaEventDisableTiming));
+        p->pipe_ready = 1;
+    }
+    for (int b = 0; b < 2; ++b) {
+        if (!p->pipe_spec[b]) FDAS_CUDA_TRY(p, cudaMalloc(&p->pipe_spec[b], spec_bytes));
+        if (!p->pipe_count[b]) FDAS_CUDA_TRY(p, cudaMalloc((void **)&p->pipe_count[b], sizeof(int)));
+        if (capacity > p->pipe_capacity || !p->pipe_peaks[b]) {
+            cudaFree(p->pipe_peaks[b]);
+            p->pipe_peaks[b] = NULL;
+            FDAS_CUDA_TRY(p, cudaMalloc((void **)&p->pipe_peaks[b], sizeof(fdas_peak_t) * (size_t)(capacity > 0 ? capacity : 1)));
+        }
+    }
+    p->pipe_capacity = capacity;
+    cudaStream_t cs = p->pipe_stream;
+    const unsigned char *src = static_cast<const unsigned char *>(spectra_host);
+    // the pipeline starts after whatever the caller queued on `stream` before this call
+    FDAS_CUDA_TRY(p, cudaEventRecord(p->pipe_ev[1][1], st));
+    FDAS_CUDA_TRY(p, cudaStreamWaitEvent(cs, p->pipe_ev[1][1], 0));
+    FDAS_CUDA_TRY(p, cudaMemcpyAsync(p->pipe_spec[0], src, spec_bytes, cudaMemcpyHostToDevice, cs));
+    FDAS_CUDA_TRY(p, cudaEventRecord(p->pipe_ev[0][0], cs));
+    for (int i = 0; i < n_series; ++i) {
+        const int b = i & 1;
+        FDAS_CUDA_TRY(p, cudaStreamWaitEvent(st, p->pipe_ev[0][b], 0));              // spectrum i is on the device
+        if (i >= 2) FDAS_CUDA_TRY(p, cudaStreamWaitEvent(st, p->pipe_ev[2][b], 0));  // peak buffers b were read back
+        rc = search_on_device(p, p->pipe_spec[b], p->stage_plane, threshold, p->pipe_peaks[b], capacity, p->pipe_count[b], st);
+        if (rc) return rc;
+        FDAS_CUDA_TRY(p, cudaEventRecord(p->pipe_ev[1][b], st));
+        if (i + 1 < n_series) {
+            // spectrum buffer b^1 was last read by search(i-1), already recorded in pipe_ev[1][b^1]
+            if (i >= 1) FDAS_CUDA_TRY(p, cudaStreamWaitEvent(cs, p->pipe_ev[1][b ^ 1], 0));
+            FDAS_CUDA_TRY(p, cudaMemcpyAsync(p->pipe_spec[b ^ 1], src + (size_t)(i + 1) * spec_bytes, spec_bytes,
+                                             cudaMemcpyHostToDevice, cs));
+            FDAS_CUDA_TRY(p, cudaEventRecord(p->pipe_ev[0][b ^ 1], cs));
+        }
+        FDAS_CUDA_TRY(p, cudaStreamWaitEvent(cs, p->pipe_ev[1][b], 0));
+        FDAS_CUDA_TRY(p, cudaMemcpyAsync(counts_host + i, p->pipe_count[b], sizeof(int), cudaMemcpyDeviceToHost, cs));
+        if (capacity > 0)
+            FDAS_CUDA_TRY(p, cudaMemcpyAsync(peaks_host + (size_t)i * capacity, p->pipe_peaks[b],
+                                             sizeof(fdas_peak_t) * (size_t)capacity, cudaMemcpyDeviceToHost, cs));
+        FDAS_CUDA_TRY(p, cudaEventRecord(p->pipe_ev[2][b], cs));
+    }
+    FDAS_CUDA_TRY(p, cudaStreamSynchronize(cs));
+    FDAS_CUDA_TRY(p, cudaStreamSynchronize(st));
     return FDAS_OK;
 }
 

@@ -28,7 +28,7 @@ EXPORTS = [
     "fdas_convolve_host", "fdas_search_host", "fdas_templates_host", "fdas_taps_host",
     "fdas_launch_count", "fdas_status_string", "fdas_last_cuda_error",
     "fdas_set_algorithm", "fdas_get_algorithm", "fdas_tapmatrix_host", "fdas_search",
-    "fdas_set_plane_format", "fdas_get_plane_format", "fdas_quick_cast", "fdas_harmonic_sum", "fdas_band_max",
+    "fdas_set_plane_format", "fdas_get_plane_format", "fdas_quick_cast", "fdas_harmonic_sum", "fdas_band_max", "fdas_search_host_batched",
 ]
 
 
@@ -83,6 +83,7 @@ def lib() -> ctypes.CDLL:
     L.fdas_quick_cast.argtypes = [vp, vp, vp, i, vp]
     L.fdas_harmonic_sum.argtypes = [vp, vp, vp, i, vp]
     L.fdas_band_max.argtypes = [vp, vp, dbl, i, vp, vp]
+    L.fdas_search_host_batched.argtypes = [vp, vp, i, ctypes.c_float, vp, i, vp, vp]
     L.fdas_status_string.argtypes = [i]
     L.fdas_status_string.restype = ctypes.c_char_p
     L.fdas_last_cuda_error.argtypes = [vp]
@@ -203,6 +204,11 @@ def fdas_harmonic_sum(h, plane_ptr, sum_ptr, n_harmonics, stream=0):
 
 def fdas_band_max(h, plane_ptr, f_bin, n_bands, out_ptr, stream=0):
     return lib().fdas_band_max(h, plane_ptr, float(f_bin), int(n_bands), out_ptr, stream)
+
+
+def fdas_search_host_batched(h, spectra_host_ptr, n_series, threshold, peaks_host_ptr, capacity, counts_host_ptr, stream=0):
+    return lib().fdas_search_host_batched(h, spectra_host_ptr, int(n_series), threshold, peaks_host_ptr, int(capacity),
+                                          counts_host_ptr, stream)
 
 
 def fdas_launch_count(h):
@@ -382,6 +388,13 @@ class Plan:
         rc, n = fdas_search_host(self._h, _host_ptr(spectrum_host), threshold, _host_ptr(peaks_host), capacity, stream)
         self._check(rc, "fdas_search_host")
         return n
+
+    def search_host_batched(self, spectra_host, threshold: float, peaks_host, counts_host, capacity: int, stream: int = 0):
+        """spectra_host [B, M]; peaks_host >= B*capacity records (12 bytes each); counts_host [B] int32 (numpy or pinned torch)."""
+        n = int(spectra_host.shape[0])
+        self._check(fdas_search_host_batched(self._h, _host_ptr(spectra_host), n, threshold, _host_ptr(peaks_host), capacity,
+                                             _host_ptr(counts_host), stream), "fdas_search_host_batched")
+        return counts_host
 
     def templates(self):
         """Bank in natural order as numpy: complex128/complex64, or uint16 [K, S, 2] bit patterns for bf16."""

@@ -64,3 +64,35 @@ def test_f32_batched_search_and_host_forms(F):
     out = np.empty((plan.K, plan.M), dtype=np.float32)
     plan.convolve_host(np.ascontiguousarray(w.spectrum), out)
     assert np.array_equal(out, P.cpu().numpy())
+
+
+@pytest.mark.parametrize("prec", ["bf16", "f32", "f64"])
+def test_search_host_batched_equals_per_series_search(F, prec):
+    # survey form (config 4 shape, shortened): 5 series, every other one carries a tone
+    import torch
+    N = 1 << 17
+    specs = []
+    for i in range(5):
+        if i % 2 == 0:
+            specs.append(workloads.harmonic_train(N, seed=100 + i, r0=3000.0 + 500 * i, z=4.0 * (i - 2), power=60.0,
+                                                  rel_amplitudes=(1.0,), zmax=20.0, dz=2.0, seglen=1024).spectrum)
+        else:
+            specs.append(workloads.noise_only(N, seed=100 + i, zmax=20.0, dz=2.0, seglen=1024).spectrum)
+    dt = np.complex128 if prec == "f64" else np.complex64
+    X = np.ascontiguousarray(np.stack(specs).astype(dt))
+    plan = F.Plan(N, 20.0, 2.0, 1024, prec)
+    cap = 256
+    peaks = np.zeros((5, cap, 3), dtype=np.int32)
+    counts = np.zeros(5, dtype=np.int32)
+    for rep in range(2):                                    # second call reuses the pipeline objects
+        plan.search_host_batched(X, 12.0, peaks, counts, cap)
+        for i in range(5):
+            one = np.zeros((cap, 3), dtype=np.int32)
+            n = plan.search_host(X[i], 12.0, one, cap)
+            assert n == counts[i] and (n >= 1 if i % 2 == 0 else True)
+            got = sorted(map(tuple, peaks[i, :min(n, cap)].tolist()))
+            assert got == sorted(map(tuple, one[:min(n, cap)].tolist()))
+    # the tone of series 0: r0 = 3000, z = -8 -> row (20 - 8) / 2 = 6
+    rows = {(int(a), int(b)) for a, b, _ in peaks[0, :counts[0]]}
+    assert (6, 3000) in rows
+    assert F.fdas_search_host_batched(plan._h, X.ctypes.data, 0, 12.0, peaks.ctypes.data, cap, counts.ctypes.data) == F.FDAS_ERR_INVALID_ARG
