@@ -379,6 +379,29 @@ def test_zero_drift_row_is_the_power_spectrum(F):
     assert np.abs(row - (X.real ** 2 + X.imag ** 2)).max() < 1e-12 * row.max()
 
 
+@pytest.mark.parametrize("prec,algo", [("f64", "fft"), ("f32", "fft"), ("f32", "mma"), ("bf16", "fft"), ("bf16", "mma")])
+@pytest.mark.parametrize("zmax,dz", [(0.0, 2.0), (2.0, 2.0), (1.0, 2.0)])
+def test_degenerate_banks(F, prec, algo, zmax, dz):
+    # smallest banks: zmax = 0 (K = 1, the z = 0 template alone: the plane IS the power spectrum, pin P2),
+    # K = 3, and zmax < dz (K = 1 at z = -1: asymmetric grid without a z = 0 row)
+    import torch
+    w = workloads.noise_only(1 << 14, seed=77, zmax=zmax, dz=dz, seglen=256)
+    plan, P = gpu_plane(F, w, prec, algorithm=algo)
+    assert plan.algorithm() == algo and P.shape[0] == (3 if zmax == 2.0 else 1)
+    exp = oracle.power_plane(w.spectrum, zmax, dz)
+    got = P.cpu().numpy().astype(np.float64)
+    if prec == "f64":
+        check_fp64(got, exp)
+    elif prec == "f32":
+        check_fp32(got, exp)
+    else:
+        assert float((np.abs(got - exp) / exp).mean()) <= 0.02
+    if zmax == 0.0 and prec != "bf16":
+        X = w.spectrum.astype(np.complex128)
+        tol = 1e-12 if prec == "f64" else 1e-5
+        assert np.abs(got[0] - (X.real ** 2 + X.imag ** 2)).max() <= tol * got.max()
+
+
 # ------------------------------------------------------------------ tensor-core (MMA) path of the bf16 variant
 def test_mma_config1_element_by_element(F):
     w = workloads.config1()
