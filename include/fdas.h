@@ -228,6 +228,19 @@ int fdas_z_of_index(const fdas_plan_t *p, int k, double *z);
 int fdas_build_templates(fdas_plan_t *p, void *stream);
 
 /*
+ * fdas_spectrum -- the "Real FFT" that feeds the convolution (Fig. 1; :85 "intentionally
+ * left in single-precision"): X[k] = (1/sqrt N) sum_j x[j] exp(-2 pi i j k / N), k = 0..N/2-1
+ * (Nyquist dropped; unit-variance noise gives unit mean power per bin, readings A8, A9).
+ *   timeseries_dev  N floats (the plan's N), 16-byte aligned
+ *   spectrum_dev    M = N/2 interleaved complex in the plan's spectrum type (float2; double2 for
+ *                   FDAS_F64, widened from the fp32 result as in the paper's pipeline)
+ * fp32 arithmetic throughout.  N must be a power of two, 2^10 <= N <= 2^23.  Work arrays (8 N bytes)
+ * are owned by the plan and allocated on first use.  Asynchronous on `stream`.
+ * Errors: INVALID_ARG (NULL), UNSUPPORTED (N not a power of two in range), ALLOC, CUDA.
+ */
+int fdas_spectrum(fdas_plan_t *p, const void *timeseries_dev, void *spectrum_dev, void *stream);
+
+/*
  * fdas_convolve -- the fused hot path (PAPER.md:65-67 overlap-save; :59 power plane).
  * One kernel: per segment, load S bins (zero outside [0,M)), forward FFT once, then for
  * every template multiply by H_z, inverse FFT, |.|^2, and store only the V valid bins.

@@ -59,6 +59,8 @@ struct fdas_plan {
     fdas_peak_t *pipe_peaks[2];
     int *pipe_count[2];
     int pipe_capacity, pipe_ready;
+    // fdas_spectrum: two half-length complex work arrays of the four-step FFT
+    void *rfft_scratch;
     // fdas_band_max: per-block partial maxima
     void *band_scratch;
     size_t band_scratch_bytes;
@@ -143,6 +145,8 @@ int fdas_launch_peaks(fdas_plan *p, const void *plane, float thr, fdas_peak_t *p
                       int *count, cudaStream_t st);
 // fdas_harmonic.cu: S_H[k][r] = sum_h P[k0 + h (k - k0)][h r]
 int fdas_launch_harmonic_sum(fdas_plan *p, const void *plane, void *sum, int n_harmonics, int k0, cudaStream_t st);
+// fdas_rfft.cu: the real FFT ahead of the convolution
+int fdas_launch_spectrum(fdas_plan *p, const void *timeseries, void *spectrum, cudaStream_t st);
 // fdas_bands.cu: Table 3 band maxima
 int fdas_launch_band_max(fdas_plan *p, const void *plane, double f_bin, int n_bands, fdas_peak_t *out, cudaStream_t st);
 // fdas_cast.cu: the paper's quick cast of a bf16-stored plane

@@ -15,6 +15,7 @@ static void free_device_members(fdas_plan *p)
     cudaFree(p->taps);
     cudaFree(p->twiddle);
     cudaFree(p->band_scratch);
+    cudaFree(p->rfft_scratch);
     if (p->pipe_ready) {
         cudaStreamDestroy(p->pipe_stream);
         for (int e = 0; e < 3; ++e)
@@ -160,6 +161,12 @@ extern "C" int fdas_harmonic_sum(fdas_plan_t *p, const void *plane_dev, void *su
     const int k0 = (p->K - 1) / 2;
     if (fabs(-p->zmax + k0 * p->dz) > 1e-9 * (1.0 + p->zmax)) return FDAS_ERR_UNSUPPORTED;
     return fdas_launch_harmonic_sum(p, plane_dev, sum_dev, n_harmonics, k0, (cudaStream_t)stream);
+}
+
+extern "C" int fdas_spectrum(fdas_plan_t *p, const void *timeseries_dev, void *spectrum_dev, void *stream)
+{
+    if (!p || !timeseries_dev || !spectrum_dev) return FDAS_ERR_INVALID_ARG;
+    return fdas_launch_spectrum(p, timeseries_dev, spectrum_dev, (cudaStream_t)stream);
 }
 
 extern "C" int fdas_band_max(fdas_plan_t *p, const void *plane_dev, double f_bin, int n_bands, fdas_peak_t *out_dev, void *stream)

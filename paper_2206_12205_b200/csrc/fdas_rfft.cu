@@ -1,0 +1,170 @@
+// fdas_rfft.cu -- the "Real FFT" ahead of the convolution (include/fdas.h: fdas_spectrum).
+//
+// PAPER.md:85 (Fig. 1): "The 'Real FFT' ... was intentionally left in single-precision as it does
+// not significantly affect the overall execution time (it does not scale with K, the number of
+// filters)".  X[k] = (1/sqrt N) sum_j x[j] exp(-2 pi i j k / N), k = 0..N/2-1 (readings A8,
+// A9), computed in fp32 as a half-length complex FFT of z[m] = x[2m] + i x[2m+1] followed by the
+// real-input unpacking; the half-length FFT (L = N/2 = L1 L2 points) is a four-step FFT:
+//
+//   pass A  L2/16 CTAs: 16 adjacent columns m2, FFT of length L1 over m1 in shared memory,
+//           twiddle W_L^{m2 k1}, Y[k1 L2 + m2]                       (128-byte coalesced both ways)
+//   pass B  L1/4 CTAs: 4 rows k1, FFT of length L2 over m2, Z[k1 + L1 k2]  (32-byte segments out)
+//   pass C  X[k] = E + exp(-2 pi i k / N) O,  E = (Z[k] + conj Z[L-k]) / 2,  O = -i (Z[k] - conj Z[L-k]) / 2
+//
+// Three streaming passes over 8 L bytes: HBM-bound, and small beside one fdas_convolve.  The
+// shared-memory FFT is a plain radix-2 decimation-in-frequency (natural in, bit-reversed out; the
+// store un-reverses), twiddles from sincospif with exactly representable arguments.
+#include <math.h>
+#include "fdas_internal.h"
+
+namespace {
+
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+
+// exp(-2 pi i num / den), den a power of two <= 2^24 and 0 <= num < 2^24: 2 num / den is exact in fp32
+__device__ __forceinline__ float2 twiddle(unsigned num, unsigned den)
+{
+    float s, c;
+    sincospif(-2.0f * (float)num / (float)den, &s, &c);
+    return make_float2(c, s);
+}
+
+// In-place radix-2 DIF FFTs of length n = 2^logn on `nbatch` sequences in shared memory: element i of
+// sequence b sits at s[i * si + b * sb].  tw[j] = exp(-2 pi i j / n), j < n/2.  Output bit-reversed.
+template <bool BATCH_FASTEST>
+__device__ __forceinline__ void smem_fft_dif(float2 *s, int logn, int nbatch, int si, int sb, const float2 *tw)
+{
+    const int n = 1 << logn, nb2 = n >> 1;
+    for (int lh = logn - 1; lh >= 0; --lh) {
+        const int h = 1 << lh;
+        for (int e = threadIdx.x; e < nb2 * nbatch; e += blockDim.x) {
+            int q, b;
+            if (BATCH_FASTEST) {
+                b = e % nbatch;
+                q = e / nbatch;
+            } else {
+                q = e & (nb2 - 1);
+                b = e >> (logn - 1);
+            }
+            const int j = q & (h - 1), i0 = ((q >> lh) << (lh + 1)) + j, i1 = i0 + h;
+            const float2 a = s[i0 * si + b * sb], c = s[i1 * si + b * sb];
+            s[i0 * si + b * sb] = make_float2(a.x + c.x, a.y + c.y);
+            s[i1 * si + b * sb] = cmul(make_float2(a.x - c.x, a.y - c.y), tw[j << (logn - 1 - lh)]);
+        }
+        __syncthreads();
+    }
+}
+
+__device__ __forceinline__ unsigned bitrev(unsigned v, int bits) { return bits ? __brev(v) >> (32 - bits) : 0u; }
+
+constexpr int RF_CB = 16;   // columns per CTA in pass A
+constexpr int RF_RB = 4;    // rows per CTA in pass B
+
+// pass A: z viewed as [L1][L2]; this CTA takes columns m2 = 16 blockIdx.x .. +15
+__global__ void __launch_bounds__(512) fdas_rfft_cols_kernel(const float2 *__restrict__ z, float2 *__restrict__ Y, int l1, int l2)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2 *s = reinterpret_cast<float2 *>(smem_raw);
+    const int L1 = 1 << l1, L2 = 1 << l2;
+    float2 *tw = s + L1 * RF_CB;
+    const int m20 = blockIdx.x * RF_CB;
+    for (int j = threadIdx.x; j < L1 / 2; j += blockDim.x) tw[j] = twiddle(j, L1);
+    for (int e = threadIdx.x; e < L1 * RF_CB; e += blockDim.x) {
+        const int m1 = e / RF_CB, c = e % RF_CB;
+        s[e] = __ldg(z + (size_t)m1 * L2 + m20 + c);
+    }
+    __syncthreads();
+    smem_fft_dif<true>(s, l1, RF_CB, RF_CB, 1, tw);
+    for (int e = threadIdx.x; e < L1 * RF_CB; e += blockDim.x) {
+        const int k1 = e / RF_CB, c = e % RF_CB;
+        const float2 v = s[bitrev(k1, l1) * RF_CB + c];
+        // four-step twiddle W_L^{m2 k1}: m2 k1 < 2^22
+        Y[(size_t)k1 * L2 + m20 + c] = cmul(v, twiddle((unsigned)(m20 + c) * (unsigned)k1, 1u << (l1 + l2)));
+    }
+}
+
+// pass B: rows k1 = 4 blockIdx.x .. +3 of Y [L1][L2] (or the single row when L1 == 1) -> Z[k1 + L1 k2]
+__global__ void __launch_bounds__(512) fdas_rfft_rows_kernel(const float2 *__restrict__ Y, float2 *__restrict__ Z, int l1, int l2, int rb)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2 *s = reinterpret_cast<float2 *>(smem_raw);
+    const int L1 = 1 << l1, L2 = 1 << l2;
+    float2 *tw = s + L2 * rb;
+    const int k10 = blockIdx.x * rb;
+    for (int j = threadIdx.x; j < L2 / 2; j += blockDim.x) tw[j] = twiddle(j, L2);
+    for (int e = threadIdx.x; e < L2 * rb; e += blockDim.x) s[e] = __ldg(Y + (size_t)k10 * L2 + e);   // rows are contiguous
+    __syncthreads();
+    smem_fft_dif<false>(s, l2, rb, 1, L2, tw);
+    for (int e = threadIdx.x; e < L2 * rb; e += blockDim.x) {
+        const int r = e % rb, k2 = e / rb;
+        Z[(size_t)k2 * L1 + k10 + r] = s[r * L2 + bitrev(k2, l2)];
+    }
+}
+
+// pass C: real-input unpacking, scale 1/sqrt(N); thread k handles bins k and L - k
+template <typename OT2>
+__global__ void __launch_bounds__(256) fdas_rfft_unpack_kernel(const float2 *__restrict__ Z, OT2 *__restrict__ X, unsigned L, float scale)
+{
+    for (unsigned k = blockIdx.x * blockDim.x + threadIdx.x; k <= L / 2; k += gridDim.x * blockDim.x) {
+        const float2 a = Z[k], zb = Z[(L - k) & (L - 1)];
+        const float2 b = make_float2(zb.x, -zb.y);
+        const float2 E = make_float2(0.5f * (a.x + b.x), 0.5f * (a.y + b.y));
+        const float2 d = make_float2(0.5f * (a.x - b.x), 0.5f * (a.y - b.y));
+        const float2 O = make_float2(d.y, -d.x);                     // -i d
+        float sn, cs;
+        sincospif(-(float)k / (float)L, &sn, &cs);                   // exp(-2 pi i k / N), N = 2 L
+        const float2 wO = cmul(make_float2(cs, sn), O);
+        X[k].x = scale * (E.x + wO.x);
+        X[k].y = scale * (E.y + wO.y);
+        if (k != 0 && k != L - k) {                                  // X[L-k] = conj(E - w O)
+            X[L - k].x = scale * (E.x - wO.x);
+            X[L - k].y = -scale * (E.y - wO.y);
+        }
+    }
+}
+
+}  // namespace
+
+int fdas_launch_spectrum(fdas_plan *p, const void *timeseries, void *spectrum, cudaStream_t st)
+{
+    int n = 0;
+    while ((1LL << n) < p->N) ++n;
+    if ((1LL << n) != p->N || n < 10 || n > 23) return FDAS_ERR_UNSUPPORTED;
+    const int l = n - 1, l2 = l < 12 ? l : 12, l1 = l - l2;
+    const size_t L = (size_t)1 << l;
+    if (!p->rfft_scratch) FDAS_CUDA_TRY(p, cudaMalloc(&p->rfft_scratch, 2 * L * sizeof(float2)));
+    float2 *Y = static_cast<float2 *>(p->rfft_scratch), *Z = Y + L;
+    const float2 *z = static_cast<const float2 *>(timeseries);
+    if (l1 > 0) {
+        const size_t smem = ((size_t)(1 << l1) * RF_CB + (1 << l1) / 2) * sizeof(float2);
+        static size_t attr = 0;
+        if (smem > attr) {
+            FDAS_CUDA_TRY(p, cudaFuncSetAttribute(fdas_rfft_cols_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            attr = smem;
+        }
+        fdas_rfft_cols_kernel<<<(1 << l2) / RF_CB, 512, smem, st>>>(z, Y, l1, l2);
+        FDAS_CUDA_TRY(p, cudaGetLastError());
+        p->launches += 1;
+    }
+    {
+        const int rb = l1 >= 2 ? RF_RB : 1;
+        const size_t smem = ((size_t)(1 << l2) * rb + (1 << l2) / 2) * sizeof(float2);
+        static size_t attr = 0;
+        if (smem > attr) {
+            FDAS_CUDA_TRY(p, cudaFuncSetAttribute(fdas_rfft_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            attr = smem;
+        }
+        fdas_rfft_rows_kernel<<<(1 << l1) / rb, 512, smem, st>>>(l1 > 0 ? Y : z, Z, l1, l2, rb);
+        FDAS_CUDA_TRY(p, cudaGetLastError());
+        p->launches += 1;
+    }
+    const float scale = (float)(1.0 / sqrt((double)p->N));
+    const unsigned blocks = (unsigned)((L / 2 + 256) / 256 < (size_t)p->num_sms * 8 ? (L / 2 + 256) / 256 : (size_t)p->num_sms * 8);
+    if (p->precision == FDAS_F64)
+        fdas_rfft_unpack_kernel<double2><<<blocks, 256, 0, st>>>(Z, static_cast<double2 *>(spectrum), (unsigned)L, scale);
+    else
+        fdas_rfft_unpack_kernel<float2><<<blocks, 256, 0, st>>>(Z, static_cast<float2 *>(spectrum), (unsigned)L, scale);
+    FDAS_CUDA_TRY(p, cudaGetLastError());
+    p->launches += 1;
+    return FDAS_OK;
+}

@@ -28,7 +28,7 @@ EXPORTS = [
     "fdas_convolve_host", "fdas_search_host", "fdas_templates_host", "fdas_taps_host",
     "fdas_launch_count", "fdas_status_string", "fdas_last_cuda_error",
     "fdas_set_algorithm", "fdas_get_algorithm", "fdas_tapmatrix_host", "fdas_search",
-    "fdas_set_plane_format", "fdas_get_plane_format", "fdas_quick_cast", "fdas_harmonic_sum", "fdas_band_max", "fdas_search_host_batched",
+    "fdas_set_plane_format", "fdas_get_plane_format", "fdas_quick_cast", "fdas_harmonic_sum", "fdas_band_max", "fdas_search_host_batched", "fdas_spectrum",
 ]
 
 
@@ -83,6 +83,7 @@ def lib() -> ctypes.CDLL:
     L.fdas_quick_cast.argtypes = [vp, vp, vp, i, vp]
     L.fdas_harmonic_sum.argtypes = [vp, vp, vp, i, vp]
     L.fdas_band_max.argtypes = [vp, vp, dbl, i, vp, vp]
+    L.fdas_spectrum.argtypes = [vp, vp, vp, vp]
     L.fdas_search_host_batched.argtypes = [vp, vp, i, ctypes.c_float, vp, i, vp, vp]
     L.fdas_status_string.argtypes = [i]
     L.fdas_status_string.restype = ctypes.c_char_p
@@ -211,6 +212,10 @@ def fdas_search_host_batched(h, spectra_host_ptr, n_series, threshold, peaks_hos
                                           counts_host_ptr, stream)
 
 
+def fdas_spectrum(h, timeseries_ptr, spectrum_ptr, stream=0):
+    return lib().fdas_spectrum(h, timeseries_ptr, spectrum_ptr, stream)
+
+
 def fdas_launch_count(h):
     n = ctypes.c_int64()
     rc = lib().fdas_launch_count(h, ctypes.byref(n))
@@ -315,6 +320,19 @@ class Plan:
     def spectrum_dtype(self):
         import torch
         return torch.complex128 if self.precision == FDAS_F64 else torch.complex64
+
+    def spectrum(self, timeseries, out=None, stream: Optional[int] = None):
+        """fdas_spectrum: float32 CUDA tensor [N] -> complex spectrum [M] (the real FFT of PAPER.md:85)."""
+        import torch
+        assert timeseries.is_cuda and timeseries.is_contiguous() and timeseries.dtype == torch.float32
+        assert timeseries.numel() == 2 * self.M
+        if out is None:
+            out = torch.empty(self.M, dtype=self.spectrum_dtype(), device=timeseries.device)
+        assert out.is_cuda and out.is_contiguous() and out.dtype == self.spectrum_dtype() and out.numel() == self.M
+        if stream is None:
+            stream = torch.cuda.current_stream().cuda_stream
+        self._check(fdas_spectrum(self._h, timeseries.data_ptr(), out.data_ptr(), stream), "fdas_spectrum")
+        return out
 
     def build_templates(self, stream: int = 0):
         self._check(fdas_build_templates(self._h, stream), "fdas_build_templates")
