@@ -6,14 +6,15 @@
 // A9), computed in fp32 as a half-length complex FFT of z[m] = x[2m] + i x[2m+1] followed by the
 // real-input unpacking; the half-length FFT (L = N/2 = L1 L2 points) is a four-step FFT:
 //
-//   pass A  L2/16 CTAs: 16 adjacent columns m2, FFT of length L1 over m1 in shared memory,
-//           twiddle W_L^{m2 k1}, Y[k1 L2 + m2]                       (128-byte coalesced both ways)
-//   pass B  L1/4 CTAs: 4 rows k1, FFT of length L2 over m2, Z[k1 + L1 k2]  (32-byte segments out)
+//   pass A  L2/8 CTAs: 8 adjacent columns m2, FFT of length L1 over m1 in shared memory,
+//           twiddle W_L^{m2 k1}, Y[k1 L2 + m2]                        (64-byte segments both ways)
+//   pass B  L1/2 CTAs: 2 rows k1, FFT of length L2 over m2, Z[k1 + L1 k2]  (16-byte segments out)
 //   pass C  X[k] = E + exp(-2 pi i k / N) O,  E = (Z[k] + conj Z[L-k]) / 2,  O = -i (Z[k] - conj Z[L-k]) / 2
 //
 // Three streaming passes over 8 L bytes: HBM-bound, and small beside one fdas_convolve.  The
-// shared-memory FFT is a plain radix-2 decimation-in-frequency (natural in, bit-reversed out; the
-// store un-reverses), twiddles from sincospif with exactly representable arguments.
+// shared-memory FFT is a decimation-in-frequency with two radix-2 stages fused per barrier (natural
+// in, bit-reversed out; the store un-reverses), twiddles from sincospif with exactly representable
+// arguments.
 #include <math.h>
 #include "fdas_internal.h"
 
@@ -29,27 +30,57 @@ __device__ __forceinline__ float2 twiddle(unsigned num, unsigned den)
     return make_float2(c, s);
 }
 
-// In-place radix-2 DIF FFTs of length n = 2^logn on `nbatch` sequences in shared memory: element i of
-// sequence b sits at s[i * si + b * sb].  tw[j] = exp(-2 pi i j / n), j < n/2.  Output bit-reversed.
+// In-place decimation-in-frequency FFTs of length n = 2^logn on `nbatch` sequences in shared memory:
+// element i of sequence b sits at s[i * si + b * sb].  tw[j] = exp(-2 pi i j / n), j < n/2.  Two radix-2
+// stages are fused in registers (one shared-memory round trip and one barrier per pair of stages);
+// an odd logn ends with a single radix-2 stage.  Output bit-reversed.
 template <bool BATCH_FASTEST>
 __device__ __forceinline__ void smem_fft_dif(float2 *s, int logn, int nbatch, int si, int sb, const float2 *tw)
 {
-    const int n = 1 << logn, nb2 = n >> 1;
-    for (int lh = logn - 1; lh >= 0; --lh) {
-        const int h = 1 << lh;
-        for (int e = threadIdx.x; e < nb2 * nbatch; e += blockDim.x) {
-            int q, b;
+    const int n = 1 << logn;
+    int lh = logn - 1;                                  // log2 of the current half size
+    for (; lh >= 1; lh -= 2) {
+        const int q = 1 << (lh - 1), nq = n >> 2;       // quarter of the current block; butterflies per sequence
+        const int tstride = logn - 1 - lh;              // tw index shift for W_{4q}
+        for (int e = threadIdx.x; e < nq * nbatch; e += blockDim.x) {
+            int g, b;
             if (BATCH_FASTEST) {
                 b = e % nbatch;
-                q = e / nbatch;
+                g = e / nbatch;
             } else {
-                q = e & (nb2 - 1);
+                g = e & (nq - 1);
+                b = e >> (logn - 2);
+            }
+            const int j = g & (q - 1), base = ((g >> (lh - 1)) << (lh + 1)) + j;
+            float2 *p0 = s + base * si + b * sb, *p1 = p0 + q * si, *p2 = p1 + q * si, *p3 = p2 + q * si;
+            const float2 x0 = *p0, x1 = *p1, x2 = *p2, x3 = *p3;
+            const float2 w1 = tw[j << tstride], w2 = tw[(2 * j) << tstride];
+            const float2 u0 = make_float2(x0.x + x2.x, x0.y + x2.y), u1 = make_float2(x1.x + x3.x, x1.y + x3.y);
+            const float2 u2 = cmul(make_float2(x0.x - x2.x, x0.y - x2.y), w1);
+            const float2 d13 = make_float2(x1.x - x3.x, x1.y - x3.y);
+            const float2 u3 = cmul(make_float2(d13.y, -d13.x), w1);      // (x1 - x3) W^{j+q} = (x1 - x3)(-i) W^j
+            *p0 = make_float2(u0.x + u1.x, u0.y + u1.y);
+            *p1 = cmul(make_float2(u0.x - u1.x, u0.y - u1.y), w2);
+            *p2 = make_float2(u2.x + u3.x, u2.y + u3.y);
+            *p3 = cmul(make_float2(u2.x - u3.x, u2.y - u3.y), w2);
+        }
+        __syncthreads();
+    }
+    if (lh == 0) {                                      // last radix-2 stage: neighbours, twiddle 1
+        const int nb2 = n >> 1;
+        for (int e = threadIdx.x; e < nb2 * nbatch; e += blockDim.x) {
+            int g, b;
+            if (BATCH_FASTEST) {
+                b = e % nbatch;
+                g = e / nbatch;
+            } else {
+                g = e & (nb2 - 1);
                 b = e >> (logn - 1);
             }
-            const int j = q & (h - 1), i0 = ((q >> lh) << (lh + 1)) + j, i1 = i0 + h;
-            const float2 a = s[i0 * si + b * sb], c = s[i1 * si + b * sb];
-            s[i0 * si + b * sb] = make_float2(a.x + c.x, a.y + c.y);
-            s[i1 * si + b * sb] = cmul(make_float2(a.x - c.x, a.y - c.y), tw[j << (logn - 1 - lh)]);
+            float2 *p0 = s + (2 * g) * si + b * sb, *p1 = p0 + si;
+            const float2 a = *p0, c = *p1;
+            *p0 = make_float2(a.x + c.x, a.y + c.y);
+            *p1 = make_float2(a.x - c.x, a.y - c.y);
         }
         __syncthreads();
     }
@@ -57,8 +88,13 @@ __device__ __forceinline__ void smem_fft_dif(float2 *s, int logn, int nbatch, in
 
 __device__ __forceinline__ unsigned bitrev(unsigned v, int bits) { return bits ? __brev(v) >> (32 - bits) : 0u; }
 
-constexpr int RF_CB = 16;   // columns per CTA in pass A
-constexpr int RF_RB = 4;    // rows per CTA in pass B
+#ifndef FDAS_RF_CB
+#define FDAS_RF_CB 8
+#define FDAS_RF_RB 2
+#define FDAS_RF_L2MAX 12
+#endif
+constexpr int RF_CB = FDAS_RF_CB;    // columns per CTA in pass A (64-byte segments; 64 KB of shared memory -> 3 CTAs per SM)
+constexpr int RF_RB = FDAS_RF_RB;    // rows per CTA in pass B
 
 // pass A: z viewed as [L1][L2]; this CTA takes columns m2 = 16 blockIdx.x .. +15
 __global__ void __launch_bounds__(512) fdas_rfft_cols_kernel(const float2 *__restrict__ z, float2 *__restrict__ Y, int l1, int l2)
@@ -130,7 +166,7 @@ int fdas_launch_spectrum(fdas_plan *p, const void *timeseries, void *spectrum, c
     int n = 0;
     while ((1LL << n) < p->N) ++n;
     if ((1LL << n) != p->N || n < 10 || n > 23) return FDAS_ERR_UNSUPPORTED;
-    const int l = n - 1, l2 = l < 12 ? l : 12, l1 = l - l2;
+    const int l = n - 1, l2 = l < FDAS_RF_L2MAX ? l : FDAS_RF_L2MAX, l1 = l - l2;
     const size_t L = (size_t)1 << l;
     if (!p->rfft_scratch) FDAS_CUDA_TRY(p, cudaMalloc(&p->rfft_scratch, 2 * L * sizeof(float2)));
     float2 *Y = static_cast<float2 *>(p->rfft_scratch), *Z = Y + L;
