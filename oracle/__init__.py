@@ -52,6 +52,12 @@ def lib() -> ctypes.CDLL:
         L.fdas_oracle_plane.argtypes = [dp, ctypes.c_int64, ctypes.c_double, ctypes.c_double,
                                         ctypes.c_int64, ctypes.c_int64, dp]
         L.fdas_oracle_plane.restype = ctypes.c_int
+        L.fdas_oracle_halfwidth_jerk.argtypes = [ctypes.c_double, ctypes.c_double]
+        L.fdas_oracle_halfwidth_jerk.restype = ctypes.c_int
+        L.fdas_oracle_response_jerk.argtypes = [ctypes.c_double, ctypes.c_double, ctypes.c_double, dp, dp]
+        L.fdas_oracle_response_jerk.restype = None
+        L.fdas_oracle_template_jerk.argtypes = [ctypes.c_double, ctypes.c_double, ctypes.c_int, dp]
+        L.fdas_oracle_template_jerk.restype = ctypes.c_int
         L.fdas_oracle_peaks.argtypes = [dp, ctypes.c_int, ctypes.c_int64, ctypes.c_double, dp,
                                         ctypes.c_int64]
         L.fdas_oracle_peaks.restype = ctypes.c_int64
@@ -138,3 +144,33 @@ def peaks(P, thr: float, capacity: int | None = None):
     w = min(n, capacity)
     rec = [(int(out[3 * i]), int(out[3 * i + 1]), float(out[3 * i + 2])) for i in range(w)]
     return n, rec
+
+
+# ---- jerk slab (reading A25) ---------------------------------------------
+def halfwidth_jerk(z: float, w: float) -> int:
+    return int(lib().fdas_oracle_halfwidth_jerk(float(z), float(w)))
+
+
+def response_jerk(z: float, w: float, q: float) -> complex:
+    re, im = ctypes.c_double(), ctypes.c_double()
+    lib().fdas_oracle_response_jerk(float(z), float(w), float(q), ctypes.byref(re), ctypes.byref(im))
+    return complex(re.value, im.value)
+
+
+def template_taps_jerk(z: float, w: float, m: int | None = None) -> np.ndarray:
+    if m is None:
+        m = halfwidth_jerk(z, w)
+    out = np.empty(2 * (2 * m + 1), dtype=np.float64)
+    rc = lib().fdas_oracle_template_jerk(float(z), float(w), int(m), _dptr(out))
+    if rc:
+        raise RuntimeError(f"fdas_oracle_template_jerk rc={rc}")
+    return out.view(np.complex128)
+
+
+def power_plane_jerk(X, zmax: float, dz: float, w: float, r_begin: int = 0, r_end: int | None = None) -> np.ndarray:
+    """One slab of the f-fdot-fddot volume: the plane at jerk w, rows z_k = -zmax + k dz."""
+    X = _as_c128(X)
+    if r_end is None:
+        r_end = len(X)
+    K = 2 * int(np.floor(zmax / dz + 1e-9)) + 1
+    return np.stack([convolve_row(X, template_taps_jerk(-zmax + k * dz, w), r_begin, r_end) for k in range(K)])

@@ -148,6 +148,55 @@ int fdas_oracle_template(double z, int m, double *taps)
     return 0;
 }
 
+/* Jerk extension (section 2.2: "Jerk Searching takes into account a change in
+ * acceleration, and therefore extends the f-fdot plane into an f-fdot-fddot volume ... based on the
+ * same principal of convolving templates").  One slab of that volume = one f-fdot plane at a fixed
+ * jerk w (change of the drift over the observation, in Fourier bins).  Reading A25: the
+ * instantaneous frequency is r0 + z (u - 1/2) + (w/2)(u^2 - u + 1/6), whose mean is r0 and whose
+ * mean slope is z, so the response is
+ *   W_{z,w}(q) = int_0^1 exp(2 pi i [q u + (z/2)(u^2 - u) + (w/12)(2u^3 - 3u^2 + u)]) du ,
+ * taps h_{z,w}[j] = conj(W_{z,w}(j)), |j| <= m = ceil(|z|/2 + |w|/12) + 16 (the largest frequency
+ * excursion from the mean is |z|/2 + |w|/12).  w = 0 is the constant-acceleration response. */
+int fdas_oracle_halfwidth_jerk(double z, double w)
+{
+    return (int)ceil(fabs(z) / 2.0 + fabs(w) / 12.0) + 16;
+}
+
+void fdas_oracle_response_jerk(double z, double w, double q, double *re, double *im)
+{
+    long double xs[ORACLE_GL_NODES], ws[ORACLE_GL_NODES];
+    gauss_legendre(ORACLE_GL_NODES, xs, ws);
+    long double sr = 0.0L, si = 0.0L;
+    const long double h = 1.0L / ORACLE_GL_PANELS;
+    for (int p = 0; p < ORACLE_GL_PANELS; ++p) {
+        long double a = p * h;
+        for (int i = 0; i < ORACLE_GL_NODES; ++i) {
+            long double u = a + 0.5L * h * (xs[i] + 1.0L);
+            long double cyc = (long double)q * u + 0.5L * (long double)z * (u * u - u) +
+                              ((long double)w / 12.0L) * (2.0L * u * u * u - 3.0L * u * u + u);
+            cyc -= floorl(cyc);
+            long double wgt = 0.5L * h * ws[i];
+            sr += wgt * cosl(2.0L * PI_L * cyc);
+            si += wgt * sinl(2.0L * PI_L * cyc);
+        }
+    }
+    *re = (double)sr;
+    *im = (double)si;
+}
+
+int fdas_oracle_template_jerk(double z, double w, int m, double *taps)
+{
+    if (m < 0 || !taps) return 1;
+#pragma omp parallel for schedule(static)
+    for (int j = -m; j <= m; ++j) {
+        double re, im;
+        fdas_oracle_response_jerk(z, w, (double)j, &re, &im);
+        taps[2 * (j + m) + 0] = re;
+        taps[2 * (j + m) + 1] = -im; /* conj */
+    }
+    return 0;
+}
+
 /* One template row, bins r in [r_begin, r_end):
  *   Y[r] = sum_{j=-m}^{m} X[r-j] h[j]   (X = 0 outside [0,M)),  P[r] = |Y[r]|^2.
  * X is interleaved (re, im) fp64, length M complex.  out has r_end - r_begin entries.

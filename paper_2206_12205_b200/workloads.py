@@ -60,7 +60,7 @@ class Workload:
 
 
 def _add_tone(x: np.ndarray, r0: float, z: float, power: float, phi0: float,
-              harmonics=None, chunk: int = 1 << 20) -> None:
+              harmonics=None, chunk: int = 1 << 20, w: float = 0.0) -> None:
     """x += sum_h a_h cos(h * theta(u)), theta(u) = 2 pi[(r0 - z/2)u + (z/2)u^2] + phi0.
 
     ``harmonics`` = list of (h, relative amplitude); default a single fundamental.  The
@@ -75,6 +75,8 @@ def _add_tone(x: np.ndarray, r0: float, z: float, power: float, phi0: float,
         e = min(N, s + chunk)
         u = np.arange(s, e, dtype=np.float64) / N
         cyc = (r0 - 0.5 * z) * u + 0.5 * z * u * u + phi0 / (2.0 * math.pi)
+        if w != 0.0:   # jerk: frequency r0 + z (u - 1/2) + (w/2)(u^2 - u + 1/6); phase term (w/12)(2u^3 - 3u^2 + u)
+            cyc += (w / 12.0) * (2.0 * u * u * u - 3.0 * u * u + u)
         cyc -= np.floor(cyc)
         acc = np.zeros(e - s, dtype=np.float64)
         for h, rel in harmonics:
@@ -199,6 +201,15 @@ def harmonic_train(N: int, seed: int, r0: float, z: float, power: float, rel_amp
     inj = Injection(float(r0), float(z), float(power), 0.0)
     _add_tone(x, r0, z, power, 0.0, harmonics=[(h + 1, float(a)) for h, a in enumerate(rel_amplitudes)])
     return Workload("harmonic_train", N, zmax, dz, seglen, spectrum_of(x), [inj], seed)
+
+
+def jerk_tone(N: int, seed: int, r0: float, z: float, w: float, power: float, zmax: float = 20.0, dz: float = 2.0,
+              seglen: int = 1024, noise: bool = True) -> Workload:
+    """One tone with drift z and jerk w (both in Fourier bins over the observation), mean frequency r0."""
+    rng = np.random.default_rng(seed)
+    x = _noise(rng, N) if noise else np.zeros(N, dtype=np.float32)
+    _add_tone(x, r0, z, power, 0.0, w=w)
+    return Workload("jerk_tone", N, zmax, dz, seglen, spectrum_of(x), [Injection(float(r0), float(z), float(power), 0.0)], seed)
 
 
 def noise_only(N: int, seed: int, zmax: float = 96.0, dz: float = 2.0, seglen: int = 2048) -> Workload:
