@@ -127,6 +127,24 @@ int fdas_plan_create(fdas_plan_t **out, int64_t N, double zmax, double dz, int s
                      int precision);
 
 /*
+ * fdas_plan_create_jerk -- one slab of the f-fdot-fddot volume of a jerk search (PAPER.md:71-73,
+ * section 2.2: "Jerk Searching takes into account a change in acceleration, and therefore extends
+ * the f-fdot plane into an f-fdot-fddot volume.  More candidate templates are required to populate
+ * the third dimension ... based on the same principal of convolving templates").  The plan is an
+ * ordinary FDAS plan whose K templates all carry the jerk `w` (change of the drift z over the
+ * observation, in Fourier bins; reading A25):
+ *      h_{z,w}[j] = conj( int_0^1 exp(2 pi i [ j u + (z/2)(u^2 - u) + (w/12)(2u^3 - 3u^2 + u) ]) du ),
+ *      |j| <= m = ceil(|z|/2 + |w|/12) + 16,
+ * i.e. the response of a signal of mean frequency r0 and mean drift z whose frequency follows
+ * r0 + z (u - 1/2) + (w/2)(u^2 - u + 1/6).  A volume is a set of such plans, one per w; every other
+ * entry point (convolve, search, peaks, harmonic sum, ...) acts on one slab.  The +-z pairing that the
+ * tensor-core form uses survives the jerk (h_{-z,w} = conj h_{z,w}); the taps are no longer even in j.
+ * w = 0 is fdas_plan_create.  Same errors; seglen must leave S - L - m >= 32 with the wider taps.
+ */
+int fdas_plan_create_jerk(fdas_plan_t **out, int64_t N, double zmax, double dz, double w, int seglen,
+                          int precision);
+
+/*
  * fdas_set_algorithm -- choose how fdas_convolve evaluates Y_z[r] = sum_j X[r-j] h_z[j]
  * (PAPER.md:35, :59).  Both algorithms compute the same plane; they differ in rounding points:
  *   FDAS_ALGO_FFT  overlap-save FFTs; in FDAS_BF16 the spectrum, the FFT'd

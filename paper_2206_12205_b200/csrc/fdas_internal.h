@@ -15,6 +15,7 @@ struct fdas_plan {
     // problem shape
     int64_t N, M;
     double zmax, dz;
+    double jerk;       // w of this slab of the f-fdot-fddot volume (0: plain FDAS)
     int K, S, m_max, L, V, precision;
     int64_t n_seg;
     int T, R3;

@@ -7,7 +7,8 @@
 #include <vector>
 #include "fdas_internal.h"
 
-static int halfwidth_of(double z) { return (int)ceil(fabs(z) / 2.0) + 16; }
+// m = ceil(|z|/2 + |w|/12) + 16: the largest excursion of the frequency from its mean, plus 16 bins (w = 0: BASELINE.json's rule)
+static int halfwidth_of(double z, double w) { return (int)ceil(fabs(z) / 2.0 + fabs(w) / 12.0) + 16; }
 
 static void free_device_members(fdas_plan *p)
 {
@@ -42,9 +43,15 @@ static void free_device_members(fdas_plan *p)
 extern "C" int fdas_plan_create(fdas_plan_t **out, int64_t N, double zmax, double dz, int seglen,
                                 int precision)
 {
+    return fdas_plan_create_jerk(out, N, zmax, dz, 0.0, seglen, precision);
+}
+
+extern "C" int fdas_plan_create_jerk(fdas_plan_t **out, int64_t N, double zmax, double dz, double w, int seglen,
+                                     int precision)
+{
     if (!out) return FDAS_ERR_INVALID_ARG;
     *out = NULL;
-    if (!(zmax >= 0.0) || !(dz > 0.0) || !isfinite(zmax) || !isfinite(dz)) return FDAS_ERR_INVALID_ARG;
+    if (!(zmax >= 0.0) || !(dz > 0.0) || !isfinite(zmax) || !isfinite(dz) || !isfinite(w)) return FDAS_ERR_INVALID_ARG;
     if (precision != FDAS_F64 && precision != FDAS_F32 && precision != FDAS_BF16) return FDAS_ERR_INVALID_ARG;
     if (seglen == 8192) return FDAS_ERR_UNSUPPORTED;
     if (seglen != 256 && seglen != 512 && seglen != 1024 && seglen != 2048 && seglen != 4096)
@@ -53,7 +60,7 @@ extern "C" int fdas_plan_create(fdas_plan_t **out, int64_t N, double zmax, doubl
     double kk = floor(zmax / dz + 1e-9);
     if (kk > 2047.0) return FDAS_ERR_INVALID_ARG;
     const int K = 2 * (int)kk + 1;
-    const int m_max = halfwidth_of(zmax);
+    const int m_max = halfwidth_of(zmax, w);
     const int L = (m_max + 31) / 32 * 32;
     const int V = (seglen - L - m_max) / 32 * 32;
     if (V < 32) return FDAS_ERR_INVALID_ARG;
@@ -65,6 +72,7 @@ extern "C" int fdas_plan_create(fdas_plan_t **out, int64_t N, double zmax, doubl
     p->M = N / 2;
     p->zmax = zmax;
     p->dz = dz;
+    p->jerk = w;
     p->K = K;
     p->S = seglen;
     p->m_max = m_max;

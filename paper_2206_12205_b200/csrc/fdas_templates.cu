@@ -71,12 +71,12 @@ __device__ __forceinline__ double frac_of_product(double a, double b)
 
 // grid (2*m_max+1, K), block GL_PANELS
 __global__ void __launch_bounds__(GL_PANELS)
-fdas_taps_kernel(double2 *taps, int K, int m_max, double zmax, double dz, GaussLegendre rule)
+fdas_taps_kernel(double2 *taps, int K, int m_max, double zmax, double dz, double jerk, GaussLegendre rule)
 {
     const int k = blockIdx.y;
     const int j = (int)blockIdx.x - m_max;
     const double z = -zmax + k * dz;
-    const int m = (int)ceil(fabs(z) / 2.0) + 16;
+    const int m = (int)ceil(fabs(z) / 2.0 + fabs(jerk) / 12.0) + 16;
     __shared__ double sr[GL_PANELS], si[GL_PANELS];
     double accr = 0.0, acci = 0.0;
     if (abs(j) <= m) {
@@ -90,6 +90,10 @@ fdas_taps_kernel(double2 *taps, int K, int m_max, double zmax, double dz, GaussL
             const double d = rule.d[i];
             // phase in cycles: j u + (z/2)(u^2 - u), u = a + d
             double cyc = base + ((double)j * d + zh * (d * lin + d * d));
+            if (jerk != 0.0) {   // jerk slab (reading A25): + (w/12)(2u^3 - 3u^2 + u), u = a + d
+                const double u = a + d;
+                cyc += (jerk / 12.0) * (u * (u * (2.0 * u - 3.0) + 1.0));
+            }
             double s, c;
             sincospi(2.0 * cyc, &s, &c);
             accr += rule.w[i] * c;
@@ -137,13 +141,13 @@ template <> struct StoreComplex<__nv_bfloat16> {
 template <typename ST>
 __global__ void __launch_bounds__(256)
 fdas_bank_kernel(void *bank, const double2 *__restrict__ taps, int K, int S, int T, int VC, int m_max,
-                 double zmax, double dz)
+                 double zmax, double dz, double jerk)
 {
     const int k = blockIdx.y;
     const int f = blockIdx.x * blockDim.x + threadIdx.x;
     if (f >= S) return;
     const double z = -zmax + k * dz;
-    const int m = (int)ceil(fabs(z) / 2.0) + 16;
+    const int m = (int)ceil(fabs(z) / 2.0 + fabs(jerk) / 12.0) + 16;
     const double2 *h = taps + (size_t)k * (2 * m_max + 1) + m_max;
     double accr = 0.0, acci = 0.0;
     const double inv = 2.0 / S;
@@ -178,19 +182,19 @@ int fdas_launch_build_templates(fdas_plan *p, cudaStream_t st)
 {
     static const GaussLegendre rule = make_rule();
     const int ntap = 2 * p->m_max + 1;
-    fdas_taps_kernel<<<dim3(ntap, p->K), GL_PANELS, 0, st>>>(p->taps, p->K, p->m_max, p->zmax, p->dz, rule);
+    fdas_taps_kernel<<<dim3(ntap, p->K), GL_PANELS, 0, st>>>(p->taps, p->K, p->m_max, p->zmax, p->dz, p->jerk, rule);
     FDAS_CUDA_TRY(p, cudaGetLastError());
     const dim3 grid((p->S + 255) / 256, p->K);
     const int VC = fdas_bank_vc(p->precision);
     if (p->precision == FDAS_F64) {
-        fdas_bank_kernel<double><<<grid, 256, 0, st>>>(p->bank, p->taps, p->K, p->S, p->T, VC, p->m_max, p->zmax, p->dz);
+        fdas_bank_kernel<double><<<grid, 256, 0, st>>>(p->bank, p->taps, p->K, p->S, p->T, VC, p->m_max, p->zmax, p->dz, p->jerk);
         FDAS_CUDA_TRY(p, cudaGetLastError());
         fdas_twiddle_kernel<double2><<<(p->S + 255) / 256, 256, 0, st>>>((double2 *)p->twiddle, p->S);
     } else {
         if (p->precision == FDAS_F32)
-            fdas_bank_kernel<float><<<grid, 256, 0, st>>>(p->bank, p->taps, p->K, p->S, p->T, VC, p->m_max, p->zmax, p->dz);
+            fdas_bank_kernel<float><<<grid, 256, 0, st>>>(p->bank, p->taps, p->K, p->S, p->T, VC, p->m_max, p->zmax, p->dz, p->jerk);
         else
-            fdas_bank_kernel<__nv_bfloat16><<<grid, 256, 0, st>>>(p->bank, p->taps, p->K, p->S, p->T, VC, p->m_max, p->zmax, p->dz);
+            fdas_bank_kernel<__nv_bfloat16><<<grid, 256, 0, st>>>(p->bank, p->taps, p->K, p->S, p->T, VC, p->m_max, p->zmax, p->dz, p->jerk);
         FDAS_CUDA_TRY(p, cudaGetLastError());
         fdas_twiddle_kernel<float2><<<(p->S + 255) / 256, 256, 0, st>>>((float2 *)p->twiddle, p->S);
     }

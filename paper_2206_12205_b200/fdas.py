@@ -28,7 +28,7 @@ EXPORTS = [
     "fdas_convolve_host", "fdas_search_host", "fdas_templates_host", "fdas_taps_host",
     "fdas_launch_count", "fdas_status_string", "fdas_last_cuda_error",
     "fdas_set_algorithm", "fdas_get_algorithm", "fdas_tapmatrix_host", "fdas_search",
-    "fdas_set_plane_format", "fdas_get_plane_format", "fdas_quick_cast", "fdas_harmonic_sum", "fdas_band_max", "fdas_search_host_batched", "fdas_spectrum",
+    "fdas_set_plane_format", "fdas_get_plane_format", "fdas_quick_cast", "fdas_harmonic_sum", "fdas_band_max", "fdas_search_host_batched", "fdas_spectrum", "fdas_plan_create_jerk",
 ]
 
 
@@ -62,6 +62,7 @@ def lib() -> ctypes.CDLL:
     L = ctypes.CDLL(LIB_PATH)
     vp, i, i64, dbl = ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_double
     L.fdas_plan_create.argtypes = [ctypes.POINTER(vp), i64, dbl, dbl, i, i]
+    L.fdas_plan_create_jerk.argtypes = [ctypes.POINTER(vp), i64, dbl, dbl, dbl, i, i]
     L.fdas_plan_destroy.argtypes = [vp]
     L.fdas_plan_info.argtypes = [vp, ctypes.POINTER(fdas_info_t)]
     L.fdas_z_of_index.argtypes = [vp, i, ctypes.POINTER(dbl)]
@@ -107,6 +108,12 @@ class FdasError(RuntimeError):
 def fdas_plan_create(N, zmax, dz, seglen, precision):
     h = ctypes.c_void_p()
     rc = lib().fdas_plan_create(ctypes.byref(h), int(N), float(zmax), float(dz), int(seglen), int(precision))
+    return rc, h
+
+
+def fdas_plan_create_jerk(N, zmax, dz, w, seglen, precision):
+    h = ctypes.c_void_p()
+    rc = lib().fdas_plan_create_jerk(ctypes.byref(h), int(N), float(zmax), float(dz), float(w), int(seglen), int(precision))
     return rc, h
 
 
@@ -236,9 +243,9 @@ class Plan:
     torch's; all arithmetic is the library's)."""
 
     def __init__(self, N: int, zmax: float, dz: float, seglen: int, precision="f32", build: bool = True,
-                 stream: int = 0, algorithm="auto", plane="f32"):
+                 stream: int = 0, algorithm="auto", plane="f32", jerk: float = 0.0):
         prec = PRECISIONS[precision] if isinstance(precision, str) else int(precision)
-        rc, self._h = fdas_plan_create(N, zmax, dz, seglen, prec)
+        rc, self._h = fdas_plan_create_jerk(N, zmax, dz, jerk, seglen, prec) if jerk else fdas_plan_create(N, zmax, dz, seglen, prec)
         if rc:
             self._h = None
             raise FdasError(rc, "fdas_plan_create")
