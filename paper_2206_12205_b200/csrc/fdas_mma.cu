@@ -1,5 +1,5 @@
-// fdas_mma.cu -- tensor-core (tcgen05 / TMEM) form of the bf16 convolution
-// (include/fdas.h: fdas_convolve with FDAS_BF16 and FDAS_ALGO_MMA).
+// fdas_mma.cu -- tensor-core (tcgen05 / TMEM) form of the convolution
+// (include/fdas.h: fdas_convolve with FDAS_ALGO_MMA, the default for FDAS_BF16 and FDAS_F32).
 //
 // the f-fdot plane is the spectrum convolved with every template,
 //      Y_z[r] = sum_{j=-m_z..m_z} X[r-j] h_z[j],   P[k][r] = |Y_{z_k}[r]|^2 .
@@ -41,6 +41,12 @@
 //               5.8-6.0 TB/s, a linear fill 7.1 TB/s.
 //   warp  16    one thread issues tcgen05.mma and tcgen05.commit
 //   warps 17-19 loader: spectrum block -> bf16 (RNE, reading A12) -> Z rows
+//
+// Template parameters of fdas_mma_bulk_kernel: NCH (16-column chunks of the tap matrix), OT (plane
+// element: float, or __nv_bfloat16 for the bf16-stored plane of PAPER.md:91), SPLIT (1: bf16 operands;
+// 3: the fp32 variant -- x = x1 + x2 and h = h1 + h2 in bf16 terms, products x1 h1 + x1 h2 + x2 h1
+// accumulated into the same TMEM columns, four Z parts, two tap images, ONE epilogue warp set).
+// The taps may carry a jerk (fdas_plan_create_jerk): h_{-z,w} = conj h_{z,w} keeps the +-|z| pairing.
 //
 // fdas_mma_convolve_kernel (any M: bulk copies need 16-byte aligned rows)
 //   warps 0-7   epilogue: tcgen05.ld -> |.|^2 -> st.global.cs (TMEM double-buffered)
