@@ -65,3 +65,45 @@ def test_noise_free_pulse_train_closed_form():
     assert abs(S[k, r] - (P[k0 + 2, 3000] + P[k0 + 4, 6000] + P[k0 + 6, 9000])) < 1e-9
     # and it beats the brightest single harmonic by the expected margin
     assert S[k, r] > 1.8 * P.max()
+
+
+def brute_drift(P, H, k0):
+    K, M = P.shape
+    S = np.zeros((K, M))
+    for k in range(K):
+        for r in range(M):
+            for h in range(1, H + 1):
+                kh, rh, t = k0 + h * (k - k0), h * r, h // 2
+                if not (0 <= kh < K and rh < M):
+                    continue
+                S[k, r] += max(P[a, b] for a in range(max(0, kh - t), min(K, kh + t + 1))
+                               for b in range(max(0, rh - t), min(M, rh + t + 1)))
+    return S
+
+
+def test_drift_tolerant_sum_brute_force_and_bounds():
+    rng = np.random.default_rng(3)
+    for K, M, k0 in ((7, 23, 3), (9, 40, 4), (1, 9, 0)):
+        P = rng.standard_exponential((K, M))
+        for H in (1, 2, 3, 5, 8):
+            S = oh.harmonic_sum_drift(P, H, k0)
+            np.testing.assert_allclose(S, brute_drift(P, H, k0), rtol=0, atol=1e-12)
+            assert (S >= oh.harmonic_sum(P, H, k0) - 1e-12).all()           # a maximum over a window that holds the centre
+    np.testing.assert_array_equal(oh.harmonic_sum_drift(P, 1, 0), P)
+
+
+def test_drift_tolerant_sum_recovers_an_off_grid_pulse_train():
+    # quantisation drifts the harmonics into adjacent bins.  Train at r0 = 3000.4, z = 4.6:
+    # harmonic 3 sits at (13.8, 9001.2) -> cell (row of z = 14, bin 9001), not at 3 x (row of 4, 3000).
+    w = workloads.harmonic_train(1 << 15, seed=1, r0=3000.4, z=4.6, power=50.0, rel_amplitudes=(1.0, 0.9, 0.8),
+                                 zmax=20.0, dz=2.0, seglen=1024, noise=False)
+    P = oracle.power_plane(w.spectrum, w.zmax, w.dz)
+    k0 = oh.zero_row(w.zmax, w.dz)
+    k1 = k0 + 2                                             # nearest row to z = 4.6 is z = 4
+    peaks = [P[k0 + 2, 3000], P[k0 + 5, 6001], P[k0 + 7, 9001]]   # nearest cells of the three harmonics
+    assert peaks[1] == P[k0 + 3:k0 + 6, 5999:6002].max() and peaks[2] == P[k0 + 5:k0 + 8, 8999:9002].max()
+    Sd = oh.harmonic_sum_drift(P, 3, k0)
+    Se = oh.harmonic_sum(P, 3, k0)
+    assert abs(Sd[k1, 3000] - sum(peaks)) < 1e-9
+    assert Se[k1, 3000] < 0.8 * Sd[k1, 3000]               # the exact-multiple sum misses the drifted harmonics
+    assert np.unravel_index(np.argmax(Sd), Sd.shape) == (k1, 3000)
