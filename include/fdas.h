@@ -210,6 +210,18 @@ int fdas_quick_cast(fdas_plan_t *p, const void *plane_bf16_dev, void *plane_f32_
 int fdas_harmonic_sum(fdas_plan_t *p, const void *plane_dev, void *sum_dev, int n_harmonics, void *stream);
 
 /*
+ * fdas_harmonic_sum_drift -- the drift-tolerant form ("Quantisation error in both the
+ * frequency and acceleration axes of the search lead to the observed peaks drifting into adjacent
+ * bins.  To account for this, a harmonic sum algorithm is used").  DESIGN.md reading A26: a signal
+ * detected in cell (k, r) lies within half a cell of it, so its h-th harmonic lies within h/2 cells of
+ * (k0 + h (k - k0), h r); harmonic h contributes the LARGEST power of that window:
+ *      S'[k][r] = sum_h max_{|dk|,|dr| <= floor(h/2)} P[k0 + h (k - k0) + dk][h r + dr]
+ * (window cells outside the plane are skipped; S' >= S of fdas_harmonic_sum; n_harmonics = 1 gives
+ * the plane).  Arguments, types and errors as fdas_harmonic_sum.
+ */
+int fdas_harmonic_sum_drift(fdas_plan_t *p, const void *plane_dev, void *sum_dev, int n_harmonics, void *stream);
+
+/*
  * fdas_band_max -- the paper's own peak selection (section 4.3, Table 3): the
  * plane is split into harmonic bands derived from the fundamental frequency f and "the n-th
  * harmonic is taken to be the highest point in the n-th band".  Band 0 (fundamental) holds the

@@ -31,7 +31,9 @@ template <> struct hs_elem<bf16bits> {
     }
 };
 
-template <typename IT, typename OT>
+// DRIFT (fdas_harmonic_sum_drift, reading A26): harmonic h contributes the largest
+// power of its quantisation window |dk|, |dr| <= h/2 around (k0 + h (k - k0), h r) instead of that cell alone.
+template <typename IT, typename OT, bool DRIFT>
 __global__ void __launch_bounds__(256) fdas_harmonic_sum_kernel(const IT *__restrict__ P, OT *__restrict__ S, int K, long long M,
                                                                 int k0, int H)
 {
@@ -49,10 +51,27 @@ __global__ void __launch_bounds__(256) fdas_harmonic_sum_kernel(const IT *__rest
             if (kh < 0 || kh >= K) continue;
             if (r * h >= M) break;                     // this and every further harmonic start beyond the plane
             const IT *rowh = P + (size_t)kh * M;
+            if (!DRIFT) {
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const long long x = (r + j) * h;
-                if (x < M) acc[j] += (OT)hs_elem<IT>::load(rowh + x);
+                for (int j = 0; j < 4; ++j) {
+                    const long long x = (r + j) * h;
+                    if (x < M) acc[j] += (OT)hs_elem<IT>::load(rowh + x);
+                }
+            } else {
+                const int t = h >> 1;
+                const int dk0 = kh - t < 0 ? (int)-kh : -t, dk1 = kh + t >= K ? (int)(K - 1 - kh) : t;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const long long x = (r + j) * h;
+                    if (x >= M) continue;
+                    const long long x0 = x - t < 0 ? 0 : x - t, x1 = x + t >= M ? M - 1 : x + t;
+                    OT best = (OT)hs_elem<IT>::load(rowh + x);
+                    for (int dk = dk0; dk <= dk1; ++dk) {
+                        const IT *rw = rowh + (long long)dk * M;
+                        for (long long xx = x0; xx <= x1; ++xx) best = max(best, (OT)hs_elem<IT>::load(rw + xx));
+                    }
+                    acc[j] += best;
+                }
             }
         }
         if (r + 3 < M && (M & 3) == 0 && sizeof(OT) == 4) {
@@ -67,7 +86,18 @@ __global__ void __launch_bounds__(256) fdas_harmonic_sum_kernel(const IT *__rest
 
 }  // namespace
 
-int fdas_launch_harmonic_sum(fdas_plan *p, const void *plane, void *sum, int n_harmonics, int k0, cudaStream_t st)
+template <bool DRIFT>
+static void launch_hs(fdas_plan *p, const void *plane, void *sum, int n_harmonics, int k0, dim3 grid, cudaStream_t st)
+{
+    if (p->precision == FDAS_F64)
+        fdas_harmonic_sum_kernel<double, double, DRIFT><<<grid, 256, 0, st>>>((const double *)plane, (double *)sum, p->K, p->M, k0, n_harmonics);
+    else if (p->plane_bf16)
+        fdas_harmonic_sum_kernel<bf16bits, float, DRIFT><<<grid, 256, 0, st>>>((const bf16bits *)plane, (float *)sum, p->K, p->M, k0, n_harmonics);
+    else
+        fdas_harmonic_sum_kernel<float, float, DRIFT><<<grid, 256, 0, st>>>((const float *)plane, (float *)sum, p->K, p->M, k0, n_harmonics);
+}
+
+int fdas_launch_harmonic_sum(fdas_plan *p, const void *plane, void *sum, int n_harmonics, int k0, int drift, cudaStream_t st)
 {
     const long long quads = (p->M + 3) / 4;
     long long bx = (quads + 255) / 256;
@@ -75,12 +105,8 @@ int fdas_launch_harmonic_sum(fdas_plan *p, const void *plane, void *sum, int n_h
     if (bx * p->K > cap) bx = (cap + p->K - 1) / p->K;
     if (bx < 1) bx = 1;
     const dim3 grid((unsigned)bx, (unsigned)p->K);
-    if (p->precision == FDAS_F64)
-        fdas_harmonic_sum_kernel<double, double><<<grid, 256, 0, st>>>((const double *)plane, (double *)sum, p->K, p->M, k0, n_harmonics);
-    else if (p->plane_bf16)
-        fdas_harmonic_sum_kernel<bf16bits, float><<<grid, 256, 0, st>>>((const bf16bits *)plane, (float *)sum, p->K, p->M, k0, n_harmonics);
-    else
-        fdas_harmonic_sum_kernel<float, float><<<grid, 256, 0, st>>>((const float *)plane, (float *)sum, p->K, p->M, k0, n_harmonics);
+    if (drift) launch_hs<true>(p, plane, sum, n_harmonics, k0, grid, st);
+    else launch_hs<false>(p, plane, sum, n_harmonics, k0, grid, st);
     FDAS_CUDA_TRY(p, cudaGetLastError());
     p->launches += 1;
     return FDAS_OK;

@@ -145,7 +145,7 @@ static inline int fdas_uses_mma(const fdas_plan *p)
 int fdas_launch_peaks(fdas_plan *p, const void *plane, float thr, fdas_peak_t *peaks, int capacity,
                       int *count, cudaStream_t st);
 // fdas_harmonic.cu: S_H[k][r] = sum_h P[k0 + h (k - k0)][h r]
-int fdas_launch_harmonic_sum(fdas_plan *p, const void *plane, void *sum, int n_harmonics, int k0, cudaStream_t st);
+int fdas_launch_harmonic_sum(fdas_plan *p, const void *plane, void *sum, int n_harmonics, int k0, int drift, cudaStream_t st);
 // fdas_rfft.cu: the real FFT ahead of the convolution
 int fdas_launch_spectrum(fdas_plan *p, const void *timeseries, void *spectrum, cudaStream_t st);
 // fdas_bands.cu: Table 3 band maxima

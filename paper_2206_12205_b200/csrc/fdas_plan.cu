@@ -162,13 +162,25 @@ extern "C" int fdas_quick_cast(fdas_plan_t *p, const void *plane_bf16_dev, void 
     return fdas_launch_quick_cast(p, plane_bf16_dev, plane_f32_dev, (long long)batch * p->K * p->M, (cudaStream_t)stream);
 }
 
+static int harmonic_sum_common(fdas_plan_t *p, const void *plane_dev, void *sum_dev, int n_harmonics, int drift, void *stream);
+
 extern "C" int fdas_harmonic_sum(fdas_plan_t *p, const void *plane_dev, void *sum_dev, int n_harmonics, void *stream)
+{
+    return harmonic_sum_common(p, plane_dev, sum_dev, n_harmonics, 0, stream);
+}
+
+extern "C" int fdas_harmonic_sum_drift(fdas_plan_t *p, const void *plane_dev, void *sum_dev, int n_harmonics, void *stream)
+{
+    return harmonic_sum_common(p, plane_dev, sum_dev, n_harmonics, 1, stream);
+}
+
+static int harmonic_sum_common(fdas_plan_t *p, const void *plane_dev, void *sum_dev, int n_harmonics, int drift, void *stream)
 {
     if (!p || !plane_dev || !sum_dev || n_harmonics < 1 || n_harmonics > 32) return FDAS_ERR_INVALID_ARG;
     // harmonic h of row z_k is row z = h z_k: on the grid iff z = 0 is (zmax a multiple of dz)
     const int k0 = (p->K - 1) / 2;
     if (fabs(-p->zmax + k0 * p->dz) > 1e-9 * (1.0 + p->zmax)) return FDAS_ERR_UNSUPPORTED;
-    return fdas_launch_harmonic_sum(p, plane_dev, sum_dev, n_harmonics, k0, (cudaStream_t)stream);
+    return fdas_launch_harmonic_sum(p, plane_dev, sum_dev, n_harmonics, k0, drift, (cudaStream_t)stream);
 }
 
 extern "C" int fdas_spectrum(fdas_plan_t *p, const void *timeseries_dev, void *spectrum_dev, void *stream)

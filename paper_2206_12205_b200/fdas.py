@@ -28,7 +28,7 @@ EXPORTS = [
     "fdas_convolve_host", "fdas_search_host", "fdas_templates_host", "fdas_taps_host",
     "fdas_launch_count", "fdas_status_string", "fdas_last_cuda_error",
     "fdas_set_algorithm", "fdas_get_algorithm", "fdas_tapmatrix_host", "fdas_search",
-    "fdas_set_plane_format", "fdas_get_plane_format", "fdas_quick_cast", "fdas_harmonic_sum", "fdas_band_max", "fdas_search_host_batched", "fdas_spectrum", "fdas_plan_create_jerk",
+    "fdas_set_plane_format", "fdas_get_plane_format", "fdas_quick_cast", "fdas_harmonic_sum", "fdas_harmonic_sum_drift", "fdas_band_max", "fdas_search_host_batched", "fdas_spectrum", "fdas_plan_create_jerk",
 ]
 
 
@@ -83,6 +83,7 @@ def lib() -> ctypes.CDLL:
     L.fdas_get_plane_format.argtypes = [vp, ctypes.POINTER(i)]
     L.fdas_quick_cast.argtypes = [vp, vp, vp, i, vp]
     L.fdas_harmonic_sum.argtypes = [vp, vp, vp, i, vp]
+    L.fdas_harmonic_sum_drift.argtypes = [vp, vp, vp, i, vp]
     L.fdas_band_max.argtypes = [vp, vp, dbl, i, vp, vp]
     L.fdas_spectrum.argtypes = [vp, vp, vp, vp]
     L.fdas_search_host_batched.argtypes = [vp, vp, i, ctypes.c_float, vp, i, vp, vp]
@@ -210,6 +211,10 @@ def fdas_harmonic_sum(h, plane_ptr, sum_ptr, n_harmonics, stream=0):
     return lib().fdas_harmonic_sum(h, plane_ptr, sum_ptr, int(n_harmonics), stream)
 
 
+def fdas_harmonic_sum_drift(h, plane_ptr, sum_ptr, n_harmonics, stream=0):
+    return lib().fdas_harmonic_sum_drift(h, plane_ptr, sum_ptr, int(n_harmonics), stream)
+
+
 def fdas_band_max(h, plane_ptr, f_bin, n_bands, out_ptr, stream=0):
     return lib().fdas_band_max(h, plane_ptr, float(f_bin), int(n_bands), out_ptr, stream)
 
@@ -284,8 +289,9 @@ class Plan:
             return torch.bfloat16          # the library writes bf16 bit patterns; torch reads them as bfloat16
         return torch.float64 if self.precision == FDAS_F64 else torch.float32
 
-    def harmonic_sum(self, plane, n_harmonics: int, out=None, stream: Optional[int] = None):
-        """fdas_harmonic_sum: S[k][r] = sum_h P[k0 + h (k - k0)][h r]."""
+    def harmonic_sum(self, plane, n_harmonics: int, out=None, stream: Optional[int] = None, drift: bool = False):
+        """fdas_harmonic_sum: S[k][r] = sum_h P[k0 + h (k - k0)][h r]; drift=True takes the
+        largest power of each harmonic's quantisation window (fdas_harmonic_sum_drift)."""
         import torch
         assert plane.is_cuda and plane.is_contiguous() and tuple(plane.shape) == (self.K, self.M)
         assert plane.dtype == self.plane_dtype()
@@ -295,7 +301,8 @@ class Plan:
         assert out.is_cuda and out.is_contiguous() and out.dtype == odt and tuple(out.shape) == (self.K, self.M)
         if stream is None:
             stream = torch.cuda.current_stream().cuda_stream
-        self._check(fdas_harmonic_sum(self._h, plane.data_ptr(), out.data_ptr(), n_harmonics, stream), "fdas_harmonic_sum")
+        fn = fdas_harmonic_sum_drift if drift else fdas_harmonic_sum
+        self._check(fn(self._h, plane.data_ptr(), out.data_ptr(), n_harmonics, stream), "fdas_harmonic_sum")
         return out
 
     def band_max(self, plane, f_bin: float, n_bands: int, stream: Optional[int] = None):

@@ -82,3 +82,36 @@ def test_harmonic_sum_errors(F):
     assert F.fdas_harmonic_sum(plan2._h, P.data_ptr(), S.data_ptr(), 33) == F.FDAS_ERR_INVALID_ARG
     assert F.fdas_harmonic_sum(plan2._h, 0, S.data_ptr(), 2) == F.FDAS_ERR_INVALID_ARG
     assert F.fdas_harmonic_sum(plan2._h, P.data_ptr(), S.data_ptr(), 2) == 0
+
+
+@pytest.mark.parametrize("K_zmax,M,prec", [(20.0, 4096, "f32"), (20.0, 4099, "f32"), (8.0, 1501, "f64"), (0.0, 1101, "f32")])
+def test_drift_tolerant_sum_on_seeded_planes(F, K_zmax, M, prec):
+    import torch
+    plan = F.Plan(2 * M, K_zmax, 2.0, 1024, prec, build=False)
+    rng = np.random.default_rng(M + 1)
+    P = rng.standard_exponential((plan.K, M)).astype(np.float64 if prec == "f64" else np.float32)
+    Pd = torch.from_numpy(P).cuda()
+    k0 = oh.zero_row(K_zmax, 2.0)
+    for H in (1, 2, 3, 5, 8):
+        S = plan.harmonic_sum(Pd, H, drift=True).cpu().numpy()
+        check_sum(S, oh.harmonic_sum_drift(P.astype(np.float64), H, k0), H, 2.0 ** -52 if prec == "f64" else 2.0 ** -23)
+
+
+def test_drift_tolerant_sum_gathers_an_off_grid_pulse_train(F):
+    # harmonics drift into adjacent bins; the exact-multiple sum misses them, the window sum does not
+    import torch
+    w = workloads.harmonic_train(1 << 18, seed=9, r0=9000.4, z=6.6, power=16.0, rel_amplitudes=(1.0, 0.9, 0.8, 0.7),
+                                 zmax=40.0, dz=2.0, seglen=1024)
+    plan = F.Plan(w.N, w.zmax, w.dz, w.seglen, "bf16")
+    P = plan.convolve(torch.from_numpy(w.spectrum).cuda())
+    Sd = plan.harmonic_sum(P, 4, drift=True)
+    Se = plan.harmonic_sum(P, 4)
+    assert bool((Sd >= Se).all())
+    k0 = oh.zero_row(w.zmax, w.dz)
+    cell = (k0 + 3, 9000)                                   # nearest cell of (z = 6.6, r0 = 9000.4)
+    exp = oh.harmonic_sum_drift(P.cpu().numpy().astype(np.float64), 4, k0)
+    assert abs(float(Sd[cell]) - exp[cell]) <= 4 * 2.0 ** -23 * exp[cell]
+    assert float(Sd[cell]) > 1.25 * float(Se[cell])
+    # the detection stands out of the summed noise where no single harmonic reaches the single-plane threshold
+    assert float(P.max().item()) < THRESH < float(Sd[cell])
+    assert float(Sd[cell]) >= 0.99 * float(Sd[:, 8000:10000].max().item())
