@@ -33,9 +33,23 @@ def stale() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False, extra_flags=(), out: str = LIB) -> str:
-    """extra_flags / out: build a tuning variant elsewhere (e.g. -DFDAS_F32_REGS=168)."""
+    """extra_flags / out: build a tuning variant elsewhere (e.g. -DFDAS_F32_REGS=168).
+    Safe to call from several processes at once (one rank per GPU): an exclusive file lock
+    serialises the compile and the others find the library fresh when they get the lock."""
     if not force and out == LIB and not stale():
         return LIB
+    import fcntl
+    with open(os.path.join(HERE, ".build.lock"), "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        try:
+            if not force and out == LIB and not stale():
+                return LIB
+            return _build_locked(verbose, extra_flags, out)
+        finally:
+            fcntl.flock(lock, fcntl.LOCK_UN)
+
+
+def _build_locked(verbose, extra_flags, out) -> str:
     objs = []
     procs = []
     for src in sources():
