@@ -63,6 +63,23 @@ def hsum_bytes(K, M, H, elem=4):
     return elem * (reads + K * M)
 
 
+def split_mma_columns(zmax, dz):
+    """Columns each 16-tap K step of the fp32 tensor-core form multiplies (one template group, symmetric grid):
+    templates whose taps do not reach a K step are skipped (fdas_mma.cu).  Accounting only."""
+    m_max = int(math.ceil(zmax / 2)) + 16
+    KS = -(-(2 * m_max + 1) // 16)
+    nz = int(math.floor(zmax / dz + 1e-9)) + 1
+    NT = -(-2 * nz // 16) * 16
+    cols = []
+    for ks in range(KS):
+        jhi = m_max - 16 * ks
+        jlo = jhi - 15
+        minabs = 0 if jlo <= 0 <= jhi else min(abs(jlo), abs(jhi))
+        need = sum(1 for e in range(nz) if int(math.ceil((zmax - e * dz) / 2)) + 16 >= minabs)
+        cols.append(min(NT, max(16, -(-4 * ((need + 1) // 2) // 16) * 16)))
+    return cols
+
+
 def nominal_flops(K, M, S, V):
     """per segment 5 S log2 S (forward) + K (6S + 5 S log2 S + 3V)."""
     n_seg = -(-M // V)
@@ -361,6 +378,7 @@ def main():
     NT = -(-2 * nz // 16) * 16
     KS = -(-(2 * (int(math.ceil(ZMAX / 2)) + 16) + 1) // 16)
     mma_flops = (-(-M // 128)) * 2 * KS * 2 * 128 * NT * 16
+    split_flops = (-(-M // 128)) * 2 * 3 * sum(2 * 128 * c * 16 for c in split_mma_columns(ZMAX, DZ))
     tensor_peak = float(peaks_json.get("bf16_tflops", 1590.0))
     tensor_src = "measured (MEASURED_PEAKS.json bf16_tflops, burst)" if "bf16_tflops" in peaks_json else "fallback 1.59 PFLOP/s"
     traffic = None
@@ -401,9 +419,10 @@ def main():
                             "flops_per_launch": mma_flops, "peak_source": tensor_src,
                             "count": "issued dense MMA flops: tiles x 2 parts x 9 K-steps x 2*128*112*16 (padding included)"},
         "roofline_tensor_fp32": {"bound": "tensor", "kernel": "fdas_mma_bulk_kernel<7,float,3> (fdas_convolve, fp32 variant: bf16 x 3 split operands)",
-                                 "achieved": 3 * mma_flops / (rf["conv_ms"] * 1e-3) / 1e12, "peak": tensor_peak, "unit": "TFLOP/s",
-                                 "frac": 3 * mma_flops / (rf["conv_ms"] * 1e-3) / 1e12 / tensor_peak, "flops_per_launch": 3 * mma_flops,
-                                 "peak_source": tensor_src, "count": "issued dense MMA flops: 3 products per tap"},
+                                 "achieved": split_flops / (rf["conv_ms"] * 1e-3) / 1e12, "peak": tensor_peak, "unit": "TFLOP/s",
+                                 "frac": split_flops / (rf["conv_ms"] * 1e-3) / 1e12 / tensor_peak, "flops_per_launch": split_flops,
+                                 "peak_source": tensor_src,
+                                 "count": "issued dense MMA flops: 3 products per tap, columns per K step " + str(split_mma_columns(ZMAX, DZ))},
         "roofline_alu_fp32_fft": {"bound": "alu", "kernel": "fdas_convolve_kernel<TraitsF32,2048>",
                                   "achieved": flops / (rff["conv_ms"] * 1e-3) / 1e12, "peak": alu_peak,
                                   "unit": "TFLOP/s", "frac": flops / (rff["conv_ms"] * 1e-3) / 1e12 / alu_peak,

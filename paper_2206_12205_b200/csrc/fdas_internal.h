@@ -29,6 +29,8 @@ struct fdas_plan {
     int algo;          // fdas_algorithm_t requested by the caller
     int tc_supported;  // the MMA kernel can run this shape
     int tc_groups, tc_nzg, tc_NT, tc_KS, tc_full_chunks;
+    unsigned long long tc_nks_lo[8], tc_nks_hi[8];   // columns per K step (nibble = columns / 16; 0 = all), per group
+    int tc_ks_first[8];                               // a K step that runs at full width (initialises the accumulators)
     int tc_force_scalar_stores;   // testing: run the generic (scalar-store) tensor-core kernel
     void *tc_bmat;     // [groups][2 KS][NT][8] bf16
     size_t tc_bmat_bytes;
