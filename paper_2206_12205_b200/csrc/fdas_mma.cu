@@ -937,13 +937,26 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
                     const int cnt_n = rg.y & 0xFFFF, cnt_p = rg.w & 0xFFFF;
                     if (col0 + lt < p.M) {
                         OT *const out = static_cast<OT *>(p.planes) + (size_t)ser * p.K * p.M + col0 + lt;
+                        const uint32_t Mu = (uint32_t)p.M;
+                        if (cnt_n == 2 * NCH && cnt_p == 2 * NCH) {
+                            // full column group: straight-line code, row offsets by addition
+                            uint32_t offn = (uint32_t)rg.x * Mu, offp = (uint32_t)(rg.z + cnt_p - 1) * Mu;
 #pragma unroll
-                        for (int pr = 0; pr < NCH; ++pr) {
+                            for (int el = 0; el < 2 * NCH; ++el) {
+                                st_cs_at<OT>(out, offn, pw[pass][4 * (el >> 1) + (el & 1)]);
+                                st_cs_at<OT>(out, offp, pw[pass][4 * (el >> 1) + 2 + (el & 1)]);
+                                offn += Mu;
+                                offp -= Mu;
+                            }
+                        } else {
 #pragma unroll
-                            for (int e = 0; e < 2; ++e) {
-                                const int el = 2 * pr + e;
-                                if (el < cnt_n) st_cs_at<OT>(out, (uint32_t)((long long)(rg.x + el) * p.M), pw[pass][4 * pr + e]);
-                                if (el < cnt_p) st_cs_at<OT>(out, (uint32_t)((long long)(rg.z + cnt_p - 1 - el) * p.M), pw[pass][4 * pr + 2 + e]);
+                            for (int pr = 0; pr < NCH; ++pr) {
+#pragma unroll
+                                for (int e = 0; e < 2; ++e) {
+                                    const int el = 2 * pr + e;
+                                    if (el < cnt_n) st_cs_at<OT>(out, (uint32_t)(rg.x + el) * Mu, pw[pass][4 * pr + e]);
+                                    if (el < cnt_p) st_cs_at<OT>(out, (uint32_t)(rg.z + cnt_p - 1 - el) * Mu, pw[pass][4 * pr + 2 + e]);
+                                }
                             }
                         }
                     }
