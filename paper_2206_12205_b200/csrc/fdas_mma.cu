@@ -940,13 +940,23 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
                         const uint32_t Mu = (uint32_t)p.M;
                         if (cnt_n == 2 * NCH && cnt_p == 2 * NCH) {
                             // full column group: straight-line code, row offsets by addition
-                            uint32_t offn = (uint32_t)rg.x * Mu, offp = (uint32_t)(rg.z + cnt_p - 1) * Mu;
+                            // two running row pointers, each advanced by one IMAD.WIDE (ptr += +-M * sizeof(OT))
+                            long long pn, pp;
+                            asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(pn) : "r"((uint32_t)rg.x * Mu), "n"((int)sizeof(OT)), "l"(out));
+                            asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(pp) : "r"((uint32_t)(rg.z + cnt_p - 1) * Mu), "n"((int)sizeof(OT)), "l"(out));
+                            const int Mi = (int)Mu;
 #pragma unroll
                             for (int el = 0; el < 2 * NCH; ++el) {
-                                st_cs_at<OT>(out, offn, pw[pass][4 * (el >> 1) + (el & 1)]);
-                                st_cs_at<OT>(out, offp, pw[pass][4 * (el >> 1) + 2 + (el & 1)]);
-                                offn += Mu;
-                                offp -= Mu;
+                                const float vn = pw[pass][4 * (el >> 1) + (el & 1)], vp = pw[pass][4 * (el >> 1) + 2 + (el & 1)];
+                                if constexpr (sizeof(OT) == 2) {
+                                    asm volatile("st.global.cs.u16 [%0], %1;" ::"l"(pn), "h"(__bfloat16_as_ushort(__float2bfloat16_rn(vn))) : "memory");
+                                    asm volatile("st.global.cs.u16 [%0], %1;" ::"l"(pp), "h"(__bfloat16_as_ushort(__float2bfloat16_rn(vp))) : "memory");
+                                } else {
+                                    asm volatile("st.global.cs.f32 [%0], %1;" ::"l"(pn), "f"(vn) : "memory");
+                                    asm volatile("st.global.cs.f32 [%0], %1;" ::"l"(pp), "f"(vp) : "memory");
+                                }
+                                asm("mad.wide.s32 %0, %1, %2, %0;" : "+l"(pn) : "r"(Mi), "n"((int)sizeof(OT)));
+                                asm("mad.wide.s32 %0, %1, %2, %0;" : "+l"(pp) : "r"(-Mi), "n"((int)sizeof(OT)));
                             }
                         } else {
 #pragma unroll
