@@ -382,9 +382,12 @@ def main():
     tensor_peak = float(peaks_json.get("bf16_tflops", 1590.0))
     tensor_src = "measured (MEASURED_PEAKS.json bf16_tflops, burst)" if "bf16_tflops" in peaks_json else "fallback 1.59 PFLOP/s"
     traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    tp = os.path.join(ROOT, "profiles", "traffic.csv")       # ncu dram__bytes_read.sum + dram__bytes_write.sum per launch
     if os.path.exists(tp):
-        traffic = json.load(open(tp)).get("bf16_conv_dram_bytes_per_launch")
+        import csv
+        for row in csv.DictReader(open(tp)):
+            if row["key"] == "bf16_conv":
+                traffic = float(row["dram_bytes_per_launch"])
 
     cpu = None
     if not args.no_cpu_baseline:
