@@ -32,29 +32,28 @@ def stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False, extra_flags=(), out: str = LIB) -> str:
-    """extra_flags / out: build a tuning variant elsewhere (e.g. -DFDAS_F32_REGS=168).
-    Safe to call from several processes at once (one rank per GPU): an exclusive file lock
+def build(force: bool = False, verbose: bool = False) -> str:
+    """Safe to call from several processes at once (one rank per GPU): an exclusive file lock
     serialises the compile and the others find the library fresh when they get the lock."""
-    if not force and out == LIB and not stale():
+    if not force and not stale():
         return LIB
     import fcntl
     with open(os.path.join(HERE, ".build.lock"), "w") as lock:
         fcntl.flock(lock, fcntl.LOCK_EX)
         try:
-            if not force and out == LIB and not stale():
+            if not force and not stale():
                 return LIB
-            return _build_locked(verbose, extra_flags, out)
+            return _build_locked(verbose)
         finally:
             fcntl.flock(lock, fcntl.LOCK_UN)
 
 
-def _build_locked(verbose, extra_flags, out) -> str:
+def _build_locked(verbose) -> str:
     objs = []
     procs = []
     for src in sources():
-        obj = (out[:-3] + "_" if out != LIB else os.path.join(CSRC, "")) + os.path.basename(src)[:-3] + ".o"
-        cmd = [NVCC, *FLAGS, *extra_flags, "-c", src, "-o", obj]
+        obj = os.path.join(CSRC, os.path.basename(src)[:-3] + ".o")
+        cmd = [NVCC, *FLAGS, "-c", src, "-o", obj]
         if verbose:
             cmd[1:1] = ["-Xptxas", "-v"]
         procs.append((src, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
@@ -67,8 +66,8 @@ def _build_locked(verbose, extra_flags, out) -> str:
         failed |= pr.returncode != 0
     if failed:
         raise RuntimeError("nvcc failed")
-    subprocess.run([NVCC, "-shared", "-o", out, *objs, "-lcudart"], check=True)
-    return out
+    subprocess.run([NVCC, "-shared", "-o", LIB, *objs, "-lcudart"], check=True)
+    return LIB
 
 
 if __name__ == "__main__":

@@ -11,6 +11,14 @@
 #define FDAS_MAX_BANDS 32     // harmonic bands one fdas_band_max call can take
 #define FDAS_TC_MAX_BOXES 8   // distinct plane-row run lengths the tensor-core kernel's box stores can serve
 
+// Kernels that need the opt-in to more than 48 KB of dynamic shared memory.  The opt-in is a per-device function
+// attribute; a plan lives on one device, so the largest size requested so far is remembered per plan.
+enum {
+    FDAS_OPTIN_FFT = 0, FDAS_OPTIN_MMA_BULK, FDAS_OPTIN_MMA_BULK16, FDAS_OPTIN_MMA_SPLIT, FDAS_OPTIN_MMA_SCALAR,
+    FDAS_OPTIN_MMA_SCALAR16, FDAS_OPTIN_MMA_NOPLANE, FDAS_OPTIN_MMA_NOPLANE_SPLIT, FDAS_OPTIN_MMA_RECHECK,
+    FDAS_OPTIN_MMA_RECHECK_SPLIT, FDAS_OPTIN_RFFT_COLS, FDAS_OPTIN_RFFT_ROWS, FDAS_OPTIN_HSUM, FDAS_OPTIN_SLOTS
+};
+
 struct fdas_plan {
     // problem shape
     int64_t N, M;
@@ -68,6 +76,7 @@ struct fdas_plan {
     void *band_scratch;
     size_t band_scratch_bytes;
     // bookkeeping
+    size_t smem_optin[FDAS_OPTIN_SLOTS];   // dynamic shared memory already opted in to, per kernel kind (this plan's device)
     int device, num_sms;
     cudaError_t last_err;
     int64_t launches;
@@ -124,6 +133,15 @@ struct fdas_search_args {
             return FDAS_ERR_CUDA;                               \
         }                                                       \
     } while (0)
+
+template <class Kern>
+static inline int fdas_optin_smem(fdas_plan *p, int slot, Kern kern, size_t bytes)
+{
+    if (bytes <= p->smem_optin[slot] || bytes <= 48u * 1024u) return FDAS_OK;
+    FDAS_CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    p->smem_optin[slot] = bytes;
+    return FDAS_OK;
+}
 
 // implemented in fdas_templates.cu / fdas_convolve.cu / fdas_peaks.cu
 int fdas_launch_build_templates(fdas_plan *p, cudaStream_t st);

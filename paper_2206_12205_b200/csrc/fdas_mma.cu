@@ -68,7 +68,9 @@ constexpr int TC_LOAD_THREADS = 32 * TC_LOAD_WARPS;
 constexpr int TC_THREADS = 32 * (TC_EPI_WARPS + 1 + TC_LOAD_WARPS);   // 384
 constexpr int TC_TMEM_COLS = 512;       // whole TMEM: 2 stages x (re | im) x NT <= 128 columns
 constexpr int TC_STAGE_COLS = 256;
-constexpr long long TC_SPIN_LIMIT = 1LL << 26;   // a stuck pipeline traps instead of hanging the GPU
+#ifdef FDAS_SPIN_TRAP   // debug builds only (-DFDAS_SPIN_TRAP): a stuck pipeline traps instead of hanging the GPU
+constexpr long long TC_SPIN_LIMIT = 1LL << 26;
+#endif
 
 struct TcParams {
     const float2 *spectra;   // [batch][M] complex64
@@ -92,17 +94,6 @@ struct TcParams {
     fdas_search_args search; // fused threshold pass (fdas_search); enabled = 0 for plain fdas_convolve
 };
 
-#ifdef FDAS_MMA_TRACE   // tuning builds only: clock64 time line of CTA 0 (warp, tile, event)
-__device__ long long g_trace[24][64][16];
-#define TR(tile_idx, ev)                                                                              \
-    do {                                                                                              \
-        if (blockIdx.x == 0 && (threadIdx.x & 31) == 0 && (tile_idx) >= 64u && (tile_idx) < 128u)     \
-            g_trace[threadIdx.x >> 5][(tile_idx) - 64u][ev] = clock64();                              \
-    } while (0)
-#else
-#define TR(tile_idx, ev)
-#endif
-
 // ---- PTX wrappers ---------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -118,7 +109,9 @@ template <int SLEEP_NS = 0>
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
     uint32_t done;
+#ifdef FDAS_SPIN_TRAP
     long long spins = 0;
+#endif
     do {
         asm volatile(
             "{\n\t.reg .pred p;\n\t"
@@ -128,7 +121,9 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
             : "r"(bar), "r"(parity)
             : "memory");
         if (!done) {
+#ifdef FDAS_SPIN_TRAP
             if (++spins > TC_SPIN_LIMIT) __trap();
+#endif
             if (SLEEP_NS > 0) __nanosleep(SLEEP_NS);
         }
     } while (!done);
@@ -338,9 +333,6 @@ __device__ __forceinline__ void epilogue_tile(uint32_t taddr, const uint4 *otab4
             __syncwarp();
             if (lane == 0) mbar_arrive(empty_bar);
         }
-#ifdef FDAS_MMA_DEBUG_NOSTORE
-        ok = false; inside = false;
-#endif
         float mx;
         if (inside && c < full_chunks) mx = epilogue_chunk<true, OT>(v[i & 1], otab4 + 4 * c, out, true);
         else mx = epilogue_chunk<false, OT>(v[i & 1], otab4 + 4 * c, out, ok);
@@ -413,17 +405,13 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
         const long long blk0 = (long long)(it % (uint32_t)p.n_blocks) * p.R;
         const long long left = p.M - blk0;
         const int n_tiles = (int)((left < p.R ? left : p.R) + TC_TILE - 1) / TC_TILE;
-        TR(t, 3);
         mbar_wait(z_full + 8 * buf, zuse & 1);
         tc_fence_after();
-        TR(t, 4);
         const uint32_t z_addr = s_base + off_z + buf * z_buf_bytes;
         for (int tile = 0; tile < n_tiles; ++tile, ++t) {
             const uint32_t stage = t & 1, use = t >> 1;
-            TR(t, 0);
             mbar_wait(t_empty + 8 * stage, (use & 1) ^ 1);
             tc_fence_after();
-            TR(t, 1);
             const uint32_t d_re = tmem_base + stage * TC_STAGE_COLS, d_im = d_re + NT;
             // descriptors advance by adding to their 14-bit address field (units of 16 bytes; shared
             // memory is < 256 KB, so no carry leaves the field)
@@ -468,7 +456,6 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
                 }
             }
             umma_commit_elected(t_full + 8 * stage, elected);
-            TR(t, 2);
         }
         umma_commit_elected(z_empty + 8 * buf, elected);
     }
@@ -863,16 +850,8 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
                 const uint32_t sblk = SETS == 2 ? stage : 0;   // staging buffer of this tile (per column group)
                 const long long col0 = blk0 + tile * TC_TILE;
                 const uint32_t taddr0 = tmem_base + ((uint32_t)(q * 32) << 16) + stage * TC_STAGE_COLS;
-                TR(t, 0);
                 mbar_wait(t_full + 8 * stage, use & 1);
                 tc_fence_after();
-                TR(t, 1);
-#ifdef FDAS_MMA_DEBUG_NOEPI
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(t_empty + 8 * stage);
-                continue;
-#endif
                 // ---- TMEM -> powers in registers, for both column groups, then hand the stage back at once:
                 // the MMA of tile t+2 never waits for the store path (shared-memory staging, TMA backlog)
                 float pw[2][NC];   // per column group: (pm0, pm1, pp0, pp1) of each entry pair
@@ -926,7 +905,6 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
                     }
                     mx2[pass] = stored_value<OT>(mx);   // rounding is monotone: the largest stored value
                 }
-                TR(t, 2);
                 // bf16-stored plane: the powers go straight from registers to the plane (one 64-byte row segment per
                 // warp and store).  Measured on config 3: 0.291 ms against 0.317 ms through staging + box stores (the
                 // 16-bit staging stores cost more shared-memory time than the halved bytes save); for the float plane
@@ -987,9 +965,7 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
                     // staging block (cg, stage) last fed this issuer's store of two commits ago (tile t-2, same
                     // pass): at most the newest group may still be reading shared memory
                     if (issuer) bulk_wait_read<1>();
-                    TR(t, 3 + 5 * pass);
                     named_bar_sync(bar_id, 128);
-                    TR(t, 4 + 5 * pass);
                     unsigned char *const stage_buf = smem + L.off_stage + (size_t)(SETS * cg + sblk) * L.stage_cg_bytes;
                     OT *const sb = reinterpret_cast<OT *>(stage_buf) + lt;
 #pragma unroll
@@ -999,23 +975,18 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
                         sb[(NC - 1 - 2 * pr) * TC_TILE] = (OT)pw[pass][4 * pr + 2];
                         sb[(NC - 2 - 2 * pr) * TC_TILE] = (OT)pw[pass][4 * pr + 3];
                     }
-                    TR(t, 5 + 5 * pass);
                     fence_proxy_async();                    // staging writes -> visible to the bulk copy engine
                     named_bar_sync(bar_id, 128);
-                    TR(t, 6 + 5 * pass);
                     if (issuer) {
                         const uint32_t sst = smem_u32(stage_buf);
                         const int row_s = (int)ser * p.K;
-#ifndef FDAS_MMA_DEBUG_NOSTORE
                         // one box per run: warp q = 0 pushes the -|z| rows, warp q = 1 the +|z| rows
                         const int cnt = (q ? rg.w : rg.y) & 0xFFFF, box = (q ? rg.w : rg.y) >> 16;
                         if (cnt > 0)
                             tensor_store(&maps.m[box], sst + (q ? (uint32_t)(NC - cnt) * ROWB : 0u), (int)col0,
                                          row_s + (q ? rg.z : rg.x));
-#endif
                         bulk_commit();                      // one group per pass, empty or not: bulk_wait_read<1> counts them
                     }
-                    TR(t, 7 + 5 * pass);
                     if (mx2[pass] > thr && col0 + lt < p.M && 2 * cg * NCH < p.nzg)
                         flag_candidate(p.search.cand, p.search.cand_count, p.search.cand_capacity,
                                        grp * p.nzg + 2 * cg * NCH, (int)(col0 + lt), mx2[pass]);
@@ -1079,13 +1050,6 @@ __global__ void fdas_tapmatrix_kernel(__nv_bfloat16 *bmat, const double2 *__rest
 }
 
 }  // namespace
-
-#ifdef FDAS_MMA_TRACE
-extern "C" int fdas_debug_trace(void *dst_host)
-{
-    return (int)cudaMemcpyFromSymbol(dst_host, g_trace, sizeof(g_trace));
-}
-#endif
 
 // Host: the |z| grouping.  Templates z_k = -zmax + k dz pair up as (k, K-1-k) when zmax is a
 // multiple of dz; otherwise every template stands alone.
@@ -1302,11 +1266,7 @@ template <int NCH>
 static int launch_mma_split(fdas_plan *p, const TcParams &tp, unsigned gx, size_t smem_bytes, const TbMaps *maps, cudaStream_t st)
 {
     auto kern = fdas_mma_bulk_kernel<NCH, float, 3>;
-    static size_t attr_bytes = 0;
-    if (smem_bytes > attr_bytes) {
-        FDAS_CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
-        attr_bytes = smem_bytes;
-    }
+    { const int rc = fdas_optin_smem(p, FDAS_OPTIN_MMA_SPLIT, kern, smem_bytes); if (rc) return rc; }
     kern<<<dim3(gx, p->tc_groups), tb_threads(3), smem_bytes, st>>>(tp, *maps);
     FDAS_CUDA_TRY(p, cudaGetLastError());
     p->launches += 1;
@@ -1318,19 +1278,11 @@ static int launch_mma(fdas_plan *p, const TcParams &tp, unsigned gx, size_t smem
 {
     if (maps) {
         auto kern = fdas_mma_bulk_kernel<NCH, OT, 1>;
-        static size_t attr_bytes = 0;
-        if (smem_bytes > attr_bytes) {
-            FDAS_CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
-            attr_bytes = smem_bytes;
-        }
+        { const int rc = fdas_optin_smem(p, sizeof(OT) == 2 ? FDAS_OPTIN_MMA_BULK16 : FDAS_OPTIN_MMA_BULK, kern, smem_bytes); if (rc) return rc; }
         kern<<<dim3(gx, p->tc_groups), tb_threads(1), smem_bytes, st>>>(tp, *maps);
     } else {
         auto kern = fdas_mma_convolve_kernel<NCH, OT>;
-        static size_t attr_bytes = 0;
-        if (smem_bytes > attr_bytes) {
-            FDAS_CUDA_TRY(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
-            attr_bytes = smem_bytes;
-        }
+        { const int rc = fdas_optin_smem(p, sizeof(OT) == 2 ? FDAS_OPTIN_MMA_SCALAR16 : FDAS_OPTIN_MMA_SCALAR, kern, smem_bytes); if (rc) return rc; }
         kern<<<dim3(gx, p->tc_groups), TC_THREADS, smem_bytes, st>>>(tp);
     }
     FDAS_CUDA_TRY(p, cudaGetLastError());
@@ -1365,9 +1317,6 @@ int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, in
         const long long items = (long long)batch * ((p->M + R - 1) / R);
         if (R == 128 || (smem_total(R) <= smem_cap && items >= 2LL * sms_per_group)) break;
     }
-#ifdef FDAS_MMA_TUNE
-    if (getenv("FDAS_TC_R")) R = atoi(getenv("FDAS_TC_R"));
-#endif
     const uint32_t total = smem_total(R);
     if (total > smem_cap) return FDAS_ERR_UNSUPPORTED;
     TcParams tp;

@@ -273,11 +273,25 @@ static int search_on_device(fdas_plan *p, const void *spectrum_dev, void *plane_
         if (rc) return rc;
         return fdas_launch_peaks(p, plane_dev, threshold, peaks_dev, capacity, count_dev, st);
     }
-    if (!p->cand) {
+    if (!p->cand || !p->cand_ctr) {   // both or neither: a failed second allocation must not leave a NULL counter behind
+        cudaFree(p->cand);
+        cudaFree(p->cand_ctr);
+        p->cand = NULL;
+        p->cand_ctr = NULL;
         p->cand_capacity = 1 << 18;
-        FDAS_CUDA_TRY(p, cudaMalloc((void **)&p->cand, sizeof(fdas_peak_t) * (size_t)p->cand_capacity));
-        FDAS_CUDA_TRY(p, cudaMalloc((void **)&p->cand_ctr, 2 * sizeof(int)));
-        FDAS_CUDA_TRY(p, cudaMemsetAsync(p->cand_ctr, 0, 2 * sizeof(int), st));
+        fdas_peak_t *c = NULL;
+        int *ctr = NULL;
+        cudaError_t e = cudaMalloc((void **)&c, sizeof(fdas_peak_t) * (size_t)p->cand_capacity);
+        if (e == cudaSuccess) e = cudaMalloc((void **)&ctr, 2 * sizeof(int));
+        if (e == cudaSuccess) e = cudaMemsetAsync(ctr, 0, 2 * sizeof(int), st);
+        if (e != cudaSuccess) {
+            cudaFree(c);
+            cudaFree(ctr);
+            p->last_err = e;
+            return e == cudaErrorMemoryAllocation ? FDAS_ERR_ALLOC : FDAS_ERR_CUDA;
+        }
+        p->cand = c;
+        p->cand_ctr = ctr;
     }
     fdas_search_args sa;
     sa.enabled = 1;

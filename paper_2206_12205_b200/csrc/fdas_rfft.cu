@@ -88,13 +88,9 @@ __device__ __forceinline__ void smem_fft_dif(float2 *s, int logn, int nbatch, in
 
 __device__ __forceinline__ unsigned bitrev(unsigned v, int bits) { return bits ? __brev(v) >> (32 - bits) : 0u; }
 
-#ifndef FDAS_RF_CB
-#define FDAS_RF_CB 8
-#define FDAS_RF_RB 2
-#define FDAS_RF_L2MAX 12
-#endif
-constexpr int RF_CB = FDAS_RF_CB;    // columns per CTA in pass A (64-byte segments; 64 KB of shared memory -> 3 CTAs per SM)
-constexpr int RF_RB = FDAS_RF_RB;    // rows per CTA in pass B
+constexpr int RF_CB = 8;      // columns per CTA in pass A (64-byte segments; 64 KB of shared memory -> 3 CTAs per SM)
+constexpr int RF_RB = 2;      // rows per CTA in pass B
+constexpr int RF_L2MAX = 12;  // log2 of the longest row FFT
 
 // pass A: z viewed as [L1][L2]; this CTA takes columns m2 = 16 blockIdx.x .. +15
 __global__ void __launch_bounds__(512) fdas_rfft_cols_kernel(const float2 *__restrict__ z, float2 *__restrict__ Y, int l1, int l2)
@@ -166,18 +162,14 @@ int fdas_launch_spectrum(fdas_plan *p, const void *timeseries, void *spectrum, c
     int n = 0;
     while ((1LL << n) < p->N) ++n;
     if ((1LL << n) != p->N || n < 10 || n > 23) return FDAS_ERR_UNSUPPORTED;
-    const int l = n - 1, l2 = l < FDAS_RF_L2MAX ? l : FDAS_RF_L2MAX, l1 = l - l2;
+    const int l = n - 1, l2 = l < RF_L2MAX ? l : RF_L2MAX, l1 = l - l2;
     const size_t L = (size_t)1 << l;
     if (!p->rfft_scratch) FDAS_CUDA_TRY(p, cudaMalloc(&p->rfft_scratch, 2 * L * sizeof(float2)));
     float2 *Y = static_cast<float2 *>(p->rfft_scratch), *Z = Y + L;
     const float2 *z = static_cast<const float2 *>(timeseries);
     if (l1 > 0) {
         const size_t smem = ((size_t)(1 << l1) * RF_CB + (1 << l1) / 2) * sizeof(float2);
-        static size_t attr = 0;
-        if (smem > attr) {
-            FDAS_CUDA_TRY(p, cudaFuncSetAttribute(fdas_rfft_cols_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            attr = smem;
-        }
+        { const int rc = fdas_optin_smem(p, FDAS_OPTIN_RFFT_COLS, fdas_rfft_cols_kernel, smem); if (rc) return rc; }
         fdas_rfft_cols_kernel<<<(1 << l2) / RF_CB, 512, smem, st>>>(z, Y, l1, l2);
         FDAS_CUDA_TRY(p, cudaGetLastError());
         p->launches += 1;
@@ -185,11 +177,7 @@ int fdas_launch_spectrum(fdas_plan *p, const void *timeseries, void *spectrum, c
     {
         const int rb = l1 >= 2 ? RF_RB : 1;
         const size_t smem = ((size_t)(1 << l2) * rb + (1 << l2) / 2) * sizeof(float2);
-        static size_t attr = 0;
-        if (smem > attr) {
-            FDAS_CUDA_TRY(p, cudaFuncSetAttribute(fdas_rfft_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            attr = smem;
-        }
+        { const int rc = fdas_optin_smem(p, FDAS_OPTIN_RFFT_ROWS, fdas_rfft_rows_kernel, smem); if (rc) return rc; }
         fdas_rfft_rows_kernel<<<(1 << l1) / rb, 512, smem, st>>>(l1 > 0 ? Y : z, Z, l1, l2, rb);
         FDAS_CUDA_TRY(p, cudaGetLastError());
         p->launches += 1;

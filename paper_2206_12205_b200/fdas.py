@@ -11,7 +11,7 @@ import os
 from typing import Optional
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("FDAS_LIBRARY", os.path.join(_HERE, "libfdas.so"))   # FDAS_LIBRARY: alternative build of the same library
+LIB_PATH = os.path.join(_HERE, "libfdas.so")
 
 FDAS_F64, FDAS_F32, FDAS_BF16 = 0, 1, 2
 FDAS_OK, FDAS_ERR_INVALID_ARG, FDAS_ERR_ALLOC, FDAS_ERR_CUDA, FDAS_ERR_NOT_BUILT, FDAS_ERR_UNSUPPORTED = range(6)
@@ -248,7 +248,7 @@ class Plan:
     torch's; all arithmetic is the library's)."""
 
     def __init__(self, N: int, zmax: float, dz: float, seglen: int, precision="f32", build: bool = True,
-                 stream: int = 0, algorithm="auto", plane="f32", jerk: float = 0.0):
+                 stream: Optional[int] = None, algorithm="auto", plane="f32", jerk: float = 0.0):
         prec = PRECISIONS[precision] if isinstance(precision, str) else int(precision)
         rc, self._h = fdas_plan_create_jerk(N, zmax, dz, jerk, seglen, prec) if jerk else fdas_plan_create(N, zmax, dz, seglen, prec)
         if rc:
@@ -348,7 +348,12 @@ class Plan:
         self._check(fdas_spectrum(self._h, timeseries.data_ptr(), out.data_ptr(), stream), "fdas_spectrum")
         return out
 
-    def build_templates(self, stream: int = 0):
+    def build_templates(self, stream: Optional[int] = None):
+        """Enqueued on torch's current stream unless one is given, like every other call: the build must
+        precede fdas_convolve in stream order (include/fdas.h)."""
+        if stream is None:
+            import torch
+            stream = torch.cuda.current_stream().cuda_stream if torch.cuda.is_available() else 0
         self._check(fdas_build_templates(self._h, stream), "fdas_build_templates")
 
     def convolve(self, spectrum, plane=None, stream: Optional[int] = None):
@@ -410,19 +415,23 @@ class Plan:
         rec["power"] = raw[:, 2].copy().view(np.float32)
         return plane, n, rec
 
-    def convolve_host(self, spectrum_host, plane_host, stream: int = 0):
+    def convolve_host(self, spectrum_host, plane_host, stream: Optional[int] = None):
         """numpy or pinned torch CPU buffers; copies are inside the call."""
+        stream = _current_stream(stream)
         self._check(fdas_convolve_host(self._h, _host_ptr(spectrum_host), _host_ptr(plane_host), stream),
                     "fdas_convolve_host")
         return plane_host
 
-    def search_host(self, spectrum_host, threshold: float, peaks_host, capacity: int, stream: int = 0):
+    def search_host(self, spectrum_host, threshold: float, peaks_host, capacity: int, stream: Optional[int] = None):
+        stream = _current_stream(stream)
         rc, n = fdas_search_host(self._h, _host_ptr(spectrum_host), threshold, _host_ptr(peaks_host), capacity, stream)
         self._check(rc, "fdas_search_host")
         return n
 
-    def search_host_batched(self, spectra_host, threshold: float, peaks_host, counts_host, capacity: int, stream: int = 0):
+    def search_host_batched(self, spectra_host, threshold: float, peaks_host, counts_host, capacity: int,
+                            stream: Optional[int] = None):
         """spectra_host [B, M]; peaks_host >= B*capacity records (12 bytes each); counts_host [B] int32 (numpy or pinned torch)."""
+        stream = _current_stream(stream)
         n = int(spectra_host.shape[0])
         self._check(fdas_search_host_batched(self._h, _host_ptr(spectra_host), n, threshold, _host_ptr(peaks_host), capacity,
                                              _host_ptr(counts_host), stream), "fdas_search_host_batched")
@@ -473,6 +482,14 @@ class Plan:
             self.close()
         except Exception:
             pass
+
+
+def _current_stream(stream: Optional[int]) -> int:
+    """torch's current stream when the caller names none (the stream the templates were built on by default)."""
+    if stream is not None:
+        return stream
+    import torch
+    return torch.cuda.current_stream().cuda_stream
 
 
 def _host_ptr(buf) -> int:
