@@ -27,7 +27,9 @@
  *     synchronise.
  *   - Output is bit-reproducible run to run (no atomics touch the plane).  The ORDER of
  *     peak records is unspecified.
- *   - A plan may be used from one host thread at a time; distinct plans are independent.
+ *   - A plan may be used from one host thread and on one stream at a time (its scratch buffers, candidate
+ *     lists and tensor-map caches are per plan, not per call); distinct plans are independent.  A plan
+ *     belongs to the device that was current when it was created; that device must be current in every call.
  *   - There is no CPU fallback: without a CUDA device every compute entry point returns
  *     FDAS_ERR_CUDA.
  */
@@ -310,9 +312,33 @@ int fdas_peaks(fdas_plan_t *p, const void *plane_dev, float threshold, fdas_peak
  * those cells only, so the plane is never read back from HBM.  Other plans run the two kernels
  * of fdas_convolve and fdas_peaks.  Arguments, ownership and the snprintf convention for
  * count_dev are those of fdas_convolve and fdas_peaks.  Asynchronous on `stream`.
+ *
+ * plane_dev == NULL: the PLANE-FREE form (what a search keeps of the plane is its peak
+ * list; surveys run batches of 256 series whose planes nobody reads).  Nothing but the
+ * spectrum is read from HBM and nothing but the peak list is written: a first launch runs the whole
+ * convolution without storing, listing the 128-bin tiles that hold a power above `threshold`; a second launch
+ * recomputes the listed tiles (the same tensor-core instructions and the same fp32 arithmetic, so every power is
+ * bit-identical to what fdas_convolve stores) and applies the peak rule there.  The peak set and the powers equal
+ * those of the call with a plane.  Cost grows with the number of listed tiles: with a threshold inside the
+ * noise every tile is listed and the call costs about four convolutions.  Needs a plan that runs the
+ * tensor-core kernels (fdas_get_algorithm != FDAS_ALGO_FFT; FDAS_F32 with M % 4 == 0) with the float plane
+ * format and at most 8 template groups (K <= 1023 on a symmetric grid); otherwise FDAS_ERR_UNSUPPORTED.
  */
 int fdas_search(fdas_plan_t *p, const void *spectrum_dev, void *plane_dev, float threshold,
                 fdas_peak_t *peaks_dev, int capacity, int *count_dev, void *stream);
+
+/*
+ * fdas_search_batched -- fdas_search over `batch` independent series sharing the plan (BASELINE.json config 4).
+ *   spectra_dev  [batch][M]
+ *   planes_dev   [batch][K][M], or NULL for the plane-free form: ONE scan launch and ONE recheck launch
+ *                for the whole batch (config 4's 256 planes would be 208 GB)
+ *   peaks_dev    [batch][capacity] records; series b's first min(counts_dev[b], capacity) are valid
+ *   counts_dev   [batch] totals (snprintf convention per series)
+ * Per series the peak set equals that of fdas_search.  Asynchronous on `stream`.
+ * Errors: INVALID_ARG (NULL, batch < 1, capacity < 0), NOT_BUILT, UNSUPPORTED (plane-free form, see fdas_search), ALLOC, CUDA.
+ */
+int fdas_search_batched(fdas_plan_t *p, const void *spectra_dev, void *planes_dev, int batch, float threshold,
+                        fdas_peak_t *peaks_dev, int capacity, int *counts_dev, void *stream);
 
 /*
  * Host-buffer forms (end-to-end path): copy the spectrum host->device, run fdas_convolve
@@ -320,7 +346,8 @@ int fdas_search(fdas_plan_t *p, const void *spectrum_dev, void *plane_dev, float
  * Device staging buffers are owned by the plan and allocated on first use.  Pinned host
  * memory makes the copies asynchronous and fast; pageable memory also works.
  *   fdas_convolve_host   plane_host receives [K][M]
- *   fdas_search_host     fdas_search; the plane stays on the device; peaks_host
+ *   fdas_search_host     fdas_search in its plane-free form where the plan allows it (no plane is allocated
+ *                        anywhere), else with a plane that stays on the device; peaks_host
  *                        receives min(count, capacity) records and *count_host the total.
  */
 int fdas_convolve_host(fdas_plan_t *p, const void *spectrum_host, void *plane_host, void *stream);
@@ -330,8 +357,8 @@ int fdas_search_host(fdas_plan_t *p, const void *spectrum_host, float threshold,
 /*
  * fdas_search_host_batched -- survey form of fdas_search_host for many independent series sharing
  * one plan (BASELINE.json config 4; PAPER.md:295-297 times 256-run batches): series i+1 is copied
- * host->device on an internal copy stream while series i is searched on `stream`; the plane never
- * leaves the device (one plane buffer is reused), only the peak lists come back.
+ * host->device on an internal copy stream while series i is searched on `stream` (plane-free where the plan
+ * allows it; otherwise one device plane buffer is reused); only the peak lists come back.
  *   spectra_host  [n_series][M] interleaved complex (pinned memory makes the overlap real)
  *   peaks_host    [n_series][capacity] records; for series i the first min(counts_host[i], capacity)
  *                 are valid (the whole slot of `capacity` records is copied: keep capacity modest)

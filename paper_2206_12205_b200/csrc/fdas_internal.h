@@ -58,6 +58,13 @@ struct fdas_plan {
     int *cand_ctr;         // two counters used alternately: call n appends to [n & 1] and clears [(n + 1) & 1]
     int cand_capacity;
     unsigned search_calls;
+    // plane-free search: tile flags / list / counters, the recheck scratch and its tensor maps
+    int *tf_flags, *tf_list, *tf_ctr;
+    long long tf_tiles;            // entries allocated in tf_flags / tf_list
+    float *tf_scratch;
+    size_t tf_scratch_bytes;
+    void *tf_maps;                 // host: tensor maps of tf_scratch
+    unsigned tf_calls;
     // host-buffer entry points: lazily allocated device staging
     void *stage_spectrum, *stage_plane;
     fdas_peak_t *stage_peaks;
@@ -123,7 +130,18 @@ struct fdas_search_args {
     int cand_capacity;
     int *count_out;        // caller's peak counter, cleared by this launch
     int cand_span;         // |z| table entries one candidate covers (set by the convolve launch)
+    // plane-free search (fdas_search with plane_dev == NULL; fdas_mma_search.cu): the scan launch flags the 128-bin
+    // tiles that hold a cell above the threshold, the recheck launch recomputes those tiles and applies the peak rule
+    int *tile_flags;       // [batch * tiles_per_series]: bit 0 = a cell above thr; bits 1, 2 = its first / last bin is one
+    int *tile_list;        // flagged tiles (series * tiles_per_series + tile), each appended once
+    int *tile_count;       // entries of tile_list: this call's counter ...
+    int *tile_count_next;  // ... and the other one, cleared by the scan launch for the next call
+    float *scratch;        // recheck launch: [gridDim.x][K][FDAS_TC_STRIP] powers of the tiles of one work item
+    fdas_peak_t *peaks;    // [batch][capacity] records out
+    int capacity;
+    int *counts;           // [batch] totals out (cleared by the scan launch)
 };
+#define FDAS_TC_STRIP 384   // bins per recheck work item: the flagged tile and its two neighbours
 
 #define FDAS_CUDA_TRY(p, call)                                  \
     do {                                                        \
@@ -151,6 +169,13 @@ int fdas_mma_plan(fdas_plan *p);
 int fdas_launch_build_tapmatrix(fdas_plan *p, cudaStream_t st);
 int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, int batch, cudaStream_t st,
                              fdas_search_args *search = nullptr);
+// fdas_mma_search.cu: convolve + peaks without a plane (scan launch + recheck launch); FDAS_ERR_UNSUPPORTED when
+// the plan does not run the tensor-core kernels with a float plane format
+int fdas_launch_search_noplane(fdas_plan *p, const void *spectra, int batch, float thr, fdas_peak_t *peaks, int capacity,
+                               int *counts, cudaStream_t st);
+// fdas_mma.cu: the work-item size the tensor-core launch picks, and tensor maps of a [rows][cols] matrix with one box
+// per distinct run length (shared with fdas_mma_search.cu)
+int fdas_tc_encode_maps(fdas_plan *p, void *base, long long cols, long long rows, size_t elem_bytes, void *maps_out);
 // fdas_peaks.cu: turns the candidates of a fused search into the peak list (same rule as fdas_peaks)
 int fdas_launch_resolve(fdas_plan *p, const void *plane, const fdas_search_args &sa, fdas_peak_t *peaks, int capacity,
                         cudaStream_t st);

@@ -217,9 +217,9 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-static int plane_maps(fdas_plan *p, void *planes, int batch, const TbMaps **out)
+int fdas_tc_encode_maps(fdas_plan *p, void *base, long long cols, long long rows, size_t elem_bytes, void *maps_out)
 {
-    static EncodeTiledFn encode = nullptr;
+    static EncodeTiledFn encode = nullptr;   // a driver entry point: the same for every device and thread
     if (!encode) {
         void *fn = nullptr;
         cudaDriverEntryPointQueryResult qres;
@@ -227,32 +227,37 @@ static int plane_maps(fdas_plan *p, void *planes, int batch, const TbMaps **out)
         if (!fn || qres != cudaDriverEntryPointSuccess) return FDAS_ERR_UNSUPPORTED;
         encode = (EncodeTiledFn)fn;
     }
+    TbMaps *maps = static_cast<TbMaps *>(maps_out);
+    const cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)cols * elem_bytes};
+    const cuuint32_t estr[2] = {1, 1};
+    for (int b = 0; b < p->tc_n_boxes; ++b) {
+        const cuuint32_t box[2] = {(cuuint32_t)TC_TILE, (cuuint32_t)p->tc_box_heights[b]};
+        const CUresult r = encode(&maps->m[b], elem_bytes == 2 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2,
+                                  base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                  CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return FDAS_ERR_UNSUPPORTED;
+    }
+    return FDAS_OK;
+}
+
+static int plane_maps(fdas_plan *p, void *planes, int batch, const TbMaps **out)
+{
     if (!p->tc_maps) {
         p->tc_maps = aligned_alloc(64, sizeof(TbMaps));
         if (!p->tc_maps) return FDAS_ERR_ALLOC;
         p->tc_maps_plane = nullptr;
     }
-    TbMaps *maps = static_cast<TbMaps *>(p->tc_maps);
     const size_t esz = p->plane_bf16 ? 2 : 4;
     if (p->tc_maps_plane != planes || p->tc_maps_batch != batch || p->tc_maps_elem != (int)esz) {
-        const cuuint64_t dims[2] = {(cuuint64_t)p->M, (cuuint64_t)batch * (cuuint64_t)p->K};
-        const cuuint64_t strides[1] = {(cuuint64_t)p->M * esz};
-        const cuuint32_t estr[2] = {1, 1};
-        for (int b = 0; b < p->tc_n_boxes; ++b) {
-            const cuuint32_t box[2] = {(cuuint32_t)TC_TILE, (cuuint32_t)p->tc_box_heights[b]};
-            const CUresult r = encode(&maps->m[b], p->plane_bf16 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, planes, dims, strides, box, estr,
-                                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                                      CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-            if (r != CUDA_SUCCESS) {
-                p->tc_maps_plane = nullptr;
-                return FDAS_ERR_UNSUPPORTED;
-            }
-        }
+        p->tc_maps_plane = nullptr;
+        const int rc = fdas_tc_encode_maps(p, planes, p->M, (long long)batch * p->K, esz, p->tc_maps);
+        if (rc != FDAS_OK) return rc;
         p->tc_maps_plane = planes;
         p->tc_maps_batch = batch;
         p->tc_maps_elem = (int)esz;
     }
-    *out = maps;
+    *out = static_cast<TbMaps *>(p->tc_maps);
     return FDAS_OK;
 }
 
@@ -314,31 +319,13 @@ int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, in
     const uint32_t total = smem_total(R);
     if (total > smem_cap) return FDAS_ERR_UNSUPPORTED;
     TcParams tp;
-    tp.spectra = static_cast<const float2 *>(spectra);
-    tp.planes = planes;
-    tp.bmat = static_cast<const uint4 *>(p->tc_bmat);
-    tp.ktab = p->tc_ktab;
-    tp.ranges = p->tc_ranges;
-    tp.M = p->M;
-    tp.K = p->K;
-    tp.batch = batch;
-    tp.R = R;
-    tp.n_blocks = (int)((p->M + R - 1) / R);
-    tp.M0 = p->m_max;
-    tp.KS = p->tc_KS;
-    tp.NT = p->tc_NT;
-    tp.nzg = p->tc_nzg;
-    tp.full_chunks = p->tc_full_chunks;
-    for (int g = 0; g < 8; ++g) {
-        tp.nks_lo[g] = p->tc_nks_lo[g];
-        tp.nks_hi[g] = p->tc_nks_hi[g];
-        tp.ks_first[g] = p->tc_ks_first[g];
-    }
+    tc_fill_params(p, tp, spectra, planes, batch, R);
     if (search) {
         search->cand_span = bulk ? p->tc_NT / 8 : 8;   // |z| entries per column group (2 NCH) / per 16-column chunk
         tp.search = *search;
     } else {
-        tp.search = fdas_search_args{0, 0.f, nullptr, nullptr, nullptr, 0, nullptr, 8};
+        tp.search = fdas_search_args{};
+        tp.search.cand_span = 8;
     }
     const long long items = (long long)batch * tp.n_blocks;
     if (items >= 0x7FFFFFFFLL) return FDAS_ERR_UNSUPPORTED;   // the kernels count work items in 32 bits

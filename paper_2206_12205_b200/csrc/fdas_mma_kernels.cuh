@@ -92,8 +92,91 @@ struct TcParams {
     // 16 * nibble(ks) columns -- the taps of narrower templates are zero there -- and K step ks_first is full width
     unsigned long long nks_lo[8], nks_hi[8];
     int ks_first[8];
+    int tiles_per_series;    // ceil(M / 128): plane-free search numbers the tiles series * tiles_per_series + tile
+    int clustered;           // recheck launch with more than one template group: the groups of one item form a cluster
     fdas_search_args search; // fused threshold pass (fdas_search); enabled = 0 for plain fdas_convolve
 };
+
+// host: everything of TcParams that follows from the plan and the work-item size R (search left disabled)
+static inline void tc_fill_params(const fdas_plan *p, TcParams &tp, const void *spectra, void *planes, int batch, int R)
+{
+    tp.spectra = static_cast<const float2 *>(spectra);
+    tp.planes = planes;
+    tp.bmat = static_cast<const uint4 *>(p->tc_bmat);
+    tp.ktab = p->tc_ktab;
+    tp.ranges = p->tc_ranges;
+    tp.M = p->M;
+    tp.K = p->K;
+    tp.batch = batch;
+    tp.R = R;
+    tp.n_blocks = (int)((p->M + R - 1) / R);
+    tp.M0 = p->m_max;
+    tp.KS = p->tc_KS;
+    tp.NT = p->tc_NT;
+    tp.nzg = p->tc_nzg;
+    tp.full_chunks = p->tc_full_chunks;
+    for (int g = 0; g < 8; ++g) {
+        tp.nks_lo[g] = p->tc_nks_lo[g];
+        tp.nks_hi[g] = p->tc_nks_hi[g];
+        tp.ks_first[g] = p->tc_ks_first[g];
+    }
+    tp.tiles_per_series = (int)((p->M + 127) / 128);
+    tp.clustered = 0;
+    tp.search = fdas_search_args{};
+    tp.search.cand_span = 8;
+}
+
+// What a launch of fdas_mma_bulk_kernel does with the powers (template parameter MODE):
+//   TB_PLANE    writes the plane (fdas_convolve; fdas_search with a plane also flags candidate cells)
+//   TB_SCAN     plane-free search, first launch: no stores at all; flags the 128-bin tiles holding a power above the
+//               threshold (search.tile_flags / tile_list)
+//   TB_RECHECK  plane-free search, second launch: work items are the flagged tiles (with the neighbour tile where the
+//               first / last bin is a candidate); the same MMAs and the same epilogue arithmetic recompute them --
+//               bit-identical to what TB_PLANE stores -- into a private strip of scratch memory, then the epilogue
+//               warps apply the peak rule of fdas_peaks to the cells of the flagged tile
+constexpr int TB_PLANE = 0, TB_SCAN = 1, TB_RECHECK = 2;
+
+// work item -> (series, first bin, tiles, index of the tile whose cells are tested [TB_RECHECK])
+template <int MODE>
+__device__ __forceinline__ void tb_item(const TcParams &p, uint32_t it, long long &ser, long long &blk0, int &n_tiles, int &centre)
+{
+    if constexpr (MODE == TB_RECHECK) {
+        const int tg = __ldcg(p.search.tile_list + it);
+        const int fl = __ldcg(p.search.tile_flags + tg);
+        const int t = tg % p.tiles_per_series;
+        ser = tg / p.tiles_per_series;
+        const int hl = ((fl & 2) && t > 0) ? 1 : 0, hr = ((fl & 4) && t + 1 < p.tiles_per_series) ? 1 : 0;
+        blk0 = (long long)(t - hl) * 128;
+        n_tiles = 1 + hl + hr;
+        centre = hl;
+    } else {
+        ser = it / (uint32_t)p.n_blocks;   // 32-bit division: items < 2^31 (checked by the launcher)
+        blk0 = (long long)(it % (uint32_t)p.n_blocks) * p.R;
+        const long long left = p.M - blk0;
+        n_tiles = (int)((left < p.R ? left : p.R) + 128 - 1) / 128;
+        centre = 0;
+    }
+}
+// work items of this launch
+template <int MODE>
+__device__ __forceinline__ uint32_t tb_items(const TcParams &p)
+{
+    if constexpr (MODE == TB_RECHECK) {
+        const long long all = (long long)p.batch * p.tiles_per_series;
+        const long long n = __ldcg(p.search.tile_count);
+        return (uint32_t)(n < all ? n : all);
+    } else {
+        return (uint32_t)p.batch * (uint32_t)p.n_blocks;
+    }
+}
+// TB_RECHECK: every thread of the CTA (of the cluster, when the template groups of an item are spread over one)
+// meets here twice per work item: once when the item's powers are in scratch, once when they have been tested
+__device__ __forceinline__ void tb_item_sync(int clustered, int threads)
+{
+    __syncwarp();
+    if (clustered) asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+    else asm volatile("bar.sync 7, %0;" ::"r"(threads) : "memory");
+}
 
 // ---- PTX wrappers ---------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -384,7 +467,7 @@ __device__ __forceinline__ void umma_commit_elected(uint32_t bar, uint32_t elect
 
 // The MMA warp of both kernels.  Per tile 2 KS MMAs (K steps outermost, so consecutive MMAs
 // alternate between the re and im accumulators), then a commit that signals the epilogue.
-template <int NT, int SPLIT = 1>
+template <int NT, int SPLIT = 1, int MODE = TB_PLANE>
 __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, uint32_t off_z, uint32_t z_buf_bytes,
                                            uint32_t z_part_bytes, uint32_t z_full, uint32_t z_empty, uint32_t t_full,
                                            uint32_t t_empty, uint32_t tmem_base, uint32_t n_items)
@@ -403,9 +486,9 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
     uint32_t n = 0, t = 0;
     for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x, ++n) {
         const uint32_t buf = n & 1, zuse = n >> 1;
-        const long long blk0 = (long long)(it % (uint32_t)p.n_blocks) * p.R;
-        const long long left = p.M - blk0;
-        const int n_tiles = (int)((left < p.R ? left : p.R) + TC_TILE - 1) / TC_TILE;
+        long long ser_, blk0;
+        int n_tiles, centre_;
+        tb_item<MODE>(p, it, ser_, blk0, n_tiles, centre_);
         mbar_wait(z_full + 8 * buf, zuse & 1);
         tc_fence_after();
         const uint32_t z_addr = s_base + off_z + buf * z_buf_bytes;
@@ -459,6 +542,10 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
             umma_commit_elected(t_full + 8 * stage, elected);
         }
         umma_commit_elected(z_empty + 8 * buf, elected);
+        if constexpr (MODE == TB_RECHECK) {
+            tb_item_sync(p.clustered, (int)blockDim.x);
+            tb_item_sync(p.clustered, (int)blockDim.x);
+        }
     }
 }
 
@@ -468,11 +555,14 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
 // their latency hides behind the tensor core working on the previous items.
 constexpr int TC_LD_ITERS = 8;   // sample pairs per loader thread: (R + 16 KS) / 2 / 96 <= (1024 + 512) / 192
 
+template <int MODE = TB_PLANE>
 __device__ __forceinline__ void loader_fetch(const TcParams &p, uint32_t it, uint32_t xn, int lt, float2 (&a)[TC_LD_ITERS],
                                              float2 (&b)[TC_LD_ITERS])
 {
-    const long long ser = it / (uint32_t)p.n_blocks;   // 32-bit division: items < 2^31 (checked by the launcher)
-    const long long g0 = (long long)(it % (uint32_t)p.n_blocks) * p.R - p.M0;   // sample index of xs[0]
+    long long ser, blk0;
+    int n_tiles_, centre_;
+    tb_item<MODE>(p, it, ser, blk0, n_tiles_, centre_);
+    const long long g0 = blk0 - p.M0;   // sample index of xs[0]
     const float2 *__restrict__ X = p.spectra + (size_t)ser * p.M;
 #pragma unroll
     for (int i = 0; i < TC_LD_ITERS; ++i) {
@@ -490,7 +580,7 @@ __device__ __forceinline__ void loader_fetch(const TcParams &p, uint32_t it, uin
 // residual of the bf16 rounding: x - bf16(x) is exact in fp32 (x has 24 significant bits, bf16(x) the top 8)
 __device__ __forceinline__ float bf16_residual(float x) { return x - __bfloat162float(__float2bfloat16_rn(x)); }
 
-template <int SPLIT = 1>
+template <int SPLIT = 1, int MODE = TB_PLANE>
 __device__ __forceinline__ void spectrum_loader(const TcParams &p, unsigned char *smem, uint32_t off_xs,
                                                 uint32_t xs_part_bytes, uint32_t xn, uint32_t off_z, uint32_t z_buf_bytes,
                                                 uint32_t z_part_bytes, uint32_t zr, uint32_t z_full, uint32_t z_empty,
@@ -502,7 +592,7 @@ __device__ __forceinline__ void spectrum_loader(const TcParams &p, unsigned char
     uint32_t *xs_im = reinterpret_cast<uint32_t *>(smem + off_xs + xs_part_bytes);
     float2 a[TC_LD_ITERS], b[TC_LD_ITERS];
     uint32_t n = 0;
-    if (blockIdx.x < n_items) loader_fetch(p, blockIdx.x, xn, lt, a, b);
+    if (blockIdx.x < n_items) loader_fetch<MODE>(p, blockIdx.x, xn, lt, a, b);
     for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x, ++n) {
         const uint32_t buf = n & 1, zuse = n >> 1;
         // phase A: spectrum block -> bf16 (round-to-nearest-even), re and im planes
@@ -519,7 +609,7 @@ __device__ __forceinline__ void spectrum_loader(const TcParams &p, unsigned char
             }
         }
         named_bar_sync(1, TC_LOAD_THREADS);
-        if (it + gridDim.x < n_items) loader_fetch(p, it + gridDim.x, xn, lt, a, b);
+        if (it + gridDim.x < n_items) loader_fetch<MODE>(p, it + gridDim.x, xn, lt, a, b);
         mbar_wait<64>(z_empty + 8 * buf, (zuse & 1) ^ 1);
         // phase B: Z row i = samples i .. i+7 (16 bytes), for both parts
         unsigned char *zb = smem + off_z + buf * z_buf_bytes;
@@ -543,6 +633,10 @@ __device__ __forceinline__ void spectrum_loader(const TcParams &p, unsigned char
         fence_proxy_async();   // generic-proxy writes of Z -> visible to tcgen05.mma
         mbar_arrive(z_full + 8 * buf);
         named_bar_sync(1, TC_LOAD_THREADS);   // xs is rewritten by the next item
+        if constexpr (MODE == TB_RECHECK) {
+            tb_item_sync(p.clustered, (int)blockDim.x);
+            tb_item_sync(p.clustered, (int)blockDim.x);
+        }
     }
 }
 
@@ -665,7 +759,7 @@ struct TbSmem {
     uint32_t off_z, off_xs, off_stage, off_bars, off_holder, total;
     // split = 1: bf16 operands; split = 3: the fp32 variant, every operand split into two bf16 terms
     // (two tap-matrix images, four Z parts) and one epilogue warp set (one staging buffer per column group)
-    __host__ __device__ TbSmem(int R, int KS, int NT, int rowb, int split)
+    __host__ __device__ TbSmem(int R, int KS, int NT, int rowb, int split, bool staging = true)
     {
         const uint32_t TP = 16u * KS;
         const uint32_t nb = split == 3 ? 2u : 1u, np = 2u * nb, sets = split == 3 ? 1u : 2u;
@@ -680,7 +774,7 @@ struct TbSmem {
         off_z = nb * b_bytes;
         off_xs = off_z + 2u * z_buf_bytes;
         off_stage = (off_xs + np * xs_part_bytes + 127u) & ~127u;
-        off_bars = (off_stage + sets * TB_CGROUPS * stage_cg_bytes + 15u) & ~15u;
+        off_bars = (off_stage + (staging ? sets * TB_CGROUPS * stage_cg_bytes : 0u) + 15u) & ~15u;
         off_holder = off_bars + 8u * 8u;
         total = off_holder + 16u;
     }
@@ -770,20 +864,22 @@ template <int N>
 __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 
-template <int NCH, typename OT, int SPLIT>
+template <int NCH, typename OT, int SPLIT, int MODE = TB_PLANE>
 __global__ void __launch_bounds__(tb_threads(SPLIT), 1)
 fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
 {
+    static_assert(MODE == TB_PLANE || sizeof(OT) == 4, "plane-free search computes float powers");
     constexpr int SETS = tb_sets(SPLIT), TB_EPI_WARPS = tb_epi_warps(SPLIT), TB_MMA_WARP = TB_EPI_WARPS,
                   TB_LOAD_WARP0 = TB_EPI_WARPS + 1, TB_THREADS = tb_threads(SPLIT);
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int NT = 16 * NCH;
     constexpr int NC = 4 * NCH;            // columns per part per column group = staging rows (slots)
     constexpr uint32_t ROWB = TC_TILE * sizeof(OT);   // bytes of one staging row
-    const TbSmem L(p.R, p.KS, NT, ROWB, SPLIT);
+    const TbSmem L(p.R, p.KS, NT, ROWB, SPLIT, MODE != TB_SCAN);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int grp = blockIdx.y;
-    const uint32_t n_items = (uint32_t)p.batch * (uint32_t)p.n_blocks;
+    const uint32_t n_items = tb_items<MODE>(p);
+    if (MODE == TB_RECHECK && blockIdx.x >= n_items) return;   // nothing flagged for this CTA (its whole cluster: same x)
 
     const uint32_t s_base = smem_u32(smem);
     const uint32_t bars = s_base + L.off_bars;
@@ -800,9 +896,13 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
         }
         fence_proxy_async();
     }
-    if (threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0 && p.search.enabled) {
+    if (MODE == TB_PLANE && threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0 && p.search.enabled) {
         *p.search.cand_count_next = 0;
         *p.search.count_out = 0;
+    }
+    if (MODE == TB_SCAN && blockIdx.x == 0 && blockIdx.y == 0) {
+        if (threadIdx.x == 0) *p.search.tile_count_next = 0;
+        for (int i = threadIdx.x; i < p.batch; i += TB_THREADS) p.search.counts[i] = 0;
     }
     if (threadIdx.x == 0) {
         for (int s = 0; s < 2; ++s) {
@@ -841,10 +941,9 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
         const int4 rg2[2] = {p.ranges[grp * TB_CGROUPS + 2 * half], p.ranges[grp * TB_CGROUPS + 2 * half + 1]};
         uint32_t t = 0;
         for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
-            const long long ser = it / (uint32_t)p.n_blocks;   // 32-bit division: items < 2^31 (checked by the launcher)
-            const long long blk0 = (long long)(it % (uint32_t)p.n_blocks) * p.R;
-            const long long left = p.M - blk0;
-            const int n_tiles = (int)((left < p.R ? left : p.R) + TC_TILE - 1) / TC_TILE;
+            long long ser, blk0;
+            int n_tiles, centre;
+            tb_item<MODE>(p, it, ser, blk0, n_tiles, centre);
             for (int tile = 0; tile < n_tiles; ++tile, ++t) {
                 if (SETS == 2 && (int)(t & 1) != set) continue;
                 const uint32_t stage = t & 1, use = t >> 1;
@@ -905,6 +1004,21 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
                         }
                     }
                     mx2[pass] = stored_value<OT>(mx);   // rounding is monotone: the largest stored value
+                }
+                if constexpr (MODE == TB_SCAN) {
+                    // plane-free search, first launch: nothing is stored.  A tile with a power above the threshold is
+                    // listed once; bits 1 / 2 ask the recheck launch for the left / right neighbour tile as well
+                    // (the 8-neighbourhood of a candidate in the first / last bin reaches into it).  Padded columns
+                    // give exactly zero; a row that is not in the plane can only list a tile needlessly.
+                    const bool hit = fmaxf(mx2[0], mx2[1]) > thr && col0 + lt < p.M;
+                    const unsigned ball = __ballot_sync(0xffffffffu, hit);
+                    if (ball != 0u && lane == 0) {
+                        const int bits = 1 | ((q == 0 && (ball & 1u)) ? 2 : 0) | ((q == 3 && (ball >> 31)) ? 4 : 0);
+                        const int tg = (int)(ser * p.tiles_per_series + (col0 >> 7));
+                        if (atomicOr(p.search.tile_flags + tg, bits) == 0)
+                            p.search.tile_list[atomicAdd(p.search.tile_count, 1)] = tg;
+                    }
+                    continue;
                 }
                 // bf16-stored plane: the powers go straight from registers to the plane (one 64-byte row segment per
                 // warp and store).  Measured on config 3: 0.291 ms against 0.317 ms through staging + box stores (the
@@ -980,29 +1094,79 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
                     named_bar_sync(bar_id, 128);
                     if (issuer) {
                         const uint32_t sst = smem_u32(stage_buf);
-                        const int row_s = (int)ser * p.K;
+                        // TB_PLANE: the planes as [batch K rows][M bins]; TB_RECHECK: this CTA's strip of scratch,
+                        // [gridDim.x K rows][FDAS_TC_STRIP bins], tile j of the item in bins 128 j ..
+                        const int row_s = MODE == TB_RECHECK ? (int)blockIdx.x * p.K : (int)ser * p.K;
+                        const int col_s = MODE == TB_RECHECK ? tile * TC_TILE : (int)col0;
                         // one box per run: warp q = 0 pushes the -|z| rows, warp q = 1 the +|z| rows
                         const int cnt = (q ? rg.w : rg.y) & 0xFFFF, box = (q ? rg.w : rg.y) >> 16;
                         if (cnt > 0)
-                            tensor_store(&maps.m[box], sst + (q ? (uint32_t)(NC - cnt) * ROWB : 0u), (int)col0,
+                            tensor_store(&maps.m[box], sst + (q ? (uint32_t)(NC - cnt) * ROWB : 0u), col_s,
                                          row_s + (q ? rg.z : rg.x));
                         bulk_commit();                      // one group per pass, empty or not: bulk_wait_read<1> counts them
                     }
-                    if (mx2[pass] > thr && col0 + lt < p.M && 2 * cg * NCH < p.nzg)
+                    if (MODE == TB_PLANE && mx2[pass] > thr && col0 + lt < p.M && 2 * cg * NCH < p.nzg)
                         flag_candidate(p.search.cand, p.search.cand_count, p.search.cand_capacity,
                                        grp * p.nzg + 2 * cg * NCH, (int)(col0 + lt), mx2[pass]);
                 }
+            }
+            if constexpr (MODE == TB_RECHECK) {
+                // ---- the item's powers are on their way to scratch: wait for this thread's boxes, meet every other
+                // thread that wrote (all template groups), apply the peak rule of fdas_peaks (reading A14) to
+                // the cells of the flagged tile, meet again before the strip is overwritten
+                if (issuer) bulk_wait_all();
+                __threadfence();
+                tb_item_sync(p.clustered, TB_THREADS);
+                {
+                    const int G = (int)gridDim.y;
+                    const int k_lo = (int)((long long)p.K * grp / G), k_hi = (int)((long long)p.K * (grp + 1) / G);
+                    const float *S = p.search.scratch + (size_t)blockIdx.x * p.K * FDAS_TC_STRIP;
+                    const long long r_first = blk0;                    // plane bin of strip column 0
+                    const int c_lo = centre * TC_TILE, c_end = n_tiles * TC_TILE;
+                    for (int idx = threadIdx.x; idx < (k_hi - k_lo) * TC_TILE; idx += TB_EPI_WARPS * 32) {
+                        const int k = k_lo + idx / TC_TILE, c = c_lo + idx % TC_TILE;
+                        const long long r = r_first + c;
+                        if (r >= p.M) continue;
+                        const float v = __ldcg(S + (size_t)k * FDAS_TC_STRIP + c);
+                        if (!(v > thr)) continue;
+                        bool ok = true;
+#pragma unroll
+                        for (int dk = -1; dk <= 1; ++dk) {
+#pragma unroll
+                            for (int dr = -1; dr <= 1; ++dr) {
+                                if (dk == 0 && dr == 0) continue;
+                                const int kk = k + dk, cc = c + dr;
+                                if (kk < 0 || kk >= p.K || cc < 0 || cc >= c_end || r + dr < 0 || r + dr >= p.M) continue;
+                                const float nb = __ldcg(S + (size_t)kk * FDAS_TC_STRIP + cc);
+                                const bool precedes = (dk < 0) || (dk == 0 && dr < 0);
+                                ok = ok && (precedes ? (v > nb) : (v >= nb));
+                            }
+                        }
+                        if (ok) {
+                            const int slot = atomicAdd(p.search.counts + ser, 1);
+                            if (slot < p.search.capacity) {
+                                fdas_peak_t rec;
+                                rec.z_index = k;
+                                rec.r = (int32_t)r;
+                                rec.power = v;
+                                p.search.peaks[(size_t)ser * p.search.capacity + slot] = rec;
+                            }
+                        }
+                    }
+                    if (threadIdx.x == 0 && grp == 0) p.search.tile_flags[__ldcg(p.search.tile_list + it)] = 0;   // flags are all zero again after this launch
+                }
+                tb_item_sync(p.clustered, TB_THREADS);
             }
         }
         if (issuer) bulk_wait_all();
     } else if (warp == TB_MMA_WARP) {
         // =========================== MMA issuer ===========================
-        mma_issuer<NT, SPLIT>(p, s_base, L.off_z, L.z_buf_bytes, L.z_part_bytes, z_full, z_empty, t_full, t_empty,
-                              __shfl_sync(0xffffffffu, tmem_base, 0), n_items);
+        mma_issuer<NT, SPLIT, MODE>(p, s_base, L.off_z, L.z_buf_bytes, L.z_part_bytes, z_full, z_empty, t_full, t_empty,
+                                    __shfl_sync(0xffffffffu, tmem_base, 0), n_items);
     } else {
         // =========================== loader ===========================
-        spectrum_loader<SPLIT>(p, smem, L.off_xs, L.xs_part_bytes, L.xn, L.off_z, L.z_buf_bytes, L.z_part_bytes, L.zr, z_full,
-                               z_empty, threadIdx.x - TB_LOAD_WARP0 * 32, n_items);
+        spectrum_loader<SPLIT, MODE>(p, smem, L.off_xs, L.xs_part_bytes, L.xn, L.off_z, L.z_buf_bytes, L.z_part_bytes, L.zr,
+                                     z_full, z_empty, threadIdx.x - TB_LOAD_WARP0 * 32, n_items);
     }
 
     tc_fence_before();

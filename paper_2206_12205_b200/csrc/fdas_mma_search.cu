@@ -1,0 +1,161 @@
+// fdas_mma_search.cu -- plane-free search (include/fdas.h: fdas_search / fdas_search_batched with a NULL plane).
+//
+// PAPER.md:184-188 (section 4.3): what a search keeps of the f-fdot plane is a list of peaks, not the plane;
+// PAPER.md:295-297 (section 5.4) times batches of 256 series, whose planes (BASELINE.json config 4: 208 GB) nobody
+// reads.  SURVEY.md 8(f) NEXT-2: emit the candidates from the convolution itself and skip the plane write.
+//
+// Two launches of the tensor-core kernel (fdas_mma_kernels.cuh), no plane in HBM:
+//   TB_SCAN     the whole convolution, powers formed in registers exactly as for a plane, nothing stored; every
+//               128-bin tile holding a power above the threshold is listed (a few hundred of 32 768 on config 3)
+//   TB_RECHECK  the listed tiles (with the neighbour tile where a first / last bin is a candidate) are computed
+//               again by the same MMAs and the same epilogue arithmetic -- bit-identical to what fdas_convolve
+//               stores -- into a per-CTA strip of scratch memory ([K][384] floats, L2 resident), and the epilogue
+//               warps apply the peak rule of fdas_peaks to the cells of the listed tile.
+// The peak set (and every power) equals that of fdas_search with a float plane.  The only HBM stream left is the
+// spectrum read: the path is bound by the tensor pipe (bf16 operands) instead of the plane write.
+#include <stdlib.h>
+#include "fdas_mma_kernels.cuh"
+
+namespace {
+
+template <int NCH, int SPLIT, int MODE>
+int launch_mode(fdas_plan *p, const TcParams &tp, unsigned gx, size_t smem_bytes, const TbMaps *maps, cudaStream_t st)
+{
+    auto kern = fdas_mma_bulk_kernel<NCH, float, SPLIT, MODE>;
+    const int slot = MODE == TB_SCAN ? (SPLIT == 3 ? FDAS_OPTIN_MMA_NOPLANE_SPLIT : FDAS_OPTIN_MMA_NOPLANE)
+                                     : (SPLIT == 3 ? FDAS_OPTIN_MMA_RECHECK_SPLIT : FDAS_OPTIN_MMA_RECHECK);
+    { const int rc = fdas_optin_smem(p, slot, kern, smem_bytes); if (rc) return rc; }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(gx, p->tc_groups);
+    cfg.blockDim = dim3(tb_threads(SPLIT));
+    cfg.dynamicSmemBytes = smem_bytes;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    if (MODE == TB_RECHECK && p->tc_groups > 1) {   // the template groups of one work item meet at a cluster barrier
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 1;
+        attr[0].val.clusterDim.y = (unsigned)p->tc_groups;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+    }
+    FDAS_CUDA_TRY(p, cudaLaunchKernelEx(&cfg, kern, tp, *maps));
+    p->launches += 1;
+    return FDAS_OK;
+}
+
+template <int SPLIT, int MODE>
+int launch_nch(fdas_plan *p, const TcParams &tp, unsigned gx, size_t smem_bytes, const TbMaps *maps, cudaStream_t st)
+{
+    switch (p->tc_NT / 16) {
+    case 1: return launch_mode<1, SPLIT, MODE>(p, tp, gx, smem_bytes, maps, st);
+    case 2: return launch_mode<2, SPLIT, MODE>(p, tp, gx, smem_bytes, maps, st);
+    case 3: return launch_mode<3, SPLIT, MODE>(p, tp, gx, smem_bytes, maps, st);
+    case 4: return launch_mode<4, SPLIT, MODE>(p, tp, gx, smem_bytes, maps, st);
+    case 5: return launch_mode<5, SPLIT, MODE>(p, tp, gx, smem_bytes, maps, st);
+    case 6: return launch_mode<6, SPLIT, MODE>(p, tp, gx, smem_bytes, maps, st);
+    case 7: return launch_mode<7, SPLIT, MODE>(p, tp, gx, smem_bytes, maps, st);
+    case 8: return launch_mode<8, SPLIT, MODE>(p, tp, gx, smem_bytes, maps, st);
+    default: return FDAS_ERR_UNSUPPORTED;
+    }
+}
+
+}  // namespace
+
+int fdas_launch_search_noplane(fdas_plan *p, const void *spectra, int batch, float thr, fdas_peak_t *peaks, int capacity,
+                               int *counts, cudaStream_t st)
+{
+    // the tensor-core kernels with a float plane format; the strip stores need the row runs of the box-store path; the
+    // template groups of one item must fit one cluster
+    if (!fdas_uses_mma(p) || p->plane_bf16 || !p->tc_bulk_ok || p->tc_groups > 8) return FDAS_ERR_UNSUPPORTED;
+    const int split = p->precision == FDAS_F32 ? 3 : 1;
+    const long long tps = (p->M + TC_TILE - 1) / TC_TILE;
+    const long long tiles = (long long)batch * tps;
+    if (tiles >= 0x7FFFFFFFLL) return FDAS_ERR_UNSUPPORTED;
+    const int sms_per_group = p->num_sms / p->tc_groups > 0 ? p->num_sms / p->tc_groups : 1;
+    const uint32_t smem_cap = 227u * 1024u;
+
+    // ---- buffers: tile flags (all zero between calls: the recheck launch clears what the scan launch set), tile list,
+    // two counters used alternately, the recheck strips and their tensor maps
+    if (tiles > p->tf_tiles) {
+        cudaFree(p->tf_flags);
+        cudaFree(p->tf_list);
+        p->tf_flags = p->tf_list = NULL;
+        p->tf_tiles = 0;
+        int *f = NULL, *l = NULL;
+        cudaError_t e = cudaMalloc((void **)&f, sizeof(int) * (size_t)tiles);
+        if (e == cudaSuccess) e = cudaMalloc((void **)&l, sizeof(int) * (size_t)tiles);
+        if (e == cudaSuccess) e = cudaMemsetAsync(f, 0, sizeof(int) * (size_t)tiles, st);
+        if (e != cudaSuccess) {
+            cudaFree(f);
+            cudaFree(l);
+            p->last_err = e;
+            return e == cudaErrorMemoryAllocation ? FDAS_ERR_ALLOC : FDAS_ERR_CUDA;
+        }
+        p->tf_flags = f;
+        p->tf_list = l;
+        p->tf_tiles = tiles;
+    }
+    if (!p->tf_ctr) {
+        FDAS_CUDA_TRY(p, cudaMalloc((void **)&p->tf_ctr, 2 * sizeof(int)));
+        FDAS_CUDA_TRY(p, cudaMemsetAsync(p->tf_ctr, 0, 2 * sizeof(int), st));
+    }
+    const size_t strip_bytes = (size_t)sms_per_group * p->K * FDAS_TC_STRIP * sizeof(float);
+    if (!p->tf_scratch) {
+        FDAS_CUDA_TRY(p, cudaMalloc((void **)&p->tf_scratch, strip_bytes));
+        p->tf_scratch_bytes = strip_bytes;
+        if (!p->tf_maps) p->tf_maps = aligned_alloc(64, sizeof(TbMaps));
+        if (!p->tf_maps) return FDAS_ERR_ALLOC;
+        const int rc = fdas_tc_encode_maps(p, p->tf_scratch, FDAS_TC_STRIP, (long long)sms_per_group * p->K, sizeof(float), p->tf_maps);
+        if (rc != FDAS_OK) {
+            cudaFree(p->tf_scratch);
+            p->tf_scratch = NULL;
+            return rc;
+        }
+    }
+    const TbMaps *maps = static_cast<const TbMaps *>(p->tf_maps);
+
+    fdas_search_args sa = {};
+    sa.enabled = 1;
+    sa.thr = thr;
+    sa.cand_span = 8;
+    sa.tile_flags = p->tf_flags;
+    sa.tile_list = p->tf_list;
+    sa.tile_count = p->tf_ctr + (p->tf_calls & 1);
+    sa.tile_count_next = p->tf_ctr + ((p->tf_calls + 1) & 1);
+    sa.scratch = p->tf_scratch;
+    sa.peaks = peaks;
+    sa.capacity = capacity;
+    sa.counts = counts;
+    p->tf_calls += 1;
+
+    // ---- scan launch: work items as for a plane (the largest of 1024..128 bins that fits and leaves two items per CTA)
+    {
+        int R = 1024;
+        for (;; R >>= 1) {
+            const long long items = (long long)batch * ((p->M + R - 1) / R);
+            if (R == 128 || (TbSmem(R, p->tc_KS, p->tc_NT, TC_TILE * 4, split, false).total <= smem_cap && items >= 2LL * sms_per_group)) break;
+        }
+        const uint32_t total = TbSmem(R, p->tc_KS, p->tc_NT, TC_TILE * 4, split, false).total;
+        if (total > smem_cap) return FDAS_ERR_UNSUPPORTED;
+        TcParams tp;
+        tc_fill_params(p, tp, spectra, nullptr, batch, R);
+        tp.search = sa;
+        const long long items = (long long)batch * tp.n_blocks;
+        if (items >= 0x7FFFFFFFLL) return FDAS_ERR_UNSUPPORTED;
+        const unsigned gx = (unsigned)(items < sms_per_group ? items : sms_per_group);
+        const int rc = split == 3 ? launch_nch<3, TB_SCAN>(p, tp, gx, total, maps, st) : launch_nch<1, TB_SCAN>(p, tp, gx, total, maps, st);
+        if (rc) return rc;
+    }
+    // ---- recheck launch: one CTA (one cluster of template groups) per strip; CTAs without a listed tile leave at once
+    {
+        const uint32_t total = TbSmem(FDAS_TC_STRIP, p->tc_KS, p->tc_NT, TC_TILE * 4, split, true).total;
+        if (total > smem_cap) return FDAS_ERR_UNSUPPORTED;
+        TcParams tp;
+        tc_fill_params(p, tp, spectra, nullptr, batch, FDAS_TC_STRIP);
+        tp.search = sa;
+        tp.clustered = p->tc_groups > 1;
+        const unsigned gx = (unsigned)(tiles < sms_per_group ? tiles : sms_per_group);
+        return split == 3 ? launch_nch<3, TB_RECHECK>(p, tp, gx, total, maps, st) : launch_nch<1, TB_RECHECK>(p, tp, gx, total, maps, st);
+    }
+}

@@ -34,6 +34,11 @@ static void free_device_members(fdas_plan *p)
     free(p->tc_maps);
     cudaFree(p->cand);
     cudaFree(p->cand_ctr);
+    cudaFree(p->tf_flags);
+    cudaFree(p->tf_list);
+    cudaFree(p->tf_ctr);
+    cudaFree(p->tf_scratch);
+    free(p->tf_maps);
     cudaFree(p->stage_spectrum);
     cudaFree(p->stage_plane);
     cudaFree(p->stage_peaks);
@@ -268,6 +273,8 @@ extern "C" int fdas_peaks(fdas_plan_t *p, const void *plane_dev, float threshold
 static int search_on_device(fdas_plan *p, const void *spectrum_dev, void *plane_dev, float threshold,
                             fdas_peak_t *peaks_dev, int capacity, int *count_dev, cudaStream_t st)
 {
+    if (!plane_dev)   // plane-free form: scan launch + recheck launch (fdas_mma_search.cu)
+        return fdas_launch_search_noplane(p, spectrum_dev, 1, threshold, peaks_dev, capacity, count_dev, st);
     if (!fdas_uses_mma(p)) {
         int rc = fdas_launch_convolve(p, spectrum_dev, plane_dev, 1, st);
         if (rc) return rc;
@@ -318,11 +325,37 @@ static int search_on_device(fdas_plan *p, const void *spectrum_dev, void *plane_
 extern "C" int fdas_search(fdas_plan_t *p, const void *spectrum_dev, void *plane_dev, float threshold,
                            fdas_peak_t *peaks_dev, int capacity, int *count_dev, void *stream)
 {
-    if (!p || !spectrum_dev || !plane_dev || !count_dev || capacity < 0 || (capacity > 0 && !peaks_dev))
+    if (!p || !spectrum_dev || !count_dev || capacity < 0 || (capacity > 0 && !peaks_dev))
         return FDAS_ERR_INVALID_ARG;
     if (!p->built) return FDAS_ERR_NOT_BUILT;
     return search_on_device(p, spectrum_dev, plane_dev, threshold, peaks_dev, capacity, count_dev,
                             (cudaStream_t)stream);
+}
+
+extern "C" int fdas_search_batched(fdas_plan_t *p, const void *spectra_dev, void *planes_dev, int batch, float threshold,
+                                   fdas_peak_t *peaks_dev, int capacity, int *counts_dev, void *stream)
+{
+    if (!p || !spectra_dev || !counts_dev || batch < 1 || capacity < 0 || (capacity > 0 && !peaks_dev))
+        return FDAS_ERR_INVALID_ARG;
+    if (!p->built) return FDAS_ERR_NOT_BUILT;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (!planes_dev)   // one scan launch and one recheck launch for the whole batch
+        return fdas_launch_search_noplane(p, spectra_dev, batch, threshold, peaks_dev, capacity, counts_dev, st);
+    const size_t spec_bytes = (size_t)p->M * (p->precision == FDAS_F64 ? 16 : 8);
+    const size_t plane_bytes = (size_t)p->K * p->M * fdas_plane_elem_bytes(p);
+    for (int b = 0; b < batch; ++b) {
+        const int rc = search_on_device(p, static_cast<const unsigned char *>(spectra_dev) + (size_t)b * spec_bytes,
+                                        static_cast<unsigned char *>(planes_dev) + (size_t)b * plane_bytes, threshold,
+                                        peaks_dev + (size_t)b * capacity, capacity, counts_dev + b, st);
+        if (rc) return rc;
+    }
+    return FDAS_OK;
+}
+
+// true when fdas_search can run without a plane for this plan (fdas_launch_search_noplane's own test)
+static bool search_is_plane_free(const fdas_plan *p)
+{
+    return fdas_uses_mma(p) && !p->plane_bf16 && p->tc_bulk_ok && p->tc_groups <= 8;
 }
 
 static int ensure_staging(fdas_plan *p, bool want_plane, int peaks_capacity)
@@ -367,11 +400,12 @@ extern "C" int fdas_search_host(fdas_plan_t *p, const void *spectrum_host, float
         return FDAS_ERR_INVALID_ARG;
     if (!p->built) return FDAS_ERR_NOT_BUILT;
     cudaStream_t st = (cudaStream_t)stream;
-    int rc = ensure_staging(p, true, capacity);
+    const bool plane_free = search_is_plane_free(p);   // no staging plane then: nothing but the spectrum and the peak list in HBM
+    int rc = ensure_staging(p, !plane_free, capacity);
     if (rc) return rc;
     const size_t spec_bytes = (size_t)p->M * (p->precision == FDAS_F64 ? 16 : 8);
     FDAS_CUDA_TRY(p, cudaMemcpyAsync(p->stage_spectrum, spectrum_host, spec_bytes, cudaMemcpyHostToDevice, st));
-    rc = search_on_device(p, p->stage_spectrum, p->stage_plane, threshold, p->stage_peaks, capacity,
+    rc = search_on_device(p, p->stage_spectrum, plane_free ? NULL : p->stage_plane, threshold, p->stage_peaks, capacity,
                           p->stage_count, st);
     if (rc) return rc;
     FDAS_CUDA_TRY(p, cudaMemcpyAsync(count_host, p->stage_count, sizeof(int), cudaMemcpyDeviceToHost, st));
@@ -395,7 +429,8 @@ extern "C" int fdas_search_host_batched(fdas_plan_t *p, const void *spectra_host
         return FDAS_ERR_INVALID_ARG;
     if (!p->built) return FDAS_ERR_NOT_BUILT;
     cudaStream_t st = (cudaStream_t)stream;
-    int rc = ensure_staging(p, true, 0);
+    const bool plane_free = search_is_plane_free(p);
+    int rc = ensure_staging(p, !plane_free, 0);
     if (rc) return rc;
     const size_t spec_bytes = (size_t)p->M * (p->precision == FDAS_F64 ? 16 : 8);
     if (!p->pipe_ready) {
@@ -425,7 +460,8 @@ extern "C" int fdas_search_host_batched(fdas_plan_t *p, const void *spectra_host
         const int b = i & 1;
         FDAS_CUDA_TRY(p, cudaStreamWaitEvent(st, p->pipe_ev[0][b], 0));              // spectrum i is on the device
         if (i >= 2) FDAS_CUDA_TRY(p, cudaStreamWaitEvent(st, p->pipe_ev[2][b], 0));  // peak buffers b were read back
-        rc = search_on_device(p, p->pipe_spec[b], p->stage_plane, threshold, p->pipe_peaks[b], capacity, p->pipe_count[b], st);
+        rc = search_on_device(p, p->pipe_spec[b], plane_free ? NULL : p->stage_plane, threshold, p->pipe_peaks[b], capacity,
+                              p->pipe_count[b], st);
         if (rc) return rc;
         FDAS_CUDA_TRY(p, cudaEventRecord(p->pipe_ev[1][b], st));
         if (i + 1 < n_series) {

@@ -29,6 +29,7 @@ EXPORTS = [
     "fdas_launch_count", "fdas_status_string", "fdas_last_cuda_error",
     "fdas_set_algorithm", "fdas_get_algorithm", "fdas_tapmatrix_host", "fdas_search",
     "fdas_set_plane_format", "fdas_get_plane_format", "fdas_quick_cast", "fdas_harmonic_sum", "fdas_harmonic_sum_drift", "fdas_band_max", "fdas_search_host_batched", "fdas_spectrum", "fdas_plan_create_jerk",
+    "fdas_search_batched",
 ]
 
 
@@ -71,6 +72,7 @@ def lib() -> ctypes.CDLL:
     L.fdas_convolve_batched.argtypes = [vp, vp, vp, i, vp]
     L.fdas_peaks.argtypes = [vp, vp, ctypes.c_float, vp, i, vp, vp]
     L.fdas_search.argtypes = [vp, vp, vp, ctypes.c_float, vp, i, vp, vp]
+    L.fdas_search_batched.argtypes = [vp, vp, vp, i, ctypes.c_float, vp, i, vp, vp]
     L.fdas_convolve_host.argtypes = [vp, vp, vp, vp]
     L.fdas_search_host.argtypes = [vp, vp, ctypes.c_float, vp, i, ctypes.POINTER(i), vp]
     L.fdas_templates_host.argtypes = [vp, vp, ctypes.c_size_t]
@@ -156,6 +158,12 @@ def fdas_search(h, spectrum_ptr, plane_ptr, threshold, peaks_ptr, capacity, coun
     return lib().fdas_search(h, ctypes.c_void_p(spectrum_ptr), ctypes.c_void_p(plane_ptr), float(threshold),
                              ctypes.c_void_p(peaks_ptr), int(capacity), ctypes.c_void_p(count_ptr),
                              ctypes.c_void_p(stream))
+
+
+def fdas_search_batched(h, spectra_ptr, planes_ptr, batch, threshold, peaks_ptr, capacity, counts_ptr, stream=0):
+    return lib().fdas_search_batched(h, ctypes.c_void_p(spectra_ptr), ctypes.c_void_p(planes_ptr), int(batch), float(threshold),
+                                     ctypes.c_void_p(peaks_ptr), int(capacity), ctypes.c_void_p(counts_ptr),
+                                     ctypes.c_void_p(stream))
 
 
 def fdas_convolve_host(h, spectrum_host_ptr, plane_host_ptr, stream=0):
@@ -392,19 +400,20 @@ class Plan:
         rec["power"] = raw[:, 2].copy().view(np.float32)
         return n, rec
 
-    def search(self, spectrum, threshold: float, plane=None, capacity: int = 1 << 16, stream: Optional[int] = None):
-        """fdas_search: returns (plane, total_count, records)."""
+    def search(self, spectrum, threshold: float, plane=None, capacity: int = 1 << 16, stream: Optional[int] = None,
+               plane_free: bool = False):
+        """fdas_search: returns (plane, total_count, records); plane_free=True passes a NULL plane (returns None for it)."""
         import numpy as np
         import torch
         assert spectrum.is_cuda and spectrum.is_contiguous() and spectrum.dtype == self.spectrum_dtype()
         assert tuple(spectrum.shape) == (self.M,)
-        if plane is None:
+        if plane is None and not plane_free:
             plane = torch.empty((self.K, self.M), dtype=self.plane_dtype(), device=spectrum.device)
         if stream is None:
             stream = torch.cuda.current_stream().cuda_stream
-        buf = torch.empty(max(capacity, 1) * 3, dtype=torch.int32, device=plane.device)
-        cnt = torch.zeros(1, dtype=torch.int32, device=plane.device)
-        self._check(fdas_search(self._h, spectrum.data_ptr(), plane.data_ptr(), threshold,
+        buf = torch.empty(max(capacity, 1) * 3, dtype=torch.int32, device=spectrum.device)
+        cnt = torch.zeros(1, dtype=torch.int32, device=spectrum.device)
+        self._check(fdas_search(self._h, spectrum.data_ptr(), 0 if plane_free else plane.data_ptr(), threshold,
                                 buf.data_ptr() if capacity else 0, capacity, cnt.data_ptr(), stream), "fdas_search")
         n = int(cnt.item())
         w = min(n, capacity)
@@ -414,6 +423,32 @@ class Plan:
         rec["r"] = raw[:, 1]
         rec["power"] = raw[:, 2].copy().view(np.float32)
         return plane, n, rec
+
+    def search_batched(self, spectra, threshold: float, capacity: int = 4096, planes=None, stream: Optional[int] = None):
+        """fdas_search_batched: spectra [B, M] on the device; planes [B, K, M] or None (plane-free form).
+        Returns (counts [B] numpy, records [B, capacity] numpy structured array; series b's first
+        min(counts[b], capacity) records are valid)."""
+        import numpy as np
+        import torch
+        assert spectra.is_cuda and spectra.is_contiguous() and spectra.dtype == self.spectrum_dtype()
+        assert spectra.dim() == 2 and spectra.shape[1] == self.M
+        B = int(spectra.shape[0])
+        if planes is not None:
+            assert planes.is_cuda and planes.is_contiguous() and tuple(planes.shape) == (B, self.K, self.M)
+            assert planes.dtype == self.plane_dtype()
+        if stream is None:
+            stream = torch.cuda.current_stream().cuda_stream
+        buf = torch.empty((B, max(capacity, 1), 3), dtype=torch.int32, device=spectra.device)
+        cnt = torch.zeros(B, dtype=torch.int32, device=spectra.device)
+        self._check(fdas_search_batched(self._h, spectra.data_ptr(), 0 if planes is None else planes.data_ptr(), B, threshold,
+                                        buf.data_ptr() if capacity else 0, capacity, cnt.data_ptr(), stream),
+                    "fdas_search_batched")
+        raw = buf.cpu().numpy()
+        rec = np.zeros((B, max(capacity, 1)), dtype=[("z_index", np.int32), ("r", np.int32), ("power", np.float32)])
+        rec["z_index"] = raw[..., 0]
+        rec["r"] = raw[..., 1]
+        rec["power"] = raw[..., 2].copy().view(np.float32)
+        return cnt.cpu().numpy(), rec
 
     def convolve_host(self, spectrum_host, plane_host, stream: Optional[int] = None):
         """numpy or pinned torch CPU buffers; copies are inside the call."""

@@ -47,3 +47,7 @@ def test_random_plan_shapes(F, S, dz, zmax, jerk, M, prec, algo, batch):
         P2, n, rec = plan.search(x, 6.0, capacity=1 << 18)
         assert torch.equal(P2, P) and n == n_ref
         assert sorted(map(tuple, rec.tolist())) == sorted(map(tuple, rec_ref.tolist()))
+        if plan.algorithm() != "fft":                   # plane-free form: the same peak set without a plane
+            _, n3, rec3 = plan.search(x, 6.0, capacity=1 << 18, plane_free=True)
+            assert n3 == n_ref
+            assert sorted(map(tuple, rec3.tolist())) == sorted(map(tuple, rec_ref.tolist()))
