@@ -386,6 +386,27 @@ int fdas_taps_host(const fdas_plan_t *p, void *dst_host, size_t bytes);
  */
 int fdas_tapmatrix_host(const fdas_plan_t *p, void *dst_host, size_t bytes);
 
+/*
+ * fdas_describe_convolve -- what fdas_convolve_batched(p, ., plane_dev, batch, .) would launch, so that a benchmark
+ * can name the kernel it times and count its work without restating the launcher.  plane_dev is
+ * only inspected for its alignment (the tensor-core form stores through tensor maps when the plane rows are 16-byte
+ * aligned); plane_dev == NULL describes the scan launch of the plane-free fdas_search.  Launches nothing.
+ * Errors: INVALID_ARG, UNSUPPORTED (plane-free form on a plan that cannot run it).
+ */
+typedef struct {
+    int32_t algorithm;         /* FDAS_ALGO_FFT, FDAS_ALGO_MMA or FDAS_ALGO_MMA_SCALAR                               */
+    int32_t split;             /* tensor-core forms: 1 = bf16 operands, 3 = fp32 operands as 3 products of bf16 terms;
+                                  0 = FFT form                                                                      */
+    int32_t groups;            /* template groups (grid y)                                                          */
+    int32_t nch, k_steps;      /* tensor-core forms: UMMA N = 16 nch columns per part, K steps of 16 taps           */
+    int32_t work_item_bins;    /* bins per work item (tensor-core forms) / valid bins per segment (FFT form)        */
+    int32_t grid_x, grid_y, block_threads;
+    size_t dynamic_smem_bytes;
+    double tensor_flops;       /* dense MMA flops the launch issues, padding included (0 for the FFT form)          */
+    char kernel[128];          /* kernel name with its template arguments                                           */
+} fdas_kernel_info_t;
+int fdas_describe_convolve(fdas_plan_t *p, const void *plane_dev, int batch, fdas_kernel_info_t *out);
+
 /* Number of kernels this plan has launched so far (template build + convolve + peaks). */
 int fdas_launch_count(const fdas_plan_t *p, int64_t *count);
 

@@ -18,6 +18,7 @@
 // A; the bank is stored in layout A as well, so the per-template work is
 //   G = F * H_k  ->  pass 1..3  ->  |y|^2  ->  store bins [L, L+V).
 #include <cuda_bf16.h>
+#include <stdio.h>
 #include "fdas_fft.cuh"
 #include "fdas_internal.h"
 
@@ -398,6 +399,32 @@ int launch_one(fdas_plan *p, const ConvParams &cp, int batch, int groups, cudaSt
     return FDAS_OK;
 }
 
+// template groups of the FFT form: one forward FFT per (segment, group); the K templates are split only when there
+// are too few segments to fill the GPU (e.g. config 1: 35 segments)
+int fft_groups(const fdas_plan *p, int batch, int *k_per_group)
+{
+    const long long ctas = (long long)batch * p->n_seg;
+    const long long want = 8LL * p->num_sms;
+    int groups = 1;
+    if (ctas < want) groups = (int)((want + ctas - 1) / ctas);
+    if (groups > p->K) groups = p->K;
+    *k_per_group = (p->K + groups - 1) / groups;
+    return (p->K + *k_per_group - 1) / *k_per_group;
+}
+
+template <class Tr>
+size_t smem_of(int S)
+{
+    switch (S) {
+    case 256: return Geo<Tr, 256>::SMEM_BYTES;
+    case 512: return Geo<Tr, 512>::SMEM_BYTES;
+    case 1024: return Geo<Tr, 1024>::SMEM_BYTES;
+    case 2048: return Geo<Tr, 2048>::SMEM_BYTES;
+    case 4096: return Geo<Tr, 4096>::SMEM_BYTES;
+    default: return 0;
+    }
+}
+
 template <class Tr>
 int launch_prec(fdas_plan *p, const ConvParams &cp, int batch, int groups, cudaStream_t st)
 {
@@ -430,19 +457,31 @@ int fdas_launch_convolve(fdas_plan *p, const void *spectra, void *planes, int ba
     cp.K = p->K;
     cp.L = p->L;
     cp.V = p->V;
-    // Template groups: one forward FFT per (segment, group).  Split the K templates only
-    // when there are too few segments to fill the GPU (e.g. config 1: 35 segments).
-    const long long ctas = (long long)batch * p->n_seg;
-    const long long want = 8LL * p->num_sms;
-    int groups = 1;
-    if (ctas < want) groups = (int)((want + ctas - 1) / ctas);
-    if (groups > p->K) groups = p->K;
-    cp.k_per_group = (p->K + groups - 1) / groups;
-    groups = (p->K + cp.k_per_group - 1) / cp.k_per_group;
+    const int groups = fft_groups(p, batch, &cp.k_per_group);
     switch (p->precision) {
     case FDAS_F64: return launch_prec<TraitsF64>(p, cp, batch, groups, st);
     case FDAS_F32: return launch_prec<TraitsF32>(p, cp, batch, groups, st);
     case FDAS_BF16: return launch_prec<TraitsBF16>(p, cp, batch, groups, st);
     default: return FDAS_ERR_INVALID_ARG;
     }
+}
+
+int fdas_fft_describe(fdas_plan *p, int batch, fdas_kernel_info_t *out)
+{
+    int kpg = 0;
+    const int groups = fft_groups(p, batch, &kpg);
+    out->algorithm = FDAS_ALGO_FFT;
+    out->split = 0;
+    out->groups = groups;
+    out->nch = 0;
+    out->k_steps = 0;
+    out->work_item_bins = p->V;
+    out->grid_x = (int32_t)((long long)batch * p->n_seg);
+    out->grid_y = groups;
+    out->block_threads = p->S / 16;
+    out->dynamic_smem_bytes = p->precision == FDAS_F64 ? smem_of<TraitsF64>(p->S) : p->precision == FDAS_F32 ? smem_of<TraitsF32>(p->S) : smem_of<TraitsBF16>(p->S);
+    out->tensor_flops = 0.0;
+    snprintf(out->kernel, sizeof(out->kernel), "fdas_convolve_kernel<%s, %d>",
+             p->precision == FDAS_F64 ? "TraitsF64" : p->precision == FDAS_F32 ? "TraitsF32" : "TraitsBF16", p->S);
+    return FDAS_OK;
 }

@@ -176,6 +176,12 @@ int fdas_launch_search_noplane(fdas_plan *p, const void *spectra, int batch, flo
 // fdas_mma.cu: the work-item size the tensor-core launch picks, and tensor maps of a [rows][cols] matrix with one box
 // per distinct run length (shared with fdas_mma_search.cu)
 int fdas_tc_encode_maps(fdas_plan *p, void *base, long long cols, long long rows, size_t elem_bytes, void *maps_out);
+// what fdas_convolve_batched would launch (fdas_describe_convolve): tensor-core forms (fdas_mma.cu; the scan launch of the
+// plane-free search when plane_dev is NULL, fdas_mma_search.cu) and the overlap-save FFT form (fdas_convolve.cu)
+int fdas_tc_describe(fdas_plan *p, const void *plane_dev, int batch, fdas_kernel_info_t *out);
+int fdas_tc_describe_noplane(fdas_plan *p, int batch, fdas_kernel_info_t *out);
+int fdas_fft_describe(fdas_plan *p, int batch, fdas_kernel_info_t *out);
+double fdas_tc_issued_flops(const fdas_plan *p, int batch);
 // fdas_peaks.cu: turns the candidates of a fused search into the peak list (same rule as fdas_peaks)
 int fdas_launch_resolve(fdas_plan *p, const void *plane, const fdas_search_args &sa, fdas_peak_t *peaks, int capacity,
                         cudaStream_t st);

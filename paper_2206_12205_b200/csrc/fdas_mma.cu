@@ -2,6 +2,7 @@
 // FDAS_ALGO_MMA, the default for FDAS_BF16 and FDAS_F32): |z| grouping, tap-matrix build, tensor maps, launch.
 // The kernels and their design notes are in fdas_mma_kernels.cuh.
 #include <math.h>
+#include <stdio.h>
 #include <stdlib.h>
 #include "fdas_mma_kernels.cuh"
 
@@ -289,24 +290,34 @@ static int launch_mma(fdas_plan *p, const TcParams &tp, unsigned gx, size_t smem
     return FDAS_OK;
 }
 
-int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, int batch, cudaStream_t st,
-                             fdas_search_args *search)
+// What fdas_launch_convolve_mma launches for (plane buffer, batch): decided once, used by the launch and by
+// fdas_describe_convolve.
+struct TcDecision {
+    bool bulk;          // box stores through tensor maps (fdas_mma_bulk_kernel) or per-thread stores (fdas_mma_convolve_kernel)
+    int split;          // 1: bf16 operands; 3: fp32 operands split into bf16 terms
+    int R;              // bins per work item
+    uint32_t smem;      // dynamic shared memory
+    unsigned gx;        // CTAs per template group
+    const TbMaps *maps;
+};
+
+static int tc_decide(fdas_plan *p, void *planes, int batch, bool want_maps, TcDecision &d)
 {
     if ((p->precision != FDAS_BF16 && p->precision != FDAS_F32) || !p->tc_supported) return FDAS_ERR_UNSUPPORTED;
-    const int split = p->precision == FDAS_F32 ? 3 : 1;
+    d.split = p->precision == FDAS_F32 ? 3 : 1;
     // tensor-map stores need 16-byte aligned plane rows: M % 4 == 0 (% 8 for a bf16 plane) and a 16-byte aligned plane
     const uint32_t esz = p->plane_bf16 ? 2u : 4u;
-    bool bulk = ((p->M * esz) % 16 == 0) && ((reinterpret_cast<uintptr_t>(planes) & 15u) == 0) && !p->tc_force_scalar_stores &&
-                p->tc_bulk_ok && (long long)batch * p->K < 0x7FFFFFFFLL;
-    const TbMaps *maps = nullptr;
-    if (bulk && plane_maps(p, planes, batch, &maps) != FDAS_OK) {   // no encoder in this driver: scalar stores
-        bulk = false;
-        maps = nullptr;
+    d.bulk = ((p->M * esz) % 16 == 0) && ((reinterpret_cast<uintptr_t>(planes) & 15u) == 0) && !p->tc_force_scalar_stores &&
+             p->tc_bulk_ok && (long long)batch * p->K < 0x7FFFFFFFLL;
+    d.maps = nullptr;
+    if (d.bulk && want_maps && plane_maps(p, planes, batch, &d.maps) != FDAS_OK) {   // no encoder in this driver: scalar stores
+        d.bulk = false;
+        d.maps = nullptr;
     }
-    if (split == 3 && !bulk) return FDAS_ERR_UNSUPPORTED;   // the split-operand form exists with box stores only
+    if (d.split == 3 && !d.bulk) return FDAS_ERR_UNSUPPORTED;   // the split-operand form exists with box stores only
     const uint32_t smem_cap = 227u * 1024u;
     auto smem_total = [&](int R) -> uint32_t {
-        return bulk ? TbSmem(R, p->tc_KS, p->tc_NT, TC_TILE * esz, split).total : TcSmem(R, p->tc_KS, p->tc_NT).total;
+        return d.bulk ? TbSmem(R, p->tc_KS, p->tc_NT, TC_TILE * esz, d.split).total : TcSmem(R, p->tc_KS, p->tc_NT).total;
     };
     // outputs per work item: the largest of 1024..128 that fits shared memory and leaves at
     // least two items per CTA
@@ -316,8 +327,64 @@ int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, in
         const long long items = (long long)batch * ((p->M + R - 1) / R);
         if (R == 128 || (smem_total(R) <= smem_cap && items >= 2LL * sms_per_group)) break;
     }
-    const uint32_t total = smem_total(R);
-    if (total > smem_cap) return FDAS_ERR_UNSUPPORTED;
+    d.R = R;
+    d.smem = smem_total(R);
+    if (d.smem > smem_cap) return FDAS_ERR_UNSUPPORTED;
+    const long long items = (long long)batch * ((p->M + R - 1) / R);
+    if (items >= 0x7FFFFFFFLL) return FDAS_ERR_UNSUPPORTED;   // the kernels count work items in 32 bits
+    d.gx = (unsigned)(items < sms_per_group ? items : sms_per_group);
+    return FDAS_OK;
+}
+
+// dense MMA flops one launch over `batch` series issues (padding included): per 128-bin tile and template group,
+// 2 parts x sum over the K steps of 2 * 128 * N_ks * 16, three products per tap in the split form
+double fdas_tc_issued_flops(const fdas_plan *p, int batch)
+{
+    const int split = p->precision == FDAS_F32 ? 3 : 1;
+    double per_tile = 0.0;
+    for (int g = 0; g < p->tc_groups; ++g)
+        for (int ks = 0; ks < p->tc_KS; ++ks) {
+            unsigned nib = 0;
+            if (split == 3 && g < 8) nib = (unsigned)((ks < 16 ? p->tc_nks_lo[g] >> (4 * ks) : p->tc_nks_hi[g] >> (4 * (ks - 16))) & 15ull);
+            const int n = nib ? 16 * (int)nib : p->tc_NT;       // the bf16 form runs every K step at full width
+            per_tile += 2.0 * 2.0 * TC_TILE * n * 16.0 * (split == 3 ? 3.0 : 1.0);
+        }
+    return per_tile * (double)batch * (double)((p->M + TC_TILE - 1) / TC_TILE);
+}
+
+int fdas_tc_describe(fdas_plan *p, const void *plane_dev, int batch, fdas_kernel_info_t *out)
+{
+    TcDecision d;
+    const int rc = tc_decide(p, const_cast<void *>(plane_dev), batch, false, d);
+    if (rc) return rc;
+    out->algorithm = d.bulk ? FDAS_ALGO_MMA : FDAS_ALGO_MMA_SCALAR;
+    out->split = d.split;
+    out->groups = p->tc_groups;
+    out->nch = p->tc_NT / 16;
+    out->k_steps = p->tc_KS;
+    out->work_item_bins = d.R;
+    out->grid_x = (int32_t)d.gx;
+    out->grid_y = p->tc_groups;
+    out->block_threads = d.bulk ? tb_threads(d.split) : TC_THREADS;
+    out->dynamic_smem_bytes = d.smem;
+    out->tensor_flops = fdas_tc_issued_flops(p, batch);
+    if (d.bulk)
+        snprintf(out->kernel, sizeof(out->kernel), "fdas_mma_bulk_kernel<%d, %s, %d>", p->tc_NT / 16, p->plane_bf16 ? "__nv_bfloat16" : "float", d.split);
+    else
+        snprintf(out->kernel, sizeof(out->kernel), "fdas_mma_convolve_kernel<%d, %s>", p->tc_NT / 16, p->plane_bf16 ? "__nv_bfloat16" : "float");
+    return FDAS_OK;
+}
+
+int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, int batch, cudaStream_t st,
+                             fdas_search_args *search)
+{
+    TcDecision d;
+    { const int rc = tc_decide(p, planes, batch, true, d); if (rc) return rc; }
+    const bool bulk = d.bulk;
+    const int split = d.split, R = d.R;
+    const uint32_t total = d.smem;
+    const TbMaps *maps = d.maps;
+    const unsigned gx = d.gx;
     TcParams tp;
     tc_fill_params(p, tp, spectra, planes, batch, R);
     if (search) {
@@ -327,9 +394,6 @@ int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, in
         tp.search = fdas_search_args{};
         tp.search.cand_span = 8;
     }
-    const long long items = (long long)batch * tp.n_blocks;
-    if (items >= 0x7FFFFFFFLL) return FDAS_ERR_UNSUPPORTED;   // the kernels count work items in 32 bits
-    const unsigned gx = (unsigned)(items < sms_per_group ? items : sms_per_group);
     switch (p->tc_NT / 16) {
     case 1: if (split == 3) return launch_mma_split<1>(p, tp, gx, total, maps, st);
             return p->plane_bf16 ? launch_mma<1, __nv_bfloat16>(p, tp, gx, total, maps, st) : launch_mma<1, float>(p, tp, gx, total, maps, st);

@@ -169,8 +169,10 @@ __device__ __forceinline__ uint32_t tb_items(const TcParams &p)
         return (uint32_t)p.batch * (uint32_t)p.n_blocks;
     }
 }
-// TB_RECHECK: every thread of the CTA (of the cluster, when the template groups of an item are spread over one)
-// meets here twice per work item: once when the item's powers are in scratch, once when they have been tested
+// TB_RECHECK: the epilogue threads meet here twice per work item: once when the item's powers are in scratch, once
+// when they have been tested.  One template group: a named barrier over the epilogue warps only, so the loader and
+// the MMA warp run ahead into the next item.  Several groups (one CTA each, forming a cluster): a cluster barrier,
+// which counts EVERY thread of the cluster -- the loader and MMA warps then call this too.
 __device__ __forceinline__ void tb_item_sync(int clustered, int threads)
 {
     __syncwarp();
@@ -543,8 +545,10 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
         }
         umma_commit_elected(z_empty + 8 * buf, elected);
         if constexpr (MODE == TB_RECHECK) {
-            tb_item_sync(p.clustered, (int)blockDim.x);
-            tb_item_sync(p.clustered, (int)blockDim.x);
+            if (p.clustered) {   // a cluster barrier counts every thread (see tb_item_sync)
+                tb_item_sync(1, 0);
+                tb_item_sync(1, 0);
+            }
         }
     }
 }
@@ -634,8 +638,10 @@ __device__ __forceinline__ void spectrum_loader(const TcParams &p, unsigned char
         mbar_arrive(z_full + 8 * buf);
         named_bar_sync(1, TC_LOAD_THREADS);   // xs is rewritten by the next item
         if constexpr (MODE == TB_RECHECK) {
-            tb_item_sync(p.clustered, (int)blockDim.x);
-            tb_item_sync(p.clustered, (int)blockDim.x);
+            if (p.clustered) {
+                tb_item_sync(1, 0);
+                tb_item_sync(1, 0);
+            }
         }
     }
 }
@@ -1116,46 +1122,56 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
                 // the cells of the flagged tile, meet again before the strip is overwritten
                 if (issuer) bulk_wait_all();
                 __threadfence();
-                tb_item_sync(p.clustered, TB_THREADS);
+                tb_item_sync(p.clustered, TB_EPI_WARPS * 32);
                 {
                     const int G = (int)gridDim.y;
                     const int k_lo = (int)((long long)p.K * grp / G), k_hi = (int)((long long)p.K * (grp + 1) / G);
                     const float *S = p.search.scratch + (size_t)blockIdx.x * p.K * FDAS_TC_STRIP;
                     const long long r_first = blk0;                    // plane bin of strip column 0
                     const int c_lo = centre * TC_TILE, c_end = n_tiles * TC_TILE;
-                    for (int idx = threadIdx.x; idx < (k_hi - k_lo) * TC_TILE; idx += TB_EPI_WARPS * 32) {
-                        const int k = k_lo + idx / TC_TILE, c = c_lo + idx % TC_TILE;
-                        const long long r = r_first + c;
-                        if (r >= p.M) continue;
-                        const float v = __ldcg(S + (size_t)k * FDAS_TC_STRIP + c);
-                        if (!(v > thr)) continue;
-                        bool ok = true;
+                    // thread -> one bin of the tile and every (TB_EPI_WARPS / 4)-th row; the loads of eight rows are in
+                    // flight together (the strip is in L2: ~1 us per dependent load otherwise)
+                    constexpr int RPP = TB_EPI_WARPS / 4, UB = 8;
+                    const int c = c_lo + (threadIdx.x & (TC_TILE - 1));
+                    const long long r = r_first + c;
+                    for (int kb = k_lo + (threadIdx.x >> 7); kb < k_hi && r < p.M; kb += UB * RPP) {
+                        float vv[UB];
 #pragma unroll
-                        for (int dk = -1; dk <= 1; ++dk) {
+                        for (int u = 0; u < UB; ++u)
+                            vv[u] = kb + u * RPP < k_hi ? __ldcg(S + (size_t)(kb + u * RPP) * FDAS_TC_STRIP + c) : -__int_as_float(0x7f800000);
 #pragma unroll
-                            for (int dr = -1; dr <= 1; ++dr) {
-                                if (dk == 0 && dr == 0) continue;
-                                const int kk = k + dk, cc = c + dr;
-                                if (kk < 0 || kk >= p.K || cc < 0 || cc >= c_end || r + dr < 0 || r + dr >= p.M) continue;
-                                const float nb = __ldcg(S + (size_t)kk * FDAS_TC_STRIP + cc);
-                                const bool precedes = (dk < 0) || (dk == 0 && dr < 0);
-                                ok = ok && (precedes ? (v > nb) : (v >= nb));
+                        for (int u = 0; u < UB; ++u) {
+                            const float v = vv[u];
+                            if (!(v > thr)) continue;
+                            const int k = kb + u * RPP;
+                            bool ok = true;
+#pragma unroll
+                            for (int dk = -1; dk <= 1; ++dk) {
+#pragma unroll
+                                for (int dr = -1; dr <= 1; ++dr) {
+                                    if (dk == 0 && dr == 0) continue;
+                                    const int kk = k + dk, cc = c + dr;
+                                    if (kk < 0 || kk >= p.K || cc < 0 || cc >= c_end || r + dr < 0 || r + dr >= p.M) continue;
+                                    const float nb = __ldcg(S + (size_t)kk * FDAS_TC_STRIP + cc);
+                                    const bool precedes = (dk < 0) || (dk == 0 && dr < 0);
+                                    ok = ok && (precedes ? (v > nb) : (v >= nb));
+                                }
                             }
-                        }
-                        if (ok) {
-                            const int slot = atomicAdd(p.search.counts + ser, 1);
-                            if (slot < p.search.capacity) {
-                                fdas_peak_t rec;
-                                rec.z_index = k;
-                                rec.r = (int32_t)r;
-                                rec.power = v;
-                                p.search.peaks[(size_t)ser * p.search.capacity + slot] = rec;
+                            if (ok) {
+                                const int slot = atomicAdd(p.search.counts + ser, 1);
+                                if (slot < p.search.capacity) {
+                                    fdas_peak_t rec;
+                                    rec.z_index = k;
+                                    rec.r = (int32_t)r;
+                                    rec.power = v;
+                                    p.search.peaks[(size_t)ser * p.search.capacity + slot] = rec;
+                                }
                             }
                         }
                     }
                     if (threadIdx.x == 0 && grp == 0) p.search.tile_flags[__ldcg(p.search.tile_list + it)] = 0;   // flags are all zero again after this launch
                 }
-                tb_item_sync(p.clustered, TB_THREADS);
+                tb_item_sync(p.clustered, TB_EPI_WARPS * 32);
             }
         }
         if (issuer) bulk_wait_all();

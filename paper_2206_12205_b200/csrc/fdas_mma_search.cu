@@ -13,6 +13,7 @@
 //               warps apply the peak rule of fdas_peaks to the cells of the listed tile.
 // The peak set (and every power) equals that of fdas_search with a float plane.  The only HBM stream left is the
 // spectrum read: the path is bound by the tensor pipe (bf16 operands) instead of the plane write.
+#include <stdio.h>
 #include <stdlib.h>
 #include "fdas_mma_kernels.cuh"
 
@@ -61,6 +62,39 @@ int launch_nch(fdas_plan *p, const TcParams &tp, unsigned gx, size_t smem_bytes,
 }
 
 }  // namespace
+
+// work item of the scan launch: as for a plane (the largest of 1024..128 bins that fits and leaves two items per CTA)
+static int scan_item_bins(const fdas_plan *p, int batch, int split, int sms_per_group)
+{
+    int R = 1024;
+    for (;; R >>= 1) {
+        const long long items = (long long)batch * ((p->M + R - 1) / R);
+        if (R == 128 || (TbSmem(R, p->tc_KS, p->tc_NT, TC_TILE * 4, split, false).total <= 227u * 1024u && items >= 2LL * sms_per_group)) break;
+    }
+    return R;
+}
+
+int fdas_tc_describe_noplane(fdas_plan *p, int batch, fdas_kernel_info_t *out)
+{
+    if (!fdas_uses_mma(p) || p->plane_bf16 || !p->tc_bulk_ok || p->tc_groups > 8) return FDAS_ERR_UNSUPPORTED;
+    const int split = p->precision == FDAS_F32 ? 3 : 1;
+    const int sms_per_group = p->num_sms / p->tc_groups > 0 ? p->num_sms / p->tc_groups : 1;
+    const int R = scan_item_bins(p, batch, split, sms_per_group);
+    const long long items = (long long)batch * ((p->M + R - 1) / R);
+    out->algorithm = FDAS_ALGO_MMA;
+    out->split = split;
+    out->groups = p->tc_groups;
+    out->nch = p->tc_NT / 16;
+    out->k_steps = p->tc_KS;
+    out->work_item_bins = R;
+    out->grid_x = (int32_t)(items < sms_per_group ? items : sms_per_group);
+    out->grid_y = p->tc_groups;
+    out->block_threads = tb_threads(split);
+    out->dynamic_smem_bytes = TbSmem(R, p->tc_KS, p->tc_NT, TC_TILE * 4, split, false).total;
+    out->tensor_flops = fdas_tc_issued_flops(p, batch);
+    snprintf(out->kernel, sizeof(out->kernel), "fdas_mma_bulk_kernel<%d, float, %d, TB_SCAN> (+ TB_RECHECK on the listed tiles)", p->tc_NT / 16, split);
+    return FDAS_OK;
+}
 
 int fdas_launch_search_noplane(fdas_plan *p, const void *spectra, int batch, float thr, fdas_peak_t *peaks, int capacity,
                                int *counts, cudaStream_t st)
@@ -129,13 +163,9 @@ int fdas_launch_search_noplane(fdas_plan *p, const void *spectra, int batch, flo
     sa.counts = counts;
     p->tf_calls += 1;
 
-    // ---- scan launch: work items as for a plane (the largest of 1024..128 bins that fits and leaves two items per CTA)
+    // ---- scan launch
     {
-        int R = 1024;
-        for (;; R >>= 1) {
-            const long long items = (long long)batch * ((p->M + R - 1) / R);
-            if (R == 128 || (TbSmem(R, p->tc_KS, p->tc_NT, TC_TILE * 4, split, false).total <= smem_cap && items >= 2LL * sms_per_group)) break;
-        }
+        const int R = scan_item_bins(p, batch, split, sms_per_group);
         const uint32_t total = TbSmem(R, p->tc_KS, p->tc_NT, TC_TILE * 4, split, false).total;
         if (total > smem_cap) return FDAS_ERR_UNSUPPORTED;
         TcParams tp;

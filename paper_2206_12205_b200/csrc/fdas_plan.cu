@@ -562,6 +562,19 @@ extern "C" int fdas_tapmatrix_host(const fdas_plan_t *p, void *dst_host, size_t 
     return FDAS_OK;
 }
 
+extern "C" int fdas_describe_convolve(fdas_plan_t *p, const void *plane_dev, int batch, fdas_kernel_info_t *out)
+{
+    if (!p || !out || batch < 1) return FDAS_ERR_INVALID_ARG;
+    memset(out, 0, sizeof(*out));
+    if (!plane_dev) return fdas_tc_describe_noplane(p, batch, out);
+    if (fdas_uses_mma(p)) {
+        const int rc = fdas_tc_describe(p, plane_dev, batch, out);
+        // fp32 under FDAS_ALGO_AUTO: a plane buffer the split-operand kernel cannot take goes to the FFT kernel
+        if (!(rc == FDAS_ERR_UNSUPPORTED && p->precision == FDAS_F32 && p->algo == FDAS_ALGO_AUTO)) return rc;
+    }
+    return fdas_fft_describe(p, batch, out);
+}
+
 extern "C" int fdas_launch_count(const fdas_plan_t *p, int64_t *count)
 {
     if (!p || !count) return FDAS_ERR_INVALID_ARG;

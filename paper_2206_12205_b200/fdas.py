@@ -29,7 +29,7 @@ EXPORTS = [
     "fdas_launch_count", "fdas_status_string", "fdas_last_cuda_error",
     "fdas_set_algorithm", "fdas_get_algorithm", "fdas_tapmatrix_host", "fdas_search",
     "fdas_set_plane_format", "fdas_get_plane_format", "fdas_quick_cast", "fdas_harmonic_sum", "fdas_harmonic_sum_drift", "fdas_band_max", "fdas_search_host_batched", "fdas_spectrum", "fdas_plan_create_jerk",
-    "fdas_search_batched",
+    "fdas_search_batched", "fdas_describe_convolve",
 ]
 
 
@@ -45,6 +45,15 @@ class fdas_info_t(ctypes.Structure):
         ("n_segments", ctypes.c_int64), ("plane_row_pitch", ctypes.c_int64),
         ("plane_elem_bytes", ctypes.c_size_t), ("spectrum_elem_bytes", ctypes.c_size_t),
         ("bank_bytes", ctypes.c_size_t),
+    ]
+
+
+class fdas_kernel_info_t(ctypes.Structure):
+    _fields_ = [
+        ("algorithm", ctypes.c_int32), ("split", ctypes.c_int32), ("groups", ctypes.c_int32), ("nch", ctypes.c_int32),
+        ("k_steps", ctypes.c_int32), ("work_item_bins", ctypes.c_int32), ("grid_x", ctypes.c_int32),
+        ("grid_y", ctypes.c_int32), ("block_threads", ctypes.c_int32), ("dynamic_smem_bytes", ctypes.c_size_t),
+        ("tensor_flops", ctypes.c_double), ("kernel", ctypes.c_char * 128),
     ]
 
 
@@ -73,6 +82,7 @@ def lib() -> ctypes.CDLL:
     L.fdas_peaks.argtypes = [vp, vp, ctypes.c_float, vp, i, vp, vp]
     L.fdas_search.argtypes = [vp, vp, vp, ctypes.c_float, vp, i, vp, vp]
     L.fdas_search_batched.argtypes = [vp, vp, vp, i, ctypes.c_float, vp, i, vp, vp]
+    L.fdas_describe_convolve.argtypes = [vp, vp, i, ctypes.POINTER(fdas_kernel_info_t)]
     L.fdas_convolve_host.argtypes = [vp, vp, vp, vp]
     L.fdas_search_host.argtypes = [vp, vp, ctypes.c_float, vp, i, ctypes.POINTER(i), vp]
     L.fdas_templates_host.argtypes = [vp, vp, ctypes.c_size_t]
@@ -234,6 +244,12 @@ def fdas_search_host_batched(h, spectra_host_ptr, n_series, threshold, peaks_hos
 
 def fdas_spectrum(h, timeseries_ptr, spectrum_ptr, stream=0):
     return lib().fdas_spectrum(h, timeseries_ptr, spectrum_ptr, stream)
+
+
+def fdas_describe_convolve(h, plane_ptr, batch=1):
+    info = fdas_kernel_info_t()
+    rc = lib().fdas_describe_convolve(h, ctypes.c_void_p(plane_ptr), int(batch), ctypes.byref(info))
+    return rc, info
 
 
 def fdas_launch_count(h):
@@ -503,6 +519,16 @@ class Plan:
         rc, a = fdas_get_algorithm(self._h)
         self._check(rc, "fdas_get_algorithm")
         return {FDAS_ALGO_FFT: "fft", FDAS_ALGO_MMA: "mma", FDAS_ALGO_MMA_SCALAR: "mma_scalar"}[a]
+
+    def describe(self, plane=None, batch: int = 1) -> dict:
+        """fdas_describe_convolve as a dict: the kernel fdas_convolve would launch for this plane buffer (None: the scan
+        launch of the plane-free search), its grid and the tensor flops it issues."""
+        rc, info = fdas_describe_convolve(self._h, 0 if plane is None else plane.data_ptr(), batch)
+        self._check(rc, "fdas_describe_convolve")
+        d = {name: getattr(info, name) for name, _ in info._fields_}
+        d["kernel"] = info.kernel.decode()
+        d["algorithm"] = {FDAS_ALGO_FFT: "fft", FDAS_ALGO_MMA: "mma", FDAS_ALGO_MMA_SCALAR: "mma_scalar"}[info.algorithm]
+        return d
 
     def launch_count(self) -> int:
         return fdas_launch_count(self._h)[1]
