@@ -61,6 +61,8 @@ def lib() -> ctypes.CDLL:
         L.fdas_oracle_peaks.argtypes = [dp, ctypes.c_int, ctypes.c_int64, ctypes.c_double, dp,
                                         ctypes.c_int64]
         L.fdas_oracle_peaks.restype = ctypes.c_int64
+        L.fdas_oracle_peaks3.argtypes = [dp, ctypes.c_int, ctypes.c_int, ctypes.c_int64, ctypes.c_double, dp, ctypes.c_int64]
+        L.fdas_oracle_peaks3.restype = ctypes.c_int64
         _lib = L
     return _lib
 
@@ -174,3 +176,28 @@ def power_plane_jerk(X, zmax: float, dz: float, w: float, r_begin: int = 0, r_en
         r_end = len(X)
     K = 2 * int(np.floor(zmax / dz + 1e-9)) + 1
     return np.stack([convolve_row(X, template_taps_jerk(-zmax + k * dz, w), r_begin, r_end) for k in range(K)])
+
+
+# ---- jerk volume (readings A25, A27) ----------------------------------------
+def jerk_values(wmax: float, dw: float) -> np.ndarray:
+    """w_i = -wmax + i dw, i = 0..2 floor(wmax/dw): the slabs of the volume (the same grid rule as z)."""
+    n = int(np.floor(wmax / dw + 1e-9)) if dw > 0 else 0
+    return -wmax + dw * np.arange(2 * n + 1)
+
+
+def power_volume(X, zmax: float, dz: float, wmax: float, dw: float, r_begin: int = 0, r_end: int | None = None) -> np.ndarray:
+    """V[i][k][r - r_begin]: the slab of every jerk value, float64 [W, K, r_end - r_begin]."""
+    return np.stack([power_plane_jerk(X, zmax, dz, float(w), r_begin, r_end) for w in jerk_values(wmax, dw)])
+
+
+def peaks3(V, thr: float, capacity: int | None = None):
+    """Returns (total_count, list of (i, k, r, power)) under the 26-neighbour peak rule."""
+    V = np.ascontiguousarray(np.asarray(V, dtype=np.float64))
+    W, K, M = V.shape
+    if capacity is None:
+        capacity = int(np.count_nonzero(V > thr))
+    out = np.empty(4 * max(capacity, 1), dtype=np.float64)
+    n = int(lib().fdas_oracle_peaks3(_dptr(V), W, K, M, float(thr), _dptr(out), int(capacity)))
+    w = min(n, capacity)
+    rec = [(int(out[4 * i]), int(out[4 * i + 1]), int(out[4 * i + 2]), float(out[4 * i + 3])) for i in range(w)]
+    return n, rec

@@ -282,3 +282,46 @@ int64_t fdas_oracle_peaks(const double *P, int K, int64_t M, double thr,
     }
     return count;
 }
+
+/* Peaks of an f-fdot-fddot volume (the jerk search "extends the f-fdot plane into an
+ * f-fdot-fddot volume"; reading A27): V[i][k][r], i = 0..W-1 the jerk slab, k the template row, r the
+ * bin.  The plane rule (reading A14) with one more axis: (i, k, r) is a peak iff V > thr and V >= every existing
+ * one of its 26 neighbours, strictly > for neighbours that precede it in (i, k, r) lexicographic order (a
+ * plateau gives exactly one peak).  out[4*n] = i, k, r, power; returns the TOTAL count; only the first
+ * `capacity` (in scan order) are written.  W = 1 is fdas_oracle_peaks. */
+int64_t fdas_oracle_peaks3(const double *V, int W, int K, int64_t M, double thr, double *out, int64_t capacity)
+{
+    int64_t count = 0;
+    for (int i = 0; i < W; ++i) {
+        for (int k = 0; k < K; ++k) {
+            for (int64_t r = 0; r < M; ++r) {
+                double v = V[((int64_t)i * K + k) * M + r];
+                if (!(v > thr)) continue;
+                int ok = 1;
+                for (int di = -1; di <= 1 && ok; ++di) {
+                    for (int dk = -1; dk <= 1 && ok; ++dk) {
+                        for (int dr = -1; dr <= 1; ++dr) {
+                            if (di == 0 && dk == 0 && dr == 0) continue;
+                            int ii = i + di, kk = k + dk;
+                            int64_t rr = r + dr;
+                            if (ii < 0 || ii >= W || kk < 0 || kk >= K || rr < 0 || rr >= M) continue;
+                            double n = V[((int64_t)ii * K + kk) * M + rr];
+                            int precedes = (di < 0) || (di == 0 && (dk < 0 || (dk == 0 && dr < 0)));
+                            if (precedes ? !(v > n) : !(v >= n)) { ok = 0; break; }
+                        }
+                    }
+                }
+                if (ok) {
+                    if (count < capacity && out) {
+                        out[4 * count + 0] = (double)i;
+                        out[4 * count + 1] = (double)k;
+                        out[4 * count + 2] = (double)r;
+                        out[4 * count + 3] = v;
+                    }
+                    ++count;
+                }
+            }
+        }
+    }
+    return count;
+}
