@@ -387,6 +387,61 @@ int fdas_taps_host(const fdas_plan_t *p, void *dst_host, size_t bytes);
 int fdas_tapmatrix_host(const fdas_plan_t *p, void *dst_host, size_t bytes);
 
 /*
+ * ---- f-fdot-fddot volume: the jerk search (section 2.2: "extends the f-fdot plane into an f-fdot-fddot
+ * volume.  More candidate templates are required to populate the third dimension") ------------------------------------
+ * A volume is a stack of slabs V[i][k][r], one per jerk value w_i = -wmax + i*dw, i = 0..2*floor(wmax/dw) (the grid
+ * rule of z; w = change of the drift z over the observation, in Fourier bins); slab i is the plane of
+ * fdas_plan_create_jerk(.., w_i, ..) (reading A25).  The volume object owns one plan per slab; all slabs are
+ * convolved from the same spectrum in device memory.
+ *   fdas_volume_create          same arguments and errors as fdas_plan_create_jerk, plus the w grid (wmax >= 0, dw > 0,
+ *                               at most 511 slabs); the segment length must fit the widest taps (|w| = wmax)
+ *   fdas_volume_slab            the plan of slab i (borrowed: do not destroy it), e.g. for fdas_set_plane_format
+ *   fdas_volume_set_algorithm   fdas_set_algorithm on every slab
+ *   fdas_volume_build_templates fdas_build_templates on every slab (asynchronous on `stream`)
+ *   fdas_volume_convolve        volume_dev [n_slabs][K][M] in the slabs' plane format, fully overwritten
+ *   fdas_volume_peaks           (i, k, r) is reported iff V > threshold and V >= each of its (up to 26) existing
+ *                               neighbours, strictly greater than those that precede it in (i, k, r) lexicographic
+ *                               order: the rule of fdas_peaks with one more axis (reading A27; a plateau
+ *                               yields one peak).  snprintf convention for count_dev; record order unspecified
+ *   fdas_volume_search          fdas_volume_convolve + fdas_volume_peaks
+ *   fdas_volume_search_host     host spectrum in (copied to the device ONCE for all slabs), peak list out; the
+ *                               volume stays in device memory owned by the volume object; synchronises `stream`
+ * Errors as for the plan calls they wrap.
+ */
+typedef struct fdas_volume fdas_volume_t; /* opaque */
+typedef struct {
+    int32_t w_index; /* i, slab of the volume; w = -wmax + i*dw                          */
+    int32_t z_index; /* k, row of the slab; z = -zmax + k*dz                             */
+    int32_t r;       /* Fourier bin                                                      */
+    float power;     /* V[i][k][r]                                                       */
+} fdas_peak3_t;
+typedef struct {
+    int32_t n_slabs;     /* W = 2*floor(wmax/dw) + 1                                      */
+    int32_t n_templates; /* K rows per slab                                               */
+    int64_t n_bins;      /* M                                                             */
+    int32_t precision;   /* fdas_precision_t                                              */
+    size_t elem_bytes;   /* bytes per volume element (the slabs' plane format)            */
+    double wmax, dw;
+} fdas_volume_info_t;
+int fdas_volume_create(fdas_volume_t **out, int64_t N, double zmax, double dz, double wmax, double dw, int seglen,
+                       int precision);
+int fdas_volume_destroy(fdas_volume_t *v); /* NULL is OK; synchronises the device */
+int fdas_volume_info(const fdas_volume_t *v, fdas_volume_info_t *info);
+int fdas_volume_w_of_index(const fdas_volume_t *v, int i, double *w);
+int fdas_volume_slab(const fdas_volume_t *v, int i, fdas_plan_t **plan);
+int fdas_volume_set_algorithm(fdas_volume_t *v, int algorithm);
+int fdas_volume_build_templates(fdas_volume_t *v, void *stream);
+int fdas_volume_convolve(fdas_volume_t *v, const void *spectrum_dev, void *volume_dev, void *stream);
+int fdas_volume_peaks(fdas_volume_t *v, const void *volume_dev, float threshold, fdas_peak3_t *peaks_dev, int capacity,
+                      int *count_dev, void *stream);
+int fdas_volume_search(fdas_volume_t *v, const void *spectrum_dev, void *volume_dev, float threshold,
+                       fdas_peak3_t *peaks_dev, int capacity, int *count_dev, void *stream);
+int fdas_volume_search_host(fdas_volume_t *v, const void *spectrum_host, float threshold, fdas_peak3_t *peaks_host,
+                            int capacity, int *count_host, void *stream);
+int fdas_volume_launch_count(const fdas_volume_t *v, int64_t *count);
+int fdas_volume_last_cuda_error(const fdas_volume_t *v);
+
+/*
  * fdas_describe_convolve -- what fdas_convolve_batched(p, ., plane_dev, batch, .) would launch, so that a benchmark
  * can name the kernel it times and count its work without restating the launcher.  plane_dev is
  * only inspected for its alignment (the tensor-core form stores through tensor maps when the plane rows are 16-byte

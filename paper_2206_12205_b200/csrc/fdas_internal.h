@@ -195,6 +195,9 @@ static inline int fdas_uses_mma(const fdas_plan *p)
 }
 int fdas_launch_peaks(fdas_plan *p, const void *plane, float thr, fdas_peak_t *peaks, int capacity,
                       int *count, cudaStream_t st);
+// fdas_peaks.cu: 26-neighbour peak rule over a volume of n_slabs planes of this plan's shape
+int fdas_launch_peaks3(fdas_plan *p, const void *volume, int n_slabs, float thr, fdas_peak3_t *peaks, int capacity, int *count,
+                       cudaStream_t st);
 // fdas_harmonic.cu: S_H[k][r] = sum_h P[k0 + h (k - k0)][h r]
 int fdas_launch_harmonic_sum(fdas_plan *p, const void *plane, void *sum, int n_harmonics, int k0, int drift, cudaStream_t st);
 // fdas_rfft.cu: the real FFT ahead of the convolution

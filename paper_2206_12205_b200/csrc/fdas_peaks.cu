@@ -121,7 +121,98 @@ fdas_resolve_kernel(const PT *__restrict__ P, int K, long long M, float thr, con
     }
 }
 
+// ---- f-fdot-fddot volume (fdas_volume_peaks; reading A27): the plane rule with one more axis.  V[i][k][r],
+// i = 0..W-1; 26 neighbours, strictly greater than those that precede the cell in (i, k, r) order.
+template <typename PT>
+__device__ __forceinline__ void test_cell3(const PT *__restrict__ V, int W, int K, long long M, int i, int k, long long r,
+                                           typename elem<PT>::cmp v, float thr, fdas_peak3_t *peaks, int capacity, int *count)
+{
+    using CT = typename elem<PT>::cmp;
+    if (!(v > (CT)thr)) return;
+    bool ok = true;
+#pragma unroll
+    for (int di = -1; di <= 1; ++di) {
+#pragma unroll
+        for (int dk = -1; dk <= 1; ++dk) {
+#pragma unroll
+            for (int dr = -1; dr <= 1; ++dr) {
+                if (di == 0 && dk == 0 && dr == 0) continue;
+                const int ii = i + di, kk = k + dk;
+                const long long rr = r + dr;
+                if (ii < 0 || ii >= W || kk < 0 || kk >= K || rr < 0 || rr >= M) continue;
+                const CT n = elem<PT>::val(V[((size_t)ii * K + kk) * M + rr]);
+                const bool precedes = (di < 0) || (di == 0 && (dk < 0 || (dk == 0 && dr < 0)));
+                ok = ok && (precedes ? (v > n) : (v >= n));
+            }
+        }
+    }
+    if (ok) {
+        const int slot = atomicAdd(count, 1);
+        if (slot < capacity) {
+            fdas_peak3_t rec;
+            rec.w_index = i;
+            rec.z_index = k;
+            rec.r = (int32_t)r;
+            rec.power = (float)v;
+            peaks[slot] = rec;
+        }
+    }
+}
+
+template <typename PT, typename VT, int NE>
+__global__ void __launch_bounds__(256)
+fdas_peaks3_kernel(const PT *__restrict__ V, int W, int K, long long M, float thr, fdas_peak3_t *peaks, int capacity, int *count)
+{
+    const long long rows = (long long)W * K, total = rows * M;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (M % NE == 0) {
+        const VT *PV = reinterpret_cast<const VT *>(V);
+        const long long nv = total / NE;
+        for (long long q = tid; q < nv; q += stride) {
+            union { VT v; PT e[NE]; } u;
+            u.v = __ldcs(PV + q);   // 128-bit streaming load
+            using CT = typename elem<PT>::cmp;
+            CT m = elem<PT>::val(u.e[0]);
+#pragma unroll
+            for (int c = 1; c < NE; ++c) m = max(m, elem<PT>::val(u.e[c]));
+            if (m > (CT)thr) {
+                const long long e0 = q * NE;
+                const long long row = e0 / M;
+                const long long r = e0 - row * M;
+                const int i = (int)(row / K), k = (int)(row - (long long)i * K);
+#pragma unroll
+                for (int c = 0; c < NE; ++c) test_cell3<PT>(V, W, K, M, i, k, r + c, elem<PT>::val(u.e[c]), thr, peaks, capacity, count);
+            }
+        }
+    } else {
+        for (long long e = tid; e < total; e += stride) {
+            const long long row = e / M;
+            const int i = (int)(row / K), k = (int)(row - (long long)i * K);
+            test_cell3<PT>(V, W, K, M, i, k, e - row * M, elem<PT>::val(V[e]), thr, peaks, capacity, count);
+        }
+    }
+}
+
 }  // namespace
+
+int fdas_launch_peaks3(fdas_plan *p, const void *volume, int n_slabs, float thr, fdas_peak3_t *peaks, int capacity, int *count,
+                       cudaStream_t st)
+{
+    FDAS_CUDA_TRY(p, cudaMemsetAsync(count, 0, sizeof(int), st));
+    const long long total = (long long)n_slabs * p->K * p->M;
+    long long want = (total / 4 + 255) / 256;
+    const long long cap = (long long)p->num_sms * 8;
+    const int grid = (int)(want < cap ? (want > 0 ? want : 1) : cap);
+    if (p->precision == FDAS_F64)
+        fdas_peaks3_kernel<double, double2, 2><<<grid, 256, 0, st>>>((const double *)volume, n_slabs, p->K, p->M, thr, peaks, capacity, count);
+    else if (p->plane_bf16)
+        fdas_peaks3_kernel<bf16raw, uint4, 8><<<grid, 256, 0, st>>>((const bf16raw *)volume, n_slabs, p->K, p->M, thr, peaks, capacity, count);
+    else
+        fdas_peaks3_kernel<float, float4, 4><<<grid, 256, 0, st>>>((const float *)volume, n_slabs, p->K, p->M, thr, peaks, capacity, count);
+    FDAS_CUDA_TRY(p, cudaGetLastError());
+    return FDAS_OK;
+}
 
 int fdas_launch_resolve(fdas_plan *p, const void *plane, const fdas_search_args &sa, fdas_peak_t *peaks, int capacity,
                         cudaStream_t st)

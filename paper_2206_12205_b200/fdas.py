@@ -30,6 +30,9 @@ EXPORTS = [
     "fdas_set_algorithm", "fdas_get_algorithm", "fdas_tapmatrix_host", "fdas_search",
     "fdas_set_plane_format", "fdas_get_plane_format", "fdas_quick_cast", "fdas_harmonic_sum", "fdas_harmonic_sum_drift", "fdas_band_max", "fdas_search_host_batched", "fdas_spectrum", "fdas_plan_create_jerk",
     "fdas_search_batched", "fdas_describe_convolve",
+    "fdas_volume_create", "fdas_volume_destroy", "fdas_volume_info", "fdas_volume_w_of_index", "fdas_volume_slab",
+    "fdas_volume_set_algorithm", "fdas_volume_build_templates", "fdas_volume_convolve", "fdas_volume_peaks",
+    "fdas_volume_search", "fdas_volume_search_host", "fdas_volume_launch_count", "fdas_volume_last_cuda_error",
 ]
 
 
@@ -46,6 +49,15 @@ class fdas_info_t(ctypes.Structure):
         ("plane_elem_bytes", ctypes.c_size_t), ("spectrum_elem_bytes", ctypes.c_size_t),
         ("bank_bytes", ctypes.c_size_t),
     ]
+
+
+class fdas_peak3_t(ctypes.Structure):
+    _fields_ = [("w_index", ctypes.c_int32), ("z_index", ctypes.c_int32), ("r", ctypes.c_int32), ("power", ctypes.c_float)]
+
+
+class fdas_volume_info_t(ctypes.Structure):
+    _fields_ = [("n_slabs", ctypes.c_int32), ("n_templates", ctypes.c_int32), ("n_bins", ctypes.c_int64),
+                ("precision", ctypes.c_int32), ("elem_bytes", ctypes.c_size_t), ("wmax", ctypes.c_double), ("dw", ctypes.c_double)]
 
 
 class fdas_kernel_info_t(ctypes.Structure):
@@ -82,6 +94,19 @@ def lib() -> ctypes.CDLL:
     L.fdas_peaks.argtypes = [vp, vp, ctypes.c_float, vp, i, vp, vp]
     L.fdas_search.argtypes = [vp, vp, vp, ctypes.c_float, vp, i, vp, vp]
     L.fdas_search_batched.argtypes = [vp, vp, vp, i, ctypes.c_float, vp, i, vp, vp]
+    L.fdas_volume_create.argtypes = [ctypes.POINTER(vp), i64, dbl, dbl, dbl, dbl, i, i]
+    L.fdas_volume_destroy.argtypes = [vp]
+    L.fdas_volume_info.argtypes = [vp, ctypes.POINTER(fdas_volume_info_t)]
+    L.fdas_volume_w_of_index.argtypes = [vp, i, ctypes.POINTER(dbl)]
+    L.fdas_volume_slab.argtypes = [vp, i, ctypes.POINTER(vp)]
+    L.fdas_volume_set_algorithm.argtypes = [vp, i]
+    L.fdas_volume_build_templates.argtypes = [vp, vp]
+    L.fdas_volume_convolve.argtypes = [vp, vp, vp, vp]
+    L.fdas_volume_peaks.argtypes = [vp, vp, ctypes.c_float, vp, i, vp, vp]
+    L.fdas_volume_search.argtypes = [vp, vp, vp, ctypes.c_float, vp, i, vp, vp]
+    L.fdas_volume_search_host.argtypes = [vp, vp, ctypes.c_float, vp, i, ctypes.POINTER(i), vp]
+    L.fdas_volume_launch_count.argtypes = [vp, ctypes.POINTER(i64)]
+    L.fdas_volume_last_cuda_error.argtypes = [vp]
     L.fdas_describe_convolve.argtypes = [vp, vp, i, ctypes.POINTER(fdas_kernel_info_t)]
     L.fdas_convolve_host.argtypes = [vp, vp, vp, vp]
     L.fdas_search_host.argtypes = [vp, vp, ctypes.c_float, vp, i, ctypes.POINTER(i), vp]
@@ -264,6 +289,74 @@ def fdas_status_string(status):
 
 def fdas_last_cuda_error(h):
     return lib().fdas_last_cuda_error(h)
+
+
+# ---- f-fdot-fddot volume (jerk search) ----------------------------------------------------
+def fdas_volume_create(N, zmax, dz, wmax, dw, seglen, precision):
+    h = ctypes.c_void_p()
+    rc = lib().fdas_volume_create(ctypes.byref(h), int(N), float(zmax), float(dz), float(wmax), float(dw), int(seglen), int(precision))
+    return rc, h
+
+
+def fdas_volume_destroy(v):
+    return lib().fdas_volume_destroy(v)
+
+
+def fdas_volume_info(v):
+    info = fdas_volume_info_t()
+    rc = lib().fdas_volume_info(v, ctypes.byref(info))
+    return rc, info
+
+
+def fdas_volume_w_of_index(v, i):
+    w = ctypes.c_double()
+    rc = lib().fdas_volume_w_of_index(v, int(i), ctypes.byref(w))
+    return rc, w.value
+
+
+def fdas_volume_slab(v, i):
+    h = ctypes.c_void_p()
+    rc = lib().fdas_volume_slab(v, int(i), ctypes.byref(h))
+    return rc, h
+
+
+def fdas_volume_set_algorithm(v, algorithm):
+    return lib().fdas_volume_set_algorithm(v, int(algorithm))
+
+
+def fdas_volume_build_templates(v, stream=0):
+    return lib().fdas_volume_build_templates(v, ctypes.c_void_p(stream))
+
+
+def fdas_volume_convolve(v, spectrum_ptr, volume_ptr, stream=0):
+    return lib().fdas_volume_convolve(v, ctypes.c_void_p(spectrum_ptr), ctypes.c_void_p(volume_ptr), ctypes.c_void_p(stream))
+
+
+def fdas_volume_peaks(v, volume_ptr, threshold, peaks_ptr, capacity, count_ptr, stream=0):
+    return lib().fdas_volume_peaks(v, ctypes.c_void_p(volume_ptr), float(threshold), ctypes.c_void_p(peaks_ptr), int(capacity),
+                                   ctypes.c_void_p(count_ptr), ctypes.c_void_p(stream))
+
+
+def fdas_volume_search(v, spectrum_ptr, volume_ptr, threshold, peaks_ptr, capacity, count_ptr, stream=0):
+    return lib().fdas_volume_search(v, ctypes.c_void_p(spectrum_ptr), ctypes.c_void_p(volume_ptr), float(threshold),
+                                    ctypes.c_void_p(peaks_ptr), int(capacity), ctypes.c_void_p(count_ptr), ctypes.c_void_p(stream))
+
+
+def fdas_volume_search_host(v, spectrum_host_ptr, threshold, peaks_host_ptr, capacity, stream=0):
+    n = ctypes.c_int(0)
+    rc = lib().fdas_volume_search_host(v, ctypes.c_void_p(spectrum_host_ptr), float(threshold), ctypes.c_void_p(peaks_host_ptr),
+                                       int(capacity), ctypes.byref(n), ctypes.c_void_p(stream))
+    return rc, n.value
+
+
+def fdas_volume_launch_count(v):
+    n = ctypes.c_int64()
+    rc = lib().fdas_volume_launch_count(v, ctypes.byref(n))
+    return rc, n.value
+
+
+def fdas_volume_last_cuda_error(v):
+    return lib().fdas_volume_last_cuda_error(v)
 
 
 # ---- convenience wrapper ------------------------------------------------------------------
@@ -537,6 +630,105 @@ class Plan:
         if getattr(self, "_h", None):
             fdas_plan_destroy(self._h)
             self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class Volume:
+    """Owns one fdas_volume_t (the f-fdot-fddot volume of a jerk search): slabs w_i = -wmax + i dw."""
+
+    def __init__(self, N: int, zmax: float, dz: float, wmax: float, dw: float, seglen: int, precision="f32",
+                 algorithm="auto", stream: Optional[int] = None):
+        prec = PRECISIONS[precision] if isinstance(precision, str) else int(precision)
+        rc, self._v = fdas_volume_create(N, zmax, dz, wmax, dw, seglen, prec)
+        if rc:
+            self._v = None
+            raise FdasError(rc, "fdas_volume_create")
+        self.precision = prec
+        rc, self.info = fdas_volume_info(self._v)
+        self._check(rc, "fdas_volume_info")
+        algo = ALGORITHMS[algorithm] if isinstance(algorithm, str) else int(algorithm)
+        if algo != FDAS_ALGO_AUTO:
+            self._check(fdas_volume_set_algorithm(self._v, algo), "fdas_volume_set_algorithm")
+        self._check(fdas_volume_build_templates(self._v, _current_stream(stream)), "fdas_volume_build_templates")
+
+    def _check(self, rc, where):
+        if rc:
+            raise FdasError(rc, where, fdas_volume_last_cuda_error(self._v))
+
+    @property
+    def W(self): return int(self.info.n_slabs)
+    @property
+    def K(self): return int(self.info.n_templates)
+    @property
+    def M(self): return int(self.info.n_bins)
+
+    def w_values(self):
+        return [fdas_volume_w_of_index(self._v, i)[1] for i in range(self.W)]
+
+    def dtype(self):
+        import torch
+        return torch.float64 if self.precision == FDAS_F64 else torch.float32
+
+    def convolve(self, spectrum, volume=None, stream: Optional[int] = None):
+        import torch
+        assert spectrum.is_cuda and spectrum.is_contiguous() and tuple(spectrum.shape) == (self.M,)
+        if volume is None:
+            volume = torch.empty((self.W, self.K, self.M), dtype=self.dtype(), device=spectrum.device)
+        assert volume.is_cuda and volume.is_contiguous() and tuple(volume.shape) == (self.W, self.K, self.M) and volume.dtype == self.dtype()
+        self._check(fdas_volume_convolve(self._v, spectrum.data_ptr(), volume.data_ptr(), _current_stream(stream)), "fdas_volume_convolve")
+        return volume
+
+    @staticmethod
+    def _records(buf, n, capacity):
+        import numpy as np
+        w = min(n, capacity)
+        raw = buf[: 4 * w].cpu().numpy().reshape(w, 4)
+        rec = np.zeros(w, dtype=[("w_index", np.int32), ("z_index", np.int32), ("r", np.int32), ("power", np.float32)])
+        rec["w_index"], rec["z_index"], rec["r"] = raw[:, 0], raw[:, 1], raw[:, 2]
+        rec["power"] = raw[:, 3].copy().view(np.float32)
+        return rec
+
+    def peaks(self, volume, threshold: float, capacity: int = 1 << 16, stream: Optional[int] = None):
+        """fdas_volume_peaks: returns (total_count, records (w_index, z_index, r, power))."""
+        import torch
+        assert volume.is_cuda and volume.is_contiguous() and tuple(volume.shape) == (self.W, self.K, self.M)
+        buf = torch.empty(max(capacity, 1) * 4, dtype=torch.int32, device=volume.device)
+        cnt = torch.zeros(1, dtype=torch.int32, device=volume.device)
+        self._check(fdas_volume_peaks(self._v, volume.data_ptr(), threshold, buf.data_ptr() if capacity else 0, capacity,
+                                      cnt.data_ptr(), _current_stream(stream)), "fdas_volume_peaks")
+        n = int(cnt.item())
+        return n, self._records(buf, n, capacity)
+
+    def search(self, spectrum, threshold: float, volume=None, capacity: int = 1 << 16, stream: Optional[int] = None):
+        """fdas_volume_search: returns (volume, total_count, records)."""
+        import torch
+        assert spectrum.is_cuda and spectrum.is_contiguous() and tuple(spectrum.shape) == (self.M,)
+        if volume is None:
+            volume = torch.empty((self.W, self.K, self.M), dtype=self.dtype(), device=spectrum.device)
+        buf = torch.empty(max(capacity, 1) * 4, dtype=torch.int32, device=spectrum.device)
+        cnt = torch.zeros(1, dtype=torch.int32, device=spectrum.device)
+        self._check(fdas_volume_search(self._v, spectrum.data_ptr(), volume.data_ptr(), threshold, buf.data_ptr() if capacity else 0,
+                                       capacity, cnt.data_ptr(), _current_stream(stream)), "fdas_volume_search")
+        n = int(cnt.item())
+        return volume, n, self._records(buf, n, capacity)
+
+    def search_host(self, spectrum_host, threshold: float, peaks_host, capacity: int, stream: Optional[int] = None):
+        rc, n = fdas_volume_search_host(self._v, _host_ptr(spectrum_host), threshold, _host_ptr(peaks_host), capacity, _current_stream(stream))
+        self._check(rc, "fdas_volume_search_host")
+        return n
+
+    def launch_count(self) -> int:
+        return fdas_volume_launch_count(self._v)[1]
+
+    def close(self):
+        if getattr(self, "_v", None):
+            fdas_volume_destroy(self._v)
+            self._v = None
 
     def __del__(self):
         try:

@@ -54,20 +54,7 @@ def test_jerk_slab_all_precisions_and_forms(F, jerk):
     assert float((np.abs(Pbf.cpu().numpy() - exp) / exp).mean()) <= 0.02
 
 
-def test_volume_search_finds_the_jerk_of_the_signal(F):
-    # a small f-fdot-fddot volume: five slabs w = -72..72; the injected (z = 4, w = 36) tone is brightest in ITS slab
-    import torch
-    w = workloads.jerk_tone(1 << 17, seed=5, r0=20000.0, z=4.0, w=36.0, power=60.0, zmax=12.0, dz=2.0, seglen=1024)
-    x = torch.from_numpy(w.spectrum).cuda()
-    best = {}
-    for jerk in (-72.0, -36.0, 0.0, 36.0, 72.0):
-        plan = F.Plan(w.N, w.zmax, w.dz, w.seglen, "bf16", jerk=jerk)
-        P, n, rec = plan.search(x, THRESH)
-        k, r, v = max(rec.tolist(), key=lambda t: t[2]) if n else (-1, -1, 0.0)
-        best[jerk] = (int(k), int(r), float(v))
-    assert max(best, key=lambda j: best[j][2]) == 36.0
-    assert best[36.0][:2] == (8, 20000)                      # z = -12 + 2 k = 4
-    assert best[36.0][2] > 1.3 * best[0.0][2]                # plain FDAS (w = 0) loses part of the power
+# (the volume as a whole -- all slabs and the 26-neighbour peak rule in one library call -- is tested in test_gpu_volume.py)
 
 
 def test_jerk_plan_errors(F):
