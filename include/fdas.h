@@ -370,6 +370,19 @@ int fdas_search_host_batched(fdas_plan_t *p, const void *spectra_host, int n_ser
                              fdas_peak_t *peaks_host, int capacity, int *counts_host, void *stream);
 
 /*
+ * fdas_search_host_timeseries / _batched -- the end-to-end flow of the paper's Fig. 1 from the TIME SERIES
+ * (PAPER.md:63-67, :85): the N fp32 samples are copied host->device (the same bytes as the spectrum they replace),
+ * fdas_spectrum takes the real FFT on the device, fdas_search follows.  timeseries_host: [N] floats
+ * ([n_series][N] for the batched form, whose copy of series i+1 overlaps the FFT and search of series i).
+ * Every other argument, the result and the errors are those of fdas_search_host / fdas_search_host_batched, plus
+ * fdas_spectrum's UNSUPPORTED (N not a power of two in 2^10 .. 2^23).
+ */
+int fdas_search_host_timeseries(fdas_plan_t *p, const void *timeseries_host, float threshold,
+                                fdas_peak_t *peaks_host, int capacity, int *count_host, void *stream);
+int fdas_search_host_timeseries_batched(fdas_plan_t *p, const void *timeseries_host, int n_series, float threshold,
+                                        fdas_peak_t *peaks_host, int capacity, int *counts_host, void *stream);
+
+/*
  * Debug / test access to the bank: copies H_z[f] in NATURAL order, [K][S] interleaved
  * complex of the storage type (double2 / float2 / 2 x bf16 bit patterns), to host memory.
  * `bytes` must equal K*S*2*sizeof(storage scalar).  Synchronises.

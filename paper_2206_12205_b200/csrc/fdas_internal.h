@@ -66,14 +66,14 @@ struct fdas_plan {
     void *tf_maps;                 // host: tensor maps of tf_scratch
     unsigned tf_calls;
     // host-buffer entry points: lazily allocated device staging
-    void *stage_spectrum, *stage_plane;
+    void *stage_spectrum, *stage_plane, *stage_series;
     fdas_peak_t *stage_peaks;
     int *stage_count;
     int stage_peaks_capacity;
     // fdas_search_host_batched: copy stream, events and double-buffered staging of the host pipeline
     cudaStream_t pipe_stream;
     cudaEvent_t pipe_ev[3][2];     // [h2d done | search done | d2h done][buffer]
-    void *pipe_spec[2];
+    void *pipe_spec[2], *pipe_series[2];
     fdas_peak_t *pipe_peaks[2];
     int *pipe_count[2];
     int pipe_capacity, pipe_ready;

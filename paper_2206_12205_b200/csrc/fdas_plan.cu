@@ -24,6 +24,7 @@ static void free_device_members(fdas_plan *p)
     }
     for (int b = 0; b < 2; ++b) {
         cudaFree(p->pipe_spec[b]);
+        cudaFree(p->pipe_series[b]);
         cudaFree(p->pipe_peaks[b]);
         cudaFree(p->pipe_count[b]);
     }
@@ -40,6 +41,7 @@ static void free_device_members(fdas_plan *p)
     cudaFree(p->tf_scratch);
     free(p->tf_maps);
     cudaFree(p->stage_spectrum);
+    cudaFree(p->stage_series);
     cudaFree(p->stage_plane);
     cudaFree(p->stage_peaks);
     cudaFree(p->stage_count);
@@ -393,10 +395,12 @@ extern "C" int fdas_convolve_host(fdas_plan_t *p, const void *spectrum_host, voi
     return FDAS_OK;
 }
 
-extern "C" int fdas_search_host(fdas_plan_t *p, const void *spectrum_host, float threshold,
-                                fdas_peak_t *peaks_host, int capacity, int *count_host, void *stream)
+// host input of the *_host search entry points: the complex spectrum, or (timeseries) the N fp32 samples, which
+// fdas_spectrum turns into the spectrum on the device (the accelerated flow of the paper's Fig. 1 starts at the series)
+static int search_host_common(fdas_plan_t *p, const void *input_host, bool timeseries, float threshold,
+                              fdas_peak_t *peaks_host, int capacity, int *count_host, void *stream)
 {
-    if (!p || !spectrum_host || !count_host || capacity < 0 || (capacity > 0 && !peaks_host))
+    if (!p || !input_host || !count_host || capacity < 0 || (capacity > 0 && !peaks_host))
         return FDAS_ERR_INVALID_ARG;
     if (!p->built) return FDAS_ERR_NOT_BUILT;
     cudaStream_t st = (cudaStream_t)stream;
@@ -404,7 +408,15 @@ extern "C" int fdas_search_host(fdas_plan_t *p, const void *spectrum_host, float
     int rc = ensure_staging(p, !plane_free, capacity);
     if (rc) return rc;
     const size_t spec_bytes = (size_t)p->M * (p->precision == FDAS_F64 ? 16 : 8);
-    FDAS_CUDA_TRY(p, cudaMemcpyAsync(p->stage_spectrum, spectrum_host, spec_bytes, cudaMemcpyHostToDevice, st));
+    if (timeseries) {
+        const size_t ts_bytes = (size_t)p->N * sizeof(float);
+        if (!p->stage_series) FDAS_CUDA_TRY(p, cudaMalloc(&p->stage_series, ts_bytes));
+        FDAS_CUDA_TRY(p, cudaMemcpyAsync(p->stage_series, input_host, ts_bytes, cudaMemcpyHostToDevice, st));
+        rc = fdas_launch_spectrum(p, p->stage_series, p->stage_spectrum, st);
+        if (rc) return rc;
+    } else {
+        FDAS_CUDA_TRY(p, cudaMemcpyAsync(p->stage_spectrum, input_host, spec_bytes, cudaMemcpyHostToDevice, st));
+    }
     rc = search_on_device(p, p->stage_spectrum, plane_free ? NULL : p->stage_plane, threshold, p->stage_peaks, capacity,
                           p->stage_count, st);
     if (rc) return rc;
@@ -419,11 +431,23 @@ extern "C" int fdas_search_host(fdas_plan_t *p, const void *spectrum_host, float
     return FDAS_OK;
 }
 
+extern "C" int fdas_search_host(fdas_plan_t *p, const void *spectrum_host, float threshold,
+                                fdas_peak_t *peaks_host, int capacity, int *count_host, void *stream)
+{
+    return search_host_common(p, spectrum_host, false, threshold, peaks_host, capacity, count_host, stream);
+}
+
+extern "C" int fdas_search_host_timeseries(fdas_plan_t *p, const void *timeseries_host, float threshold,
+                                           fdas_peak_t *peaks_host, int capacity, int *count_host, void *stream)
+{
+    return search_host_common(p, timeseries_host, true, threshold, peaks_host, capacity, count_host, stream);
+}
+
 // Survey form of the host path: series i+1 crosses PCIe while series i is searched.
 //   copy stream:    [wait search(i-1)] H2D spectrum(i+1)            [wait search(i)] D2H count(i), peaks(i)
 //   caller stream:  [wait H2D(i)] [wait D2H(i-2)] fdas_search(i)
-extern "C" int fdas_search_host_batched(fdas_plan_t *p, const void *spectra_host, int n_series, float threshold,
-                                        fdas_peak_t *peaks_host, int capacity, int *counts_host, void *stream)
+static int search_host_pipeline(fdas_plan_t *p, const void *spectra_host, bool timeseries, int n_series, float threshold,
+                                fdas_peak_t *peaks_host, int capacity, int *counts_host, void *stream)
 {
     if (!p || !spectra_host || !counts_host || n_series < 1 || capacity < 0 || (capacity > 0 && !peaks_host))
         return FDAS_ERR_INVALID_ARG;
@@ -433,6 +457,11 @@ extern "C" int fdas_search_host_batched(fdas_plan_t *p, const void *spectra_host
     int rc = ensure_staging(p, !plane_free, 0);
     if (rc) return rc;
     const size_t spec_bytes = (size_t)p->M * (p->precision == FDAS_F64 ? 16 : 8);
+    const size_t in_bytes = timeseries ? (size_t)p->N * sizeof(float) : spec_bytes;   // what crosses the host link per series
+    if (timeseries) {
+        rc = ensure_staging(p, false, 0);   // stage_spectrum: fdas_spectrum's output, consumed by the search that follows it
+        if (rc) return rc;
+    }
     if (!p->pipe_ready) {
         FDAS_CUDA_TRY(p, cudaStreamCreateWithFlags(&p->pipe_stream, cudaStreamNonBlocking));
         for (int e = 0; e < 3; ++e)
@@ -440,7 +469,8 @@ extern "C" int fdas_search_host_batched(fdas_plan_t *p, const void *spectra_host
         p->pipe_ready = 1;
     }
     for (int b = 0; b < 2; ++b) {
-        if (!p->pipe_spec[b]) FDAS_CUDA_TRY(p, cudaMalloc(&p->pipe_spec[b], spec_bytes));
+        if (!timeseries && !p->pipe_spec[b]) FDAS_CUDA_TRY(p, cudaMalloc(&p->pipe_spec[b], spec_bytes));
+        if (timeseries && !p->pipe_series[b]) FDAS_CUDA_TRY(p, cudaMalloc(&p->pipe_series[b], in_bytes));
         if (!p->pipe_count[b]) FDAS_CUDA_TRY(p, cudaMalloc((void **)&p->pipe_count[b], sizeof(int)));
         if (capacity > p->pipe_capacity || !p->pipe_peaks[b]) {
             cudaFree(p->pipe_peaks[b]);
@@ -451,23 +481,30 @@ extern "C" int fdas_search_host_batched(fdas_plan_t *p, const void *spectra_host
     p->pipe_capacity = capacity;
     cudaStream_t cs = p->pipe_stream;
     const unsigned char *src = static_cast<const unsigned char *>(spectra_host);
+    void *const *in_buf = timeseries ? p->pipe_series : p->pipe_spec;
     // the pipeline starts after whatever the caller queued on `stream` before this call
     FDAS_CUDA_TRY(p, cudaEventRecord(p->pipe_ev[1][1], st));
     FDAS_CUDA_TRY(p, cudaStreamWaitEvent(cs, p->pipe_ev[1][1], 0));
-    FDAS_CUDA_TRY(p, cudaMemcpyAsync(p->pipe_spec[0], src, spec_bytes, cudaMemcpyHostToDevice, cs));
+    FDAS_CUDA_TRY(p, cudaMemcpyAsync(in_buf[0], src, in_bytes, cudaMemcpyHostToDevice, cs));
     FDAS_CUDA_TRY(p, cudaEventRecord(p->pipe_ev[0][0], cs));
     for (int i = 0; i < n_series; ++i) {
         const int b = i & 1;
         FDAS_CUDA_TRY(p, cudaStreamWaitEvent(st, p->pipe_ev[0][b], 0));              // spectrum i is on the device
         if (i >= 2) FDAS_CUDA_TRY(p, cudaStreamWaitEvent(st, p->pipe_ev[2][b], 0));  // peak buffers b were read back
-        rc = search_on_device(p, p->pipe_spec[b], plane_free ? NULL : p->stage_plane, threshold, p->pipe_peaks[b], capacity,
+        const void *spec = in_buf[b];
+        if (timeseries) {   // the real FFT of PAPER.md:85 on the device, into the one spectrum buffer (stream order protects it)
+            rc = fdas_launch_spectrum(p, in_buf[b], p->stage_spectrum, st);
+            if (rc) return rc;
+            spec = p->stage_spectrum;
+        }
+        rc = search_on_device(p, spec, plane_free ? NULL : p->stage_plane, threshold, p->pipe_peaks[b], capacity,
                               p->pipe_count[b], st);
         if (rc) return rc;
         FDAS_CUDA_TRY(p, cudaEventRecord(p->pipe_ev[1][b], st));
         if (i + 1 < n_series) {
             // spectrum buffer b^1 was last read by search(i-1), already recorded in pipe_ev[1][b^1]
             if (i >= 1) FDAS_CUDA_TRY(p, cudaStreamWaitEvent(cs, p->pipe_ev[1][b ^ 1], 0));
-            FDAS_CUDA_TRY(p, cudaMemcpyAsync(p->pipe_spec[b ^ 1], src + (size_t)(i + 1) * spec_bytes, spec_bytes,
+            FDAS_CUDA_TRY(p, cudaMemcpyAsync(in_buf[b ^ 1], src + (size_t)(i + 1) * in_bytes, in_bytes,
                                              cudaMemcpyHostToDevice, cs));
             FDAS_CUDA_TRY(p, cudaEventRecord(p->pipe_ev[0][b ^ 1], cs));
         }
@@ -481,6 +518,18 @@ extern "C" int fdas_search_host_batched(fdas_plan_t *p, const void *spectra_host
     FDAS_CUDA_TRY(p, cudaStreamSynchronize(cs));
     FDAS_CUDA_TRY(p, cudaStreamSynchronize(st));
     return FDAS_OK;
+}
+
+extern "C" int fdas_search_host_batched(fdas_plan_t *p, const void *spectra_host, int n_series, float threshold,
+                                        fdas_peak_t *peaks_host, int capacity, int *counts_host, void *stream)
+{
+    return search_host_pipeline(p, spectra_host, false, n_series, threshold, peaks_host, capacity, counts_host, stream);
+}
+
+extern "C" int fdas_search_host_timeseries_batched(fdas_plan_t *p, const void *timeseries_host, int n_series, float threshold,
+                                                   fdas_peak_t *peaks_host, int capacity, int *counts_host, void *stream)
+{
+    return search_host_pipeline(p, timeseries_host, true, n_series, threshold, peaks_host, capacity, counts_host, stream);
 }
 
 extern "C" int fdas_templates_host(const fdas_plan_t *p, void *dst_host, size_t bytes)

@@ -11,11 +11,13 @@
 //   pass B  L1/2 CTAs: 2 rows k1, FFT of length L2 over m2, Z[k1 + L1 k2]  (16-byte segments out)
 //   pass C  X[k] = E + exp(-2 pi i k / N) O,  E = (Z[k] + conj Z[L-k]) / 2,  O = -i (Z[k] - conj Z[L-k]) / 2
 //
-// Three streaming passes over 8 L bytes: HBM-bound, and small beside one fdas_convolve.  The
-// shared-memory FFT is a decimation-in-frequency with two radix-2 stages fused per barrier (natural
-// in, bit-reversed out; the store un-reverses), twiddles from sincospif with exactly representable
-// arguments.
+// N >= 2^17 (both factors >= 256): passes A and B run the transforms in REGISTERS -- 16 points per thread, three
+// butterfly passes of radix 16 / 16 / n/256 (the butterflies of fdas_fft.cuh), two shared-memory exchanges, output in
+// natural order (fdas_rfft_fast_kernel below); the 8 L-byte intermediates stay in the 126 MB L2.  Smaller N keep the
+// shared-memory decimation-in-frequency kernels (two radix-2 stages fused per barrier; natural in, bit-reversed
+// out; the store un-reverses).  Twiddles come from sincospif with exactly representable arguments.
 #include <math.h>
+#include "fdas_fft.cuh"
 #include "fdas_internal.h"
 
 namespace {
@@ -91,6 +93,7 @@ __device__ __forceinline__ unsigned bitrev(unsigned v, int bits) { return bits ?
 constexpr int RF_CB = 8;      // columns per CTA in pass A (64-byte segments; 64 KB of shared memory -> 3 CTAs per SM)
 constexpr int RF_RB = 2;      // rows per CTA in pass B
 constexpr int RF_L2MAX = 12;  // log2 of the longest row FFT
+constexpr int RF_NSEQ = 4;    // register FFT passes: adjacent columns / rows per CTA (32-byte segments; 8 needs 1024 threads at n = 2048)
 
 // pass A: z viewed as [L1][L2]; this CTA takes columns m2 = 16 blockIdx.x .. +15
 __global__ void __launch_bounds__(512) fdas_rfft_cols_kernel(const float2 *__restrict__ z, float2 *__restrict__ Y, int l1, int l2)
@@ -133,6 +136,147 @@ __global__ void __launch_bounds__(512) fdas_rfft_rows_kernel(const float2 *__res
     }
 }
 
+
+// ---- register FFT passes (N >= 2^17) ---------------------------------------------------------------
+// One length-n transform, n = 256 R3 (R3 = 1, 2, 4, 8, 16), by T = n / 16 threads holding 16 points each:
+//   pass 1  thread t, slot a <-> input index t + T a: 16-point DFT over a -> k1; twiddle W_n^{t k1}
+//   pass 2  thread (k1, t2), slot b <-> t = t2 + (T/16) b: 16-point DFT over b -> k2; twiddle W_T^{t2 k2}
+//   pass 3  thread (k1, k2): R3-point DFTs over the remaining index (16 / R3 of them) -> k3
+// output index k1 + 16 k2 + 256 k3: natural order, consecutive threads hold consecutive outputs.
+// The butterflies are inverse-sign (exp(+2 pi i ..)); the forward transform is taken on data with re and im
+// swapped and swapped back at the end (fdas_fft.cuh).  Sequences are interleaved by NSEQ in shared memory and in
+// the thread index (sequence fastest) so that pass A reads / writes NSEQ adjacent columns (64-byte segments).
+template <int R3>
+struct FastGeo {
+    static constexpr int N = 256 * R3, T = N / 16, U = 16 / R3;   // U radix-R3 butterflies per thread in pass 3
+    static constexpr int STR1 = T + 1;                            // exchange 1: row k1 holds y_k1[t], padded
+    static constexpr int STR2 = R3 + 2;                           // exchange 2: row (k2, k1) holds the R3 values t2, padded
+    static constexpr int NEED = 16 * STR1 > 256 * STR2 ? 16 * STR1 : 256 * STR2;
+    // elements per sequence, = 4 (mod 16): the sequences of a warp (8 of them x 4 consecutive t) then fall into
+    // different 8-byte slots of a 128-byte wavefront
+    static constexpr int SE = (NEED + 11) / 16 * 16 + 4;
+};
+
+// One transform per `seq`; re[], im[] hold the 16 inputs t + T a of thread t on entry and the outputs on exit:
+// output index (t + T u) + 256 k3 sits in slot u R3 + DftSlot<R3>::of(k3).  tw[j] = exp(+2 pi i j / n), j < n.
+template <int R3>
+__device__ __forceinline__ void fast_fft(float *re, float *im, float2 *sx, const float2 *tw, int t, int seq)
+{
+    using G = FastGeo<R3>;
+    using namespace fdas;
+    constexpr int T = G::T, N = G::N;
+    float2 *s1 = sx + (size_t)seq * G::SE;
+    // pass 1: DFT16 over a; y_k1[t] = W_n^{t k1} sum_a x[t + T a] W_16^{a k1}
+    Dft<float, 16>::run(re, im);
+#pragma unroll
+    for (int k1 = 0; k1 < 16; ++k1) {
+        const int sl = DftSlot<16>::of(k1);
+        float xr = re[sl], xi = im[sl];
+        if (k1) {
+            const float2 w = tw[(t * k1) & (N - 1)];
+            fdas::cmul(xr, xi, w.x, w.y);
+        }
+        s1[k1 * G::STR1 + t] = make_float2(xr, xi);
+    }
+    __syncthreads();
+    // pass 2: thread (k1, t2), t2 < R3: DFT16 over b of y_k1[t2 + R3 b]; twiddle W_T^{t2 k2} = W_n^{16 t2 k2}
+    const int k1 = t / R3, t2 = t % R3;
+#pragma unroll
+    for (int b = 0; b < 16; ++b) {
+        const float2 v = s1[k1 * G::STR1 + t2 + R3 * b];
+        re[b] = v.x;
+        im[b] = v.y;
+    }
+    __syncthreads();
+    Dft<float, 16>::run(re, im);
+#pragma unroll
+    for (int k2 = 0; k2 < 16; ++k2) {
+        const int sl = DftSlot<16>::of(k2);
+        float xr = re[sl], xi = im[sl];
+        if (k2 && R3 > 1) {
+            const float2 w = tw[(t2 * k2 * 16) & (N - 1)];
+            fdas::cmul(xr, xi, w.x, w.y);
+        }
+        s1[(k2 * 16 + k1) * G::STR2 + t2] = make_float2(xr, xi);
+    }
+    __syncthreads();
+    // pass 3: rows q = t + T u (q = k1 + 16 k2), R3-point DFT over t2 -> k3
+#pragma unroll
+    for (int u = 0; u < G::U; ++u) {
+        const int row = t + T * u;
+        const int rk1 = row & 15, rk2 = row >> 4;
+#pragma unroll
+        for (int j = 0; j < R3; ++j) {
+            const float2 v = s1[(rk2 * 16 + rk1) * G::STR2 + j];
+            re[u * R3 + j] = v.x;
+            im[u * R3 + j] = v.y;
+        }
+        Dft<float, R3>::run(re + u * R3, im + u * R3);
+    }
+}
+
+// Pass A (COLS = true): z viewed as [L1][L2]; CTA = NSEQ adjacent columns m2, transform over m1 (stride L2), output
+// Y[k L2 + m2] = W_L^{m2 k} FFT_m1(z)[k].  Pass B (COLS = false): CTA = NSEQ rows k1 of Y [L1][L2] (contiguous),
+// transform over m2, output Z[k1 + L1 k2].
+template <int R3, bool COLS, int NSEQ>
+__global__ void __launch_bounds__(FastGeo<R3>::T * NSEQ)
+fdas_rfft_fast_kernel(const float2 *__restrict__ in, float2 *__restrict__ out, int l1, int l2)
+{
+    using G = FastGeo<R3>;
+    using namespace fdas;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2 *tw = reinterpret_cast<float2 *>(smem_raw);
+    float2 *sx = tw + G::N;
+    const int L2 = 1 << l2, L1 = 1 << l1;
+    const int seq = threadIdx.x % NSEQ, t = threadIdx.x / NSEQ;
+    for (int j = threadIdx.x; j < G::N; j += blockDim.x) {
+        float sn, cs;
+        sincospif(2.0f * (float)j / (float)G::N, &sn, &cs);
+        tw[j] = make_float2(cs, sn);
+    }
+    float re[16], im[16];
+    if (COLS) {
+        const int m2 = blockIdx.x * NSEQ + seq;
+#pragma unroll
+        for (int a = 0; a < 16; ++a) {
+            const float2 v = __ldg(in + (size_t)(t + G::T * a) * L2 + m2);
+            re[a] = v.y;   // swapped: forward transform through the inverse-sign butterflies
+            im[a] = v.x;
+        }
+    } else {
+        const int k1 = blockIdx.x * NSEQ + seq;
+#pragma unroll
+        for (int a = 0; a < 16; ++a) {
+            const float2 v = __ldg(in + (size_t)k1 * L2 + t + G::T * a);
+            re[a] = v.y;
+            im[a] = v.x;
+        }
+    }
+    __syncthreads();   // twiddle table
+    fast_fft<R3>(re, im, sx, tw, t, seq);
+    constexpr int U = G::U;
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+#pragma unroll
+        for (int k3 = 0; k3 < R3; ++k3) {
+            const int sl = u * R3 + DftSlot<R3>::of(k3);
+            const int k = t + G::T * u + 256 * k3;
+            float xr = im[sl], xi = re[sl];            // swap back: forward transform
+            if (COLS) {
+                const int m2 = blockIdx.x * NSEQ + seq;
+                float sn, cs;
+                // four-step twiddle W_L^{m2 k} = exp(-2 pi i m2 k / L): m2 k < 2^24, 2 m2 k / L exact in fp32
+                sincospif(-2.0f * (float)((unsigned)m2 * (unsigned)k) / (float)(1u << (l1 + l2)), &sn, &cs);
+                fdas::cmul(xr, xi, cs, sn);
+                out[(size_t)k * L2 + m2] = make_float2(xr, xi);
+            } else {
+                const int k1 = blockIdx.x * NSEQ + seq;
+                out[(size_t)k * L1 + k1] = make_float2(xr, xi);
+            }
+        }
+    }
+}
+
 // pass C: real-input unpacking, scale 1/sqrt(N); thread k handles bins k and L - k
 template <typename OT2>
 __global__ void __launch_bounds__(256) fdas_rfft_unpack_kernel(const float2 *__restrict__ Z, OT2 *__restrict__ X, unsigned L, float scale)
@@ -155,6 +299,33 @@ __global__ void __launch_bounds__(256) fdas_rfft_unpack_kernel(const float2 *__r
     }
 }
 
+template <int R3, bool COLS>
+int launch_fast_r(fdas_plan *p, int l1, int l2, const float2 *in, float2 *out, cudaStream_t st)
+{
+    using G = FastGeo<R3>;
+    constexpr int NSEQ = RF_NSEQ;
+    auto kern = fdas_rfft_fast_kernel<R3, COLS, NSEQ>;
+    const size_t smem = ((size_t)G::N + (size_t)NSEQ * G::SE) * sizeof(float2);
+    { const int rc = fdas_optin_smem(p, (COLS ? FDAS_OPTIN_RFFT_COLS : FDAS_OPTIN_RFFT_ROWS), kern, smem); if (rc) return rc; }
+    const int seqs = COLS ? (1 << l2) : (1 << l1);       // columns m2 / rows k1
+    kern<<<seqs / NSEQ, G::T * NSEQ, smem, st>>>(in, out, l1, l2);
+    FDAS_CUDA_TRY(p, cudaGetLastError());
+    p->launches += 1;
+    return FDAS_OK;
+}
+
+// transforms of length 2^ln: down the columns of [L1][L2] (cols) or along its rows
+int launch_fast(fdas_plan *p, bool cols, int ln, int l1, int l2, const float2 *in, float2 *out, cudaStream_t st)
+{
+    switch (ln - 8) {
+    case 0: return cols ? launch_fast_r<1, true>(p, l1, l2, in, out, st) : launch_fast_r<1, false>(p, l1, l2, in, out, st);
+    case 1: return cols ? launch_fast_r<2, true>(p, l1, l2, in, out, st) : launch_fast_r<2, false>(p, l1, l2, in, out, st);
+    case 2: return cols ? launch_fast_r<4, true>(p, l1, l2, in, out, st) : launch_fast_r<4, false>(p, l1, l2, in, out, st);
+    case 3: return cols ? launch_fast_r<8, true>(p, l1, l2, in, out, st) : launch_fast_r<8, false>(p, l1, l2, in, out, st);
+    default: return FDAS_ERR_UNSUPPORTED;
+    }
+}
+
 }  // namespace
 
 int fdas_launch_spectrum(fdas_plan *p, const void *timeseries, void *spectrum, cudaStream_t st)
@@ -162,25 +333,34 @@ int fdas_launch_spectrum(fdas_plan *p, const void *timeseries, void *spectrum, c
     int n = 0;
     while ((1LL << n) < p->N) ++n;
     if ((1LL << n) != p->N || n < 10 || n > 23) return FDAS_ERR_UNSUPPORTED;
-    const int l = n - 1, l2 = l < RF_L2MAX ? l : RF_L2MAX, l1 = l - l2;
+    const int l = n - 1;
     const size_t L = (size_t)1 << l;
     if (!p->rfft_scratch) FDAS_CUDA_TRY(p, cudaMalloc(&p->rfft_scratch, 2 * L * sizeof(float2)));
     float2 *Y = static_cast<float2 *>(p->rfft_scratch), *Z = Y + L;
     const float2 *z = static_cast<const float2 *>(timeseries);
-    if (l1 > 0) {
-        const size_t smem = ((size_t)(1 << l1) * RF_CB + (1 << l1) / 2) * sizeof(float2);
-        { const int rc = fdas_optin_smem(p, FDAS_OPTIN_RFFT_COLS, fdas_rfft_cols_kernel, smem); if (rc) return rc; }
-        fdas_rfft_cols_kernel<<<(1 << l2) / RF_CB, 512, smem, st>>>(z, Y, l1, l2);
-        FDAS_CUDA_TRY(p, cudaGetLastError());
-        p->launches += 1;
-    }
-    {
-        const int rb = l1 >= 2 ? RF_RB : 1;
-        const size_t smem = ((size_t)(1 << l2) * rb + (1 << l2) / 2) * sizeof(float2);
-        { const int rc = fdas_optin_smem(p, FDAS_OPTIN_RFFT_ROWS, fdas_rfft_rows_kernel, smem); if (rc) return rc; }
-        fdas_rfft_rows_kernel<<<(1 << l1) / rb, 512, smem, st>>>(l1 > 0 ? Y : z, Z, l1, l2, rb);
-        FDAS_CUDA_TRY(p, cudaGetLastError());
-        p->launches += 1;
+    if (l >= 16) {
+        // register FFT passes: L = L1 L2 with both factors in 256 .. 2048
+        const int l1 = (l + 1) / 2, l2 = l - l1;
+        int rc = launch_fast(p, true, l1, l1, l2, z, Y, st);       // pass A: transforms of length L1 down the columns
+        if (rc == FDAS_OK) rc = launch_fast(p, false, l2, l1, l2, Y, Z, st);   // pass B: transforms of length L2 along the rows
+        if (rc) return rc;
+    } else {
+        const int l2 = l < RF_L2MAX ? l : RF_L2MAX, l1 = l - l2;
+        if (l1 > 0) {
+            const size_t smem = ((size_t)(1 << l1) * RF_CB + (1 << l1) / 2) * sizeof(float2);
+            { const int rc = fdas_optin_smem(p, FDAS_OPTIN_RFFT_COLS, fdas_rfft_cols_kernel, smem); if (rc) return rc; }
+            fdas_rfft_cols_kernel<<<(1 << l2) / RF_CB, 512, smem, st>>>(z, Y, l1, l2);
+            FDAS_CUDA_TRY(p, cudaGetLastError());
+            p->launches += 1;
+        }
+        {
+            const int rb = l1 >= 2 ? RF_RB : 1;
+            const size_t smem = ((size_t)(1 << l2) * rb + (1 << l2) / 2) * sizeof(float2);
+            { const int rc = fdas_optin_smem(p, FDAS_OPTIN_RFFT_ROWS, fdas_rfft_rows_kernel, smem); if (rc) return rc; }
+            fdas_rfft_rows_kernel<<<(1 << l1) / rb, 512, smem, st>>>(l1 > 0 ? Y : z, Z, l1, l2, rb);
+            FDAS_CUDA_TRY(p, cudaGetLastError());
+            p->launches += 1;
+        }
     }
     const float scale = (float)(1.0 / sqrt((double)p->N));
     const unsigned blocks = (unsigned)((L / 2 + 256) / 256 < (size_t)p->num_sms * 8 ? (L / 2 + 256) / 256 : (size_t)p->num_sms * 8);

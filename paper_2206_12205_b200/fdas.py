@@ -29,7 +29,7 @@ EXPORTS = [
     "fdas_launch_count", "fdas_status_string", "fdas_last_cuda_error",
     "fdas_set_algorithm", "fdas_get_algorithm", "fdas_tapmatrix_host", "fdas_search",
     "fdas_set_plane_format", "fdas_get_plane_format", "fdas_quick_cast", "fdas_harmonic_sum", "fdas_harmonic_sum_drift", "fdas_band_max", "fdas_search_host_batched", "fdas_spectrum", "fdas_plan_create_jerk",
-    "fdas_search_batched", "fdas_describe_convolve",
+    "fdas_search_batched", "fdas_describe_convolve", "fdas_search_host_timeseries", "fdas_search_host_timeseries_batched",
     "fdas_volume_create", "fdas_volume_destroy", "fdas_volume_info", "fdas_volume_w_of_index", "fdas_volume_slab",
     "fdas_volume_set_algorithm", "fdas_volume_build_templates", "fdas_volume_convolve", "fdas_volume_peaks",
     "fdas_volume_search", "fdas_volume_search_host", "fdas_volume_launch_count", "fdas_volume_last_cuda_error",
@@ -124,6 +124,8 @@ def lib() -> ctypes.CDLL:
     L.fdas_band_max.argtypes = [vp, vp, dbl, i, vp, vp]
     L.fdas_spectrum.argtypes = [vp, vp, vp, vp]
     L.fdas_search_host_batched.argtypes = [vp, vp, i, ctypes.c_float, vp, i, vp, vp]
+    L.fdas_search_host_timeseries.argtypes = [vp, vp, ctypes.c_float, vp, i, ctypes.POINTER(i), vp]
+    L.fdas_search_host_timeseries_batched.argtypes = [vp, vp, i, ctypes.c_float, vp, i, vp, vp]
     L.fdas_status_string.argtypes = [i]
     L.fdas_status_string.restype = ctypes.c_char_p
     L.fdas_last_cuda_error.argtypes = [vp]
@@ -265,6 +267,18 @@ def fdas_band_max(h, plane_ptr, f_bin, n_bands, out_ptr, stream=0):
 def fdas_search_host_batched(h, spectra_host_ptr, n_series, threshold, peaks_host_ptr, capacity, counts_host_ptr, stream=0):
     return lib().fdas_search_host_batched(h, spectra_host_ptr, int(n_series), threshold, peaks_host_ptr, int(capacity),
                                           counts_host_ptr, stream)
+
+
+def fdas_search_host_timeseries(h, timeseries_host_ptr, threshold, peaks_host_ptr, capacity, stream=0):
+    n = ctypes.c_int(0)
+    rc = lib().fdas_search_host_timeseries(h, ctypes.c_void_p(timeseries_host_ptr), float(threshold),
+                                           ctypes.c_void_p(peaks_host_ptr), int(capacity), ctypes.byref(n), ctypes.c_void_p(stream))
+    return rc, n.value
+
+
+def fdas_search_host_timeseries_batched(h, timeseries_host_ptr, n_series, threshold, peaks_host_ptr, capacity, counts_host_ptr, stream=0):
+    return lib().fdas_search_host_timeseries_batched(h, timeseries_host_ptr, int(n_series), threshold, peaks_host_ptr, int(capacity),
+                                                     counts_host_ptr, stream)
 
 
 def fdas_spectrum(h, timeseries_ptr, spectrum_ptr, stream=0):
@@ -573,13 +587,22 @@ class Plan:
         return n
 
     def search_host_batched(self, spectra_host, threshold: float, peaks_host, counts_host, capacity: int,
-                            stream: Optional[int] = None):
-        """spectra_host [B, M]; peaks_host >= B*capacity records (12 bytes each); counts_host [B] int32 (numpy or pinned torch)."""
+                            stream: Optional[int] = None, timeseries: bool = False):
+        """spectra_host [B, M] (timeseries=True: the fp32 series [B, N]); peaks_host >= B*capacity records (12 bytes each);
+        counts_host [B] int32 (numpy or pinned torch)."""
         stream = _current_stream(stream)
         n = int(spectra_host.shape[0])
-        self._check(fdas_search_host_batched(self._h, _host_ptr(spectra_host), n, threshold, _host_ptr(peaks_host), capacity,
-                                             _host_ptr(counts_host), stream), "fdas_search_host_batched")
+        fn = fdas_search_host_timeseries_batched if timeseries else fdas_search_host_batched
+        self._check(fn(self._h, _host_ptr(spectra_host), n, threshold, _host_ptr(peaks_host), capacity,
+                       _host_ptr(counts_host), stream), "fdas_search_host_batched")
         return counts_host
+
+    def search_host_timeseries(self, timeseries_host, threshold: float, peaks_host, capacity: int, stream: Optional[int] = None):
+        """fdas_search_host_timeseries: fp32 series [N] on the host in, peak list out (real FFT and search on the device)."""
+        stream = _current_stream(stream)
+        rc, n = fdas_search_host_timeseries(self._h, _host_ptr(timeseries_host), threshold, _host_ptr(peaks_host), capacity, stream)
+        self._check(rc, "fdas_search_host_timeseries")
+        return n
 
     def templates(self):
         """Bank in natural order as numpy: complex128/complex64, or uint16 [K, S, 2] bit patterns for bf16."""

@@ -49,6 +49,7 @@ class Workload:
     spectrum: np.ndarray   # complex64 [M] (or [B, M] for a batch)
     injections: List[Injection]
     seed: int
+    series: Optional[np.ndarray] = None   # the fp32 time series itself, kept on request (inputs of fdas_spectrum)
 
     @property
     def M(self) -> int:
@@ -96,7 +97,7 @@ def _noise(rng: np.random.Generator, N: int) -> np.ndarray:
     return rng.standard_normal(N, dtype=np.float32)
 
 
-def config1(noise: bool = True) -> Workload:
+def config1(noise: bool = True, keep_series: bool = False) -> Workload:
     """Tiny series: N=2^16, seed 1, one tone r0=10000.25, z=+20, power 100; K=21, S=1024.
 
     ``noise=False`` gives the noise-free twin used by the closed-form pin (reading A19).
@@ -108,7 +109,7 @@ def config1(noise: bool = True) -> Workload:
         x = np.zeros(N, dtype=np.float32)
     inj = Injection(r0=10000.25, z=20.0, power=100.0, phi0=0.0)
     _add_tone(x, inj.r0, inj.z, inj.power, inj.phi0)
-    return Workload("config1", N, 20.0, 2.0, 1024, spectrum_of(x), [inj], seed)
+    return Workload("config1", N, 20.0, 2.0, 1024, spectrum_of(x), [inj], seed, series=x if keep_series else None)
 
 
 def _draw_tones(rng, n, r_lo, r_hi, z_lo, z_hi) -> List[Injection]:

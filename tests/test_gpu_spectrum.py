@@ -88,3 +88,31 @@ def test_time_series_to_peaks_through_the_library(F):
     # same series through the harness FFT (what every other test feeds): planes agree to the bf16 rule
     P2 = plan.convolve(torch.from_numpy(workloads.spectrum_of(x)).cuda())
     assert float(((P - P2).abs() / P2).mean().item()) < 0.02
+
+
+def test_search_from_the_time_series_on_the_host(F):
+    # the paper's accelerated flow starts at the time series (Fig. 1, :85): host series in, peak list out, checked
+    # against oracle.spectrum -> oracle.power_plane -> oracle.peaks on config 1
+    import oracle
+    w = workloads.config1(keep_series=True)
+    X = osp.spectrum(w.series)
+    exp = oracle.power_plane(X, w.zmax, w.dz)
+    n_exp, rec_exp = oracle.peaks(exp, THRESH)
+    for prec in ("f32", "bf16", "f64"):
+        plan = F.Plan(w.N, w.zmax, w.dz, w.seglen, prec)
+        rec = np.zeros(256, dtype=[("z_index", np.int32), ("r", np.int32), ("power", np.float32)])
+        n = plan.search_host_timeseries(w.series, THRESH, rec, 256)
+        assert (20, 10000) in {(int(a), int(b)) for a, b, _ in rec[:n].tolist()}           # the injected tone
+        if prec != "bf16":
+            assert n == n_exp and sorted((int(a), int(b)) for a, b, _ in rec[:n].tolist()) == sorted((k, r) for k, r, _ in rec_exp)
+            got = {(int(a), int(b)): float(c) for a, b, c in rec[:n].tolist()}
+            for k, r, pw in rec_exp:
+                assert abs(got[(k, r)] - pw) <= 1e-4 * exp.max() + 1e-4
+        # the pipelined batched form returns the same list for every copy of the series
+        B, cap = 3, 64
+        xs = np.stack([w.series] * B)
+        recs = np.zeros((B, cap), dtype=rec.dtype)
+        counts = np.zeros(B, dtype=np.int32)
+        plan.search_host_batched(xs, THRESH, recs, counts, cap, timeseries=True)
+        for b in range(B):
+            assert counts[b] == n and sorted(map(tuple, recs[b, :n].tolist())) == sorted(map(tuple, rec[:n].tolist()))
