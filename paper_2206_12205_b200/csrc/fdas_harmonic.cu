@@ -84,6 +84,90 @@ __global__ void __launch_bounds__(256) fdas_harmonic_sum_kernel(const IT *__rest
     }
 }
 
+// Drift-tolerant form, tiled: CTA = (row k, 1024 output bins).  For every harmonic the plane elements its windows cover
+// form ONE contiguous span of rows kh - t .. kh + t (windows of 2t + 1 >= h bins at stride h tile the row), so the
+// window maximum is separable: a coalesced pass takes the maximum over the rows of the span into shared memory, then
+// every output takes the maximum of its 2t + 1 consecutive entries.  (2t + 1) h coalesced loads per output instead of
+// (2t + 1)^2 scattered ones; maxima are exact, so the result is bit-identical to the gather form.  blockIdx.x = k
+// (fastest) keeps the rows that share plane rows -- output rows k and k + 1 overlap in 2t + 1 - h of them -- together
+// in L2.
+constexpr int HD_THREADS = 256, HD_OUT = 4, HD_TILE = HD_THREADS * HD_OUT, HD_SPAN = 4096 + 64;
+
+template <typename IT, typename OT>
+__global__ void __launch_bounds__(HD_THREADS) fdas_harmonic_drift_kernel(const IT *__restrict__ P, OT *__restrict__ S, int K, long long M,
+                                                                         int k0, int H)
+{
+    __shared__ __align__(16) OT buf[HD_SPAN];
+    const int k = blockIdx.x;
+    const long long r0 = (long long)blockIdx.y * HD_TILE;
+    const IT *row1 = P + (size_t)k * M;
+    OT acc[HD_OUT];
+#pragma unroll
+    for (int j = 0; j < HD_OUT; ++j) {
+        const long long r = r0 + threadIdx.x + HD_THREADS * j;      // thread -> bins r0 + tid + 256 j: coalesced, stride-h smem reads
+        acc[j] = r < M ? (OT)hs_elem<IT>::load(row1 + r) : (OT)0;
+    }
+    for (int h = 2; h <= H; ++h) {
+        const long long kh = (long long)k0 + (long long)h * (k - k0);
+        if (kh < 0 || kh >= K) continue;
+        if (r0 * h >= M) break;                        // this and every further harmonic start beyond the plane
+        const int t = h >> 1;
+        const int dk0 = kh - t < 0 ? (int)-kh : -t, dk1 = kh + t >= K ? (int)(K - 1 - kh) : t;
+        const IT *rowh = P + (size_t)kh * M;
+        const int chunk = (HD_SPAN - 2 * t - 8) / h < HD_TILE ? (HD_SPAN - 2 * t - 8) / h : HD_TILE;   // outputs per span (3 bins of alignment slack)
+        for (int c0 = 0; c0 < HD_TILE; c0 += chunk) {
+            const long long rc = r0 + c0;                              // first output bin of this chunk
+            if (rc * h >= M) break;
+            const int nout = HD_TILE - c0 < chunk ? HD_TILE - c0 : chunk;
+            const long long x_lo = rc * h - t < 0 ? 0 : rc * h - t;
+            long long x_base;                                          // plane bin of buf[0]
+            long long x_hi = (rc + nout - 1) * h + t;
+            if (x_hi > M - 1) x_hi = M - 1;
+            const int span = (int)(x_hi - x_lo + 1);
+            if (sizeof(IT) == 4 && sizeof(OT) == 4 && (M & 3) == 0) {
+                // float planes with 16-byte aligned rows: 128-bit loads from the aligned start of the span (buf index 0 = x_al)
+                const long long x_al = x_lo & ~3LL;
+                const int nq = (int)((x_hi - x_al) / 4 + 1);
+                for (int i = threadIdx.x; i < nq; i += HD_THREADS) {
+                    const float4 *src = reinterpret_cast<const float4 *>(rowh + (long long)dk0 * M + x_al) + i;
+                    float4 v = __ldg(src);
+                    for (int dk = dk0 + 1; dk <= dk1; ++dk) {
+                        const float4 w = __ldg(reinterpret_cast<const float4 *>(rowh + (long long)dk * M + x_al) + i);
+                        v.x = fmaxf(v.x, w.x); v.y = fmaxf(v.y, w.y); v.z = fmaxf(v.z, w.z); v.w = fmaxf(v.w, w.w);
+                    }
+                    reinterpret_cast<float4 *>(buf)[i] = v;
+                }
+                x_base = x_al;
+            } else {
+                for (int i = threadIdx.x; i < span; i += HD_THREADS) {
+                    OT v = (OT)hs_elem<IT>::load(rowh + (long long)dk0 * M + x_lo + i);
+                    for (int dk = dk0 + 1; dk <= dk1; ++dk) v = max(v, (OT)hs_elem<IT>::load(rowh + (long long)dk * M + x_lo + i));
+                    buf[i] = v;
+                }
+                x_base = x_lo;
+            }
+            __syncthreads();
+#pragma unroll
+            for (int j = 0; j < HD_OUT; ++j) {
+                const int o = threadIdx.x + HD_THREADS * j - c0;       // output index inside the chunk
+                if (o < 0 || o >= nout) continue;
+                const long long x = (rc + o) * h;
+                if (x >= M) continue;
+                const long long a = x - t < 0 ? 0 : x - t, b = x + t > M - 1 ? M - 1 : x + t;
+                OT best = buf[a - x_base];
+                for (long long xx = a + 1; xx <= b; ++xx) best = max(best, buf[xx - x_base]);
+                acc[j] += best;
+            }
+            __syncthreads();
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < HD_OUT; ++j) {
+        const long long r = r0 + threadIdx.x + HD_THREADS * j;
+        if (r < M) S[(size_t)k * M + r] = acc[j];
+    }
+}
+
 }  // namespace
 
 template <bool DRIFT>
@@ -105,7 +189,16 @@ int fdas_launch_harmonic_sum(fdas_plan *p, const void *plane, void *sum, int n_h
     if (bx * p->K > cap) bx = (cap + p->K - 1) / p->K;
     if (bx < 1) bx = 1;
     const dim3 grid((unsigned)bx, (unsigned)p->K);
-    if (drift) launch_hs<true>(p, plane, sum, n_harmonics, k0, grid, st);
+    const long long tiles = (p->M + HD_TILE - 1) / HD_TILE;
+    if (drift && tiles <= 65535) {
+        const dim3 gd((unsigned)p->K, (unsigned)tiles);
+        if (p->precision == FDAS_F64)
+            fdas_harmonic_drift_kernel<double, double><<<gd, HD_THREADS, 0, st>>>((const double *)plane, (double *)sum, p->K, p->M, k0, n_harmonics);
+        else if (p->plane_bf16)
+            fdas_harmonic_drift_kernel<bf16bits, float><<<gd, HD_THREADS, 0, st>>>((const bf16bits *)plane, (float *)sum, p->K, p->M, k0, n_harmonics);
+        else
+            fdas_harmonic_drift_kernel<float, float><<<gd, HD_THREADS, 0, st>>>((const float *)plane, (float *)sum, p->K, p->M, k0, n_harmonics);
+    } else if (drift) launch_hs<true>(p, plane, sum, n_harmonics, k0, grid, st);
     else launch_hs<false>(p, plane, sum, n_harmonics, k0, grid, st);
     FDAS_CUDA_TRY(p, cudaGetLastError());
     p->launches += 1;
