@@ -181,7 +181,7 @@ int fdas_tc_encode_maps(fdas_plan *p, void *base, long long cols, long long rows
 int fdas_tc_describe(fdas_plan *p, const void *plane_dev, int batch, fdas_kernel_info_t *out);
 int fdas_tc_describe_noplane(fdas_plan *p, int batch, fdas_kernel_info_t *out);
 int fdas_fft_describe(fdas_plan *p, int batch, fdas_kernel_info_t *out);
-double fdas_tc_issued_flops(const fdas_plan *p, int batch);
+double fdas_tc_issued_flops(const fdas_plan *p, int batch, int plane_free);
 // fdas_peaks.cu: turns the candidates of a fused search into the peak list (same rule as fdas_peaks)
 int fdas_launch_resolve(fdas_plan *p, const void *plane, const fdas_search_args &sa, fdas_peak_t *peaks, int capacity,
                         cudaStream_t st);

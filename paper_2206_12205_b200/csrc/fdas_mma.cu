@@ -337,16 +337,19 @@ static int tc_decide(fdas_plan *p, void *planes, int batch, bool want_maps, TcDe
 }
 
 // dense MMA flops one launch over `batch` series issues (padding included): per 128-bin tile and template group,
-// 2 parts x sum over the K steps of 2 * 128 * N_ks * 16, three products per tap in the split form
-double fdas_tc_issued_flops(const fdas_plan *p, int batch)
+// 2 parts x sum over the K steps of 2 * 128 * N_ks * 16, three products per tap in the split form; plane_free: the
+// scan launch of the plane-free search
+double fdas_tc_issued_flops(const fdas_plan *p, int batch, int plane_free)
 {
     const int split = p->precision == FDAS_F32 ? 3 : 1;
+    // mma_issuer: which launches skip the columns a K step does not reach
+    const bool trimmed = split == 3 || tb_trims(plane_free ? TB_SCAN : TB_PLANE, p->plane_bf16 ? 2 : 4);
     double per_tile = 0.0;
     for (int g = 0; g < p->tc_groups; ++g)
         for (int ks = 0; ks < p->tc_KS; ++ks) {
             unsigned nib = 0;
-            if (split == 3 && g < 8) nib = (unsigned)((ks < 16 ? p->tc_nks_lo[g] >> (4 * ks) : p->tc_nks_hi[g] >> (4 * (ks - 16))) & 15ull);
-            const int n = nib ? 16 * (int)nib : p->tc_NT;       // the bf16 form runs every K step at full width
+            if (trimmed && g < 8) nib = (unsigned)((ks < 16 ? p->tc_nks_lo[g] >> (4 * ks) : p->tc_nks_hi[g] >> (4 * (ks - 16))) & 15ull);
+            const int n = nib ? 16 * (int)nib : p->tc_NT;       // a bf16 launch that writes a plane runs every K step at full width
             per_tile += 2.0 * 2.0 * TC_TILE * n * 16.0 * (split == 3 ? 3.0 : 1.0);
         }
     return per_tile * (double)batch * (double)((p->M + TC_TILE - 1) / TC_TILE);
@@ -367,7 +370,7 @@ int fdas_tc_describe(fdas_plan *p, const void *plane_dev, int batch, fdas_kernel
     out->grid_y = p->tc_groups;
     out->block_threads = d.bulk ? tb_threads(d.split) : TC_THREADS;
     out->dynamic_smem_bytes = d.smem;
-    out->tensor_flops = fdas_tc_issued_flops(p, batch);
+    out->tensor_flops = fdas_tc_issued_flops(p, batch, 0);
     if (d.bulk)
         snprintf(out->kernel, sizeof(out->kernel), "fdas_mma_bulk_kernel<%d, %s, %d>", p->tc_NT / 16, p->plane_bf16 ? "__nv_bfloat16" : "float", d.split);
     else

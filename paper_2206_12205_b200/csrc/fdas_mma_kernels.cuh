@@ -135,6 +135,8 @@ static inline void tc_fill_params(const fdas_plan *p, TcParams &tp, const void *
 //               bit-identical to what TB_PLANE stores -- into a private strip of scratch memory, then the epilogue
 //               warps apply the peak rule of fdas_peaks to the cells of the flagged tile
 constexpr int TB_PLANE = 0, TB_SCAN = 1, TB_RECHECK = 2;
+// bf16 operands: does this launch skip the columns a K step does not reach (mma_issuer)?  The split form always does.
+__host__ __device__ constexpr bool tb_trims(int mode, size_t plane_elem) { return mode != TB_PLANE || plane_elem == 2; }
 
 // work item -> (series, first bin, tiles, index of the tile whose cells are tested [TB_RECHECK])
 template <int MODE>
@@ -469,7 +471,15 @@ __device__ __forceinline__ void umma_commit_elected(uint32_t bar, uint32_t elect
 
 // The MMA warp of both kernels.  Per tile 2 KS MMAs (K steps outermost, so consecutive MMAs
 // alternate between the re and im accumulators), then a commit that signals the epilogue.
-template <int NT, int SPLIT = 1, int MODE = TB_PLANE>
+//
+// The tensor pipe queues only a few MMAs (measured with clock64 stamps: the issuing thread reaches the end of a
+// tile when that tile is one or two MMAs from done), so whatever the thread does between the last MMA of one tile
+// and the first of the next is idle tensor time (measured: ~100 cycles per tile, 400-550 per item boundary with the
+// waits and the item arithmetic at the top of the loops).  Everything the next tile needs -- its TMEM stage handed
+// back by the epilogue, across an item boundary also the next Z buffer, the next item's tile count, the next tile's
+// descriptors -- is therefore waited for / worked out BEFORE the last K step of the current tile is issued, and the
+// loop is flat: commit, a few register moves, next tile's first MMA.
+template <int NT, int SPLIT = 1, int MODE = TB_PLANE, bool TRIM = false>
 __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, uint32_t off_z, uint32_t z_buf_bytes,
                                            uint32_t z_part_bytes, uint32_t z_full, uint32_t z_empty, uint32_t t_full,
                                            uint32_t t_empty, uint32_t tmem_base, uint32_t n_items)
@@ -485,71 +495,137 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
     constexpr uint32_t b_lbo = (uint32_t)NT * 16u;   // next 8-tap chunk of the tap matrix
     const uint32_t elected = elect_one();
     const uint64_t b_desc0 = smem_desc(s_base, b_lbo, 128u);
-    uint32_t n = 0, t = 0;
-    for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x, ++n) {
-        const uint32_t buf = n & 1, zuse = n >> 1;
-        long long ser_, blk0;
-        int n_tiles, centre_;
-        tb_item<MODE>(p, it, ser_, blk0, n_tiles, centre_);
-        mbar_wait(z_full + 8 * buf, zuse & 1);
-        tc_fence_after();
-        const uint32_t z_addr = s_base + off_z + buf * z_buf_bytes;
-        for (int tile = 0; tile < n_tiles; ++tile, ++t) {
-            const uint32_t stage = t & 1, use = t >> 1;
-            mbar_wait(t_empty + 8 * stage, (use & 1) ^ 1);
-            tc_fence_after();
-            const uint32_t d_re = tmem_base + stage * TC_STAGE_COLS, d_im = d_re + NT;
-            // descriptors advance by adding to their 14-bit address field (units of 16 bytes; shared
-            // memory is < 256 KB, so no carry leaves the field)
-            uint64_t a_re = smem_desc(z_addr + (uint32_t)(tile * TC_TILE) * 16u, 128u, 128u);
-            uint64_t a_im = smem_desc(z_addr + z_part_bytes + (uint32_t)(tile * TC_TILE) * 16u, 128u, 128u);
-            uint64_t bd = b_desc0;
-            // SPLIT == 3 (fp32 variant): x = x1 + x2, h = h1 + h2 in bf16 terms; x h ~ x1 h1 + x1 h2 + x2 h1
-            // (the dropped x2 h2 is <= 2^-18 |x h|).  Z parts: re1, im1, re2, im2; tap images: h1, h2.
-            const uint32_t b2_off = (2u * (uint32_t)p.KS * b_lbo) >> 4;   // second tap-matrix image
-            const uint32_t a2_off = (2u * z_part_bytes) >> 4;             // re2 / im2 parts
-            if constexpr (SPLIT == 1) {
-                // bf16 variant: the kernel is bound by the plane stores, not by the tensor pipe; trimming the
-                // columns of the outer K steps measured no gain (0.300 -> 0.31 ms), so every K step runs full width
-                constexpr uint32_t idesc = idesc0 | ((uint32_t)(NT >> 3) << 17);
-                uint64_t ar = a_re, ai = a_im, bk = bd;
-#pragma unroll 3
-                for (int ks = 0; ks < p.KS; ++ks) {
-                    umma_bf16_elected(d_re, ar, bk, idesc, ks > 0, elected);
-                    umma_bf16_elected(d_im, ai, bk, idesc, ks > 0, elected);
-                    ar += 256u >> 4;
-                    ai += 256u >> 4;
-                    bk += (2u * b_lbo) >> 4;
-                }
-            } else {
-                // fp32 variant (tensor-bound, 6 MMAs per K step): outer K steps multiply only the columns whose
-                // templates reach that far (0.487 -> 0.419 ms on config 3)
-                int ks = ks_first;                              // a full-width K step initialises every column
-#pragma unroll 3
-                for (int i = 0; i < p.KS; ++i) {
-                    const uint32_t nib = (uint32_t)((ks < 16 ? nk_lo >> (4 * ks) : nk_hi >> (4 * (ks - 16))) & 15ull);
-                    const uint32_t nk = nib ? 16u * nib : (uint32_t)NT;
-                    const uint32_t idesc = idesc0 | ((nk >> 3) << 17);
-                    const uint64_t ar = a_re + (uint32_t)ks * (256u >> 4), ai = a_im + (uint32_t)ks * (256u >> 4);
-                    const uint64_t bk = bd + (uint32_t)ks * ((2u * b_lbo) >> 4);
-                    umma_bf16_elected(d_re, ar, bk, idesc, i > 0, elected);
-                    umma_bf16_elected(d_im, ai, bk, idesc, i > 0, elected);
-                    umma_bf16_elected(d_re, ar, bk + b2_off, idesc, 1, elected);
-                    umma_bf16_elected(d_im, ai, bk + b2_off, idesc, 1, elected);
-                    umma_bf16_elected(d_re, ar + a2_off, bk, idesc, 1, elected);
-                    umma_bf16_elected(d_im, ai + a2_off, bk, idesc, 1, elected);
-                    ks = ks + 1 == p.KS ? 0 : ks + 1;
-                }
-            }
-            umma_commit_elected(t_full + 8 * stage, elected);
+    // SPLIT == 3 (fp32 variant): x = x1 + x2, h = h1 + h2 in bf16 terms; x h ~ x1 h1 + x1 h2 + x2 h1
+    // (the dropped x2 h2 is <= 2^-18 |x h|).  Z parts: re1, im1, re2, im2; tap images: h1, h2.
+    const uint32_t b2_off = (2u * (uint32_t)p.KS * b_lbo) >> 4;   // second tap-matrix image
+    const uint32_t a2_off = (2u * z_part_bytes) >> 4;             // re2 / im2 parts
+    // One K step of one tile.  K steps run in the same rotated order in every launch (the sums must agree bit for
+    // bit between fdas_convolve and the plane-free search): the full-width step holding tap 0 first, it initialises
+    // every column.  TRIM: a step multiplies only the columns whose templates reach it -- always in the fp32 form
+    // (tensor-bound: 0.487 -> 0.419 ms on config 3), with bf16 operands in the plane-free launches (0.227 -> 0.196 ms)
+    // and for the bf16-stored plane (0.264 -> 0.248 ms); the launch that writes a float plane is bound by its stores
+    // and measured slower with it (0.297 -> 0.309 ms), so it runs every K step at full width.
+    auto issue_step = [&](uint32_t d_re, uint32_t d_im, uint64_t a_re, uint64_t a_im, int ks, uint32_t acc) {
+        uint32_t nk = (uint32_t)NT;
+        if constexpr (TRIM || SPLIT == 3) {
+            const uint32_t nib = (uint32_t)((ks < 16 ? nk_lo >> (4 * ks) : nk_hi >> (4 * (ks - 16))) & 15ull);
+            if (nib) nk = 16u * nib;
         }
-        umma_commit_elected(z_empty + 8 * buf, elected);
+        const uint32_t idesc = idesc0 | ((nk >> 3) << 17);
+        // descriptors advance by adding to their 14-bit address field (units of 16 bytes; shared memory is
+        // < 256 KB, so no carry leaves the field)
+        const uint64_t ar = a_re + (uint32_t)ks * (256u >> 4), ai = a_im + (uint32_t)ks * (256u >> 4);
+        const uint64_t bk = b_desc0 + (uint32_t)ks * ((2u * b_lbo) >> 4);
+        umma_bf16_elected(d_re, ar, bk, idesc, acc, elected);
+        umma_bf16_elected(d_im, ai, bk, idesc, acc, elected);
+        if constexpr (SPLIT == 3) {
+            umma_bf16_elected(d_re, ar, bk + b2_off, idesc, 1, elected);
+            umma_bf16_elected(d_im, ai, bk + b2_off, idesc, 1, elected);
+            umma_bf16_elected(d_re, ar + a2_off, bk, idesc, 1, elected);
+            umma_bf16_elected(d_im, ai + a2_off, bk, idesc, 1, elected);
+        }
+    };
+    // TB_RECHECK: the items are separated by barriers the loader and (clustered) this warp take part in, so nothing
+    // of the next item is waited for early there
+    constexpr bool AHEAD_ITEM = MODE != TB_RECHECK;
+    if (blockIdx.x >= n_items) return;
+    // Tiles of an item.  Everything the issue loop branches on must be warp-uniform IN THE COMPILER'S EYES: the
+    // descriptors live in uniform registers, and one branch on a value held in a vector register drags every
+    // loop-carried descriptor into vector registers at the price of a R2UR per MMA operand (measured: 1120 -> 1360
+    // cycles per tile).  The tile counts therefore pass through a warp reduction (REDUX writes a uniform register);
+    // the block index inside the series is tracked by subtraction instead of it % n_blocks (no division between MMAs).
+    n_items = __reduce_max_sync(0xffffffffu, n_items);
+    uint32_t blk_cur = blockIdx.x;
+    auto blk_wrap = [&](uint32_t b) {
+        while (b >= (uint32_t)p.n_blocks) b -= (uint32_t)p.n_blocks;
+        return b;
+    };
+    auto tiles_of = [&](uint32_t item, uint32_t blk) {
         if constexpr (MODE == TB_RECHECK) {
-            if (p.clustered) {   // a cluster barrier counts every thread (see tb_item_sync)
-                tb_item_sync(1, 0);
-                tb_item_sync(1, 0);
+            long long ser_, blk0_;
+            int nt, centre_;
+            tb_item<MODE>(p, item, ser_, blk0_, nt, centre_);
+            return (int)__reduce_max_sync(0xffffffffu, (unsigned)nt);
+        } else {
+            const long long left = p.M - (long long)blk * p.R;
+            return (int)__reduce_max_sync(0xffffffffu, (unsigned)(((left < p.R ? left : (long long)p.R) + 128 - 1) >> 7));
+        }
+    };
+    blk_cur = blk_wrap(blk_cur);
+    auto wait_stage = [&](uint32_t tt) { mbar_wait(t_empty + 8 * (tt & 1), ((tt >> 1) & 1) ^ 1); };
+    auto wait_z = [&](uint32_t nn) { mbar_wait(z_full + 8 * (nn & 1), (nn >> 1) & 1); };
+    // the tile being issued: item `it` (the n-th of this CTA, `n_tiles` tiles), tile `tile` of it, the t-th tile overall
+    uint32_t it = blockIdx.x, n = 0, t = 0;
+    int tile = 0, n_tiles = tiles_of(it, blk_cur), n_tiles_next = 0;
+    uint32_t z_addr = s_base + off_z;
+    wait_z(0);
+    wait_stage(0);
+    tc_fence_after();
+    uint32_t d_re = tmem_base;
+    uint64_t a_re = smem_desc(z_addr, 128u, 128u), a_im = smem_desc(z_addr + z_part_bytes, 128u, 128u);
+    for (;;) {
+        const uint32_t stage = t & 1;
+        int ks = ks_first;
+        issue_step(d_re, d_re + NT, a_re, a_im, ks, 0);
+        ks = ks + 1 == p.KS ? 0 : ks + 1;
+        // the next item's tile count, early in the current item
+        const bool has_next = it + gridDim.x < n_items;
+        if (tile == 0 && has_next) {
+            blk_cur = blk_wrap(blk_cur + gridDim.x);
+            n_tiles_next = tiles_of(it + gridDim.x, blk_cur);
+        }
+#pragma unroll 2
+        for (int i = 1; i + 1 < p.KS; ++i) {
+            issue_step(d_re, d_re + NT, a_re, a_im, ks, 1);
+            ks = ks + 1 == p.KS ? 0 : ks + 1;
+        }
+        // ---- ahead of the last K step: the next tile's operands, and what it waits for
+        const bool item_ends = tile + 1 == n_tiles;
+        bool more = true, late_waits = false;
+        uint32_t nz_addr = z_addr;
+        if (!item_ends) {
+            wait_stage(t + 1);
+        } else if (!has_next) {
+            more = false;
+        } else {
+            nz_addr = s_base + off_z + ((n + 1) & 1) * z_buf_bytes;
+            if (AHEAD_ITEM) {
+                wait_z(n + 1);
+                wait_stage(t + 1);
+            } else {
+                late_waits = true;
             }
         }
+        const int ntile = item_ends ? 0 : tile + 1;
+        const uint32_t nd_re = tmem_base + ((t + 1) & 1) * TC_STAGE_COLS;
+        const uint64_t na_re = smem_desc(nz_addr + (uint32_t)(ntile * TC_TILE) * 16u, 128u, 128u);
+        const uint64_t na_im = smem_desc(nz_addr + z_part_bytes + (uint32_t)(ntile * TC_TILE) * 16u, 128u, 128u);
+        if (p.KS > 1) issue_step(d_re, d_re + NT, a_re, a_im, ks, 1);
+        umma_commit_elected(t_full + 8 * stage, elected);
+        if (item_ends) {
+            umma_commit_elected(z_empty + 8 * (n & 1), elected);
+            if constexpr (MODE == TB_RECHECK) {
+                if (p.clustered) {   // a cluster barrier counts every thread (see tb_item_sync)
+                    tb_item_sync(1, 0);
+                    tb_item_sync(1, 0);
+                }
+            }
+            if (!more) break;
+            it += gridDim.x;
+            n += 1;
+            n_tiles = n_tiles_next;
+        }
+        ++t;
+        tile = ntile;
+        z_addr = nz_addr;
+        d_re = nd_re;
+        a_re = na_re;
+        a_im = na_im;
+        if (late_waits) {
+            wait_z(n);
+            wait_stage(t);
+        }
+        tc_fence_after();
     }
 }
 
@@ -558,6 +634,7 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
 // item n+1 are issued before the wait for buffer n and stay in registers across it, so that
 // their latency hides behind the tensor core working on the previous items.
 constexpr int TC_LD_ITERS = 8;   // sample pairs per loader thread: (R + 16 KS) / 2 / 96 <= (1024 + 512) / 192
+constexpr int TC_LD_PAIRS = 2;   // Z row pairs a loader thread has in flight (phase B of spectrum_loader)
 
 template <int MODE = TB_PLANE>
 __device__ __forceinline__ void loader_fetch(const TcParams &p, uint32_t it, uint32_t xn, int lt, float2 (&a)[TC_LD_ITERS],
@@ -615,23 +692,44 @@ __device__ __forceinline__ void spectrum_loader(const TcParams &p, unsigned char
         named_bar_sync(1, TC_LOAD_THREADS);
         if (it + gridDim.x < n_items) loader_fetch<MODE>(p, it + gridDim.x, xn, lt, a, b);
         mbar_wait<64>(z_empty + 8 * buf, (zuse & 1) ^ 1);
-        // phase B: Z row i = samples i .. i+7 (16 bytes), for both parts
+        // phase B: Z row i = samples i .. i+7 (16 bytes), for every part.  A thread builds the row pair (2q, 2q+1)
+        // from the five words xs[q .. q+4] (the odd row is the even one shifted by one sample); the loads of TC_LD_PAIRS
+        // pairs and all parts are issued before the first store: the tensor core's operand reads keep shared memory
+        // ~90 % busy, a dependent load -> store chain per row took the loader a whole item period (measured), which
+        // left the MMA warp waiting at every item boundary.  Lanes with bit 2 set store their odd row first: the
+        // eight lanes of a quarter warp then cover 32 distinct banks (rows 2q of lanes 0-3, rows 2q+1 of lanes 4-7).
         unsigned char *zb = smem + off_z + buf * z_buf_bytes;
-        for (uint32_t row = lt; row < zr; row += TC_LOAD_THREADS) {
+        const uint32_t n_pairs = zr >> 1;   // zr = R + 16 KS - 8 is even
+        const bool odd_first = (lt & 4) != 0;
+        for (uint32_t q0 = lt; q0 < n_pairs; q0 += TC_LD_PAIRS * TC_LOAD_THREADS) {
+            uint32_t w[TC_LD_PAIRS][NP][5];
 #pragma unroll
-            for (int part = 0; part < NP; ++part) {
-                const uint32_t *w = xs_re + part * (xs_part_bytes / 4) + (row >> 1);
-                uint4 o;
-                if (row & 1) {
-                    const uint32_t w0 = w[0], w1 = w[1], w2 = w[2], w3 = w[3], w4 = w[4];
-                    o.x = __byte_perm(w0, w1, 0x5432);
-                    o.y = __byte_perm(w1, w2, 0x5432);
-                    o.z = __byte_perm(w2, w3, 0x5432);
-                    o.w = __byte_perm(w3, w4, 0x5432);
-                } else {
-                    o = make_uint4(w[0], w[1], w[2], w[3]);
+            for (int u = 0; u < TC_LD_PAIRS; ++u) {
+                const uint32_t q = q0 + u * TC_LOAD_THREADS;
+                if (q < n_pairs) {
+#pragma unroll
+                    for (int part = 0; part < NP; ++part) {
+                        const uint32_t *src = xs_re + part * (xs_part_bytes / 4) + q;
+#pragma unroll
+                        for (int j = 0; j < 5; ++j) w[u][part][j] = src[j];
+                    }
                 }
-                *reinterpret_cast<uint4 *>(zb + part * z_part_bytes + (size_t)row * 16) = o;
+            }
+#pragma unroll
+            for (int u = 0; u < TC_LD_PAIRS; ++u) {
+                const uint32_t q = q0 + u * TC_LOAD_THREADS;
+                if (q < n_pairs) {
+#pragma unroll
+                    for (int part = 0; part < NP; ++part) {
+                        const uint32_t *v = w[u][part];
+                        const uint4 even = make_uint4(v[0], v[1], v[2], v[3]);
+                        const uint4 odd = make_uint4(__byte_perm(v[0], v[1], 0x5432), __byte_perm(v[1], v[2], 0x5432),
+                                                     __byte_perm(v[2], v[3], 0x5432), __byte_perm(v[3], v[4], 0x5432));
+                        uint4 *rows = reinterpret_cast<uint4 *>(zb + part * z_part_bytes) + 2 * (size_t)q;
+                        rows[odd_first ? 1 : 0] = odd_first ? odd : even;
+                        rows[odd_first ? 0 : 1] = odd_first ? even : odd;
+                    }
+                }
             }
         }
         fence_proxy_async();   // generic-proxy writes of Z -> visible to tcgen05.mma
@@ -727,8 +825,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1) fdas_mma_convolve_kernel(const 
         }
     } else if (warp == TC_MMA_WARP) {
         // =========================== MMA issuer ===========================
-        mma_issuer<NT>(p, s_base, L.off_z, L.z_buf_bytes, L.z_part_bytes, z_full, z_empty, t_full, t_empty,
-                       __shfl_sync(0xffffffffu, tmem_base, 0), n_items);
+        mma_issuer<NT, 1, TB_PLANE, tb_trims(TB_PLANE, sizeof(OT))>(p, s_base, L.off_z, L.z_buf_bytes, L.z_part_bytes, z_full, z_empty,
+                                                                    t_full, t_empty, __shfl_sync(0xffffffffu, tmem_base, 0), n_items);
     } else {
         // =========================== loader ===========================
         spectrum_loader(p, smem, L.off_xs, L.xs_part_bytes, L.xn, L.off_z, L.z_buf_bytes, L.z_part_bytes, L.zr, z_full,
@@ -1177,8 +1275,8 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
         if (issuer) bulk_wait_all();
     } else if (warp == TB_MMA_WARP) {
         // =========================== MMA issuer ===========================
-        mma_issuer<NT, SPLIT, MODE>(p, s_base, L.off_z, L.z_buf_bytes, L.z_part_bytes, z_full, z_empty, t_full, t_empty,
-                                    __shfl_sync(0xffffffffu, tmem_base, 0), n_items);
+        mma_issuer<NT, SPLIT, MODE, tb_trims(MODE, sizeof(OT))>(p, s_base, L.off_z, L.z_buf_bytes, L.z_part_bytes, z_full, z_empty,
+                                                                t_full, t_empty, __shfl_sync(0xffffffffu, tmem_base, 0), n_items);
     } else {
         // =========================== loader ===========================
         spectrum_loader<SPLIT, MODE>(p, smem, L.off_xs, L.xs_part_bytes, L.xn, L.off_z, L.z_buf_bytes, L.z_part_bytes, L.zr,

@@ -91,7 +91,7 @@ int fdas_tc_describe_noplane(fdas_plan *p, int batch, fdas_kernel_info_t *out)
     out->grid_y = p->tc_groups;
     out->block_threads = tb_threads(split);
     out->dynamic_smem_bytes = TbSmem(R, p->tc_KS, p->tc_NT, TC_TILE * 4, split, false).total;
-    out->tensor_flops = fdas_tc_issued_flops(p, batch);
+    out->tensor_flops = fdas_tc_issued_flops(p, batch, 1);
     snprintf(out->kernel, sizeof(out->kernel), "fdas_mma_bulk_kernel<%d, float, %d, TB_SCAN> (+ TB_RECHECK on the listed tiles)", p->tc_NT / 16, split);
     return FDAS_OK;
 }
