@@ -10,13 +10,15 @@
 #define FDAS_PTS 16
 #define FDAS_MAX_BANDS 32     // harmonic bands one fdas_band_max call can take
 #define FDAS_TC_MAX_BOXES 8   // distinct plane-row run lengths the tensor-core kernel's box stores can serve
+#define FDAS_TC_MAX_KS 32     // K steps of 16 taps: 2 m_max + 1 <= 512 taps
+#define FDAS_TC_STEP_TABLES 9 // K-step tables of the tensor-core kernels: template groups 0..7, then one for every other group
 
 // Kernels that need the opt-in to more than 48 KB of dynamic shared memory.  The opt-in is a per-device function
 // attribute; a plan lives on one device, so the largest size requested so far is remembered per plan.
 enum {
     FDAS_OPTIN_FFT = 0, FDAS_OPTIN_MMA_BULK, FDAS_OPTIN_MMA_BULK16, FDAS_OPTIN_MMA_SPLIT, FDAS_OPTIN_MMA_SCALAR,
     FDAS_OPTIN_MMA_SCALAR16, FDAS_OPTIN_MMA_NOPLANE, FDAS_OPTIN_MMA_NOPLANE_SPLIT, FDAS_OPTIN_MMA_RECHECK,
-    FDAS_OPTIN_MMA_RECHECK_SPLIT, FDAS_OPTIN_RFFT_COLS, FDAS_OPTIN_RFFT_ROWS, FDAS_OPTIN_HSUM, FDAS_OPTIN_SLOTS
+    FDAS_OPTIN_MMA_RECHECK_SPLIT, FDAS_OPTIN_RFFT_COLS, FDAS_OPTIN_RFFT_ROWS, FDAS_OPTIN_RFFT_ROWS64, FDAS_OPTIN_HSUM, FDAS_OPTIN_SLOTS
 };
 
 struct fdas_plan {
@@ -39,6 +41,7 @@ struct fdas_plan {
     int tc_groups, tc_nzg, tc_NT, tc_KS, tc_full_chunks;
     unsigned long long tc_nks_lo[8], tc_nks_hi[8];   // columns per K step (nibble = columns / 16; 0 = all), per group
     int tc_ks_first[8];                               // a K step that runs at full width (initialises the accumulators)
+    unsigned long long tc_steps[FDAS_TC_STEP_TABLES][FDAS_TC_MAX_KS];   // the K steps in issue order (tc_step_entry, fdas_mma_kernels.cuh)
     int tc_force_scalar_stores;   // testing: run the generic (scalar-store) tensor-core kernel
     void *tc_bmat;     // [groups][2 KS][NT][8] bf16
     size_t tc_bmat_bytes;

@@ -59,7 +59,7 @@ int fdas_mma_plan(fdas_plan *p)
     const int NT = (2 * nzg + 15) / 16 * 16;
     const int KS = (2 * p->m_max + 1 + 15) / 16;
     // row offsets k*M are 32-bit plane-element offsets inside the kernel
-    p->tc_supported = (KS <= 32 && NT <= 128 && (long long)K * p->M < 0xFFFFFFFFLL);
+    p->tc_supported = (KS <= FDAS_TC_MAX_KS && NT <= 128 && (long long)K * p->M < 0xFFFFFFFFLL);
     // fp32 variant (two tap images, four Z parts): must fit shared memory at the smallest work item
     if (p->precision == FDAS_F32 && TbSmem(128, KS, NT, TC_TILE * 4, 3).total > 227u * 1024u) p->tc_supported = 0;
     p->tc_groups = groups;
@@ -122,6 +122,16 @@ int fdas_mma_plan(fdas_plan *p)
             }
         }
     }
+    // the K steps in issue order: the full-width step first, then on through the taps, wrapping round.  Table 8 serves
+    // the groups beyond the eighth: natural order, every step at full width.
+    for (int g = 0; g < FDAS_TC_STEP_TABLES; ++g)
+        for (int i = 0; i < FDAS_TC_MAX_KS; ++i) {
+            const bool own = g < 8;
+            const int ks = i < KS ? ((own ? p->tc_ks_first[g] : 0) + i) % KS : 0;
+            unsigned nib = 0;
+            if (own && i < KS) nib = (unsigned)((ks < 16 ? p->tc_nks_lo[g] >> (4 * ks) : p->tc_nks_hi[g] >> (4 * (ks - 16))) & 15ull);
+            p->tc_steps[g][i] = tc_step_entry(nib ? 16u * nib : (uint32_t)NT, (uint32_t)ks, (uint32_t)NT);
+        }
     // leading 16-column chunks (8 |z| each) in which every entry has both plane rows, in every group
     p->tc_full_chunks = NT / 16;
     for (int g = 0; g < groups; ++g) {

@@ -73,6 +73,21 @@ constexpr int TC_STAGE_COLS = 256;
 constexpr long long TC_SPIN_LIMIT = 1LL << 26;
 #endif
 
+// tcgen05 instruction descriptor (cute::UMMA::InstrDescriptor): fp32 accumulate, bf16 A and B, both K-major, M = 128,
+// N = n_cols (a multiple of 16)
+__host__ __device__ constexpr uint32_t tc_idesc(uint32_t n_cols)
+{
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(TC_TILE >> 4) << 24) | ((n_cols >> 3) << 17);
+}
+// one K step of the issue order: bits 0-31 the instruction descriptor (N = the columns whose templates reach the
+// step), bits 32-47 the offset of the step's Z rows, bits 48-63 the offset of its tap chunk pair, both in units of
+// 16 bytes (what a shared-memory descriptor's address field counts)
+__host__ __device__ constexpr unsigned long long tc_step_entry(uint32_t n_cols, uint32_t ks, uint32_t NT)
+{
+    return (unsigned long long)tc_idesc(n_cols) | ((unsigned long long)(ks * 16u) << 32) |
+           ((unsigned long long)(ks * 2u * NT) << 48);
+}
+
 struct TcParams {
     const float2 *spectra;   // [batch][M] complex64
     void *planes;            // [batch][K][M] float, or bf16 bit patterns when the plan stores a bf16 plane
@@ -88,10 +103,10 @@ struct TcParams {
     int NT;                  // UMMA N: columns per part (multiple of 16, <= 128) = 16 NCH
     int nzg;                 // |z| values per group
     int full_chunks;         // 16-column chunks whose 8 |z| entries all have both plane rows
-    // per template group (first 8 groups; others run every K step at full width): K step ks needs only the first
-    // 16 * nibble(ks) columns -- the taps of narrower templates are zero there -- and K step ks_first is full width
-    unsigned long long nks_lo[8], nks_hi[8];
-    int ks_first[8];
+    // K steps in issue order, per template group (the first 8 groups; the others use row 8: every step at full width):
+    // tc_step_entry(instruction descriptor with the columns the step needs, offset of its A rows, offset of its tap
+    // chunk).  Read through the constant bank with a uniform index: the MMA warp never leaves the uniform datapath.
+    unsigned long long steps[FDAS_TC_STEP_TABLES][FDAS_TC_MAX_KS];
     int tiles_per_series;    // ceil(M / 128): plane-free search numbers the tiles series * tiles_per_series + tile
     int clustered;           // recheck launch with more than one template group: the groups of one item form a cluster
     fdas_search_args search; // fused threshold pass (fdas_search); enabled = 0 for plain fdas_convolve
@@ -115,11 +130,8 @@ static inline void tc_fill_params(const fdas_plan *p, TcParams &tp, const void *
     tp.NT = p->tc_NT;
     tp.nzg = p->tc_nzg;
     tp.full_chunks = p->tc_full_chunks;
-    for (int g = 0; g < 8; ++g) {
-        tp.nks_lo[g] = p->tc_nks_lo[g];
-        tp.nks_hi[g] = p->tc_nks_hi[g];
-        tp.ks_first[g] = p->tc_ks_first[g];
-    }
+    for (int g = 0; g < FDAS_TC_STEP_TABLES; ++g)
+        for (int i = 0; i < FDAS_TC_MAX_KS; ++i) tp.steps[g][i] = p->tc_steps[g][i];
     tp.tiles_per_series = (int)((p->M + 127) / 128);
     tp.clustered = 0;
     tp.search = fdas_search_args{};
@@ -288,6 +300,13 @@ __device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo_bytes,
     return (uint64_t)((addr >> 4) & 0x3FFFu) | ((uint64_t)((lbo_bytes >> 4) & 0x3FFFu) << 16) |
            ((uint64_t)((sbo_bytes >> 4) & 0x3FFFu) << 32) | (1ull << 46);
 }
+// the same descriptor as two words: every operand of these kernels has stride byte offset 128 (consecutive 8-row
+// groups are adjacent), so the high word is one constant
+constexpr uint32_t TC_DESC_HI = (128u >> 4) | (1u << 14);
+__device__ __forceinline__ uint32_t smem_desc_lo(uint32_t addr, uint32_t lbo_bytes)
+{
+    return ((addr >> 4) & 0x3FFFu) | (((lbo_bytes >> 4) & 0x3FFFu) << 16);
+}
 
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi)
 {
@@ -447,16 +466,19 @@ __device__ __forceinline__ uint32_t elect_one()
     return pred;
 }
 // umma_bf16 issued by the elected lane only; every lane of the warp executes the surrounding code,
-// so the descriptors stay in uniform registers and MMAs issue back to back
-__device__ __forceinline__ void umma_bf16_elected(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc,
+// so the descriptors stay in uniform registers and MMAs issue back to back.  The descriptors come as their low
+// words (the address field moves, 32-bit adds) and the constant high word TC_DESC_HI.
+__device__ __forceinline__ void umma_bf16_elected(uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t idesc,
                                                   uint32_t accumulate, uint32_t elected)
 {
     asm volatile(
-        "{\n\t.reg .pred p, q;\n\t"
+        "{\n\t.reg .pred p, q;\n\t.reg .b64 da, db;\n\t"
+        "mov.b64 da, {%1, %6};\n\t"
+        "mov.b64 db, {%2, %6};\n\t"
         "setp.ne.b32 p, %4, 0;\n\t"
         "setp.ne.b32 q, %5, 0;\n\t"
-        "@q tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-        ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate), "r"(elected)
+        "@q tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %3, p;\n\t}"
+        ::"r"(d_tmem), "r"(a_lo), "r"(b_lo), "r"(idesc), "r"(accumulate), "r"(elected), "r"(TC_DESC_HI)
         : "memory");
 }
 __device__ __forceinline__ void umma_commit_elected(uint32_t bar, uint32_t elected)
@@ -484,38 +506,29 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
                                            uint32_t z_part_bytes, uint32_t z_full, uint32_t z_empty, uint32_t t_full,
                                            uint32_t t_empty, uint32_t tmem_base, uint32_t n_items)
 {
-    // instruction descriptor (cute::UMMA::InstrDescriptor): fp32 accumulate, bf16 A and B, both K-major,
-    // N = NT, M = 128
-    constexpr uint32_t idesc0 = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(TC_TILE >> 4) << 24);
-    // columns per K step: templates are ordered by descending |z| = descending tap count, so the outer K steps
-    // (large |j|) multiply only a prefix of the columns; everything beyond is an exact zero and is skipped
+    // K steps run in the same order in every launch (the sums must agree bit for bit between fdas_convolve and the
+    // plane-free search): the full-width step holding tap 0 first -- it initialises every column -- then on through
+    // the taps, wrapping round (p.steps[] lists them in that order, fdas_mma_plan).  TRIM: a step multiplies only the
+    // columns whose templates reach it, i.e. uses the table's instruction descriptor -- always in the fp32 form
+    // (tensor-bound: 0.487 -> 0.419 ms on config 3), with bf16 operands in the plane-free launches (0.227 -> 0.196 ms)
+    // and for the bf16-stored plane (0.264 -> 0.248 ms); the launch that writes a float plane is bound by its stores
+    // and measured slower with it (0.297 -> 0.309 ms), so it runs every K step at full width.
     const int grp = blockIdx.y;
-    const unsigned long long nk_lo = grp < 8 ? p.nks_lo[grp] : 0ull, nk_hi = grp < 8 ? p.nks_hi[grp] : 0ull;
-    const int ks_first = grp < 8 ? p.ks_first[grp] : 0;
+    const unsigned long long *const steps = p.steps[grp < FDAS_TC_STEP_TABLES - 1 ? grp : FDAS_TC_STEP_TABLES - 1];
     constexpr uint32_t b_lbo = (uint32_t)NT * 16u;   // next 8-tap chunk of the tap matrix
     const uint32_t elected = elect_one();
-    const uint64_t b_desc0 = smem_desc(s_base, b_lbo, 128u);
+    const uint32_t b_lo0 = smem_desc_lo(s_base, b_lbo);
     // SPLIT == 3 (fp32 variant): x = x1 + x2, h = h1 + h2 in bf16 terms; x h ~ x1 h1 + x1 h2 + x2 h1
     // (the dropped x2 h2 is <= 2^-18 |x h|).  Z parts: re1, im1, re2, im2; tap images: h1, h2.
     const uint32_t b2_off = (2u * (uint32_t)p.KS * b_lbo) >> 4;   // second tap-matrix image
     const uint32_t a2_off = (2u * z_part_bytes) >> 4;             // re2 / im2 parts
-    // One K step of one tile.  K steps run in the same rotated order in every launch (the sums must agree bit for
-    // bit between fdas_convolve and the plane-free search): the full-width step holding tap 0 first, it initialises
-    // every column.  TRIM: a step multiplies only the columns whose templates reach it -- always in the fp32 form
-    // (tensor-bound: 0.487 -> 0.419 ms on config 3), with bf16 operands in the plane-free launches (0.227 -> 0.196 ms)
-    // and for the bf16-stored plane (0.264 -> 0.248 ms); the launch that writes a float plane is bound by its stores
-    // and measured slower with it (0.297 -> 0.309 ms), so it runs every K step at full width.
-    auto issue_step = [&](uint32_t d_re, uint32_t d_im, uint64_t a_re, uint64_t a_im, int ks, uint32_t acc) {
-        uint32_t nk = (uint32_t)NT;
-        if constexpr (TRIM || SPLIT == 3) {
-            const uint32_t nib = (uint32_t)((ks < 16 ? nk_lo >> (4 * ks) : nk_hi >> (4 * (ks - 16))) & 15ull);
-            if (nib) nk = 16u * nib;
-        }
-        const uint32_t idesc = idesc0 | ((nk >> 3) << 17);
-        // descriptors advance by adding to their 14-bit address field (units of 16 bytes; shared memory is
-        // < 256 KB, so no carry leaves the field)
-        const uint64_t ar = a_re + (uint32_t)ks * (256u >> 4), ai = a_im + (uint32_t)ks * (256u >> 4);
-        const uint64_t bk = b_desc0 + (uint32_t)ks * ((2u * b_lbo) >> 4);
+    // One K step of one tile; descriptors advance by adding to their 14-bit address field (units of 16 bytes;
+    // shared memory is < 256 KB, so no carry leaves the field).
+    auto issue_step = [&](uint32_t d_re, uint32_t d_im, uint32_t a_re, uint32_t a_im, int i, uint32_t acc) {
+        const unsigned long long e = steps[i];
+        const uint32_t idesc = (TRIM || SPLIT == 3) ? (uint32_t)e : tc_idesc((uint32_t)NT);
+        const uint32_t a_off = (uint32_t)(e >> 32) & 0xFFFFu, b_off = (uint32_t)(e >> 48);
+        const uint32_t ar = a_re + a_off, ai = a_im + a_off, bk = b_lo0 + b_off;
         umma_bf16_elected(d_re, ar, bk, idesc, acc, elected);
         umma_bf16_elected(d_im, ai, bk, idesc, acc, elected);
         if constexpr (SPLIT == 3) {
@@ -562,12 +575,10 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
     wait_stage(0);
     tc_fence_after();
     uint32_t d_re = tmem_base;
-    uint64_t a_re = smem_desc(z_addr, 128u, 128u), a_im = smem_desc(z_addr + z_part_bytes, 128u, 128u);
+    uint32_t a_re = smem_desc_lo(z_addr, 128u), a_im = smem_desc_lo(z_addr + z_part_bytes, 128u);
     for (;;) {
         const uint32_t stage = t & 1;
-        int ks = ks_first;
-        issue_step(d_re, d_re + NT, a_re, a_im, ks, 0);
-        ks = ks + 1 == p.KS ? 0 : ks + 1;
+        issue_step(d_re, d_re + NT, a_re, a_im, 0, 0);
         // the next item's tile count, early in the current item
         const bool has_next = it + gridDim.x < n_items;
         if (tile == 0 && has_next) {
@@ -575,10 +586,7 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
             n_tiles_next = tiles_of(it + gridDim.x, blk_cur);
         }
 #pragma unroll 2
-        for (int i = 1; i + 1 < p.KS; ++i) {
-            issue_step(d_re, d_re + NT, a_re, a_im, ks, 1);
-            ks = ks + 1 == p.KS ? 0 : ks + 1;
-        }
+        for (int i = 1; i + 1 < p.KS; ++i) issue_step(d_re, d_re + NT, a_re, a_im, i, 1);
         // ---- ahead of the last K step: the next tile's operands, and what it waits for
         const bool item_ends = tile + 1 == n_tiles;
         bool more = true, late_waits = false;
@@ -598,9 +606,9 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
         }
         const int ntile = item_ends ? 0 : tile + 1;
         const uint32_t nd_re = tmem_base + ((t + 1) & 1) * TC_STAGE_COLS;
-        const uint64_t na_re = smem_desc(nz_addr + (uint32_t)(ntile * TC_TILE) * 16u, 128u, 128u);
-        const uint64_t na_im = smem_desc(nz_addr + z_part_bytes + (uint32_t)(ntile * TC_TILE) * 16u, 128u, 128u);
-        if (p.KS > 1) issue_step(d_re, d_re + NT, a_re, a_im, ks, 1);
+        const uint32_t na_re = smem_desc_lo(nz_addr + (uint32_t)(ntile * TC_TILE) * 16u, 128u);
+        const uint32_t na_im = smem_desc_lo(nz_addr + z_part_bytes + (uint32_t)(ntile * TC_TILE) * 16u, 128u);
+        if (p.KS > 1) issue_step(d_re, d_re + NT, a_re, a_im, p.KS - 1, 1);
         umma_commit_elected(t_full + 8 * stage, elected);
         if (item_ends) {
             umma_commit_elected(z_empty + 8 * (n & 1), elected);

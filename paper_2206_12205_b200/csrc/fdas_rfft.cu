@@ -13,7 +13,8 @@
 //
 // N >= 2^17 (both factors >= 256): passes A and B run the transforms in REGISTERS -- 16 points per thread, three
 // butterfly passes of radix 16 / 16 / n/256 (the butterflies of fdas_fft.cuh), two shared-memory exchanges, output in
-// natural order (fdas_rfft_fast_kernel below); the 8 L-byte intermediates stay in the 126 MB L2.  Smaller N keep the
+// natural order (fdas_rfft_fast_kernel below) -- and pass C is fused into pass B (a CTA takes rows and their mirror
+// rows): two launches, the series read once, Y (8 L bytes, L2-resident) written and read once, the spectrum written once.  Smaller N keep the
 // shared-memory decimation-in-frequency kernels (two radix-2 stages fused per barrier; natural in, bit-reversed
 // out; the store un-reverses).  Twiddles come from sincospif with exactly representable arguments.
 #include <math.h>
@@ -217,13 +218,17 @@ __device__ __forceinline__ void fast_fft(float *re, float *im, float2 *sx, const
 
 // Pass A (COLS = true): z viewed as [L1][L2]; CTA = NSEQ adjacent columns m2, transform over m1 (stride L2), output
 // Y[k L2 + m2] = W_L^{m2 k} FFT_m1(z)[k].  Pass B (COLS = false): CTA = NSEQ rows k1 of Y [L1][L2] (contiguous),
-// transform over m2, output Z[k1 + L1 k2].
-template <int R3, bool COLS, int NSEQ>
+// transform over m2; Z[k1 + L1 k2] never goes to memory: pass C (the real-input unpacking, file header) is done here.
+// Bin k = k1 + L1 k2 needs Z[L - k], which sits in row L1 - k1 at k2' = L2 - 1 - k2 (rows 0 and L1/2 mirror onto
+// themselves, row 0 at k2' = (L2 - k2) mod L2), so a CTA takes two rows and their two mirror rows -- rows
+// 2b+1, 2b+2, L1-2b-1, L1-2b-2, the last CTA rows L1/2-1, L1/2+1, 0, L1/2 -- and the four transforms meet in shared memory.
+template <int R3, bool COLS, int NSEQ, typename OT2>
 __global__ void __launch_bounds__(FastGeo<R3>::T * NSEQ)
-fdas_rfft_fast_kernel(const float2 *__restrict__ in, float2 *__restrict__ out, int l1, int l2)
+fdas_rfft_fast_kernel(const float2 *__restrict__ in, void *__restrict__ out_, int l1, int l2, float scale)
 {
     using G = FastGeo<R3>;
     using namespace fdas;
+    static_assert(COLS || NSEQ == 4, "pass B pairs two rows with their two mirror rows");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2 *tw = reinterpret_cast<float2 *>(smem_raw);
     float2 *sx = tw + G::N;
@@ -235,6 +240,7 @@ fdas_rfft_fast_kernel(const float2 *__restrict__ in, float2 *__restrict__ out, i
         tw[j] = make_float2(cs, sn);
     }
     float re[16], im[16];
+    int k1 = 0, mate = seq;          // pass B: this thread's row; the sequence of this CTA that holds the mirror row
     if (COLS) {
         const int m2 = blockIdx.x * NSEQ + seq;
 #pragma unroll
@@ -244,7 +250,14 @@ fdas_rfft_fast_kernel(const float2 *__restrict__ in, float2 *__restrict__ out, i
             im[a] = v.x;
         }
     } else {
-        const int k1 = blockIdx.x * NSEQ + seq;
+        const int b = blockIdx.x;
+        if (b + 1 < (int)gridDim.x) {
+            k1 = seq < 2 ? 2 * b + 1 + seq : L1 - 2 * b - 1 - (seq - 2);
+            mate = seq ^ 2;
+        } else {
+            k1 = seq == 0 ? L1 / 2 - 1 : seq == 1 ? L1 / 2 + 1 : seq == 2 ? 0 : L1 / 2;
+            mate = seq < 2 ? seq ^ 1 : seq;
+        }
 #pragma unroll
         for (int a = 0; a < 16; ++a) {
             const float2 v = __ldg(in + (size_t)k1 * L2 + t + G::T * a);
@@ -255,23 +268,58 @@ fdas_rfft_fast_kernel(const float2 *__restrict__ in, float2 *__restrict__ out, i
     __syncthreads();   // twiddle table
     fast_fft<R3>(re, im, sx, tw, t, seq);
     constexpr int U = G::U;
+    if (COLS) {
+        float2 *out = static_cast<float2 *>(out_);
 #pragma unroll
-    for (int u = 0; u < U; ++u) {
+        for (int u = 0; u < U; ++u) {
 #pragma unroll
-        for (int k3 = 0; k3 < R3; ++k3) {
-            const int sl = u * R3 + DftSlot<R3>::of(k3);
-            const int k = t + G::T * u + 256 * k3;
-            float xr = im[sl], xi = re[sl];            // swap back: forward transform
-            if (COLS) {
+            for (int k3 = 0; k3 < R3; ++k3) {
+                const int sl = u * R3 + DftSlot<R3>::of(k3);
+                const int k = t + G::T * u + 256 * k3;
+                float xr = im[sl], xi = re[sl];            // swap back: forward transform
                 const int m2 = blockIdx.x * NSEQ + seq;
                 float sn, cs;
                 // four-step twiddle W_L^{m2 k} = exp(-2 pi i m2 k / L): m2 k < 2^24, 2 m2 k / L exact in fp32
                 sincospif(-2.0f * (float)((unsigned)m2 * (unsigned)k) / (float)(1u << (l1 + l2)), &sn, &cs);
                 fdas::cmul(xr, xi, cs, sn);
                 out[(size_t)k * L2 + m2] = make_float2(xr, xi);
-            } else {
-                const int k1 = blockIdx.x * NSEQ + seq;
-                out[(size_t)k * L1 + k1] = make_float2(xr, xi);
+            }
+        }
+    } else {
+        // Z rows of this CTA -> shared memory (the exchange buffers are free after the barrier), natural k2 order
+        OT2 *X = static_cast<OT2 *>(out_);
+        float2 *zrow = sx + (size_t)seq * G::SE;
+        __syncthreads();
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+#pragma unroll
+            for (int k3 = 0; k3 < R3; ++k3) {
+                const int sl = u * R3 + DftSlot<R3>::of(k3);
+                zrow[t + G::T * u + 256 * k3] = make_float2(im[sl], re[sl]);   // swap back: forward transform
+            }
+        }
+        __syncthreads();
+        // pass C: X[k] = (E + exp(-2 pi i k / N) O) / sqrt N, E = (Z[k] + conj Z[L-k]) / 2, O = -i (Z[k] - conj Z[L-k]) / 2
+        const float2 *zmate = sx + (size_t)mate * G::SE;
+        const float inv_L = 1.0f / (float)(1u << (l1 + l2));
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+#pragma unroll
+            for (int k3 = 0; k3 < R3; ++k3) {
+                const int sl = u * R3 + DftSlot<R3>::of(k3);
+                const int k2 = t + G::T * u + 256 * k3;
+                const int k2m = k1 == 0 ? (L2 - k2) & (L2 - 1) : L2 - 1 - k2;
+                const float2 a = make_float2(im[sl], re[sl]), zb = zmate[k2m];
+                const float2 bq = make_float2(zb.x, -zb.y);
+                const float2 E = make_float2(0.5f * (a.x + bq.x), 0.5f * (a.y + bq.y));
+                const float2 d = make_float2(0.5f * (a.x - bq.x), 0.5f * (a.y - bq.y));
+                const float2 O = make_float2(d.y, -d.x);                     // -i d
+                const unsigned k = (unsigned)k1 + ((unsigned)k2 << l1);
+                float sn, cs;
+                sincospif(-(float)k * inv_L, &sn, &cs);                      // exp(-2 pi i k / N), N = 2 L; k / L exact in fp32
+                const float2 wO = cmul(make_float2(cs, sn), O);
+                X[k].x = scale * (E.x + wO.x);
+                X[k].y = scale * (E.y + wO.y);
             }
         }
     }
@@ -299,29 +347,41 @@ __global__ void __launch_bounds__(256) fdas_rfft_unpack_kernel(const float2 *__r
     }
 }
 
-template <int R3, bool COLS>
-int launch_fast_r(fdas_plan *p, int l1, int l2, const float2 *in, float2 *out, cudaStream_t st)
+template <int R3, bool COLS, typename OT2>
+int launch_fast_r(fdas_plan *p, int l1, int l2, const float2 *in, void *out, float scale, cudaStream_t st)
 {
     using G = FastGeo<R3>;
     constexpr int NSEQ = RF_NSEQ;
-    auto kern = fdas_rfft_fast_kernel<R3, COLS, NSEQ>;
+    auto kern = fdas_rfft_fast_kernel<R3, COLS, NSEQ, OT2>;
     const size_t smem = ((size_t)G::N + (size_t)NSEQ * G::SE) * sizeof(float2);
-    { const int rc = fdas_optin_smem(p, (COLS ? FDAS_OPTIN_RFFT_COLS : FDAS_OPTIN_RFFT_ROWS), kern, smem); if (rc) return rc; }
+    { const int rc = fdas_optin_smem(p, (COLS ? FDAS_OPTIN_RFFT_COLS : sizeof(OT2) == 16 ? FDAS_OPTIN_RFFT_ROWS64 : FDAS_OPTIN_RFFT_ROWS), kern, smem); if (rc) return rc; }
     const int seqs = COLS ? (1 << l2) : (1 << l1);       // columns m2 / rows k1
-    kern<<<seqs / NSEQ, G::T * NSEQ, smem, st>>>(in, out, l1, l2);
+    kern<<<seqs / NSEQ, G::T * NSEQ, smem, st>>>(in, out, l1, l2, scale);
     FDAS_CUDA_TRY(p, cudaGetLastError());
     p->launches += 1;
     return FDAS_OK;
 }
 
-// transforms of length 2^ln: down the columns of [L1][L2] (cols) or along its rows
-int launch_fast(fdas_plan *p, bool cols, int ln, int l1, int l2, const float2 *in, float2 *out, cudaStream_t st)
+// pass A: transforms of length 2^l1 down the columns of [L1][L2]
+int launch_fast_cols(fdas_plan *p, int l1, int l2, const float2 *in, float2 *out, cudaStream_t st)
 {
-    switch (ln - 8) {
-    case 0: return cols ? launch_fast_r<1, true>(p, l1, l2, in, out, st) : launch_fast_r<1, false>(p, l1, l2, in, out, st);
-    case 1: return cols ? launch_fast_r<2, true>(p, l1, l2, in, out, st) : launch_fast_r<2, false>(p, l1, l2, in, out, st);
-    case 2: return cols ? launch_fast_r<4, true>(p, l1, l2, in, out, st) : launch_fast_r<4, false>(p, l1, l2, in, out, st);
-    case 3: return cols ? launch_fast_r<8, true>(p, l1, l2, in, out, st) : launch_fast_r<8, false>(p, l1, l2, in, out, st);
+    switch (l1 - 8) {
+    case 0: return launch_fast_r<1, true, float2>(p, l1, l2, in, out, 1.f, st);
+    case 1: return launch_fast_r<2, true, float2>(p, l1, l2, in, out, 1.f, st);
+    case 2: return launch_fast_r<4, true, float2>(p, l1, l2, in, out, 1.f, st);
+    case 3: return launch_fast_r<8, true, float2>(p, l1, l2, in, out, 1.f, st);
+    default: return FDAS_ERR_UNSUPPORTED;
+    }
+}
+// pass B + C: transforms of length 2^l2 along the rows, unpacked and scaled into the spectrum
+template <typename OT2>
+int launch_fast_rows(fdas_plan *p, int l1, int l2, const float2 *in, void *spectrum, float scale, cudaStream_t st)
+{
+    switch (l2 - 8) {
+    case 0: return launch_fast_r<1, false, OT2>(p, l1, l2, in, spectrum, scale, st);
+    case 1: return launch_fast_r<2, false, OT2>(p, l1, l2, in, spectrum, scale, st);
+    case 2: return launch_fast_r<4, false, OT2>(p, l1, l2, in, spectrum, scale, st);
+    case 3: return launch_fast_r<8, false, OT2>(p, l1, l2, in, spectrum, scale, st);
     default: return FDAS_ERR_UNSUPPORTED;
     }
 }
@@ -341,9 +401,12 @@ int fdas_launch_spectrum(fdas_plan *p, const void *timeseries, void *spectrum, c
     if (l >= 16) {
         // register FFT passes: L = L1 L2 with both factors in 256 .. 2048
         const int l1 = (l + 1) / 2, l2 = l - l1;
-        int rc = launch_fast(p, true, l1, l1, l2, z, Y, st);       // pass A: transforms of length L1 down the columns
-        if (rc == FDAS_OK) rc = launch_fast(p, false, l2, l1, l2, Y, Z, st);   // pass B: transforms of length L2 along the rows
-        if (rc) return rc;
+        const float scale = (float)(1.0 / sqrt((double)p->N));
+        int rc = launch_fast_cols(p, l1, l2, z, Y, st);
+        if (rc == FDAS_OK)
+            rc = p->precision == FDAS_F64 ? launch_fast_rows<double2>(p, l1, l2, Y, spectrum, scale, st)
+                                          : launch_fast_rows<float2>(p, l1, l2, Y, spectrum, scale, st);
+        return rc;
     } else {
         const int l2 = l < RF_L2MAX ? l : RF_L2MAX, l1 = l - l2;
         if (l1 > 0) {
