@@ -859,6 +859,9 @@ __host__ __device__ constexpr int tb_sets(int split) { return split == 3 ? 1 : 2
 __host__ __device__ constexpr int tb_epi_warps(int split) { return 8 * tb_sets(split); }
 __host__ __device__ constexpr int tb_threads(int split) { return 32 * (tb_epi_warps(split) + 1 + TC_LOAD_WARPS); }   // 640 / 384
 constexpr int TB_CGROUPS = 4;           // column groups: NCH entry pairs (4 NCH columns per part) each
+// Recheck launch with one template group: the powers of the listed tile go to a strip in shared memory, K rows of
+// (last bin of the left neighbour tile | the 128 bins of the tile | first bin of the right neighbour tile), padded
+constexpr int TB_STRIP_W = 132;
 constexpr int TB_BOXES = FDAS_TC_MAX_BOXES;   // tensor maps, one per distinct run length (plan->tc_box_heights)
 struct TbMaps {
     CUtensorMap m[TB_BOXES];            // the planes as a [batch*K][M] fp32 matrix, box = tc_box_heights[i] rows x 128 bins
@@ -871,7 +874,9 @@ struct TbSmem {
     uint32_t off_z, off_xs, off_stage, off_bars, off_holder, total;
     // split = 1: bf16 operands; split = 3: the fp32 variant, every operand split into two bf16 terms
     // (two tap-matrix images, four Z parts) and one epilogue warp set (one staging buffer per column group)
-    __host__ __device__ TbSmem(int R, int KS, int NT, int rowb, int split, bool staging = true)
+    // staging: the box-store staging rows; strip_rows > 0 (recheck launch, one template group): no staging, a strip
+    // of strip_rows x TB_STRIP_W floats in its place
+    __host__ __device__ TbSmem(int R, int KS, int NT, int rowb, int split, bool staging = true, int strip_rows = 0)
     {
         const uint32_t TP = 16u * KS;
         const uint32_t nb = split == 3 ? 2u : 1u, np = 2u * nb, sets = split == 3 ? 1u : 2u;
@@ -886,7 +891,7 @@ struct TbSmem {
         off_z = nb * b_bytes;
         off_xs = off_z + 2u * z_buf_bytes;
         off_stage = (off_xs + np * xs_part_bytes + 127u) & ~127u;
-        off_bars = (off_stage + (staging ? sets * TB_CGROUPS * stage_cg_bytes : 0u) + 15u) & ~15u;
+        off_bars = (off_stage + (strip_rows > 0 ? (uint32_t)strip_rows * TB_STRIP_W * 4u : staging ? sets * TB_CGROUPS * stage_cg_bytes : 0u) + 15u) & ~15u;
         off_holder = off_bars + 8u * 8u;
         total = off_holder + 16u;
     }
@@ -987,7 +992,9 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
     constexpr int NT = 16 * NCH;
     constexpr int NC = 4 * NCH;            // columns per part per column group = staging rows (slots)
     constexpr uint32_t ROWB = TC_TILE * sizeof(OT);   // bytes of one staging row
-    const TbSmem L(p.R, p.KS, NT, ROWB, SPLIT, MODE != TB_SCAN);
+    // recheck launch of a single template group: the strip lives in shared memory (no scratch round trip through L2)
+    const bool smem_strip = MODE == TB_RECHECK && gridDim.y == 1;
+    const TbSmem L(p.R, p.KS, NT, ROWB, SPLIT, MODE != TB_SCAN, smem_strip ? p.K : 0);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int grp = blockIdx.y;
     const uint32_t n_items = tb_items<MODE>(p);
@@ -1184,6 +1191,28 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
                     direct_pass(1);
                     continue;
                 }
+                if (MODE == TB_RECHECK && smem_strip) {
+                    // powers -> the strip: every bin of the listed tile, the one adjacent bin of a neighbour tile
+                    const int scol = tile == centre ? 1 + lt : tile < centre ? (lt == TC_TILE - 1 ? 0 : -1) : (lt == 0 ? TC_TILE + 1 : -1);
+                    if (scol >= 0) {
+                        float *const S = reinterpret_cast<float *>(smem + L.off_stage) + scol;
+#pragma unroll
+                        for (int pass = 0; pass < 2; ++pass) {
+                            const int4 rg = rg2[pass];
+                            const int cnt_n = rg.y & 0xFFFF, cnt_p = rg.w & 0xFFFF;
+#pragma unroll
+                            for (int pr = 0; pr < NCH; ++pr) {
+#pragma unroll
+                                for (int e = 0; e < 2; ++e) {
+                                    const int el = 2 * pr + e;
+                                    if (el < cnt_n) S[(rg.x + el) * TB_STRIP_W] = pw[pass][4 * pr + e];
+                                    if (el < cnt_p) S[(rg.z + cnt_p - 1 - el) * TB_STRIP_W] = pw[pass][4 * pr + 2 + e];
+                                }
+                            }
+                        }
+                    }
+                    continue;
+                }
                 // ---- registers -> staging rows -> one tensor-map box per run
 #pragma unroll
                 for (int pass = 0; pass < 2; ++pass) {
@@ -1226,6 +1255,44 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
                 // ---- the item's powers are on their way to scratch: wait for this thread's boxes, meet every other
                 // thread that wrote (all template groups), apply the peak rule of fdas_peaks (reading A14) to
                 // the cells of the flagged tile, meet again before the strip is overwritten
+                if (smem_strip) {
+                    tb_item_sync(0, TB_EPI_WARPS * 32);
+                    const float *S = reinterpret_cast<const float *>(smem + L.off_stage);
+                    const int c = threadIdx.x & (TC_TILE - 1);
+                    const long long r = blk0 + (long long)centre * TC_TILE + c;
+                    const bool left_ok = centre == 1, right_ok = n_tiles > centre + 1;
+                    for (int k = threadIdx.x >> 7; k < p.K && r < p.M; k += TB_EPI_WARPS / 4) {
+                        const float v = S[k * TB_STRIP_W + 1 + c];
+                        if (!(v > thr)) continue;
+                        bool ok = true;
+#pragma unroll
+                        for (int dk = -1; dk <= 1; ++dk) {
+#pragma unroll
+                            for (int dr = -1; dr <= 1; ++dr) {
+                                if (dk == 0 && dr == 0) continue;
+                                const int kk = k + dk, cc = c + dr;
+                                if (kk < 0 || kk >= p.K || r + dr < 0 || r + dr >= p.M) continue;
+                                if ((cc < 0 && !left_ok) || (cc >= TC_TILE && !right_ok)) continue;
+                                const float nb = S[kk * TB_STRIP_W + 1 + cc];
+                                const bool precedes = (dk < 0) || (dk == 0 && dr < 0);
+                                ok = ok && (precedes ? (v > nb) : (v >= nb));
+                            }
+                        }
+                        if (ok) {
+                            const int slot = atomicAdd(p.search.counts + ser, 1);
+                            if (slot < p.search.capacity) {
+                                fdas_peak_t rec;
+                                rec.z_index = k;
+                                rec.r = (int32_t)r;
+                                rec.power = v;
+                                p.search.peaks[(size_t)ser * p.search.capacity + slot] = rec;
+                            }
+                        }
+                    }
+                    if (threadIdx.x == 0) p.search.tile_flags[__ldcg(p.search.tile_list + it)] = 0;
+                    tb_item_sync(0, TB_EPI_WARPS * 32);
+                    continue;
+                }
                 if (issuer) bulk_wait_all();
                 __threadfence();
                 tb_item_sync(p.clustered, TB_EPI_WARPS * 32);

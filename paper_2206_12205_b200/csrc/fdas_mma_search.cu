@@ -179,7 +179,9 @@ int fdas_launch_search_noplane(fdas_plan *p, const void *spectra, int batch, flo
     }
     // ---- recheck launch: one CTA (one cluster of template groups) per strip; CTAs without a listed tile leave at once
     {
-        const uint32_t total = TbSmem(FDAS_TC_STRIP, p->tc_KS, p->tc_NT, TC_TILE * 4, split, true).total;
+        // one template group: the strip of the listed tile sits in shared memory; several: staging rows for the box
+        // stores into the scratch strips the groups share
+        const uint32_t total = TbSmem(FDAS_TC_STRIP, p->tc_KS, p->tc_NT, TC_TILE * 4, split, true, p->tc_groups == 1 ? p->K : 0).total;
         if (total > smem_cap) return FDAS_ERR_UNSUPPORTED;
         TcParams tp;
         tc_fill_params(p, tp, spectra, nullptr, batch, FDAS_TC_STRIP);
