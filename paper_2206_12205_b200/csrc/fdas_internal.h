@@ -185,6 +185,7 @@ int fdas_tc_describe(fdas_plan *p, const void *plane_dev, int batch, fdas_kernel
 int fdas_tc_describe_noplane(fdas_plan *p, int batch, fdas_kernel_info_t *out);
 int fdas_fft_describe(fdas_plan *p, int batch, fdas_kernel_info_t *out);
 double fdas_tc_issued_flops(const fdas_plan *p, int batch, int plane_free);
+int fdas_tc_trims(const fdas_plan *p, bool plane_free);   // does this launch skip the columns a K step does not reach?
 // fdas_peaks.cu: turns the candidates of a fused search into the peak list (same rule as fdas_peaks)
 int fdas_launch_resolve(fdas_plan *p, const void *plane, const fdas_search_args &sa, fdas_peak_t *peaks, int capacity,
                         cudaStream_t st);

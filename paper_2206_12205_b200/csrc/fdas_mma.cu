@@ -346,14 +346,27 @@ static int tc_decide(fdas_plan *p, void *planes, int batch, bool want_maps, TcDe
     return FDAS_OK;
 }
 
+// Does a launch skip, per K step, the columns no template of that step reaches (exact zeros; the sums do not change)?
+// Always where the tensor pipe bounds the launch: the split-operand form, the plane-free search, the bf16-stored
+// plane.  A float plane with bf16 operands is bound by its stores when the MMA stream is short against them --
+// config 3 (97 templates, 9 K steps) measured 0.297 ms at full width against 0.309 ms trimmed -- and by the SM side
+// when it is not -- config 5 (201 templates in two groups, 15 K steps): 0.781 ms at full width, 0.734 ms trimmed.
+// The rule between the two: MMA cycles per 128-bin tile (groups x 2 KS x ~66) against the cycles the tile's K rows of
+// 512 bytes take at the store rate of one SM's share (~25 per row); trimmed above 0.6.
+int fdas_tc_trims(const fdas_plan *p, bool plane_free)
+{
+    if (p->precision == FDAS_F32 || plane_free || p->plane_bf16) return 1;
+    const double mma = (double)p->tc_groups * 2.0 * p->tc_KS * 66.0, store = 25.0 * p->K;
+    return mma > 0.6 * store;
+}
+
 // dense MMA flops one launch over `batch` series issues (padding included): per 128-bin tile and template group,
 // 2 parts x sum over the K steps of 2 * 128 * N_ks * 16, three products per tap in the split form; plane_free: the
 // scan launch of the plane-free search
 double fdas_tc_issued_flops(const fdas_plan *p, int batch, int plane_free)
 {
     const int split = p->precision == FDAS_F32 ? 3 : 1;
-    // mma_issuer: which launches skip the columns a K step does not reach
-    const bool trimmed = split == 3 || tb_trims(plane_free ? TB_SCAN : TB_PLANE, p->plane_bf16 ? 2 : 4);
+    const bool trimmed = fdas_tc_trims(p, plane_free != 0);
     double per_tile = 0.0;
     for (int g = 0; g < p->tc_groups; ++g)
         for (int ks = 0; ks < p->tc_KS; ++ks) {

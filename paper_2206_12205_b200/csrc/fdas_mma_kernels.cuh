@@ -107,6 +107,7 @@ struct TcParams {
     // tc_step_entry(instruction descriptor with the columns the step needs, offset of its A rows, offset of its tap
     // chunk).  Read through the constant bank with a uniform index: the MMA warp never leaves the uniform datapath.
     unsigned long long steps[FDAS_TC_STEP_TABLES][FDAS_TC_MAX_KS];
+    int trim;                // K steps skip the columns no template of theirs reaches (fdas_tc_trims)
     int tiles_per_series;    // ceil(M / 128): plane-free search numbers the tiles series * tiles_per_series + tile
     int clustered;           // recheck launch with more than one template group: the groups of one item form a cluster
     fdas_search_args search; // fused threshold pass (fdas_search); enabled = 0 for plain fdas_convolve
@@ -132,6 +133,7 @@ static inline void tc_fill_params(const fdas_plan *p, TcParams &tp, const void *
     tp.full_chunks = p->tc_full_chunks;
     for (int g = 0; g < FDAS_TC_STEP_TABLES; ++g)
         for (int i = 0; i < FDAS_TC_MAX_KS; ++i) tp.steps[g][i] = p->tc_steps[g][i];
+    tp.trim = fdas_tc_trims(p, planes == nullptr);
     tp.tiles_per_series = (int)((p->M + 127) / 128);
     tp.clustered = 0;
     tp.search = fdas_search_args{};
@@ -147,8 +149,6 @@ static inline void tc_fill_params(const fdas_plan *p, TcParams &tp, const void *
 //               bit-identical to what TB_PLANE stores -- into a private strip of scratch memory, then the epilogue
 //               warps apply the peak rule of fdas_peaks to the cells of the flagged tile
 constexpr int TB_PLANE = 0, TB_SCAN = 1, TB_RECHECK = 2;
-// bf16 operands: does this launch skip the columns a K step does not reach (mma_issuer)?  The split form always does.
-__host__ __device__ constexpr bool tb_trims(int mode, size_t plane_elem) { return mode != TB_PLANE || plane_elem == 2; }
 
 // work item -> (series, first bin, tiles, index of the tile whose cells are tested [TB_RECHECK])
 template <int MODE>
@@ -501,18 +501,15 @@ __device__ __forceinline__ void umma_commit_elected(uint32_t bar, uint32_t elect
 // back by the epilogue, across an item boundary also the next Z buffer, the next item's tile count, the next tile's
 // descriptors -- is therefore waited for / worked out BEFORE the last K step of the current tile is issued, and the
 // loop is flat: commit, a few register moves, next tile's first MMA.
-template <int NT, int SPLIT = 1, int MODE = TB_PLANE, bool TRIM = false>
+template <int NT, int SPLIT = 1, int MODE = TB_PLANE>
 __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, uint32_t off_z, uint32_t z_buf_bytes,
                                            uint32_t z_part_bytes, uint32_t z_full, uint32_t z_empty, uint32_t t_full,
                                            uint32_t t_empty, uint32_t tmem_base, uint32_t n_items)
 {
     // K steps run in the same order in every launch (the sums must agree bit for bit between fdas_convolve and the
     // plane-free search): the full-width step holding tap 0 first -- it initialises every column -- then on through
-    // the taps, wrapping round (p.steps[] lists them in that order, fdas_mma_plan).  TRIM: a step multiplies only the
-    // columns whose templates reach it, i.e. uses the table's instruction descriptor -- always in the fp32 form
-    // (tensor-bound: 0.487 -> 0.419 ms on config 3), with bf16 operands in the plane-free launches (0.227 -> 0.196 ms)
-    // and for the bf16-stored plane (0.264 -> 0.248 ms); the launch that writes a float plane is bound by its stores
-    // and measured slower with it (0.297 -> 0.309 ms), so it runs every K step at full width.
+    // the taps, wrapping round (p.steps[] lists them in that order, fdas_mma_plan).  p.trim: a step multiplies only the
+    // columns whose templates reach it, i.e. uses the table's instruction descriptor (fdas_tc_trims decides per launch).
     const int grp = blockIdx.y;
     const unsigned long long *const steps = p.steps[grp < FDAS_TC_STEP_TABLES - 1 ? grp : FDAS_TC_STEP_TABLES - 1];
     constexpr uint32_t b_lbo = (uint32_t)NT * 16u;   // next 8-tap chunk of the tap matrix
@@ -526,7 +523,7 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
     // shared memory is < 256 KB, so no carry leaves the field).
     auto issue_step = [&](uint32_t d_re, uint32_t d_im, uint32_t a_re, uint32_t a_im, int i, uint32_t acc) {
         const unsigned long long e = steps[i];
-        const uint32_t idesc = (TRIM || SPLIT == 3) ? (uint32_t)e : tc_idesc((uint32_t)NT);
+        const uint32_t idesc = p.trim ? (uint32_t)e : tc_idesc((uint32_t)NT);
         const uint32_t a_off = (uint32_t)(e >> 32) & 0xFFFFu, b_off = (uint32_t)(e >> 48);
         const uint32_t ar = a_re + a_off, ai = a_im + a_off, bk = b_lo0 + b_off;
         umma_bf16_elected(d_re, ar, bk, idesc, acc, elected);
@@ -833,8 +830,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1) fdas_mma_convolve_kernel(const 
         }
     } else if (warp == TC_MMA_WARP) {
         // =========================== MMA issuer ===========================
-        mma_issuer<NT, 1, TB_PLANE, tb_trims(TB_PLANE, sizeof(OT))>(p, s_base, L.off_z, L.z_buf_bytes, L.z_part_bytes, z_full, z_empty,
-                                                                    t_full, t_empty, __shfl_sync(0xffffffffu, tmem_base, 0), n_items);
+        mma_issuer<NT, 1, TB_PLANE>(p, s_base, L.off_z, L.z_buf_bytes, L.z_part_bytes, z_full, z_empty, t_full, t_empty,
+                                    __shfl_sync(0xffffffffu, tmem_base, 0), n_items);
     } else {
         // =========================== loader ===========================
         spectrum_loader(p, smem, L.off_xs, L.xs_part_bytes, L.xn, L.off_z, L.z_buf_bytes, L.z_part_bytes, L.zr, z_full,
@@ -1350,8 +1347,8 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
         if (issuer) bulk_wait_all();
     } else if (warp == TB_MMA_WARP) {
         // =========================== MMA issuer ===========================
-        mma_issuer<NT, SPLIT, MODE, tb_trims(MODE, sizeof(OT))>(p, s_base, L.off_z, L.z_buf_bytes, L.z_part_bytes, z_full, z_empty,
-                                                                t_full, t_empty, __shfl_sync(0xffffffffu, tmem_base, 0), n_items);
+        mma_issuer<NT, SPLIT, MODE>(p, s_base, L.off_z, L.z_buf_bytes, L.z_part_bytes, z_full, z_empty, t_full, t_empty,
+                                    __shfl_sync(0xffffffffu, tmem_base, 0), n_items);
     } else {
         // =========================== loader ===========================
         spectrum_loader<SPLIT, MODE>(p, smem, L.off_xs, L.xs_part_bytes, L.xn, L.off_z, L.z_buf_bytes, L.z_part_bytes, L.zr,
