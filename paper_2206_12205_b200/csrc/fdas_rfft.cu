@@ -269,7 +269,22 @@ fdas_rfft_fast_kernel(const float2 *__restrict__ in, void *__restrict__ out_, in
     fast_fft<R3>(re, im, sx, tw, t, seq);
     constexpr int U = G::U;
     if (COLS) {
+        // four-step twiddle W_L^{m2 k} = exp(-2 pi i m2 k / L), k = t + T (u + U k3): one sincospif per thread for
+        // W_L^{m2 t} and a table of the 16 factors W_L^{m2 T j}, j = u + U k3, per sequence (arguments m2 k < 2^24:
+        // 2 m2 k / L is exact in fp32, each factor is correctly rounded; their product adds one rounding, ~6e-8)
         float2 *out = static_cast<float2 *>(out_);
+        const int m2 = blockIdx.x * NSEQ + seq;
+        const float inv_L = 1.0f / (float)(1u << (l1 + l2));
+        float2 *fac = sx + (size_t)NSEQ * G::SE;          // [NSEQ][16], behind the exchange buffers
+        __syncthreads();
+        if (t < 16) {
+            float sn, cs;
+            sincospif(-2.0f * (float)((unsigned)m2 * (unsigned)(G::T * t)) * inv_L, &sn, &cs);
+            fac[seq * 16 + t] = make_float2(cs, sn);
+        }
+        float wsn, wcs;
+        sincospif(-2.0f * (float)((unsigned)m2 * (unsigned)t) * inv_L, &wsn, &wcs);
+        __syncthreads();
 #pragma unroll
         for (int u = 0; u < U; ++u) {
 #pragma unroll
@@ -277,10 +292,9 @@ fdas_rfft_fast_kernel(const float2 *__restrict__ in, void *__restrict__ out_, in
                 const int sl = u * R3 + DftSlot<R3>::of(k3);
                 const int k = t + G::T * u + 256 * k3;
                 float xr = im[sl], xi = re[sl];            // swap back: forward transform
-                const int m2 = blockIdx.x * NSEQ + seq;
-                float sn, cs;
-                // four-step twiddle W_L^{m2 k} = exp(-2 pi i m2 k / L): m2 k < 2^24, 2 m2 k / L exact in fp32
-                sincospif(-2.0f * (float)((unsigned)m2 * (unsigned)k) / (float)(1u << (l1 + l2)), &sn, &cs);
+                const float2 f = fac[seq * 16 + u + U * k3];
+                float cs = wcs, sn = wsn;
+                fdas::cmul(cs, sn, f.x, f.y);
                 fdas::cmul(xr, xi, cs, sn);
                 out[(size_t)k * L2 + m2] = make_float2(xr, xi);
             }
@@ -302,6 +316,9 @@ fdas_rfft_fast_kernel(const float2 *__restrict__ in, void *__restrict__ out_, in
         // pass C: X[k] = (E + exp(-2 pi i k / N) O) / sqrt N, E = (Z[k] + conj Z[L-k]) / 2, O = -i (Z[k] - conj Z[L-k]) / 2
         const float2 *zmate = sx + (size_t)mate * G::SE;
         const float inv_L = 1.0f / (float)(1u << (l1 + l2));
+        // exp(-2 pi i k / N) = exp(-i pi (k1 + L1 t) / L) (one sincospif per thread) x exp(-i pi T j / L2), j = u + U k3
+        float wsn, wcs;
+        sincospif(-(float)((unsigned)k1 + ((unsigned)t << l1)) * inv_L, &wsn, &wcs);
 #pragma unroll
         for (int u = 0; u < U; ++u) {
 #pragma unroll
@@ -315,9 +332,8 @@ fdas_rfft_fast_kernel(const float2 *__restrict__ in, void *__restrict__ out_, in
                 const float2 d = make_float2(0.5f * (a.x - bq.x), 0.5f * (a.y - bq.y));
                 const float2 O = make_float2(d.y, -d.x);                     // -i d
                 const unsigned k = (unsigned)k1 + ((unsigned)k2 << l1);
-                float sn, cs;
-                sincospif(-(float)k * inv_L, &sn, &cs);                      // exp(-2 pi i k / N), N = 2 L; k / L exact in fp32
-                const float2 wO = cmul(make_float2(cs, sn), O);
+                const float2 f = tw[(G::T / 2) * (u + U * k3)];             // exp(+i pi T j / L2): conjugate it
+                const float2 wO = cmul(cmul(make_float2(wcs, wsn), make_float2(f.x, -f.y)), O);
                 X[k].x = scale * (E.x + wO.x);
                 X[k].y = scale * (E.y + wO.y);
             }
@@ -353,7 +369,7 @@ int launch_fast_r(fdas_plan *p, int l1, int l2, const float2 *in, void *out, flo
     using G = FastGeo<R3>;
     constexpr int NSEQ = RF_NSEQ;
     auto kern = fdas_rfft_fast_kernel<R3, COLS, NSEQ, OT2>;
-    const size_t smem = ((size_t)G::N + (size_t)NSEQ * G::SE) * sizeof(float2);
+    const size_t smem = ((size_t)G::N + (size_t)NSEQ * G::SE + (size_t)NSEQ * 16) * sizeof(float2);
     { const int rc = fdas_optin_smem(p, (COLS ? FDAS_OPTIN_RFFT_COLS : sizeof(OT2) == 16 ? FDAS_OPTIN_RFFT_ROWS64 : FDAS_OPTIN_RFFT_ROWS), kern, smem); if (rc) return rc; }
     const int seqs = COLS ? (1 << l2) : (1 << l1);       // columns m2 / rows k1
     kern<<<seqs / NSEQ, G::T * NSEQ, smem, st>>>(in, out, l1, l2, scale);
