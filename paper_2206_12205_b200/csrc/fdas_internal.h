@@ -76,6 +76,7 @@ struct fdas_plan {
     // fdas_search_host_batched: copy stream, events and double-buffered staging of the host pipeline
     cudaStream_t pipe_stream;
     cudaEvent_t pipe_ev[3][2];     // [h2d done | search done | d2h done][buffer]
+    cudaEvent_t chunk_ev[5];       // fdas_search_host: [0] the caller's stream at entry, [1 + c] chunk c of the spectrum on the device
     void *pipe_spec[2], *pipe_series[2];
     fdas_peak_t *pipe_peaks[2];
     int *pipe_count[2];
@@ -176,6 +177,13 @@ int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, in
 // the plan does not run the tensor-core kernels with a float plane format
 int fdas_launch_search_noplane(fdas_plan *p, const void *spectra, int batch, float thr, fdas_peak_t *peaks, int capacity,
                                int *counts, cudaStream_t st);
+// the same in steps (fdas_mma_search.cu): begin, scan launches over block ranges, one recheck launch
+int fdas_noplane_block_bins(const fdas_plan *p, int batch);
+int fdas_noplane_begin(fdas_plan *p, int batch, float thr, fdas_peak_t *peaks, int capacity, int *counts, cudaStream_t st,
+                       fdas_search_args *out);
+int fdas_noplane_scan(fdas_plan *p, const void *spectra, int batch, const fdas_search_args *sa, int blk_first, int n_blk,
+                      cudaStream_t st);
+int fdas_noplane_recheck(fdas_plan *p, const void *spectra, int batch, const fdas_search_args *sa, cudaStream_t st);
 // fdas_mma.cu: the work-item size the tensor-core launch picks, and tensor maps of a [rows][cols] matrix with one box
 // per distinct run length (shared with fdas_mma_search.cu)
 int fdas_tc_encode_maps(fdas_plan *p, void *base, long long cols, long long rows, size_t elem_bytes, void *maps_out);

@@ -97,7 +97,8 @@ struct TcParams {
     long long M;
     int K, batch;
     int R;                   // outputs per work item (multiple of 128)
-    int n_blocks;            // ceil(M / R)
+    int n_blocks;            // work items per series in this launch: ceil(M / R), or the blocks of a bin range
+    int blk_first;           // first block of that range (0: the whole series)
     int M0;                  // m_max: T[r][kappa] = X[r - M0 + kappa]
     int KS;                  // K steps of 16 taps
     int NT;                  // UMMA N: columns per part (multiple of 16, <= 128) = 16 NCH
@@ -126,6 +127,7 @@ static inline void tc_fill_params(const fdas_plan *p, TcParams &tp, const void *
     tp.batch = batch;
     tp.R = R;
     tp.n_blocks = (int)((p->M + R - 1) / R);
+    tp.blk_first = 0;
     tp.M0 = p->m_max;
     tp.KS = p->tc_KS;
     tp.NT = p->tc_NT;
@@ -165,7 +167,7 @@ __device__ __forceinline__ void tb_item(const TcParams &p, uint32_t it, long lon
         centre = hl;
     } else {
         ser = it / (uint32_t)p.n_blocks;   // 32-bit division: items < 2^31 (checked by the launcher)
-        blk0 = (long long)(it % (uint32_t)p.n_blocks) * p.R;
+        blk0 = (long long)(p.blk_first + it % (uint32_t)p.n_blocks) * p.R;
         const long long left = p.M - blk0;
         n_tiles = (int)((left < p.R ? left : p.R) + 128 - 1) / 128;
         centre = 0;
@@ -557,7 +559,7 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
             tb_item<MODE>(p, item, ser_, blk0_, nt, centre_);
             return (int)__reduce_max_sync(0xffffffffu, (unsigned)nt);
         } else {
-            const long long left = p.M - (long long)blk * p.R;
+            const long long left = p.M - (long long)(p.blk_first + blk) * p.R;
             return (int)__reduce_max_sync(0xffffffffu, (unsigned)(((left < p.R ? left : (long long)p.R) + 128 - 1) >> 7));
         }
     };

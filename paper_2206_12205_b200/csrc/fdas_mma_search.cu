@@ -96,18 +96,29 @@ int fdas_tc_describe_noplane(fdas_plan *p, int batch, fdas_kernel_info_t *out)
     return FDAS_OK;
 }
 
-int fdas_launch_search_noplane(fdas_plan *p, const void *spectra, int batch, float thr, fdas_peak_t *peaks, int capacity,
-                               int *counts, cudaStream_t st)
+// The plane-free search in three steps, so that a caller can scan a series range by range (fdas_search_host scans
+// the chunks of the spectrum as they arrive over the host link):
+//   fdas_noplane_begin    buffers, counters, the arguments both launches share
+//   fdas_noplane_scan     scan launch over blocks [blk_first, blk_first + n_blk) of every series (n_blk <= 0: all);
+//                         block = the scan's work item, fdas_noplane_block_bins() bins
+//   fdas_noplane_recheck  recheck launch over every tile listed since fdas_noplane_begin
+int fdas_noplane_block_bins(const fdas_plan *p, int batch)
+{
+    const int split = p->precision == FDAS_F32 ? 3 : 1;
+    const int sms_per_group = p->num_sms / p->tc_groups > 0 ? p->num_sms / p->tc_groups : 1;
+    return scan_item_bins(p, batch, split, sms_per_group);
+}
+
+int fdas_noplane_begin(fdas_plan *p, int batch, float thr, fdas_peak_t *peaks, int capacity, int *counts, cudaStream_t st,
+                       fdas_search_args *out)
 {
     // the tensor-core kernels with a float plane format; the strip stores need the row runs of the box-store path; the
     // template groups of one item must fit one cluster
     if (!fdas_uses_mma(p) || p->plane_bf16 || !p->tc_bulk_ok || p->tc_groups > 8) return FDAS_ERR_UNSUPPORTED;
-    const int split = p->precision == FDAS_F32 ? 3 : 1;
     const long long tps = (p->M + TC_TILE - 1) / TC_TILE;
     const long long tiles = (long long)batch * tps;
     if (tiles >= 0x7FFFFFFFLL) return FDAS_ERR_UNSUPPORTED;
     const int sms_per_group = p->num_sms / p->tc_groups > 0 ? p->num_sms / p->tc_groups : 1;
-    const uint32_t smem_cap = 227u * 1024u;
 
     // ---- buffers: tile flags (all zero between calls: the recheck launch clears what the scan launch set), tile list,
     // two counters used alternately, the recheck strips and their tensor maps
@@ -136,7 +147,7 @@ int fdas_launch_search_noplane(fdas_plan *p, const void *spectra, int batch, flo
     }
     const size_t strip_bytes = (size_t)sms_per_group * p->K * FDAS_TC_STRIP * sizeof(float);
     if (!p->tf_scratch) {
-        FDAS_CUDA_TRY(p, cudaMalloc((void **)&p->tf_scratch, strip_bytes));
+        FDAS_CUDA_TRY(p, cudaMalloc(&p->tf_scratch, strip_bytes));
         p->tf_scratch_bytes = strip_bytes;
         if (!p->tf_maps) p->tf_maps = aligned_alloc(64, sizeof(TbMaps));
         if (!p->tf_maps) return FDAS_ERR_ALLOC;
@@ -147,8 +158,6 @@ int fdas_launch_search_noplane(fdas_plan *p, const void *spectra, int batch, flo
             return rc;
         }
     }
-    const TbMaps *maps = static_cast<const TbMaps *>(p->tf_maps);
-
     fdas_search_args sa = {};
     sa.enabled = 1;
     sa.thr = thr;
@@ -162,32 +171,58 @@ int fdas_launch_search_noplane(fdas_plan *p, const void *spectra, int batch, flo
     sa.capacity = capacity;
     sa.counts = counts;
     p->tf_calls += 1;
+    *out = sa;
+    return FDAS_OK;
+}
 
-    // ---- scan launch
-    {
-        const int R = scan_item_bins(p, batch, split, sms_per_group);
-        const uint32_t total = TbSmem(R, p->tc_KS, p->tc_NT, TC_TILE * 4, split, false).total;
-        if (total > smem_cap) return FDAS_ERR_UNSUPPORTED;
-        TcParams tp;
-        tc_fill_params(p, tp, spectra, nullptr, batch, R);
-        tp.search = sa;
-        const long long items = (long long)batch * tp.n_blocks;
-        if (items >= 0x7FFFFFFFLL) return FDAS_ERR_UNSUPPORTED;
-        const unsigned gx = (unsigned)(items < sms_per_group ? items : sms_per_group);
-        const int rc = split == 3 ? launch_nch<3, TB_SCAN>(p, tp, gx, total, maps, st) : launch_nch<1, TB_SCAN>(p, tp, gx, total, maps, st);
-        if (rc) return rc;
+int fdas_noplane_scan(fdas_plan *p, const void *spectra, int batch, const fdas_search_args *sa, int blk_first, int n_blk,
+                      cudaStream_t st)
+{
+    const int split = p->precision == FDAS_F32 ? 3 : 1;
+    const int sms_per_group = p->num_sms / p->tc_groups > 0 ? p->num_sms / p->tc_groups : 1;
+    const int R = scan_item_bins(p, batch, split, sms_per_group);
+    const uint32_t total = TbSmem(R, p->tc_KS, p->tc_NT, TC_TILE * 4, split, false).total;
+    if (total > 227u * 1024u) return FDAS_ERR_UNSUPPORTED;
+    TcParams tp;
+    tc_fill_params(p, tp, spectra, nullptr, batch, R);
+    if (n_blk > 0) {
+        if (blk_first < 0 || blk_first + n_blk > tp.n_blocks) return FDAS_ERR_INVALID_ARG;
+        tp.blk_first = blk_first;
+        tp.n_blocks = n_blk;
     }
-    // ---- recheck launch: one CTA (one cluster of template groups) per strip; CTAs without a listed tile leave at once
-    {
-        // one template group: the strip of the listed tile sits in shared memory; several: staging rows for the box
-        // stores into the scratch strips the groups share
-        const uint32_t total = TbSmem(FDAS_TC_STRIP, p->tc_KS, p->tc_NT, TC_TILE * 4, split, true, p->tc_groups == 1 ? p->K : 0).total;
-        if (total > smem_cap) return FDAS_ERR_UNSUPPORTED;
-        TcParams tp;
-        tc_fill_params(p, tp, spectra, nullptr, batch, FDAS_TC_STRIP);
-        tp.search = sa;
-        tp.clustered = p->tc_groups > 1;
-        const unsigned gx = (unsigned)(tiles < sms_per_group ? tiles : sms_per_group);
-        return split == 3 ? launch_nch<3, TB_RECHECK>(p, tp, gx, total, maps, st) : launch_nch<1, TB_RECHECK>(p, tp, gx, total, maps, st);
-    }
+    tp.search = *sa;
+    const long long items = (long long)batch * tp.n_blocks;
+    if (items >= 0x7FFFFFFFLL) return FDAS_ERR_UNSUPPORTED;
+    const unsigned gx = (unsigned)(items < sms_per_group ? items : sms_per_group);
+    const TbMaps *maps = static_cast<const TbMaps *>(p->tf_maps);
+    return split == 3 ? launch_nch<3, TB_SCAN>(p, tp, gx, total, maps, st) : launch_nch<1, TB_SCAN>(p, tp, gx, total, maps, st);
+}
+
+// one CTA (one cluster of template groups) per strip; CTAs without a listed tile leave at once
+int fdas_noplane_recheck(fdas_plan *p, const void *spectra, int batch, const fdas_search_args *sa, cudaStream_t st)
+{
+    const int split = p->precision == FDAS_F32 ? 3 : 1;
+    const int sms_per_group = p->num_sms / p->tc_groups > 0 ? p->num_sms / p->tc_groups : 1;
+    const long long tiles = (long long)batch * ((p->M + TC_TILE - 1) / TC_TILE);
+    // one template group: the strip of the listed tile sits in shared memory; several: staging rows for the box
+    // stores into the scratch strips the groups share
+    const uint32_t total = TbSmem(FDAS_TC_STRIP, p->tc_KS, p->tc_NT, TC_TILE * 4, split, true, p->tc_groups == 1 ? p->K : 0).total;
+    if (total > 227u * 1024u) return FDAS_ERR_UNSUPPORTED;
+    TcParams tp;
+    tc_fill_params(p, tp, spectra, nullptr, batch, FDAS_TC_STRIP);
+    tp.search = *sa;
+    tp.clustered = p->tc_groups > 1;
+    const unsigned gx = (unsigned)(tiles < sms_per_group ? tiles : sms_per_group);
+    const TbMaps *maps = static_cast<const TbMaps *>(p->tf_maps);
+    return split == 3 ? launch_nch<3, TB_RECHECK>(p, tp, gx, total, maps, st) : launch_nch<1, TB_RECHECK>(p, tp, gx, total, maps, st);
+}
+
+int fdas_launch_search_noplane(fdas_plan *p, const void *spectra, int batch, float thr, fdas_peak_t *peaks, int capacity,
+                               int *counts, cudaStream_t st)
+{
+    fdas_search_args sa;
+    int rc = fdas_noplane_begin(p, batch, thr, peaks, capacity, counts, st, &sa);
+    if (rc == FDAS_OK) rc = fdas_noplane_scan(p, spectra, batch, &sa, 0, 0, st);
+    if (rc == FDAS_OK) rc = fdas_noplane_recheck(p, spectra, batch, &sa, st);
+    return rc;
 }

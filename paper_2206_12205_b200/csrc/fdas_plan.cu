@@ -21,6 +21,7 @@ static void free_device_members(fdas_plan *p)
         cudaStreamDestroy(p->pipe_stream);
         for (int e = 0; e < 3; ++e)
             for (int b = 0; b < 2; ++b) cudaEventDestroy(p->pipe_ev[e][b]);
+        for (int c = 0; c < 5; ++c) cudaEventDestroy(p->chunk_ev[c]);
     }
     for (int b = 0; b < 2; ++b) {
         cudaFree(p->pipe_spec[b]);
@@ -395,6 +396,18 @@ extern "C" int fdas_convolve_host(fdas_plan_t *p, const void *spectrum_host, voi
     return FDAS_OK;
 }
 
+// the second stream and the events of the host pipelines
+static int ensure_pipe(fdas_plan *p)
+{
+    if (p->pipe_ready) return FDAS_OK;
+    FDAS_CUDA_TRY(p, cudaStreamCreateWithFlags(&p->pipe_stream, cudaStreamNonBlocking));
+    for (int e = 0; e < 3; ++e)
+        for (int b = 0; b < 2; ++b) FDAS_CUDA_TRY(p, cudaEventCreateWithFlags(&p->pipe_ev[e][b], cudaEventDisableTiming));
+    for (int c = 0; c < 5; ++c) FDAS_CUDA_TRY(p, cudaEventCreateWithFlags(&p->chunk_ev[c], cudaEventDisableTiming));
+    p->pipe_ready = 1;
+    return FDAS_OK;
+}
+
 // host input of the *_host search entry points: the complex spectrum, or (timeseries) the N fp32 samples, which
 // fdas_spectrum turns into the spectrum on the device (the accelerated flow of the paper's Fig. 1 starts at the series)
 static int search_host_common(fdas_plan_t *p, const void *input_host, bool timeseries, float threshold,
@@ -408,17 +421,56 @@ static int search_host_common(fdas_plan_t *p, const void *input_host, bool times
     int rc = ensure_staging(p, !plane_free, capacity);
     if (rc) return rc;
     const size_t spec_bytes = (size_t)p->M * (p->precision == FDAS_F64 ? 16 : 8);
+    bool chunked = false;
     if (timeseries) {
         const size_t ts_bytes = (size_t)p->N * sizeof(float);
         if (!p->stage_series) FDAS_CUDA_TRY(p, cudaMalloc(&p->stage_series, ts_bytes));
         FDAS_CUDA_TRY(p, cudaMemcpyAsync(p->stage_series, input_host, ts_bytes, cudaMemcpyHostToDevice, st));
         rc = fdas_launch_spectrum(p, p->stage_series, p->stage_spectrum, st);
         if (rc) return rc;
+    } else if (plane_free && spec_bytes >= ((size_t)8 << 20)) {
+        // The spectrum crosses the host link in chunks on a second stream while the scan launch of the plane-free
+        // search works through the chunks already on the device (a chunk's last tiles read the first bins of the next
+        // chunk, so chunk c is scanned when chunk c + 1 has landed); one recheck launch at the end.  The copy takes
+        // 0.6 ms for config 3, the search 0.19 ms: overlapped, a series costs little more than its copy.
+        rc = ensure_pipe(p);
+        if (rc) return rc;
+        cudaStream_t cs = p->pipe_stream;
+        const int R = fdas_noplane_block_bins(p, 1);
+        const int blocks = (int)((p->M + R - 1) / R);
+        // chunks of 1/2, 1/4, 1/8, 1/8 of the blocks: every copy call costs ~10 us of link time, and only the scan of
+        // the LAST chunk is not hidden behind a copy
+        int first[5] = {0, blocks / 2, blocks / 2 + blocks / 4, blocks - blocks / 8, blocks};
+        const int n_chunks = blocks >= 64 ? 4 : 1;
+        if (n_chunks == 1) first[1] = blocks;
+        const size_t esz = spec_bytes / (size_t)p->M;
+        fdas_search_args sa;
+        rc = fdas_noplane_begin(p, 1, threshold, p->stage_peaks, capacity, p->stage_count, st, &sa);
+        if (rc) return rc;
+        FDAS_CUDA_TRY(p, cudaEventRecord(p->chunk_ev[0], st));           // after whatever the caller queued before
+        FDAS_CUDA_TRY(p, cudaStreamWaitEvent(cs, p->chunk_ev[0], 0));
+        for (int c = 0; c < n_chunks; ++c) {
+            const long long b0 = (long long)first[c] * R, b1 = (long long)first[c + 1] * R < p->M ? (long long)first[c + 1] * R : p->M;
+            FDAS_CUDA_TRY(p, cudaMemcpyAsync(static_cast<unsigned char *>(p->stage_spectrum) + (size_t)b0 * esz,
+                                             static_cast<const unsigned char *>(input_host) + (size_t)b0 * esz,
+                                             (size_t)(b1 - b0) * esz, cudaMemcpyHostToDevice, cs));
+            FDAS_CUDA_TRY(p, cudaEventRecord(p->chunk_ev[1 + c], cs));
+        }
+        for (int c = 0; c < n_chunks; ++c) {
+            const int need = c + 1 < n_chunks ? c + 1 : c;                   // the chunk holding this range's right halo
+            FDAS_CUDA_TRY(p, cudaStreamWaitEvent(st, p->chunk_ev[1 + need], 0));
+            rc = fdas_noplane_scan(p, p->stage_spectrum, 1, &sa, first[c], first[c + 1] - first[c], st);
+            if (rc) return rc;
+        }
+        rc = fdas_noplane_recheck(p, p->stage_spectrum, 1, &sa, st);
+        if (rc) return rc;
+        chunked = true;
     } else {
         FDAS_CUDA_TRY(p, cudaMemcpyAsync(p->stage_spectrum, input_host, spec_bytes, cudaMemcpyHostToDevice, st));
     }
-    rc = search_on_device(p, p->stage_spectrum, plane_free ? NULL : p->stage_plane, threshold, p->stage_peaks, capacity,
-                          p->stage_count, st);
+    if (!chunked)
+        rc = search_on_device(p, p->stage_spectrum, plane_free ? NULL : p->stage_plane, threshold, p->stage_peaks, capacity,
+                              p->stage_count, st);
     if (rc) return rc;
     FDAS_CUDA_TRY(p, cudaMemcpyAsync(count_host, p->stage_count, sizeof(int), cudaMemcpyDeviceToHost, st));
     FDAS_CUDA_TRY(p, cudaStreamSynchronize(st));
@@ -462,12 +514,8 @@ static int search_host_pipeline(fdas_plan_t *p, const void *spectra_host, bool t
         rc = ensure_staging(p, false, 0);   // stage_spectrum: fdas_spectrum's output, consumed by the search that follows it
         if (rc) return rc;
     }
-    if (!p->pipe_ready) {
-        FDAS_CUDA_TRY(p, cudaStreamCreateWithFlags(&p->pipe_stream, cudaStreamNonBlocking));
-        for (int e = 0; e < 3; ++e)
-            for (int b = 0; b < 2; ++b) FDAS_CUDA_TRY(p, cudaEventCreateWithFlags(&p->pipe_ev[e][b], cudaEventDisableTiming));
-        p->pipe_ready = 1;
-    }
+    rc = ensure_pipe(p);
+    if (rc) return rc;
     for (int b = 0; b < 2; ++b) {
         if (!timeseries && !p->pipe_spec[b]) FDAS_CUDA_TRY(p, cudaMalloc(&p->pipe_spec[b], spec_bytes));
         if (timeseries && !p->pipe_series[b]) FDAS_CUDA_TRY(p, cudaMalloc(&p->pipe_series[b], in_bytes));

@@ -135,3 +135,27 @@ def test_plane_free_search_config3(F):
         n = both(plan, x, THRESH, capacity=1 << 16)
         assert n >= 64
     torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("prec,N", [("bf16", 1 << 21), ("f32", 1 << 21), ("bf16", (1 << 21) + 2 * 12345)])
+def test_search_host_scans_the_spectrum_in_chunks(F, prec, N):
+    # fdas_search_host on a spectrum of 8 MB and more: the copy is split into chunks and every chunk is scanned by
+    # its own launch as soon as the next one has landed (the accelerated section starts with the
+    # host -> device copy).  Same peaks, bit for bit, as the search of the whole spectrum on the device; the ragged
+    # size ends with a partial block and a partial tile.
+    import torch
+    w = workloads.noise_only(N, seed=21, zmax=20.0, dz=2.0, seglen=1024)
+    sp = w.spectrum.copy()
+    rng = np.random.default_rng(5)
+    M = len(sp)
+    for r0 in (3, 1023, 1024, M // 8 - 1, M // 8, M // 2 + 77, M - 2):     # bright bins on and beside chunk / block boundaries
+        sp[r0] += np.complex64(12.0 * np.exp(2j * np.pi * rng.random()))
+    plan = F.Plan(w.N, w.zmax, w.dz, w.seglen, prec)
+    assert sp.nbytes >= 8 << 20
+    _, n_ref, rec_ref = plan.search(torch.from_numpy(sp).cuda(), THRESH, capacity=1 << 16)
+    assert n_ref >= 7
+    rec = np.zeros(1 << 16, dtype=rec_ref.dtype)
+    for _ in range(2):
+        n = plan.search_host(sp, THRESH, rec, 1 << 16)
+        assert n == n_ref
+        assert as_set(rec[:n]) == as_set(rec_ref)
