@@ -672,15 +672,13 @@ template <int SPLIT = 1, int MODE = TB_PLANE>
 __device__ __forceinline__ void spectrum_loader(const TcParams &p, unsigned char *smem, uint32_t off_xs,
                                                 uint32_t xs_part_bytes, uint32_t xn, uint32_t off_z, uint32_t z_buf_bytes,
                                                 uint32_t z_part_bytes, uint32_t zr, uint32_t z_full, uint32_t z_empty,
-                                                int lt, uint32_t n_items)
+                                                int lt, uint32_t n_items, float2 (&a)[TC_LD_ITERS], float2 (&b)[TC_LD_ITERS])
 {
     // sample planes: re, im of the bf16 spectrum; SPLIT == 3 adds re, im of the rounded residual (parts 2, 3)
     constexpr int NP = SPLIT == 3 ? 4 : 2;
     uint32_t *xs_re = reinterpret_cast<uint32_t *>(smem + off_xs);
     uint32_t *xs_im = reinterpret_cast<uint32_t *>(smem + off_xs + xs_part_bytes);
-    float2 a[TC_LD_ITERS], b[TC_LD_ITERS];
-    uint32_t n = 0;
-    if (blockIdx.x < n_items) loader_fetch<MODE>(p, blockIdx.x, xn, lt, a, b);
+    uint32_t n = 0;   // a, b: the first item's samples, fetched by the kernel before its set-up (tb_first_fetch)
     for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x, ++n) {
         const uint32_t buf = n & 1, zuse = n >> 1;
         // phase A: spectrum block -> bf16 (round-to-nearest-even), re and im planes
@@ -769,6 +767,11 @@ __global__ void __launch_bounds__(TC_THREADS, 1) fdas_mma_convolve_kernel(const 
     uint32_t *holder = reinterpret_cast<uint32_t *>(smem + L.off_holder);
     uint2 *otab = reinterpret_cast<uint2 *>(smem + L.off_ktab);   // [NT/2] row offsets (+|z|, -|z|)
 
+    // the loader warps put the global loads of their first item in flight before the set-up: its latency hides behind
+    // the tap-matrix copy and the TMEM allocation (a launch of config 1 is 10 us long, the set-up 3 of them)
+    float2 first_a[TC_LD_ITERS], first_b[TC_LD_ITERS];
+    if (warp >= TC_LOAD_WARP0 && blockIdx.x < n_items)
+        loader_fetch<TB_PLANE>(p, blockIdx.x, L.xn, threadIdx.x - TC_LOAD_WARP0 * 32, first_a, first_b);
     // ---- one-time setup: tap matrix image and row-offset table -> shared memory, barriers, TMEM
     {
         const uint4 *src = p.bmat + (size_t)grp * (L.b_bytes / 16);
@@ -837,7 +840,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) fdas_mma_convolve_kernel(const 
     } else {
         // =========================== loader ===========================
         spectrum_loader(p, smem, L.off_xs, L.xs_part_bytes, L.xn, L.off_z, L.z_buf_bytes, L.z_part_bytes, L.zr, z_full,
-                        z_empty, threadIdx.x - TC_LOAD_WARP0 * 32, n_items);
+                        z_empty, threadIdx.x - TC_LOAD_WARP0 * 32, n_items, first_a, first_b);
     }
 
     tc_fence_before();
@@ -1004,6 +1007,10 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
     const uint32_t z_full = bars, z_empty = bars + 16, t_full = bars + 32, t_empty = bars + 48;
     uint32_t *holder = reinterpret_cast<uint32_t *>(smem + L.off_holder);
 
+    // the loader warps put the global loads of their first item in flight before the set-up (see fdas_mma_convolve_kernel)
+    float2 first_a[TC_LD_ITERS], first_b[TC_LD_ITERS];
+    if (warp >= TB_LOAD_WARP0 && blockIdx.x < n_items)
+        loader_fetch<MODE>(p, blockIdx.x, L.xn, threadIdx.x - TB_LOAD_WARP0 * 32, first_a, first_b);
     // ---- one-time setup: tap matrix image -> shared memory, barriers, TMEM
     {
         // tap-matrix image(s) of this template group: bmat is [image][group][...]
@@ -1354,7 +1361,7 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
     } else {
         // =========================== loader ===========================
         spectrum_loader<SPLIT, MODE>(p, smem, L.off_xs, L.xs_part_bytes, L.xn, L.off_z, L.z_buf_bytes, L.z_part_bytes, L.zr,
-                                     z_full, z_empty, threadIdx.x - TB_LOAD_WARP0 * 32, n_items);
+                                     z_full, z_empty, threadIdx.x - TB_LOAD_WARP0 * 32, n_items, first_a, first_b);
     }
 
     tc_fence_before();
