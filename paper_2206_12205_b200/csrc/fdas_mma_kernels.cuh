@@ -999,6 +999,7 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
     const TbSmem L(p.R, p.KS, NT, ROWB, SPLIT, MODE != TB_SCAN, smem_strip ? p.K : 0);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int grp = blockIdx.y;
+    if (MODE == TB_RECHECK) asm volatile("griddepcontrol.wait;" ::: "memory");   // the scan launch has listed its tiles
     const uint32_t n_items = tb_items<MODE>(p);
     if (MODE == TB_RECHECK && blockIdx.x >= n_items) return;   // nothing flagged for this CTA (its whole cluster: same x)
 

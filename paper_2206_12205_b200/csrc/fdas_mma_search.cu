@@ -31,15 +31,22 @@ int launch_mode(fdas_plan *p, const TcParams &tp, unsigned gx, size_t smem_bytes
     cfg.blockDim = dim3(tb_threads(SPLIT));
     cfg.dynamicSmemBytes = smem_bytes;
     cfg.stream = st;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
+    int na = 0;
     if (MODE == TB_RECHECK && p->tc_groups > 1) {   // the template groups of one work item meet at a cluster barrier
-        attr[0].id = cudaLaunchAttributeClusterDimension;
-        attr[0].val.clusterDim.x = 1;
-        attr[0].val.clusterDim.y = (unsigned)p->tc_groups;
-        attr[0].val.clusterDim.z = 1;
-        cfg.attrs = attr;
-        cfg.numAttrs = 1;
+        attr[na].id = cudaLaunchAttributeClusterDimension;
+        attr[na].val.clusterDim.x = 1;
+        attr[na].val.clusterDim.y = (unsigned)p->tc_groups;
+        attr[na].val.clusterDim.z = 1;
+        ++na;
     }
+    if (MODE == TB_RECHECK) {   // programmatic dependent of the scan launch: set up while it drains, griddepcontrol.wait inside
+        attr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[na].val.programmaticStreamSerializationAllowed = 1;
+        ++na;
+    }
+    cfg.attrs = attr;
+    cfg.numAttrs = na;
     FDAS_CUDA_TRY(p, cudaLaunchKernelEx(&cfg, kern, tp, *maps));
     p->launches += 1;
     return FDAS_OK;

@@ -98,6 +98,7 @@ fdas_resolve_kernel(const PT *__restrict__ P, int K, long long M, float thr, con
                     const int *__restrict__ cand_count, int cand_capacity, int span, const int2 *__restrict__ ktab,
                     int nzg, fdas_peak_t *peaks, int capacity, int *count)
 {
+    asm volatile("griddepcontrol.wait;" ::: "memory");   // launched as a programmatic dependent of the convolve launch
     const int n = *cand_count;
     const long long stride = (long long)gridDim.x * blockDim.x;
     const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -217,15 +218,25 @@ int fdas_launch_peaks3(fdas_plan *p, const void *volume, int n_slabs, float thr,
 int fdas_launch_resolve(fdas_plan *p, const void *plane, const fdas_search_args &sa, fdas_peak_t *peaks, int capacity,
                         cudaStream_t st)
 {
-    const int grid = p->num_sms * 2;
+    // programmatic dependent launch: the grid is set up while the convolve launch drains; the kernel itself waits
+    // (griddepcontrol.wait) for that launch to complete before it reads the candidates
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(p->num_sms * 2));
+    cfg.blockDim = dim3(256);
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
     if (p->plane_bf16)
-        fdas_resolve_kernel<bf16raw, uint4, 8><<<grid, 256, 0, st>>>((const bf16raw *)plane, p->K, p->M, sa.thr, sa.cand,
-                                                                     sa.cand_count, sa.cand_capacity, sa.cand_span, p->tc_ktab,
-                                                                     p->tc_nzg, peaks, capacity, sa.count_out);
+        FDAS_CUDA_TRY(p, cudaLaunchKernelEx(&cfg, fdas_resolve_kernel<bf16raw, uint4, 8>, (const bf16raw *)plane, p->K, (long long)p->M, sa.thr,
+                                            (const fdas_peak_t *)sa.cand, (const int *)sa.cand_count, sa.cand_capacity, sa.cand_span,
+                                            (const int2 *)p->tc_ktab, p->tc_nzg, peaks, capacity, sa.count_out));
     else
-        fdas_resolve_kernel<float, float4, 4><<<grid, 256, 0, st>>>((const float *)plane, p->K, p->M, sa.thr, sa.cand,
-                                                                   sa.cand_count, sa.cand_capacity, sa.cand_span, p->tc_ktab,
-                                                                   p->tc_nzg, peaks, capacity, sa.count_out);
+        FDAS_CUDA_TRY(p, cudaLaunchKernelEx(&cfg, fdas_resolve_kernel<float, float4, 4>, (const float *)plane, p->K, (long long)p->M, sa.thr,
+                                            (const fdas_peak_t *)sa.cand, (const int *)sa.cand_count, sa.cand_capacity, sa.cand_span,
+                                            (const int2 *)p->tc_ktab, p->tc_nzg, peaks, capacity, sa.count_out));
     FDAS_CUDA_TRY(p, cudaGetLastError());
     p->launches += 1;
     return FDAS_OK;
