@@ -42,6 +42,9 @@ struct fdas_plan {
     unsigned long long tc_nks_lo[8], tc_nks_hi[8];   // columns per K step (nibble = columns / 16; 0 = all), per group
     int tc_ks_first[8];                               // a K step that runs at full width (initialises the accumulators)
     unsigned long long tc_steps[FDAS_TC_STEP_TABLES][FDAS_TC_MAX_KS];   // the K steps in issue order (tc_step_entry, fdas_mma_kernels.cuh)
+    int tc_nsteps[FDAS_TC_STEP_TABLES];   // entries of tc_steps[g]
+    double tc_cost[8];                    // estimated tensor-pipe cycles per 128-bin tile, per template group
+    int tc_rows[8];                       // plane rows of each template group
     int tc_force_scalar_stores;   // testing: run the generic (scalar-store) tensor-core kernel
     void *tc_bmat;     // [groups][2 KS][NT][8] bf16
     size_t tc_bmat_bytes;

@@ -115,23 +115,46 @@ int fdas_mma_plan(fdas_plan *p)
                 cols = (cols + 15) / 16 * 16;
                 if (cols < 16) cols = 16;
                 if (cols > NT) cols = NT;
-                const unsigned long long nib = (unsigned long long)(cols / 16);
+                // nibble 15 (NT / 16 <= 8 leaves it free): no template of the group reaches this step
+                const unsigned long long nib = n_need == 0 ? 15ull : (unsigned long long)(cols / 16);
                 if (ks < 16) p->tc_nks_lo[g] |= nib << (4 * ks);
                 else p->tc_nks_hi[g] |= nib << (4 * (ks - 16));
                 if (minabs == 0) p->tc_ks_first[g] = ks;              // holds tap j = 0: every entry needs it
             }
         }
     }
-    // the K steps in issue order: the full-width step first, then on through the taps, wrapping round.  Table 8 serves
-    // the groups beyond the eighth: natural order, every step at full width.
-    for (int g = 0; g < FDAS_TC_STEP_TABLES; ++g)
-        for (int i = 0; i < FDAS_TC_MAX_KS; ++i) {
-            const bool own = g < 8;
-            const int ks = i < KS ? ((own ? p->tc_ks_first[g] : 0) + i) % KS : 0;
+    // the K steps in issue order: the full-width step first, then on through the taps, wrapping round; a step no
+    // template of the group reaches (a group of narrow templates: its outer taps are all zero) is left out.  Table 8
+    // serves the groups beyond the eighth: natural order, every step at full width.  tc_cost[g]: estimated tensor-pipe
+    // cycles per 128-bin tile (an M = 128, K = 16 MMA costs max(51, (4 KB + 32 N B) / 113 B per cycle), measured).
+    for (int g = 0; g < FDAS_TC_STEP_TABLES; ++g) {
+        const bool own = g < 8 && g < groups && symmetric;
+        int n = 0;
+        double cost = 0.0;
+        for (int i = 0; i < KS; ++i) {
+            const int ks = ((own ? p->tc_ks_first[g] : 0) + i) % KS;
             unsigned nib = 0;
-            if (own && i < KS) nib = (unsigned)((ks < 16 ? p->tc_nks_lo[g] >> (4 * ks) : p->tc_nks_hi[g] >> (4 * (ks - 16))) & 15ull);
-            p->tc_steps[g][i] = tc_step_entry(nib ? 16u * nib : (uint32_t)NT, (uint32_t)ks, (uint32_t)NT);
+            if (own) {
+                nib = (unsigned)((ks < 16 ? p->tc_nks_lo[g] >> (4 * ks) : p->tc_nks_hi[g] >> (4 * (ks - 16))) & 15ull);
+                if (nib == 15u) continue;   // marked below: nobody reaches this step
+            }
+            const uint32_t cols = nib ? 16u * nib : (uint32_t)NT;
+            p->tc_steps[g][n++] = tc_step_entry(cols, (uint32_t)ks, (uint32_t)NT);
+            const double c = (4096.0 + 32.0 * cols) / 113.0;
+            cost += 2.0 * (c > 51.0 ? c : 51.0);
         }
+        for (int i = n; i < FDAS_TC_MAX_KS; ++i) p->tc_steps[g][i] = 0;
+        p->tc_nsteps[g] = n;
+        if (g < 8) {
+            p->tc_cost[g] = cost;
+            int rows = 0;
+            for (int e = 0; e < nzg && g < groups; ++e) {
+                const int2 t = tab[(size_t)g * nzg + e];
+                rows += (t.y >= 0) + (t.x >= 0 && t.x != t.y);
+            }
+            p->tc_rows[g] = rows;
+        }
+    }
     // leading 16-column chunks (8 |z| each) in which every entry has both plane rows, in every group
     p->tc_full_chunks = NT / 16;
     for (int g = 0; g < groups; ++g) {
@@ -277,7 +300,7 @@ static int launch_mma_split(fdas_plan *p, const TcParams &tp, unsigned gx, size_
 {
     auto kern = fdas_mma_bulk_kernel<NCH, float, 3>;
     { const int rc = fdas_optin_smem(p, FDAS_OPTIN_MMA_SPLIT, kern, smem_bytes); if (rc) return rc; }
-    kern<<<dim3(gx, p->tc_groups), tb_threads(3), smem_bytes, st>>>(tp, *maps);
+    kern<<<dim3(gx), tb_threads(3), smem_bytes, st>>>(tp, *maps);
     FDAS_CUDA_TRY(p, cudaGetLastError());
     p->launches += 1;
     return FDAS_OK;
@@ -289,11 +312,11 @@ static int launch_mma(fdas_plan *p, const TcParams &tp, unsigned gx, size_t smem
     if (maps) {
         auto kern = fdas_mma_bulk_kernel<NCH, OT, 1>;
         { const int rc = fdas_optin_smem(p, sizeof(OT) == 2 ? FDAS_OPTIN_MMA_BULK16 : FDAS_OPTIN_MMA_BULK, kern, smem_bytes); if (rc) return rc; }
-        kern<<<dim3(gx, p->tc_groups), tb_threads(1), smem_bytes, st>>>(tp, *maps);
+        kern<<<dim3(gx), tb_threads(1), smem_bytes, st>>>(tp, *maps);
     } else {
         auto kern = fdas_mma_convolve_kernel<NCH, OT>;
         { const int rc = fdas_optin_smem(p, sizeof(OT) == 2 ? FDAS_OPTIN_MMA_SCALAR16 : FDAS_OPTIN_MMA_SCALAR, kern, smem_bytes); if (rc) return rc; }
-        kern<<<dim3(gx, p->tc_groups), TC_THREADS, smem_bytes, st>>>(tp);
+        kern<<<dim3(gx), TC_THREADS, smem_bytes, st>>>(tp);
     }
     FDAS_CUDA_TRY(p, cudaGetLastError());
     p->launches += 1;
@@ -368,13 +391,13 @@ double fdas_tc_issued_flops(const fdas_plan *p, int batch, int plane_free)
     const int split = p->precision == FDAS_F32 ? 3 : 1;
     const bool trimmed = fdas_tc_trims(p, plane_free != 0);
     double per_tile = 0.0;
-    for (int g = 0; g < p->tc_groups; ++g)
-        for (int ks = 0; ks < p->tc_KS; ++ks) {
-            unsigned nib = 0;
-            if (trimmed && g < 8) nib = (unsigned)((ks < 16 ? p->tc_nks_lo[g] >> (4 * ks) : p->tc_nks_hi[g] >> (4 * (ks - 16))) & 15ull);
-            const int n = nib ? 16 * (int)nib : p->tc_NT;       // a bf16 launch that writes a plane runs every K step at full width
+    for (int g = 0; g < p->tc_groups; ++g) {
+        const int tb = g < FDAS_TC_STEP_TABLES - 1 ? g : FDAS_TC_STEP_TABLES - 1;
+        for (int i = 0; i < p->tc_nsteps[tb]; ++i) {
+            const int n = trimmed ? (int)(((uint32_t)p->tc_steps[tb][i] >> 17) & 63u) * 8 : p->tc_NT;   // N field of the descriptor
             per_tile += 2.0 * 2.0 * TC_TILE * n * 16.0 * (split == 3 ? 3.0 : 1.0);
         }
+    }
     return per_tile * (double)batch * (double)((p->M + TC_TILE - 1) / TC_TILE);
 }
 
@@ -389,8 +412,12 @@ int fdas_tc_describe(fdas_plan *p, const void *plane_dev, int batch, fdas_kernel
     out->nch = p->tc_NT / 16;
     out->k_steps = p->tc_KS;
     out->work_item_bins = d.R;
-    out->grid_x = (int32_t)d.gx;
-    out->grid_y = p->tc_groups;
+    {
+        TcParams tp;
+        tc_fill_params(p, tp, nullptr, const_cast<void *>(plane_dev), batch, d.R);
+        out->grid_x = (int32_t)fdas_tc_split_ctas(p, tp, (long long)batch * tp.n_blocks);   // one-dimensional: every group's CTAs
+        out->grid_y = 1;
+    }
     out->block_threads = d.bulk ? tb_threads(d.split) : TC_THREADS;
     out->dynamic_smem_bytes = d.smem;
     out->tensor_flops = fdas_tc_issued_flops(p, batch, 0);
@@ -410,9 +437,9 @@ int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, in
     const int split = d.split, R = d.R;
     const uint32_t total = d.smem;
     const TbMaps *maps = d.maps;
-    const unsigned gx = d.gx;
     TcParams tp;
     tc_fill_params(p, tp, spectra, planes, batch, R);
+    const unsigned gx = fdas_tc_split_ctas(p, tp, (long long)batch * tp.n_blocks);   // all CTAs, every group
     if (search) {
         search->cand_span = bulk ? p->tc_NT / 8 : 8;   // |z| entries per column group (2 NCH) / per 16-column chunk
         tp.search = *search;

@@ -108,6 +108,13 @@ struct TcParams {
     // tc_step_entry(instruction descriptor with the columns the step needs, offset of its A rows, offset of its tap
     // chunk).  Read through the constant bank with a uniform index: the MMA warp never leaves the uniform datapath.
     unsigned long long steps[FDAS_TC_STEP_TABLES][FDAS_TC_MAX_KS];
+    int nsteps[FDAS_TC_STEP_TABLES];   // entries of steps[g]: the K steps at least one template of the group reaches
+    // CTA -> (template group, index inside the group).  TB_PLANE / TB_SCAN launches use a one-dimensional grid: with up
+    // to 8 groups, group g owns CTAs cta0[g] .. cta0[g + 1] - 1, as many as its share of the MMA work (a group of narrow
+    // templates needs fewer K steps per tile; fdas_tc_split_ctas); with more groups cta_even CTAs each.  TB_RECHECK
+    // launches keep the grid (x, groups): the groups of one item form a cluster.
+    int groups, cta_even;
+    int cta0[FDAS_TC_STEP_TABLES];
     int trim;                // K steps skip the columns no template of theirs reaches (fdas_tc_trims)
     int tiles_per_series;    // ceil(M / 128): plane-free search numbers the tiles series * tiles_per_series + tile
     int clustered;           // recheck launch with more than one template group: the groups of one item form a cluster
@@ -133,13 +140,54 @@ static inline void tc_fill_params(const fdas_plan *p, TcParams &tp, const void *
     tp.NT = p->tc_NT;
     tp.nzg = p->tc_nzg;
     tp.full_chunks = p->tc_full_chunks;
-    for (int g = 0; g < FDAS_TC_STEP_TABLES; ++g)
+    for (int g = 0; g < FDAS_TC_STEP_TABLES; ++g) {
         for (int i = 0; i < FDAS_TC_MAX_KS; ++i) tp.steps[g][i] = p->tc_steps[g][i];
+        tp.nsteps[g] = p->tc_nsteps[g];
+        tp.cta0[g] = 0;
+    }
+    tp.groups = p->tc_groups;
+    tp.cta_even = 1;
     tp.trim = fdas_tc_trims(p, planes == nullptr);
     tp.tiles_per_series = (int)((p->M + 127) / 128);
     tp.clustered = 0;
     tp.search = fdas_search_args{};
     tp.search.cand_span = 8;
+}
+
+// CTAs of a TB_PLANE / TB_SCAN launch over `items` work items per template group: total returned, tp.cta0 / cta_even
+// filled.  Up to 8 groups share the SMs in proportion to their cost per tile (tensor work or plane stores, whichever
+// bounds the group), at least one CTA and at most `items` each; more groups get the same number each.
+static inline unsigned fdas_tc_split_ctas(const fdas_plan *p, TcParams &tp, long long items)
+{
+    const int G = p->tc_groups;
+    const int even = p->num_sms / G > 0 ? p->num_sms / G : 1;
+    tp.cta_even = (int)(items < even ? items : even);
+    if (G > FDAS_TC_STEP_TABLES - 1) return (unsigned)tp.cta_even * (unsigned)G;
+    // cost of a tile: its MMAs (three products per tap in the split form) or, if that takes longer, its plane rows at
+    // one SM's share of the store rate (~25 cycles per 512-byte row segment: config 3 is store-bound at 97 rows in
+    // 2400 cycles); a plane-free launch stores nothing
+    const double per_row = tp.planes ? (p->plane_bf16 ? 12.5 : 25.0) : 0.0, products = p->precision == FDAS_F32 ? 3.0 : 1.0;
+    double cost[FDAS_TC_STEP_TABLES - 1], total = 0.0;
+    for (int g = 0; g < G; ++g) {
+        const double mma = products * p->tc_cost[g], store = per_row * p->tc_rows[g];
+        cost[g] = mma > store ? mma : store;
+        total += cost[g];
+    }
+    int n[FDAS_TC_STEP_TABLES - 1], sum = 0;
+    for (int g = 0; g < G; ++g) {
+        n[g] = (int)(p->num_sms * cost[g] / total);
+        if (n[g] < 1) n[g] = 1;
+        sum += n[g];
+    }
+    for (int g = 0; sum < p->num_sms && G <= p->num_sms; g = (g + 1) % G, ++sum) n[g] += 1;   // rounding leftovers
+    for (int g = 0; sum > p->num_sms && g < G; ++g)
+        while (n[g] > 1 && sum > p->num_sms) { n[g] -= 1; sum -= 1; }
+    tp.cta0[0] = 0;
+    for (int g = 0; g < G; ++g) {
+        if (n[g] > items) n[g] = (int)items;
+        tp.cta0[g + 1] = tp.cta0[g] + n[g];
+    }
+    return (unsigned)tp.cta0[G];
 }
 
 // What a launch of fdas_mma_bulk_kernel does with the powers (template parameter MODE):
@@ -184,6 +232,41 @@ __device__ __forceinline__ uint32_t tb_items(const TcParams &p)
     } else {
         return (uint32_t)p.batch * (uint32_t)p.n_blocks;
     }
+}
+// This CTA's template group, its index among the CTAs of that group and their number (TcParams::cta0).  Only the
+// group is kept in a register: x and nx are re-read from the constant bank where they are used (once per work item) --
+// held in registers they cost the float-plane kernel a spill in its epilogue (96-register cap; 0.300 -> 0.309 ms).
+struct TbCta {
+    int grp;
+    template <int MODE>
+    __device__ __forceinline__ uint32_t x(const TcParams &p) const
+    {
+        if constexpr (MODE == TB_RECHECK) return blockIdx.x;
+        else if (p.groups <= FDAS_TC_STEP_TABLES - 1) return blockIdx.x - (uint32_t)p.cta0[grp];
+        else return blockIdx.x % (uint32_t)p.cta_even;
+    }
+    template <int MODE>
+    __device__ __forceinline__ uint32_t nx(const TcParams &p) const
+    {
+        if constexpr (MODE == TB_RECHECK) return gridDim.x;
+        else if (p.groups <= FDAS_TC_STEP_TABLES - 1) return (uint32_t)(p.cta0[grp + 1] - p.cta0[grp]);
+        else return (uint32_t)p.cta_even;
+    }
+};
+template <int MODE>
+__device__ __forceinline__ TbCta tb_cta(const TcParams &p)
+{
+    TbCta c;
+    if constexpr (MODE == TB_RECHECK) {
+        c.grp = (int)blockIdx.y;
+    } else if (p.groups <= FDAS_TC_STEP_TABLES - 1) {
+        int g = 0;
+        while (g + 1 < p.groups && (int)blockIdx.x >= p.cta0[g + 1]) ++g;
+        c.grp = g;
+    } else {
+        c.grp = (int)(blockIdx.x / (uint32_t)p.cta_even);
+    }
+    return c;
 }
 // TB_RECHECK: the epilogue threads meet here twice per work item: once when the item's powers are in scratch, once
 // when they have been tested.  One template group: a named barrier over the epilogue warps only, so the loader and
@@ -506,13 +589,16 @@ __device__ __forceinline__ void umma_commit_elected(uint32_t bar, uint32_t elect
 template <int NT, int SPLIT = 1, int MODE = TB_PLANE>
 __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, uint32_t off_z, uint32_t z_buf_bytes,
                                            uint32_t z_part_bytes, uint32_t z_full, uint32_t z_empty, uint32_t t_full,
-                                           uint32_t t_empty, uint32_t tmem_base, uint32_t n_items)
+                                           uint32_t t_empty, uint32_t tmem_base, uint32_t n_items, TbCta cta)
 {
     // K steps run in the same order in every launch (the sums must agree bit for bit between fdas_convolve and the
     // plane-free search): the full-width step holding tap 0 first -- it initialises every column -- then on through
     // the taps, wrapping round (p.steps[] lists them in that order, fdas_mma_plan).  p.trim: a step multiplies only the
     // columns whose templates reach it, i.e. uses the table's instruction descriptor (fdas_tc_trims decides per launch).
-    const int grp = blockIdx.y;
+    // (uniform in the compiler's eyes, see below)
+    const int grp = (int)__reduce_max_sync(0xffffffffu, (unsigned)cta.grp);
+    const uint32_t cta_x = __reduce_max_sync(0xffffffffu, cta.x<MODE>(p)), cta_nx = __reduce_max_sync(0xffffffffu, cta.nx<MODE>(p));
+    const int KSg = p.nsteps[grp < FDAS_TC_STEP_TABLES - 1 ? grp : FDAS_TC_STEP_TABLES - 1];   // K steps of this group
     const unsigned long long *const steps = p.steps[grp < FDAS_TC_STEP_TABLES - 1 ? grp : FDAS_TC_STEP_TABLES - 1];
     constexpr uint32_t b_lbo = (uint32_t)NT * 16u;   // next 8-tap chunk of the tap matrix
     const uint32_t elected = elect_one();
@@ -540,14 +626,14 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
     // TB_RECHECK: the items are separated by barriers the loader and (clustered) this warp take part in, so nothing
     // of the next item is waited for early there
     constexpr bool AHEAD_ITEM = MODE != TB_RECHECK;
-    if (blockIdx.x >= n_items) return;
+    if (cta_x >= n_items) return;
     // Tiles of an item.  Everything the issue loop branches on must be warp-uniform IN THE COMPILER'S EYES: the
     // descriptors live in uniform registers, and one branch on a value held in a vector register drags every
     // loop-carried descriptor into vector registers at the price of a R2UR per MMA operand (measured: 1120 -> 1360
     // cycles per tile).  The tile counts therefore pass through a warp reduction (REDUX writes a uniform register);
     // the block index inside the series is tracked by subtraction instead of it % n_blocks (no division between MMAs).
     n_items = __reduce_max_sync(0xffffffffu, n_items);
-    uint32_t blk_cur = blockIdx.x;
+    uint32_t blk_cur = cta_x;
     auto blk_wrap = [&](uint32_t b) {
         while (b >= (uint32_t)p.n_blocks) b -= (uint32_t)p.n_blocks;
         return b;
@@ -567,7 +653,7 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
     auto wait_stage = [&](uint32_t tt) { mbar_wait(t_empty + 8 * (tt & 1), ((tt >> 1) & 1) ^ 1); };
     auto wait_z = [&](uint32_t nn) { mbar_wait(z_full + 8 * (nn & 1), (nn >> 1) & 1); };
     // the tile being issued: item `it` (the n-th of this CTA, `n_tiles` tiles), tile `tile` of it, the t-th tile overall
-    uint32_t it = blockIdx.x, n = 0, t = 0;
+    uint32_t it = cta_x, n = 0, t = 0;
     int tile = 0, n_tiles = tiles_of(it, blk_cur), n_tiles_next = 0;
     uint32_t z_addr = s_base + off_z;
     wait_z(0);
@@ -579,13 +665,13 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
         const uint32_t stage = t & 1;
         issue_step(d_re, d_re + NT, a_re, a_im, 0, 0);
         // the next item's tile count, early in the current item
-        const bool has_next = it + gridDim.x < n_items;
+        const bool has_next = it + cta_nx < n_items;
         if (tile == 0 && has_next) {
-            blk_cur = blk_wrap(blk_cur + gridDim.x);
-            n_tiles_next = tiles_of(it + gridDim.x, blk_cur);
+            blk_cur = blk_wrap(blk_cur + cta_nx);
+            n_tiles_next = tiles_of(it + cta_nx, blk_cur);
         }
 #pragma unroll 2
-        for (int i = 1; i + 1 < p.KS; ++i) issue_step(d_re, d_re + NT, a_re, a_im, i, 1);
+        for (int i = 1; i + 1 < KSg; ++i) issue_step(d_re, d_re + NT, a_re, a_im, i, 1);
         // ---- ahead of the last K step: the next tile's operands, and what it waits for
         const bool item_ends = tile + 1 == n_tiles;
         bool more = true, late_waits = false;
@@ -607,7 +693,7 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
         const uint32_t nd_re = tmem_base + ((t + 1) & 1) * TC_STAGE_COLS;
         const uint32_t na_re = smem_desc_lo(nz_addr + (uint32_t)(ntile * TC_TILE) * 16u, 128u);
         const uint32_t na_im = smem_desc_lo(nz_addr + z_part_bytes + (uint32_t)(ntile * TC_TILE) * 16u, 128u);
-        if (p.KS > 1) issue_step(d_re, d_re + NT, a_re, a_im, p.KS - 1, 1);
+        if (KSg > 1) issue_step(d_re, d_re + NT, a_re, a_im, KSg - 1, 1);
         umma_commit_elected(t_full + 8 * stage, elected);
         if (item_ends) {
             umma_commit_elected(z_empty + 8 * (n & 1), elected);
@@ -618,7 +704,7 @@ __device__ __forceinline__ void mma_issuer(const TcParams &p, uint32_t s_base, u
                 }
             }
             if (!more) break;
-            it += gridDim.x;
+            it += cta_nx;
             n += 1;
             n_tiles = n_tiles_next;
         }
@@ -672,14 +758,14 @@ template <int SPLIT = 1, int MODE = TB_PLANE>
 __device__ __forceinline__ void spectrum_loader(const TcParams &p, unsigned char *smem, uint32_t off_xs,
                                                 uint32_t xs_part_bytes, uint32_t xn, uint32_t off_z, uint32_t z_buf_bytes,
                                                 uint32_t z_part_bytes, uint32_t zr, uint32_t z_full, uint32_t z_empty,
-                                                int lt, uint32_t n_items, float2 (&a)[TC_LD_ITERS], float2 (&b)[TC_LD_ITERS])
+                                                int lt, uint32_t n_items, TbCta cta, float2 (&a)[TC_LD_ITERS], float2 (&b)[TC_LD_ITERS])
 {
     // sample planes: re, im of the bf16 spectrum; SPLIT == 3 adds re, im of the rounded residual (parts 2, 3)
     constexpr int NP = SPLIT == 3 ? 4 : 2;
     uint32_t *xs_re = reinterpret_cast<uint32_t *>(smem + off_xs);
     uint32_t *xs_im = reinterpret_cast<uint32_t *>(smem + off_xs + xs_part_bytes);
     uint32_t n = 0;   // a, b: the first item's samples, fetched by the kernel before its set-up (tb_first_fetch)
-    for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x, ++n) {
+    for (uint32_t it = cta.x<MODE>(p); it < n_items; it += cta.nx<MODE>(p), ++n) {
         const uint32_t buf = n & 1, zuse = n >> 1;
         // phase A: spectrum block -> bf16 (round-to-nearest-even), re and im planes
 #pragma unroll
@@ -695,7 +781,7 @@ __device__ __forceinline__ void spectrum_loader(const TcParams &p, unsigned char
             }
         }
         named_bar_sync(1, TC_LOAD_THREADS);
-        if (it + gridDim.x < n_items) loader_fetch<MODE>(p, it + gridDim.x, xn, lt, a, b);
+        if (it + cta.nx<MODE>(p) < n_items) loader_fetch<MODE>(p, it + cta.nx<MODE>(p), xn, lt, a, b);
         mbar_wait<64>(z_empty + 8 * buf, (zuse & 1) ^ 1);
         // phase B: Z row i = samples i .. i+7 (16 bytes), for every part.  A thread builds the row pair (2q, 2q+1)
         // from the five words xs[q .. q+4] (the odd row is the even one shifted by one sample); the loads of TC_LD_PAIRS
@@ -756,7 +842,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1) fdas_mma_convolve_kernel(const 
     constexpr int NT = 16 * NCH;
     const TcSmem L(p.R, p.KS, NT);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int grp = blockIdx.y;
+    const TbCta cta = tb_cta<TB_PLANE>(p);
+    const int grp = cta.grp;
     const uint32_t n_items = (uint32_t)p.batch * (uint32_t)p.n_blocks;
 
     const uint32_t s_base = smem_u32(smem);
@@ -770,8 +857,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1) fdas_mma_convolve_kernel(const 
     // the loader warps put the global loads of their first item in flight before the set-up: its latency hides behind
     // the tap-matrix copy and the TMEM allocation (a launch of config 1 is 10 us long, the set-up 3 of them)
     float2 first_a[TC_LD_ITERS], first_b[TC_LD_ITERS];
-    if (warp >= TC_LOAD_WARP0 && blockIdx.x < n_items)
-        loader_fetch<TB_PLANE>(p, blockIdx.x, L.xn, threadIdx.x - TC_LOAD_WARP0 * 32, first_a, first_b);
+    if (warp >= TC_LOAD_WARP0 && cta.x<TB_PLANE>(p) < n_items)
+        loader_fetch<TB_PLANE>(p, cta.x<TB_PLANE>(p), L.xn, threadIdx.x - TC_LOAD_WARP0 * 32, first_a, first_b);
     // ---- one-time setup: tap matrix image and row-offset table -> shared memory, barriers, TMEM
     {
         const uint4 *src = p.bmat + (size_t)grp * (L.b_bytes / 16);
@@ -785,7 +872,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) fdas_mma_convolve_kernel(const 
         }
         fence_proxy_async();   // the tap matrix is read by the tensor core (async proxy)
     }
-    if (threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0 && p.search.enabled) {
+    if (threadIdx.x == 0 && blockIdx.x == 0 && p.search.enabled) {
         *p.search.cand_count_next = 0;   // the other counter: nobody appends to it during this launch
         *p.search.count_out = 0;         // written by the resolve kernel that follows in stream order
     }
@@ -811,7 +898,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) fdas_mma_convolve_kernel(const 
         const float thr = p.search.enabled ? p.search.thr : __int_as_float(0x7f800000);
         const int zi_group0 = grp * p.nzg;
         uint32_t t = 0;
-        for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
+        for (uint32_t it = cta.x<TB_PLANE>(p); it < n_items; it += cta.nx<TB_PLANE>(p)) {
             const long long ser = it / (uint32_t)p.n_blocks;   // 32-bit division: items < 2^31 (checked by the launcher)
             const long long blk0 = (long long)(it % (uint32_t)p.n_blocks) * p.R;
             const long long left = p.M - blk0;
@@ -836,11 +923,11 @@ __global__ void __launch_bounds__(TC_THREADS, 1) fdas_mma_convolve_kernel(const 
     } else if (warp == TC_MMA_WARP) {
         // =========================== MMA issuer ===========================
         mma_issuer<NT, 1, TB_PLANE>(p, s_base, L.off_z, L.z_buf_bytes, L.z_part_bytes, z_full, z_empty, t_full, t_empty,
-                                    __shfl_sync(0xffffffffu, tmem_base, 0), n_items);
+                                    __shfl_sync(0xffffffffu, tmem_base, 0), n_items, cta);
     } else {
         // =========================== loader ===========================
         spectrum_loader(p, smem, L.off_xs, L.xs_part_bytes, L.xn, L.off_z, L.z_buf_bytes, L.z_part_bytes, L.zr, z_full,
-                        z_empty, threadIdx.x - TC_LOAD_WARP0 * 32, n_items, first_a, first_b);
+                        z_empty, threadIdx.x - TC_LOAD_WARP0 * 32, n_items, cta, first_a, first_b);
     }
 
     tc_fence_before();
@@ -996,9 +1083,10 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
     constexpr uint32_t ROWB = TC_TILE * sizeof(OT);   // bytes of one staging row
     // recheck launch of a single template group: the strip lives in shared memory (no scratch round trip through L2)
     const bool smem_strip = MODE == TB_RECHECK && gridDim.y == 1;
+    const TbCta cta = tb_cta<MODE>(p);
     const TbSmem L(p.R, p.KS, NT, ROWB, SPLIT, MODE != TB_SCAN, smem_strip ? p.K : 0);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int grp = blockIdx.y;
+    const int grp = cta.grp;
     if (MODE == TB_RECHECK) asm volatile("griddepcontrol.wait;" ::: "memory");   // the scan launch has listed its tiles
     const uint32_t n_items = tb_items<MODE>(p);
     if (MODE == TB_RECHECK && blockIdx.x >= n_items) return;   // nothing flagged for this CTA (its whole cluster: same x)
@@ -1010,23 +1098,23 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
 
     // the loader warps put the global loads of their first item in flight before the set-up (see fdas_mma_convolve_kernel)
     float2 first_a[TC_LD_ITERS], first_b[TC_LD_ITERS];
-    if (warp >= TB_LOAD_WARP0 && blockIdx.x < n_items)
-        loader_fetch<MODE>(p, blockIdx.x, L.xn, threadIdx.x - TB_LOAD_WARP0 * 32, first_a, first_b);
+    if (warp >= TB_LOAD_WARP0 && cta.x<MODE>(p) < n_items)
+        loader_fetch<MODE>(p, cta.x<MODE>(p), L.xn, threadIdx.x - TB_LOAD_WARP0 * 32, first_a, first_b);
     // ---- one-time setup: tap matrix image -> shared memory, barriers, TMEM
     {
         // tap-matrix image(s) of this template group: bmat is [image][group][...]
         uint4 *dst = reinterpret_cast<uint4 *>(smem);
         for (int img = 0; img < (SPLIT == 3 ? 2 : 1); ++img) {
-            const uint4 *src = p.bmat + ((size_t)img * gridDim.y + grp) * (L.b_bytes / 16);
+            const uint4 *src = p.bmat + ((size_t)img * p.groups + grp) * (L.b_bytes / 16);
             for (uint32_t i = threadIdx.x; i < L.b_bytes / 16; i += TB_THREADS) dst[img * (L.b_bytes / 16) + i] = __ldg(src + i);
         }
         fence_proxy_async();
     }
-    if (MODE == TB_PLANE && threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0 && p.search.enabled) {
+    if (MODE == TB_PLANE && threadIdx.x == 0 && blockIdx.x == 0 && p.search.enabled) {
         *p.search.cand_count_next = 0;
         *p.search.count_out = 0;
     }
-    if (MODE == TB_SCAN && blockIdx.x == 0 && blockIdx.y == 0) {
+    if (MODE == TB_SCAN && blockIdx.x == 0) {
         if (threadIdx.x == 0) *p.search.tile_count_next = 0;
         for (int i = threadIdx.x; i < p.batch; i += TB_THREADS) p.search.counts[i] = 0;
     }
@@ -1066,7 +1154,7 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
         // of its staging block, for thousands of cycles)
         const int4 rg2[2] = {p.ranges[grp * TB_CGROUPS + 2 * half], p.ranges[grp * TB_CGROUPS + 2 * half + 1]};
         uint32_t t = 0;
-        for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
+        for (uint32_t it = cta.x<MODE>(p); it < n_items; it += cta.nx<MODE>(p)) {
             long long ser, blk0;
             int n_tiles, centre;
             tb_item<MODE>(p, it, ser, blk0, n_tiles, centre);
@@ -1358,11 +1446,11 @@ fdas_mma_bulk_kernel(const TcParams p, const __grid_constant__ TbMaps maps)
     } else if (warp == TB_MMA_WARP) {
         // =========================== MMA issuer ===========================
         mma_issuer<NT, SPLIT, MODE>(p, s_base, L.off_z, L.z_buf_bytes, L.z_part_bytes, z_full, z_empty, t_full, t_empty,
-                                    __shfl_sync(0xffffffffu, tmem_base, 0), n_items);
+                                    __shfl_sync(0xffffffffu, tmem_base, 0), n_items, cta);
     } else {
         // =========================== loader ===========================
         spectrum_loader<SPLIT, MODE>(p, smem, L.off_xs, L.xs_part_bytes, L.xn, L.off_z, L.z_buf_bytes, L.z_part_bytes, L.zr,
-                                     z_full, z_empty, threadIdx.x - TB_LOAD_WARP0 * 32, n_items, first_a, first_b);
+                                     z_full, z_empty, threadIdx.x - TB_LOAD_WARP0 * 32, n_items, cta, first_a, first_b);
     }
 
     tc_fence_before();

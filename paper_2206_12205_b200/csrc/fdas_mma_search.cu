@@ -27,7 +27,7 @@ int launch_mode(fdas_plan *p, const TcParams &tp, unsigned gx, size_t smem_bytes
                                      : (SPLIT == 3 ? FDAS_OPTIN_MMA_RECHECK_SPLIT : FDAS_OPTIN_MMA_RECHECK);
     { const int rc = fdas_optin_smem(p, slot, kern, smem_bytes); if (rc) return rc; }
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(gx, p->tc_groups);
+    cfg.gridDim = MODE == TB_RECHECK ? dim3(gx, p->tc_groups) : dim3(gx);   // scan: one-dimensional, every group's CTAs (TcParams::cta0)
     cfg.blockDim = dim3(tb_threads(SPLIT));
     cfg.dynamicSmemBytes = smem_bytes;
     cfg.stream = st;
@@ -94,8 +94,12 @@ int fdas_tc_describe_noplane(fdas_plan *p, int batch, fdas_kernel_info_t *out)
     out->nch = p->tc_NT / 16;
     out->k_steps = p->tc_KS;
     out->work_item_bins = R;
-    out->grid_x = (int32_t)(items < sms_per_group ? items : sms_per_group);
-    out->grid_y = p->tc_groups;
+    {
+        TcParams tp;
+        tc_fill_params(p, tp, nullptr, nullptr, batch, R);
+        out->grid_x = (int32_t)fdas_tc_split_ctas(p, tp, items);
+        out->grid_y = 1;
+    }
     out->block_threads = tb_threads(split);
     out->dynamic_smem_bytes = TbSmem(R, p->tc_KS, p->tc_NT, TC_TILE * 4, split, false).total;
     out->tensor_flops = fdas_tc_issued_flops(p, batch, 1);
@@ -200,7 +204,7 @@ int fdas_noplane_scan(fdas_plan *p, const void *spectra, int batch, const fdas_s
     tp.search = *sa;
     const long long items = (long long)batch * tp.n_blocks;
     if (items >= 0x7FFFFFFFLL) return FDAS_ERR_UNSUPPORTED;
-    const unsigned gx = (unsigned)(items < sms_per_group ? items : sms_per_group);
+    const unsigned gx = fdas_tc_split_ctas(p, tp, items);
     const TbMaps *maps = static_cast<const TbMaps *>(p->tf_maps);
     return split == 3 ? launch_nch<3, TB_SCAN>(p, tp, gx, total, maps, st) : launch_nch<1, TB_SCAN>(p, tp, gx, total, maps, st);
 }
