@@ -333,23 +333,6 @@ __device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t cols)
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(cols) : "memory");
 }
 
-// D[tmem] (+)= A[smem desc] * B[smem desc]^T, bf16 x bf16 -> fp32, M = 128, K = 16
-__device__ __forceinline__ void umma_bf16(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc,
-                                          uint32_t accumulate)
-{
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "setp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-        ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
-        : "memory");
-}
-// arrives on the mbarrier once every tcgen05.mma issued so far by this thread has completed
-__device__ __forceinline__ void umma_commit(uint32_t bar)
-{
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
-}
-
 // TMEM -> registers: this warp's 32 lanes x 16 columns at taddr_a (v[0..15]) and at taddr_b
 // (v[16..31]).  Asynchronous: v[] is defined only after tmem_ld_wait(v), which names the same
 // registers as in/out operands so that no use can be scheduled before tcgen05.wait::ld.
@@ -380,13 +363,8 @@ __device__ __forceinline__ void tmem_ld_wait(uint32_t *v)
 // K-major, non-swizzled shared-memory matrix descriptor (cute::UMMA::SmemDescriptor layout):
 // bits [0,14) address >> 4, [16,30) leading byte offset >> 4 (between the two 8-element K
 // chunks of one MMA), [32,46) stride byte offset >> 4 (between 8-row groups), bit 46 version.
-__device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo_bytes, uint32_t sbo_bytes)
-{
-    return (uint64_t)((addr >> 4) & 0x3FFFu) | ((uint64_t)((lbo_bytes >> 4) & 0x3FFFu) << 16) |
-           ((uint64_t)((sbo_bytes >> 4) & 0x3FFFu) << 32) | (1ull << 46);
-}
-// the same descriptor as two words: every operand of these kernels has stride byte offset 128 (consecutive 8-row
-// groups are adjacent), so the high word is one constant
+// Held as two words: every operand of these kernels has stride byte offset 128 (consecutive 8-row groups are adjacent),
+// so the high word is one constant and the low word carries the address and the leading byte offset
 constexpr uint32_t TC_DESC_HI = (128u >> 4) | (1u << 14);
 __device__ __forceinline__ uint32_t smem_desc_lo(uint32_t addr, uint32_t lbo_bytes)
 {
