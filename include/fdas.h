@@ -468,10 +468,11 @@ typedef struct {
     int32_t algorithm;         /* FDAS_ALGO_FFT, FDAS_ALGO_MMA or FDAS_ALGO_MMA_SCALAR                               */
     int32_t split;             /* tensor-core forms: 1 = bf16 operands, 3 = fp32 operands as 3 products of bf16 terms;
                                   0 = FFT form                                                                      */
-    int32_t groups;            /* template groups (grid y)                                                          */
+    int32_t groups;            /* template groups (more than one when the bank holds more than 128 templates)       */
     int32_t nch, k_steps;      /* tensor-core forms: UMMA N = 16 nch columns per part, K steps of 16 taps           */
     int32_t work_item_bins;    /* bins per work item (tensor-core forms) / valid bins per segment (FFT form)        */
-    int32_t grid_x, grid_y, block_threads;
+    int32_t grid_x, grid_y, block_threads;   /* tensor-core forms: a one-dimensional grid, the template groups share
+                                                its CTAs in proportion to their work per tile (grid_y = 1)             */
     size_t dynamic_smem_bytes;
     double tensor_flops;       /* dense MMA flops the launch issues, padding included (0 for the FFT form)          */
     char kernel[128];          /* kernel name with its template arguments                                           */
