@@ -96,3 +96,34 @@ def test_search_host_batched_equals_per_series_search(F, prec):
     rows = {(int(a), int(b)) for a, b, _ in peaks[0, :counts[0]]}
     assert (6, 3000) in rows
     assert F.fdas_search_host_batched(plan._h, X.ctypes.data, 0, 12.0, peaks.ctypes.data, cap, counts.ctypes.data) == F.FDAS_ERR_INVALID_ARG
+
+
+def test_describe_convolve_counts_the_issued_tensor_work(F):
+    # fdas_describe_convolve is what bench.py reads its kernel names, grids and tensor flops from: the counts must be
+    # the launcher's.  Config-3 bank (49 |z| entries -> 112 columns, 129 taps -> 9 K steps): a full-width launch issues
+    # tiles x 2 parts x 9 steps x 2*128*112*16 flops; a trimmed one multiplies 32, 64, 96, 112, 112, 112, 80, 48, 16
+    # columns in its 9 steps (the templates that reach the step: half-width |z|/2 + 16 taps).
+    import torch
+    N = 1 << 20
+    M = N // 2
+    tiles = M // 128
+    full = tiles * 2 * 9 * 2.0 * 128 * 112 * 16
+    trimmed = tiles * 2 * 2.0 * 128 * 16 * (32 + 64 + 96 + 112 + 112 + 112 + 80 + 48 + 16)
+    plan = F.Plan(N, 96.0, 2.0, 2048, "bf16")
+    plane = torch.empty((plan.K, plan.M), dtype=torch.float32, device="cuda")
+    d = plan.describe(plane)
+    assert d["algorithm"] == "mma" and d["split"] == 1 and d["nch"] == 7 and d["k_steps"] == 9 and d["groups"] == 1
+    assert d["kernel"] == "fdas_mma_bulk_kernel<7, float, 1>" and d["grid_y"] == 1 and 1 <= d["grid_x"] <= 1024
+    assert d["tensor_flops"] == full                       # float plane, 97 templates: store-bound, every step at full width
+    assert plan.describe(None)["tensor_flops"] == trimmed  # scan launch of the plane-free search
+    p16 = F.Plan(N, 96.0, 2.0, 2048, "bf16", plane="bf16")
+    assert p16.describe(torch.empty((p16.K, p16.M), dtype=torch.bfloat16, device="cuda"))["tensor_flops"] == trimmed
+    p32 = F.Plan(N, 96.0, 2.0, 2048, "f32")
+    d32 = p32.describe(plane)
+    assert d32["split"] == 3 and d32["tensor_flops"] == 3 * trimmed
+    # two template groups (201 templates): one grid for both, the group of narrow templates skips the K steps none of
+    # its templates reaches, so the launch issues less than groups x full
+    p5 = F.Plan(1 << 18, 200.0, 2.0, 4096, "f32")
+    d5 = p5.describe(torch.empty((p5.K, p5.M), dtype=torch.float32, device="cuda"))
+    assert d5["groups"] == 2 and d5["grid_y"] == 1 and d5["k_steps"] == 15
+    assert d5["tensor_flops"] < 0.75 * 3 * 2 * ((1 << 17) // 128) * 2 * 15 * 2.0 * 128 * d5["nch"] * 16 * 16
