@@ -405,6 +405,24 @@ def main():
             xo = torch.empty(M, dtype=torch.complex64, device="cuda")
             extra["rfft_ms"] = float(np.mean(timer(lambda: plan.spectrum(ts, xo, stream=sptr), 5, warm=1)))
             del ts, xo
+            # NEXT-4: the jerk search as a volume: 5 slabs w = -8..8 of the same bank on the same spectrum,
+            # every slab convolved and the 26-neighbour peak rule applied over (w, z, r), one library call
+            with torch.cuda.stream(stream):
+                vol = fdas.Volume(w.N, ZMAX, DZ, 8.0, 4.0, SEGLEN, "bf16", stream=sptr)
+            vbuf = torch.empty((vol.W, vol.K, vol.M), dtype=torch.float32, device="cuda")
+            vpk = torch.empty(4 * PEAK_CAPACITY, dtype=torch.int32, device="cuda")
+            vct = torch.zeros(1, dtype=torch.int32, device="cuda")
+
+            def vsearch():
+                assert fdas.fdas_volume_search(vol._v, x_dev.data_ptr(), vbuf.data_ptr(), THRESH, vpk.data_ptr(), PEAK_CAPACITY,
+                                               vct.data_ptr(), sptr) == 0
+
+            extra["volume_ms"] = float(np.mean(timer(vsearch, 3, warm=1)))
+            extra["volume_shape"] = [vol.W, vol.K, vol.M]
+            extra["volume_peaks"] = int(vct.item())
+            vol.close()
+            del vbuf, vpk, vct
+            torch.cuda.empty_cache()
         total_ms = sharding.max_over_ranks(float(sum(step_ms)), device="cuda")
         n_found = int(count_dev.item())
         res = dict(K=K, M=M, S=S, V=V, conv_ms=float(np.mean(conv_ms)), conv_ms_min=float(np.min(conv_ms)),
@@ -522,6 +540,10 @@ def main():
         "real_fft": {"ms": r["rfft_ms"], "algorithmic_gbs": 6.0 * 4 * M / (r["rfft_ms"] * 1e-3) / 1e9,
                      "note": "NEXT-4: fdas_spectrum, fp32 real FFT of the 2^23-sample series (outside the timed step, as in the paper); "
                              "bytes = series read + spectrum written"},
+        "jerk_volume_search": {"ms": r["volume_ms"], "shape_w_k_m": r["volume_shape"], "peaks_found": r["volume_peaks"],
+                               "points_per_s": float(np.prod(r["volume_shape"])) / (r["volume_ms"] * 1e-3),
+                               "note": "NEXT-4: fdas_volume_search, bf16: 5 jerk slabs (w = -8..8 step 4) x 97 templates x 2^22 bins, float volume "
+                                       "written + 26-neighbour peak rule over (w, z, r)"},
     }
 
     cpu = None

@@ -181,6 +181,9 @@ int fdas_launch_convolve_mma(fdas_plan *p, const void *spectra, void *planes, in
 int fdas_launch_search_noplane(fdas_plan *p, const void *spectra, int batch, float thr, fdas_peak_t *peaks, int capacity,
                                int *counts, cudaStream_t st);
 // the same in steps (fdas_mma_search.cu): begin, scan launches over block ranges, one recheck launch
+int fdas_launch_resolve3(fdas_plan *p, const void *volume, int n_slabs, int slab, const fdas_search_args &sa, fdas_peak3_t *peaks,
+                         int capacity, int *count, cudaStream_t st);
+int fdas_search_prepare(fdas_plan *p, float thr, int *count_dev, cudaStream_t st, fdas_search_args *sa);   // fdas_plan.cu
 int fdas_noplane_block_bins(const fdas_plan *p, int batch);
 int fdas_noplane_begin(fdas_plan *p, int batch, float thr, fdas_peak_t *peaks, int capacity, int *counts, cudaStream_t st,
                        fdas_search_args *out);

@@ -195,7 +195,52 @@ fdas_peaks3_kernel(const PT *__restrict__ V, int W, int K, long long M, float th
     }
 }
 
+// fdas_volume_search on the tensor-core path: slab i's convolve launch flagged its candidates exactly as for
+// fdas_search; each candidate cell is read back from the volume just written and tested against its 26 neighbours
+// (slabs i - 1 and i + 1 are complete: every slab is convolved before the first slab is resolved).  If the slab's
+// candidate buffer overflowed, the whole slab is scanned instead (same result).  Nothing re-reads the volume.
+template <typename PT>
+__global__ void __launch_bounds__(256)
+fdas_resolve3_kernel(const PT *__restrict__ V, int W, int K, long long M, int slab, float thr, const fdas_peak_t *__restrict__ cand,
+                     const int *__restrict__ cand_count, int cand_capacity, int span, const int2 *__restrict__ ktab, int nzg,
+                     fdas_peak3_t *peaks, int capacity, int *count)
+{
+    const int n = *cand_count;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const PT *S = V + (size_t)slab * K * M;
+    if (n <= cand_capacity) {
+        const int cells = 2 * span;
+        for (long long i = tid; i < (long long)cells * n; i += stride) {
+            const fdas_peak_t c = cand[i / cells];
+            const int zi = c.z_index + (int)((i % cells) >> 1);
+            if (zi >= (c.z_index / nzg + 1) * nzg) continue;      // past the end of this template group
+            const int2 kk = ktab[zi];
+            const int k = (i & 1) ? kk.y : kk.x;
+            if (k < 0 || ((i & 1) && kk.y == kk.x)) continue;      // no such row / z = 0 listed twice
+            test_cell3<PT>(V, W, K, M, slab, k, c.r, elem<PT>::val(S[(size_t)k * M + c.r]), thr, peaks, capacity, count);
+        }
+        return;
+    }
+    const long long total = (long long)K * M;
+    for (long long e = tid; e < total; e += stride) {
+        const int k = (int)(e / M);
+        test_cell3<PT>(V, W, K, M, slab, k, e - (long long)k * M, elem<PT>::val(S[e]), thr, peaks, capacity, count);
+    }
+}
+
 }  // namespace
+
+int fdas_launch_resolve3(fdas_plan *p, const void *volume, int n_slabs, int slab, const fdas_search_args &sa, fdas_peak3_t *peaks,
+                         int capacity, int *count, cudaStream_t st)
+{
+    const int grid = p->num_sms * 2;
+    fdas_resolve3_kernel<float><<<grid, 256, 0, st>>>((const float *)volume, n_slabs, p->K, p->M, slab, sa.thr, sa.cand, sa.cand_count,
+                                                      sa.cand_capacity, sa.cand_span, p->tc_ktab, p->tc_nzg, peaks, capacity, count);
+    FDAS_CUDA_TRY(p, cudaGetLastError());
+    p->launches += 1;
+    return FDAS_OK;
+}
 
 int fdas_launch_peaks3(fdas_plan *p, const void *volume, int n_slabs, float thr, fdas_peak3_t *peaks, int capacity, int *count,
                        cudaStream_t st)

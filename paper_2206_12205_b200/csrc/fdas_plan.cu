@@ -270,19 +270,11 @@ extern "C" int fdas_peaks(fdas_plan_t *p, const void *plane_dev, float threshold
                              (cudaStream_t)stream);
 }
 
-// fdas_search: convolve + peaks.  On the tensor-core path the convolve epilogue flags the
-// (rare) chunks holding a power above the threshold and a small second kernel applies the
-// peak rule to those cells only, so the plane is not read back from HBM.
-static int search_on_device(fdas_plan *p, const void *spectrum_dev, void *plane_dev, float threshold,
-                            fdas_peak_t *peaks_dev, int capacity, int *count_dev, cudaStream_t st)
+// The arguments of a convolve launch with the fused threshold test (fdas_search, fdas_volume_search): the plan's
+// candidate buffer and its two counters, used alternately from call to call.
+int fdas_search_prepare(fdas_plan *p, float thr, int *count_dev, cudaStream_t st, fdas_search_args *sa)
 {
-    if (!plane_dev)   // plane-free form: scan launch + recheck launch (fdas_mma_search.cu)
-        return fdas_launch_search_noplane(p, spectrum_dev, 1, threshold, peaks_dev, capacity, count_dev, st);
-    if (!fdas_uses_mma(p)) {
-        int rc = fdas_launch_convolve(p, spectrum_dev, plane_dev, 1, st);
-        if (rc) return rc;
-        return fdas_launch_peaks(p, plane_dev, threshold, peaks_dev, capacity, count_dev, st);
-    }
+    *sa = fdas_search_args{};
     if (!p->cand || !p->cand_ctr) {   // both or neither: a failed second allocation must not leave a NULL counter behind
         cudaFree(p->cand);
         cudaFree(p->cand_ctr);
@@ -303,16 +295,33 @@ static int search_on_device(fdas_plan *p, const void *spectrum_dev, void *plane_
         p->cand = c;
         p->cand_ctr = ctr;
     }
-    fdas_search_args sa;
-    sa.enabled = 1;
-    sa.thr = threshold;
-    sa.cand = p->cand;
-    sa.cand_count = p->cand_ctr + (p->search_calls & 1);
-    sa.cand_count_next = p->cand_ctr + ((p->search_calls + 1) & 1);
-    sa.cand_capacity = p->cand_capacity;
-    sa.count_out = count_dev;
-    sa.cand_span = 8;   // overwritten by the convolve launch
+    sa->enabled = 1;
+    sa->thr = thr;
+    sa->cand = p->cand;
+    sa->cand_count = p->cand_ctr + (p->search_calls & 1);
+    sa->cand_count_next = p->cand_ctr + ((p->search_calls + 1) & 1);
+    sa->cand_capacity = p->cand_capacity;
+    sa->count_out = count_dev;
+    sa->cand_span = 8;   // overwritten by the convolve launch
     p->search_calls += 1;
+    return FDAS_OK;
+}
+
+// fdas_search: convolve + peaks.  On the tensor-core path the convolve epilogue flags the
+// (rare) chunks holding a power above the threshold and a small second kernel applies the
+// peak rule to those cells only, so the plane is not read back from HBM.
+static int search_on_device(fdas_plan *p, const void *spectrum_dev, void *plane_dev, float threshold,
+                            fdas_peak_t *peaks_dev, int capacity, int *count_dev, cudaStream_t st)
+{
+    if (!plane_dev)   // plane-free form: scan launch + recheck launch (fdas_mma_search.cu)
+        return fdas_launch_search_noplane(p, spectrum_dev, 1, threshold, peaks_dev, capacity, count_dev, st);
+    if (!fdas_uses_mma(p)) {
+        int rc = fdas_launch_convolve(p, spectrum_dev, plane_dev, 1, st);
+        if (rc) return rc;
+        return fdas_launch_peaks(p, plane_dev, threshold, peaks_dev, capacity, count_dev, st);
+    }
+    fdas_search_args sa;
+    { const int rc0 = fdas_search_prepare(p, threshold, count_dev, st, &sa); if (rc0) return rc0; }
     int rc = fdas_launch_convolve_mma(p, spectrum_dev, plane_dev, 1, st, &sa);   // sets sa.cand_span
     if (rc == FDAS_ERR_UNSUPPORTED && p->precision == FDAS_F32 && p->algo == FDAS_ALGO_AUTO) {
         // the split-operand kernel cannot take this plane buffer (alignment, shared memory): FFT kernel + peak pass

@@ -160,6 +160,39 @@ extern "C" int fdas_volume_search(fdas_volume_t *v, const void *spectrum_dev, vo
                                   fdas_peak3_t *peaks_dev, int capacity, int *count_dev, void *stream)
 {
     if (!v || !spectrum_dev || !volume_dev || !count_dev || capacity < 0 || (capacity > 0 && !peaks_dev)) return FDAS_ERR_INVALID_ARG;
+    if (!v->built) return FDAS_ERR_NOT_BUILT;
+    // Tensor-core slabs with a float volume: every slab's convolve launch flags its candidate cells (the fused threshold
+    // of fdas_search), then one small launch per slab applies the 26-neighbour rule to those cells only -- the volume
+    // (8 GB for 5 slabs of config 3) is not read back.  Other plans: convolve, then the full peak pass.
+    bool fused = true;
+    for (int i = 0; i < v->n_slabs; ++i) fused = fused && fdas_uses_mma(v->slabs[i]) && !v->slabs[i]->plane_bf16;
+    if (fused) {
+        cudaStream_t st = (cudaStream_t)stream;
+        const fdas_plan *p0 = v->slabs[0];
+        const size_t slab_elems = (size_t)p0->K * p0->M;
+        fdas_search_args *sa = new (std::nothrow) fdas_search_args[v->n_slabs];
+        if (!sa) return FDAS_ERR_ALLOC;
+        int rc = FDAS_OK;
+        for (int i = 0; i < v->n_slabs && rc == FDAS_OK; ++i) {
+            rc = fdas_search_prepare(v->slabs[i], threshold, count_dev, st, &sa[i]);
+            if (rc == FDAS_OK)
+                rc = fdas_launch_convolve_mma(v->slabs[i], spectrum_dev, static_cast<float *>(volume_dev) + (size_t)i * slab_elems, 1, st, &sa[i]);
+            if (rc == FDAS_ERR_UNSUPPORTED && i == 0) {   // this volume buffer cannot take the box stores (alignment): plain path
+                v->slabs[0]->search_calls -= 1;
+                fused = false;
+                rc = FDAS_OK;
+                break;
+            }
+        }
+        if (fused) {
+            // every convolve launch cleared count_dev; the resolve launches add to it
+            for (int i = 0; i < v->n_slabs && rc == FDAS_OK; ++i)
+                rc = fdas_launch_resolve3(v->slabs[i], volume_dev, v->n_slabs, i, sa[i], peaks_dev, capacity, count_dev, st);
+            delete[] sa;
+            return rc;
+        }
+        delete[] sa;
+    }
     const int rc = fdas_volume_convolve(v, spectrum_dev, volume_dev, stream);
     if (rc) return rc;
     return fdas_volume_peaks(v, volume_dev, threshold, peaks_dev, capacity, count_dev, stream);
