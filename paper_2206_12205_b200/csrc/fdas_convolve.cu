@@ -40,6 +40,7 @@ struct ConvParams {
     long long n_seg;
     int K, L, V;
     int k_per_group;
+    fdas_search_args search;   // fdas_search: the cells above the threshold are listed while they are stored (SEARCH kernels)
 };
 
 // ---- per-precision traits -------------------------------------------------------------
@@ -206,7 +207,24 @@ __device__ __forceinline__ void pass3(typename Tr::CT *re, typename Tr::CT *im, 
     Dft<typename Tr::CT, G::R3>::run(re, im);
 }
 
-template <class Tr, int S>
+// fdas_search on the FFT forms: "one of the 16 outputs of thread i0's of segment `seg` for template k exceeds the
+// threshold" -- one record per (thread, template), appended to the plan's candidate list; the resolve launch that
+// follows expands it to the thread's valid cells and applies the peak rule to those (a few thousand of 4e8 cells on
+// config 3).  The record reuses fdas_peak_t: z_index = k, r = i0 (the thread's first output index inside the
+// segment), power = the bits of seg.
+__device__ __noinline__ void flag_outputs(fdas_peak_t *cand, int *cand_count, int cand_capacity, int k, int i0, int seg)
+{
+    const int slot = atomicAdd(cand_count, 1);
+    if (slot < cand_capacity) {
+        fdas_peak_t rec;
+        rec.z_index = k;
+        rec.r = i0;
+        rec.power = __int_as_float(seg);
+        cand[slot] = rec;
+    }
+}
+
+template <class Tr, int S, bool SEARCH = false>
 __global__ void __launch_bounds__(S / 16, Geo<Tr, S>::MIN_BLOCKS) fdas_convolve_kernel(const ConvParams p)
 {
     using G = Geo<Tr, S>;
@@ -224,6 +242,10 @@ __global__ void __launch_bounds__(S / 16, Geo<Tr, S>::MIN_BLOCKS) fdas_convolve_
     CT2 *smF = reinterpret_cast<CT2 *>(smem_raw + G::XCH_ALIGNED);
 
     const int t = threadIdx.x;
+    if (SEARCH && t == 0 && blockIdx.x == 0 && blockIdx.y == 0) {
+        *p.search.cand_count_next = 0;   // the other counter: nobody appends to it during this launch
+        *p.search.count_out = 0;         // written by the resolve kernel that follows in stream order
+    }
     const long long seg = blockIdx.x % p.n_seg;
     const long long ser = blockIdx.x / p.n_seg;
     const int k_begin = blockIdx.y * p.k_per_group;
@@ -355,6 +377,15 @@ __global__ void __launch_bounds__(S / 16, Geo<Tr, S>::MIN_BLOCKS) fdas_convolve_
                     pw[u][k3] = re[s] * re[s] + im[s] * im[s];
                 }
             }
+            if constexpr (SEARCH) {
+                CT mx = 0;
+#pragma unroll
+                for (int k3 = 0; k3 < R3; ++k3) {
+                    if (vmask & (1u << k3)) mx = max(mx, pw[0][k3]);
+                    if (vmask & (1u << (R3 + k3))) mx = max(mx, pw[1][k3]);
+                }
+                if ((PT)mx > (PT)p.search.thr) flag_outputs(p.search.cand, p.search.cand_count, p.search.cand_capacity, k, G::bfly(t, 0), (int)seg);   // the stored value, compared in the plane's type as fdas_peaks does
+            }
             if (vec2) {
 #pragma unroll
                 for (int k3 = 0; k3 < R3; ++k3)
@@ -367,17 +398,22 @@ __global__ void __launch_bounds__(S / 16, Geo<Tr, S>::MIN_BLOCKS) fdas_convolve_
                 }
             }
         } else {
+            PT mx_g = 0;
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 pass3<Tr, S>(re, im, sm2, G::bfly(t, u));
 #pragma unroll
                 for (int k3 = 0; k3 < R3; ++k3) {
                     const int s = DftSlot<R3>::of(k3);
-                    if (vmask & (1u << (u * R3 + k3)))
-                        store_stream(row + (G::bfly(t, u) - G::bfly(t, 0)) + 256 * k3,
-                                     (PT)(re[s] * re[s] + im[s] * im[s]));
+                    if (vmask & (1u << (u * R3 + k3))) {
+                        const PT pv = (PT)(re[s] * re[s] + im[s] * im[s]);
+                        store_stream(row + (G::bfly(t, u) - G::bfly(t, 0)) + 256 * k3, pv);
+                        if constexpr (SEARCH) mx_g = max(mx_g, pv);
+                    }
                 }
             }
+            if constexpr (SEARCH)
+                if (mx_g > (PT)p.search.thr) flag_outputs(p.search.cand, p.search.cand_count, p.search.cand_capacity, k, G::bfly(t, 0), (int)seg);
         }
         // no barrier needed here: the next template's first shared-memory write (exchange 1)
         // touches sm1, whose last readers finished before this template's second barrier;
@@ -385,12 +421,12 @@ __global__ void __launch_bounds__(S / 16, Geo<Tr, S>::MIN_BLOCKS) fdas_convolve_
     }
 }
 
-template <class Tr, int S>
+template <class Tr, int S, bool SEARCH>
 int launch_one(fdas_plan *p, const ConvParams &cp, int batch, int groups, cudaStream_t st)
 {
     using G = Geo<Tr, S>;
-    auto kern = fdas_convolve_kernel<Tr, S>;
-    { const int rc = fdas_optin_smem(p, FDAS_OPTIN_FFT, kern, G::SMEM_BYTES); if (rc) return rc; }
+    auto kern = fdas_convolve_kernel<Tr, S, SEARCH>;
+    { const int rc = fdas_optin_smem(p, SEARCH ? FDAS_OPTIN_FFT_SEARCH : FDAS_OPTIN_FFT, kern, G::SMEM_BYTES); if (rc) return rc; }
     const long long gx = (long long)batch * p->n_seg;
     if (gx > 2147483647LL) return FDAS_ERR_INVALID_ARG;
     kern<<<dim3((unsigned)gx, groups), G::T, G::SMEM_BYTES, st>>>(cp);
@@ -425,16 +461,36 @@ size_t smem_of(int S)
     }
 }
 
-template <class Tr>
+template <class Tr, bool SEARCH>
 int launch_prec(fdas_plan *p, const ConvParams &cp, int batch, int groups, cudaStream_t st)
 {
     switch (p->S) {
-    case 256: return launch_one<Tr, 256>(p, cp, batch, groups, st);
-    case 512: return launch_one<Tr, 512>(p, cp, batch, groups, st);
-    case 1024: return launch_one<Tr, 1024>(p, cp, batch, groups, st);
-    case 2048: return launch_one<Tr, 2048>(p, cp, batch, groups, st);
-    case 4096: return launch_one<Tr, 4096>(p, cp, batch, groups, st);
+    case 256: return launch_one<Tr, 256, SEARCH>(p, cp, batch, groups, st);
+    case 512: return launch_one<Tr, 512, SEARCH>(p, cp, batch, groups, st);
+    case 1024: return launch_one<Tr, 1024, SEARCH>(p, cp, batch, groups, st);
+    case 2048: return launch_one<Tr, 2048, SEARCH>(p, cp, batch, groups, st);
+    case 4096: return launch_one<Tr, 4096, SEARCH>(p, cp, batch, groups, st);
     default: return FDAS_ERR_UNSUPPORTED;
+    }
+}
+
+int launch_fft_form(fdas_plan *p, ConvParams &cp, int batch, const fdas_search_args *search, cudaStream_t st)
+{
+    const int groups = fft_groups(p, batch, &cp.k_per_group);
+    cp.search = search ? *search : fdas_search_args{};
+    if (search) {
+        switch (p->precision) {
+        case FDAS_F64: return launch_prec<TraitsF64, true>(p, cp, batch, groups, st);
+        case FDAS_F32: return launch_prec<TraitsF32, true>(p, cp, batch, groups, st);
+        case FDAS_BF16: return launch_prec<TraitsBF16, true>(p, cp, batch, groups, st);
+        default: return FDAS_ERR_INVALID_ARG;
+        }
+    }
+    switch (p->precision) {
+    case FDAS_F64: return launch_prec<TraitsF64, false>(p, cp, batch, groups, st);
+    case FDAS_F32: return launch_prec<TraitsF32, false>(p, cp, batch, groups, st);
+    case FDAS_BF16: return launch_prec<TraitsBF16, false>(p, cp, batch, groups, st);
+    default: return FDAS_ERR_INVALID_ARG;
     }
 }
 
@@ -457,13 +513,23 @@ int fdas_launch_convolve(fdas_plan *p, const void *spectra, void *planes, int ba
     cp.K = p->K;
     cp.L = p->L;
     cp.V = p->V;
-    const int groups = fft_groups(p, batch, &cp.k_per_group);
-    switch (p->precision) {
-    case FDAS_F64: return launch_prec<TraitsF64>(p, cp, batch, groups, st);
-    case FDAS_F32: return launch_prec<TraitsF32>(p, cp, batch, groups, st);
-    case FDAS_BF16: return launch_prec<TraitsBF16>(p, cp, batch, groups, st);
-    default: return FDAS_ERR_INVALID_ARG;
-    }
+    return launch_fft_form(p, cp, batch, nullptr, st);
+}
+
+// the overlap-save FFT form with the threshold test of fdas_search in its store loop (one series)
+int fdas_launch_convolve_fft_search(fdas_plan *p, const void *spectrum, void *plane, const fdas_search_args *search, cudaStream_t st)
+{
+    ConvParams cp;
+    cp.spectra = spectrum;
+    cp.planes = plane;
+    cp.bank = p->bank;
+    cp.twiddle = p->twiddle;
+    cp.M = p->M;
+    cp.n_seg = p->n_seg;
+    cp.K = p->K;
+    cp.L = p->L;
+    cp.V = p->V;
+    return launch_fft_form(p, cp, 1, search, st);
 }
 
 int fdas_fft_describe(fdas_plan *p, int batch, fdas_kernel_info_t *out)

@@ -16,7 +16,7 @@
 // Kernels that need the opt-in to more than 48 KB of dynamic shared memory.  The opt-in is a per-device function
 // attribute; a plan lives on one device, so the largest size requested so far is remembered per plan.
 enum {
-    FDAS_OPTIN_FFT = 0, FDAS_OPTIN_MMA_BULK, FDAS_OPTIN_MMA_BULK16, FDAS_OPTIN_MMA_SPLIT, FDAS_OPTIN_MMA_SCALAR,
+    FDAS_OPTIN_FFT = 0, FDAS_OPTIN_FFT_SEARCH, FDAS_OPTIN_MMA_BULK, FDAS_OPTIN_MMA_BULK16, FDAS_OPTIN_MMA_SPLIT, FDAS_OPTIN_MMA_SCALAR,
     FDAS_OPTIN_MMA_SCALAR16, FDAS_OPTIN_MMA_NOPLANE, FDAS_OPTIN_MMA_NOPLANE_SPLIT, FDAS_OPTIN_MMA_RECHECK,
     FDAS_OPTIN_MMA_RECHECK_SPLIT, FDAS_OPTIN_RFFT_COLS, FDAS_OPTIN_RFFT_ROWS, FDAS_OPTIN_RFFT_ROWS64, FDAS_OPTIN_HSUM, FDAS_OPTIN_SLOTS
 };
@@ -183,6 +183,8 @@ int fdas_launch_search_noplane(fdas_plan *p, const void *spectra, int batch, flo
 // the same in steps (fdas_mma_search.cu): begin, scan launches over block ranges, one recheck launch
 int fdas_launch_resolve3(fdas_plan *p, const void *volume, int n_slabs, int slab, const fdas_search_args &sa, fdas_peak3_t *peaks,
                          int capacity, int *count, cudaStream_t st);
+int fdas_launch_convolve_fft_search(fdas_plan *p, const void *spectrum, void *plane, const fdas_search_args *search, cudaStream_t st);
+int fdas_launch_resolve_cells(fdas_plan *p, const void *plane, const fdas_search_args &sa, fdas_peak_t *peaks, int capacity, cudaStream_t st);
 int fdas_search_prepare(fdas_plan *p, float thr, int *count_dev, cudaStream_t st, fdas_search_args *sa);   // fdas_plan.cu
 int fdas_noplane_block_bins(const fdas_plan *p, int batch);
 int fdas_noplane_begin(fdas_plan *p, int batch, float thr, fdas_peak_t *peaks, int capacity, int *counts, cudaStream_t st,

@@ -122,6 +122,40 @@ fdas_resolve_kernel(const PT *__restrict__ P, int K, long long M, float thr, con
     }
 }
 
+// fdas_search on the overlap-save FFT forms: the convolve launch listed, per (thread, template), "one of my 16 outputs
+// exceeds the threshold" (flag_outputs, fdas_convolve.cu: z_index = k, r = the thread's first output index i0 inside
+// its segment, power = the bits of the segment number).  A record expands to the thread's outputs
+// i = i0 + du(u) + 256 k3 (u < U = 16 / R3, k3 < R3 = S / 256; du = u for U <= 2, else (S / 16) u), of which those in
+// the segment's valid window [L, L + V) and inside the plane are read back and tested.  Overflow of the list:
+// whole-plane scan (same result).
+template <typename PT>
+__global__ void __launch_bounds__(256)
+fdas_resolve_cells_kernel(const PT *__restrict__ P, int K, long long M, float thr, const fdas_peak_t *__restrict__ cand,
+                          const int *__restrict__ cand_count, int cand_capacity, int S, int L, int V, fdas_peak_t *peaks,
+                          int capacity, int *count)
+{
+    const int n = *cand_count;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (n <= cand_capacity) {
+        const int R3 = S / 256, U = 16 / R3, T = S / 16;
+        for (long long j = tid; j < 16LL * n; j += stride) {
+            const fdas_peak_t c = cand[j >> 4];
+            const int o = (int)(j & 15), u = o / R3, k3 = o % R3;
+            const int i = c.r + (U <= 2 ? u : T * u) + 256 * k3;
+            const long long col = (long long)__float_as_int(c.power) * V - L + i;
+            if (i < L || i >= L + V || col >= M) continue;
+            test_cell<PT>(P, K, M, c.z_index, col, elem<PT>::val(P[(size_t)c.z_index * M + col]), thr, peaks, capacity, count);
+        }
+        return;
+    }
+    const long long total = (long long)K * M;
+    for (long long e = tid; e < total; e += stride) {
+        const int k = (int)(e / M);
+        test_cell<PT>(P, K, M, k, e - (long long)k * M, elem<PT>::val(P[e]), thr, peaks, capacity, count);
+    }
+}
+
 // ---- f-fdot-fddot volume (fdas_volume_peaks; reading A27): the plane rule with one more axis.  V[i][k][r],
 // i = 0..W-1; 26 neighbours, strictly greater than those that precede the cell in (i, k, r) order.
 template <typename PT>
@@ -230,6 +264,23 @@ fdas_resolve3_kernel(const PT *__restrict__ V, int W, int K, long long M, int sl
 }
 
 }  // namespace
+
+int fdas_launch_resolve_cells(fdas_plan *p, const void *plane, const fdas_search_args &sa, fdas_peak_t *peaks, int capacity, cudaStream_t st)
+{
+    const int grid = p->num_sms * 2;
+    if (p->precision == FDAS_F64)
+        fdas_resolve_cells_kernel<double><<<grid, 256, 0, st>>>((const double *)plane, p->K, p->M, sa.thr, sa.cand, sa.cand_count,
+                                                                sa.cand_capacity, p->S, p->L, p->V, peaks, capacity, sa.count_out);
+    else if (p->plane_bf16)
+        fdas_resolve_cells_kernel<bf16raw><<<grid, 256, 0, st>>>((const bf16raw *)plane, p->K, p->M, sa.thr, sa.cand, sa.cand_count,
+                                                                 sa.cand_capacity, p->S, p->L, p->V, peaks, capacity, sa.count_out);
+    else
+        fdas_resolve_cells_kernel<float><<<grid, 256, 0, st>>>((const float *)plane, p->K, p->M, sa.thr, sa.cand, sa.cand_count,
+                                                               sa.cand_capacity, p->S, p->L, p->V, peaks, capacity, sa.count_out);
+    FDAS_CUDA_TRY(p, cudaGetLastError());
+    p->launches += 1;
+    return FDAS_OK;
+}
 
 int fdas_launch_resolve3(fdas_plan *p, const void *volume, int n_slabs, int slab, const fdas_search_args &sa, fdas_peak3_t *peaks,
                          int capacity, int *count, cudaStream_t st)

@@ -316,9 +316,13 @@ static int search_on_device(fdas_plan *p, const void *spectrum_dev, void *plane_
     if (!plane_dev)   // plane-free form: scan launch + recheck launch (fdas_mma_search.cu)
         return fdas_launch_search_noplane(p, spectrum_dev, 1, threshold, peaks_dev, capacity, count_dev, st);
     if (!fdas_uses_mma(p)) {
-        int rc = fdas_launch_convolve(p, spectrum_dev, plane_dev, 1, st);
+        // overlap-save FFT forms: the store loop lists the cells above the threshold, a small launch resolves them
+        fdas_search_args sa;
+        int rc = fdas_search_prepare(p, threshold, count_dev, st, &sa);
         if (rc) return rc;
-        return fdas_launch_peaks(p, plane_dev, threshold, peaks_dev, capacity, count_dev, st);
+        rc = fdas_launch_convolve_fft_search(p, spectrum_dev, plane_dev, &sa, st);
+        if (rc) return rc;
+        return fdas_launch_resolve_cells(p, plane_dev, sa, peaks_dev, capacity, st);
     }
     fdas_search_args sa;
     { const int rc0 = fdas_search_prepare(p, threshold, count_dev, st, &sa); if (rc0) return rc0; }
