@@ -65,19 +65,28 @@ fdas_peaks_kernel(const PT *__restrict__ P, int K, long long M, float thr, fdas_
     if (M % NE == 0) {
         const VT *PV = reinterpret_cast<const VT *>(P);
         const long long nv = total / NE;
-        for (long long q = tid; q < nv; q += stride) {
-            union { VT v; PT e[NE]; } u;
-            u.v = __ldcs(PV + q);   // 128-bit streaming load
-            using CT = typename elem<PT>::cmp;
-            CT m = elem<PT>::val(u.e[0]);
+        // four 128-bit streaming loads in flight per thread; a vector holding a value above the threshold is rare
+        // (a few thousand of 1e8 on config 3) and handled out of line
+        constexpr int UNR = 4;
+        for (long long q0 = tid; q0 < nv; q0 += UNR * stride) {
+            union { VT v; PT e[NE]; } u[UNR];
 #pragma unroll
-            for (int c = 1; c < NE; ++c) m = max(m, elem<PT>::val(u.e[c]));
-            if (m > (CT)thr) {
-                const long long e0 = q * NE;
-                const int k = (int)(e0 / M);
-                const long long r = e0 - (long long)k * M;
+            for (int j = 0; j < UNR; ++j)
+                if (q0 + j * stride < nv) u[j].v = __ldcs(PV + q0 + j * stride);
 #pragma unroll
-                for (int c = 0; c < NE; ++c) test_cell<PT>(P, K, M, k, r + c, elem<PT>::val(u.e[c]), thr, peaks, capacity, count);
+            for (int j = 0; j < UNR; ++j) {
+                const long long q = q0 + j * stride;
+                if (q >= nv) break;
+                using CT = typename elem<PT>::cmp;
+                CT m = elem<PT>::val(u[j].e[0]);
+#pragma unroll
+                for (int c = 1; c < NE; ++c) m = max(m, elem<PT>::val(u[j].e[c]));
+                if (m > (CT)thr) {
+                    const long long e0 = q * NE;
+                    const int k = (int)(e0 / M);
+                    const long long r = e0 - (long long)k * M;
+                    for (int c = 0; c < NE; ++c) test_cell<PT>(P, K, M, k, r + c, elem<PT>::val(P[e0 + c]), thr, peaks, capacity, count);
+                }
             }
         }
     } else {
@@ -204,20 +213,27 @@ fdas_peaks3_kernel(const PT *__restrict__ V, int W, int K, long long M, float th
     if (M % NE == 0) {
         const VT *PV = reinterpret_cast<const VT *>(V);
         const long long nv = total / NE;
-        for (long long q = tid; q < nv; q += stride) {
-            union { VT v; PT e[NE]; } u;
-            u.v = __ldcs(PV + q);   // 128-bit streaming load
-            using CT = typename elem<PT>::cmp;
-            CT m = elem<PT>::val(u.e[0]);
+        constexpr int UNR = 4;   // four 128-bit streaming loads in flight per thread (as fdas_peaks_kernel)
+        for (long long q0 = tid; q0 < nv; q0 += UNR * stride) {
+            union { VT v; PT e[NE]; } u[UNR];
 #pragma unroll
-            for (int c = 1; c < NE; ++c) m = max(m, elem<PT>::val(u.e[c]));
-            if (m > (CT)thr) {
-                const long long e0 = q * NE;
-                const long long row = e0 / M;
-                const long long r = e0 - row * M;
-                const int i = (int)(row / K), k = (int)(row - (long long)i * K);
+            for (int j = 0; j < UNR; ++j)
+                if (q0 + j * stride < nv) u[j].v = __ldcs(PV + q0 + j * stride);
 #pragma unroll
-                for (int c = 0; c < NE; ++c) test_cell3<PT>(V, W, K, M, i, k, r + c, elem<PT>::val(u.e[c]), thr, peaks, capacity, count);
+            for (int j = 0; j < UNR; ++j) {
+                const long long q = q0 + j * stride;
+                if (q >= nv) break;
+                using CT = typename elem<PT>::cmp;
+                CT m = elem<PT>::val(u[j].e[0]);
+#pragma unroll
+                for (int c = 1; c < NE; ++c) m = max(m, elem<PT>::val(u[j].e[c]));
+                if (m > (CT)thr) {
+                    const long long e0 = q * NE;
+                    const long long row = e0 / M;
+                    const long long r = e0 - row * M;
+                    const int i = (int)(row / K), k = (int)(row - (long long)i * K);
+                    for (int c = 0; c < NE; ++c) test_cell3<PT>(V, W, K, M, i, k, r + c, elem<PT>::val(V[e0 + c]), thr, peaks, capacity, count);
+                }
             }
         }
     } else {
