@@ -26,6 +26,9 @@ template <> struct bm_elem<bm_bf16> {
     }
 };
 
+template <typename T> struct bm_cmp { using type = float; };
+template <> struct bm_cmp<double> { using type = double; };
+
 struct Best {
     double v;
     long long idx;   // k * M + r; -1 = none
@@ -79,11 +82,21 @@ __global__ void __launch_bounds__(256) fdas_band_scan_kernel(const T *__restrict
         // this block's slice of the band's columns; every row of the slice is read contiguously
         const long long per = (width + gridDim.x - 1) / gridDim.x;
         const long long c0 = r0 + (long long)blockIdx.x * per, c1 = min(c0 + per, r1 + 1);
+        // A thread meets its cells in increasing (k, r) order, so "the first cell of the largest value" is "replace on
+        // strictly greater"; compared in the plane's own type (float for float and bf16 planes: fp64 compares run at a
+        // fraction of the rate)
+        using CT = typename bm_cmp<T>::type;
+        CT bv = 0;
+        long long bi = -1;
         for (int k = 0; k < K; ++k)
             for (long long r = c0 + threadIdx.x; r < c1; r += blockDim.x) {
-                const double v = bm_elem<T>::load(P + (size_t)k * M + r);
-                mine = better(mine, Best{v, (long long)k * M + r});
+                const CT v = (CT)bm_elem<T>::load(P + (size_t)k * M + r);
+                if (bi < 0 || v > bv) {
+                    bv = v;
+                    bi = (long long)k * M + r;
+                }
             }
+        mine = Best{(double)bv, bi};
     }
     mine = block_best(mine, sh);
     if (threadIdx.x == 0) partial[(size_t)band * gridDim.x + blockIdx.x] = mine;
