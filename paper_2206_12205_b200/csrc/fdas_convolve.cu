@@ -50,7 +50,7 @@ struct TraitsF64 {
     using PT = double;        // plane element
     using E = double2;        // exchange element in shared memory
     static constexpr int VC = 1;              // complexes per 16-byte bank vector
-    static constexpr bool F_IN_REGS = false;
+    static constexpr bool F_IN_REGS = true;
     static constexpr bool TW_IN_REGS = false;
     static constexpr bool PREFETCH_H = false;
     static constexpr bool ROUND_INPUT = false;
