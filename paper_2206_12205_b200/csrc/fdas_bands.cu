@@ -82,20 +82,34 @@ __global__ void __launch_bounds__(256) fdas_band_scan_kernel(const T *__restrict
         // this block's slice of the band's columns; every row of the slice is read contiguously
         const long long per = (width + gridDim.x - 1) / gridDim.x;
         const long long c0 = r0 + (long long)blockIdx.x * per, c1 = min(c0 + per, r1 + 1);
-        // A thread meets its cells in increasing (k, r) order, so "the first cell of the largest value" is "replace on
-        // strictly greater"; compared in the plane's own type (float for float and bf16 planes: fp64 compares run at a
-        // fraction of the rate)
+        // the first cell (in (k, r) order) of the largest value; compared in the plane's own type (float for float and bf16
+        // planes: fp64 compares run at a fraction of the rate)
         using CT = typename bm_cmp<T>::type;
         CT bv = 0;
         long long bi = -1;
-        for (int k = 0; k < K; ++k)
-            for (long long r = c0 + threadIdx.x; r < c1; r += blockDim.x) {
+        // (the slice is a few hundred columns wide: a thread has one or two cells per row, so the loads of four rows are
+        // put in flight together)
+        for (long long r = c0 + threadIdx.x; r < c1; r += blockDim.x) {
+            int k = 0;
+            for (; k + 4 <= K; k += 4) {
+                CT v[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) v[j] = (CT)bm_elem<T>::load(P + (size_t)(k + j) * M + r);
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+                    if (bi < 0 || v[j] > bv || (v[j] == bv && (long long)(k + j) * M + r < bi)) {
+                        bv = v[j];
+                        bi = (long long)(k + j) * M + r;
+                    }
+            }
+            for (; k < K; ++k) {
                 const CT v = (CT)bm_elem<T>::load(P + (size_t)k * M + r);
-                if (bi < 0 || v > bv) {
+                if (bi < 0 || v > bv || (v == bv && (long long)k * M + r < bi)) {
                     bv = v;
                     bi = (long long)k * M + r;
                 }
             }
+        }
         mine = Best{(double)bv, bi};
     }
     mine = block_best(mine, sh);
