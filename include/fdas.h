@@ -86,7 +86,8 @@ typedef enum {
     FDAS_ERR_ALLOC = 2,       /* host or device allocation failed                        */
     FDAS_ERR_CUDA = 3,        /* a CUDA call failed; see fdas_last_cuda_error            */
     FDAS_ERR_NOT_BUILT = 4,   /* convolve/peaks before fdas_build_templates              */
-    FDAS_ERR_UNSUPPORTED = 5  /* legal request this build has no kernel for              */
+    FDAS_ERR_UNSUPPORTED = 5, /* legal request this build has no kernel for              */
+    FDAS_ERR_TOO_LARGE = 6    /* beyond the fixed capacity of a call that allocates nothing (fdas_search_static) */
 } fdas_status_t;
 
 /* One peak candidate (12 bytes). */
@@ -326,6 +327,27 @@ int fdas_peaks(fdas_plan_t *p, const void *plane_dev, float threshold, fdas_peak
  */
 int fdas_search(fdas_plan_t *p, const void *spectrum_dev, void *plane_dev, float threshold,
                 fdas_peak_t *peaks_dev, int capacity, int *count_dev, void *stream);
+
+/*
+ * fdas_search_static -- the plane-free fdas_search (plane_dev == NULL) of one series for callers that cannot
+ * allocate: code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  The call makes NO
+ * cudaMalloc / cudaFree and calls no allocating library routine: the scratch the two launches share (tile flags, tile
+ * list, two counters) lives in a device array compiled into the library, 262 400 bytes that every GPU loading the
+ * library holds until the process exits.  Same kernels and arithmetic as fdas_search: the same peak set, the same
+ * power bits.  The caller passes inputs and outputs as for fdas_search.
+ *   limit      M = N/2 <= FDAS_SEARCH_STATIC_MAX_BINS (2^22 bins, BASELINE.json config 3), one series per call, one
+ *              template group (K <= 127 on a symmetric grid: configs 1-4)
+ *   sharing    every call, of every plan and stream, uses the same array, which keeps the last call's contents: the
+ *              call clears what must start at zero (stream-ordered, before its first launch), and two calls that
+ *              overlap on the GPU (different streams, no ordering between them) RACE -- order them
+ *   device     the plan's device must be current (the array's address is looked up per device, once)
+ * Asynchronous on `stream`.
+ * Errors: INVALID_ARG (NULL, capacity < 0, another device current), NOT_BUILT, TOO_LARGE (M beyond the limit),
+ * UNSUPPORTED (a plan the plane-free fdas_search does not take, or more than one template group), CUDA.
+ */
+#define FDAS_SEARCH_STATIC_MAX_BINS 4194304
+int fdas_search_static(fdas_plan_t *p, const void *spectrum_dev, float threshold, fdas_peak_t *peaks_dev,
+                       int capacity, int *count_dev, void *stream);
 
 /*
  * fdas_search_batched -- fdas_search over `batch` independent series sharing the plan (BASELINE.json config 4).

@@ -15,6 +15,7 @@
 // spectrum read: the path is bound by the tensor pipe (bf16 operands) instead of the plane write.
 #include <stdio.h>
 #include <stdlib.h>
+#include <mutex>
 #include "fdas_mma_kernels.cuh"
 
 namespace {
@@ -236,4 +237,90 @@ int fdas_launch_search_noplane(fdas_plan *p, const void *spectra, int batch, flo
     if (rc == FDAS_OK) rc = fdas_noplane_scan(p, spectra, batch, &sa, 0, 0, st);
     if (rc == FDAS_OK) rc = fdas_noplane_recheck(p, spectra, batch, &sa, st);
     return rc;
+}
+
+// =====================================================================================
+// fdas_search_static (include/fdas.h): the plane-free search of ONE series with every byte of scratch in a
+// file-scope device array, for callers that may not allocate (CUDA graph capture, serving loops).  Same two
+// launches, same kernels, same arithmetic as fdas_launch_search_noplane; only where the tile flags, the tile list
+// and the two counters live differs.  One template group only: the recheck launch then keeps its strip in shared
+// memory and needs no scratch strip in global memory (and no tensor map).
+// =====================================================================================
+#define FDAS_STATIC_TILES (FDAS_SEARCH_STATIC_MAX_BINS / 128)   // 128-bin tiles of the longest series accepted
+#define FDAS_STATIC_CTR_INTS 64                                 // the two counters, padded to 256 bytes
+// [0, 64): counters | [64, 64 + TILES): tile flags | [64 + TILES, 64 + 2 TILES): tile list.  262 400 bytes, held by
+// every GPU that loads the library until the process exits; shared by every call, so calls that overlap on the GPU race.
+static __device__ __align__(256) int fdas_static_scratch[FDAS_STATIC_CTR_INTS + 2 * FDAS_STATIC_TILES];
+
+// Device address of the array on the CURRENT device.  In host code `fdas_static_scratch` is a host-side stand-in for
+// the symbol, not a device address: the address comes from cudaGetSymbolAddress, once per device, with that device
+// current (the caller checks that the plan's device is).
+static int static_scratch_address(fdas_plan *p, int **out)
+{
+    constexpr int MAX_DEV = 64;
+    static int *addr[MAX_DEV];
+    static std::mutex mu;
+    std::lock_guard<std::mutex> lock(mu);
+    const int dev = p->device;
+    if (dev >= 0 && dev < MAX_DEV && addr[dev]) {
+        *out = addr[dev];
+        return FDAS_OK;
+    }
+    int *ptr = nullptr;
+    FDAS_CUDA_TRY(p, cudaGetSymbolAddress((void **)&ptr, fdas_static_scratch));
+    if (!ptr) return FDAS_ERR_CUDA;
+    if (dev >= 0 && dev < MAX_DEV) addr[dev] = ptr;
+    *out = ptr;
+    return FDAS_OK;
+}
+
+extern "C" int fdas_search_static(fdas_plan_t *p, const void *spectrum_dev, float threshold, fdas_peak_t *peaks_dev,
+                                  int capacity, int *count_dev, void *stream)
+{
+    if (!p || !spectrum_dev || !count_dev || capacity < 0 || (capacity > 0 && !peaks_dev)) return FDAS_ERR_INVALID_ARG;
+    if (!p->built) return FDAS_ERR_NOT_BUILT;
+    // the same plans as the plane-free fdas_search, with one template group
+    if (!fdas_uses_mma(p) || p->plane_bf16 || !p->tc_bulk_ok || p->tc_groups != 1) return FDAS_ERR_UNSUPPORTED;
+    if (p->M > (long long)FDAS_SEARCH_STATIC_MAX_BINS) return FDAS_ERR_TOO_LARGE;
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = -1;
+    FDAS_CUDA_TRY(p, cudaGetDevice(&dev));
+    if (dev != p->device) return FDAS_ERR_INVALID_ARG;   // the scratch address below is that of the current device
+    int *scratch = nullptr;
+    { const int rc = static_scratch_address(p, &scratch); if (rc) return rc; }
+
+    const int split = p->precision == FDAS_F32 ? 3 : 1;
+    const int tiles = (int)((p->M + TC_TILE - 1) / TC_TILE);
+    const int R = scan_item_bins(p, 1, split, p->num_sms);
+    const uint32_t scan_smem = TbSmem(R, p->tc_KS, p->tc_NT, TC_TILE * 4, split, false).total;
+    const uint32_t recheck_smem = TbSmem(FDAS_TC_STRIP, p->tc_KS, p->tc_NT, TC_TILE * 4, split, true, p->K).total;
+    if (scan_smem > 227u * 1024u || recheck_smem > 227u * 1024u) return FDAS_ERR_UNSUPPORTED;
+
+    // the array keeps what the last call (of any plan, on any stream) left: counters and flags start at zero
+    FDAS_CUDA_TRY(p, cudaMemsetAsync(scratch, 0, sizeof(int) * (size_t)(FDAS_STATIC_CTR_INTS + tiles), st));
+    fdas_search_args sa = {};
+    sa.enabled = 1;
+    sa.thr = threshold;
+    sa.cand_span = 8;
+    sa.tile_count = scratch;
+    sa.tile_count_next = scratch + 1;
+    sa.tile_flags = scratch + FDAS_STATIC_CTR_INTS;
+    sa.tile_list = scratch + FDAS_STATIC_CTR_INTS + FDAS_STATIC_TILES;
+    sa.scratch = nullptr;   // one template group: the recheck strip is in shared memory
+    sa.peaks = peaks_dev;
+    sa.capacity = capacity;
+    sa.counts = count_dev;
+    const TbMaps no_maps = {};   // neither launch stores through a tensor map
+
+    TcParams tp;
+    tc_fill_params(p, tp, spectrum_dev, nullptr, 1, R);
+    tp.search = sa;
+    const unsigned gx = fdas_tc_split_ctas(p, tp, tp.n_blocks);
+    int rc = split == 3 ? launch_nch<3, TB_SCAN>(p, tp, gx, scan_smem, &no_maps, st) : launch_nch<1, TB_SCAN>(p, tp, gx, scan_smem, &no_maps, st);
+    if (rc) return rc;
+    tc_fill_params(p, tp, spectrum_dev, nullptr, 1, FDAS_TC_STRIP);
+    tp.search = sa;
+    tp.clustered = 0;
+    const unsigned gr = (unsigned)(tiles < p->num_sms ? tiles : p->num_sms);
+    return split == 3 ? launch_nch<3, TB_RECHECK>(p, tp, gr, recheck_smem, &no_maps, st) : launch_nch<1, TB_RECHECK>(p, tp, gr, recheck_smem, &no_maps, st);
 }

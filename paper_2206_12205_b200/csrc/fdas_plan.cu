@@ -701,6 +701,7 @@ extern "C" const char *fdas_status_string(int status)
     case FDAS_ERR_CUDA: return "FDAS_ERR_CUDA";
     case FDAS_ERR_NOT_BUILT: return "FDAS_ERR_NOT_BUILT";
     case FDAS_ERR_UNSUPPORTED: return "FDAS_ERR_UNSUPPORTED";
+    case FDAS_ERR_TOO_LARGE: return "FDAS_ERR_TOO_LARGE";
     default: return "FDAS_ERR_UNKNOWN";
     }
 }

@@ -14,7 +14,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libfdas.so")
 
 FDAS_F64, FDAS_F32, FDAS_BF16 = 0, 1, 2
-FDAS_OK, FDAS_ERR_INVALID_ARG, FDAS_ERR_ALLOC, FDAS_ERR_CUDA, FDAS_ERR_NOT_BUILT, FDAS_ERR_UNSUPPORTED = range(6)
+FDAS_OK, FDAS_ERR_INVALID_ARG, FDAS_ERR_ALLOC, FDAS_ERR_CUDA, FDAS_ERR_NOT_BUILT, FDAS_ERR_UNSUPPORTED, FDAS_ERR_TOO_LARGE = range(7)
+FDAS_SEARCH_STATIC_MAX_BINS = 1 << 22
 PRECISIONS = {"f64": FDAS_F64, "f32": FDAS_F32, "bf16": FDAS_BF16}
 FDAS_ALGO_AUTO, FDAS_ALGO_FFT, FDAS_ALGO_MMA, FDAS_ALGO_MMA_SCALAR = 0, 1, 2, 3
 ALGORITHMS = {"auto": FDAS_ALGO_AUTO, "fft": FDAS_ALGO_FFT, "mma": FDAS_ALGO_MMA,
@@ -33,6 +34,7 @@ EXPORTS = [
     "fdas_volume_create", "fdas_volume_destroy", "fdas_volume_info", "fdas_volume_w_of_index", "fdas_volume_slab",
     "fdas_volume_set_algorithm", "fdas_volume_build_templates", "fdas_volume_convolve", "fdas_volume_peaks",
     "fdas_volume_search", "fdas_volume_search_host", "fdas_volume_launch_count", "fdas_volume_last_cuda_error",
+    "fdas_search_static",
 ]
 
 
@@ -94,6 +96,7 @@ def lib() -> ctypes.CDLL:
     L.fdas_peaks.argtypes = [vp, vp, ctypes.c_float, vp, i, vp, vp]
     L.fdas_search.argtypes = [vp, vp, vp, ctypes.c_float, vp, i, vp, vp]
     L.fdas_search_batched.argtypes = [vp, vp, vp, i, ctypes.c_float, vp, i, vp, vp]
+    L.fdas_search_static.argtypes = [vp, vp, ctypes.c_float, vp, i, vp, vp]
     L.fdas_volume_create.argtypes = [ctypes.POINTER(vp), i64, dbl, dbl, dbl, dbl, i, i]
     L.fdas_volume_destroy.argtypes = [vp]
     L.fdas_volume_info.argtypes = [vp, ctypes.POINTER(fdas_volume_info_t)]
@@ -195,6 +198,11 @@ def fdas_search(h, spectrum_ptr, plane_ptr, threshold, peaks_ptr, capacity, coun
     return lib().fdas_search(h, ctypes.c_void_p(spectrum_ptr), ctypes.c_void_p(plane_ptr), float(threshold),
                              ctypes.c_void_p(peaks_ptr), int(capacity), ctypes.c_void_p(count_ptr),
                              ctypes.c_void_p(stream))
+
+
+def fdas_search_static(h, spectrum_ptr, threshold, peaks_ptr, capacity, count_ptr, stream=0):
+    return lib().fdas_search_static(h, ctypes.c_void_p(spectrum_ptr), float(threshold), ctypes.c_void_p(peaks_ptr),
+                                    int(capacity), ctypes.c_void_p(count_ptr), ctypes.c_void_p(stream))
 
 
 def fdas_search_batched(h, spectra_ptr, planes_ptr, batch, threshold, peaks_ptr, capacity, counts_ptr, stream=0):
@@ -546,6 +554,19 @@ class Plan:
         rec["r"] = raw[:, 1]
         rec["power"] = raw[:, 2].copy().view(np.float32)
         return plane, n, rec
+
+    def search_static(self, spectrum, threshold: float, peaks_buf, count_buf, capacity: int, stream: Optional[int] = None):
+        """fdas_search_static: the plane-free search with the library's built-in scratch array; the call allocates
+        nothing, so the caller brings the outputs: peaks_buf int32 [3 * capacity], count_buf int32 [1], on the device."""
+        import torch
+        assert spectrum.is_cuda and spectrum.is_contiguous() and spectrum.dtype == self.spectrum_dtype()
+        assert tuple(spectrum.shape) == (self.M,)
+        assert peaks_buf.is_cuda and peaks_buf.dtype == torch.int32 and peaks_buf.numel() >= 3 * capacity
+        assert count_buf.is_cuda and count_buf.dtype == torch.int32 and count_buf.numel() >= 1
+        if stream is None:
+            stream = torch.cuda.current_stream().cuda_stream
+        self._check(fdas_search_static(self._h, spectrum.data_ptr(), threshold, peaks_buf.data_ptr() if capacity else 0,
+                                       capacity, count_buf.data_ptr(), stream), "fdas_search_static")
 
     def search_batched(self, spectra, threshold: float, capacity: int = 4096, planes=None, stream: Optional[int] = None):
         """fdas_search_batched: spectra [B, M] on the device; planes [B, K, M] or None (plane-free form).
