@@ -43,6 +43,7 @@ METRIC = "fdas_plane_points_per_s"
 UNIT = "points/s"
 THRESH = 22.5              # DESIGN.md reading A13
 PEAK_CAPACITY = 1 << 16
+BAND_F_BIN = 100000.0      # fundamental of the band-maxima timing: bins 0 .. 16.5e5 of the 2^22 = 0.39 of the plane
 WORKLOAD = "config3: N=2^23 fp32 samples (noise seed 3 + 64 five-harmonic pulse trains), M=2^22 bins, K=97 templates (z in [-96,96] step 2), seglen 2048 -> 97 x 2^22 plane"
 N_SAMPLES = 1 << 23
 ZMAX, DZ, SEGLEN = 96.0, 2.0, 2048
@@ -405,6 +406,15 @@ def main():
             xo = torch.empty(M, dtype=torch.complex64, device="cuda")
             extra["rfft_ms"] = float(np.mean(timer(lambda: plan.spectrum(ts, xo, stream=sptr), 5, warm=1)))
             del ts, xo
+            # a6 as a pass of its own (fdas_peaks over the stored plane) and the paper's harmonic-band maxima (Table 3)
+            pk = torch.empty(3 * PEAK_CAPACITY, dtype=torch.int32, device="cuda")
+            pc = torch.zeros(1, dtype=torch.int32, device="cuda")
+            extra["peaks_ms"] = float(np.mean(timer(lambda: fdas.fdas_peaks(plan._h, plane.data_ptr(), THRESH, pk.data_ptr(), PEAK_CAPACITY,
+                                                                             pc.data_ptr(), sptr), 5, warm=1)))
+            bm = torch.empty(3 * 16, dtype=torch.int32, device="cuda")
+            extra["band_ms"] = float(np.mean(timer(lambda: fdas.fdas_band_max(plan._h, plane.data_ptr(), BAND_F_BIN, 16, bm.data_ptr(), sptr),
+                                                   5, warm=1)))
+            del pk, pc, bm
             # NEXT-4: the jerk search as a volume: 5 slabs w = -8..8 of the same bank on the same spectrum,
             # every slab convolved and the 26-neighbour peak rule applied over (w, z, r), one library call
             with torch.cuda.stream(stream):
@@ -537,6 +547,10 @@ def main():
         "harmonic_sum_4": {"ms": r["hsum_ms"], "algorithmic_gbs": hsum_bytes(K, M, 4) / (r["hsum_ms"] * 1e-3) / 1e9,
                            "note": "NEXT-3: fdas_harmonic_sum, 4 harmonics, on the headline float plane; bytes = elements read + plane written"},
         "harmonic_sum_drift_4": {"ms": r["hsum_drift_ms"], "note": "fdas_harmonic_sum_drift, 4 harmonics (window maxima, reading A26)"},
+        "peaks_pass": {"ms": r["peaks_ms"], "algorithmic_gbs": 4.0 * K * M / (r["peaks_ms"] * 1e-3) / 1e9,
+                       "note": "a6 as its own pass: fdas_peaks over the stored float plane (one read of the plane)"},
+        "band_max_16": {"ms": r["band_ms"], "algorithmic_gbs": 4.0 * K * min(M, int(16.5 * BAND_F_BIN) + 1) / (r["band_ms"] * 1e-3) / 1e9,
+                        "note": "fdas_band_max (PAPER.md Table 3): maxima of 16 harmonic bands of a %g-bin fundamental; bytes = the band columns read" % BAND_F_BIN},
         "real_fft": {"ms": r["rfft_ms"], "algorithmic_gbs": 6.0 * 4 * M / (r["rfft_ms"] * 1e-3) / 1e9,
                      "note": "NEXT-4: fdas_spectrum, fp32 real FFT of the 2^23-sample series (outside the timed step, as in the paper); "
                              "bytes = series read + spectrum written"},
