@@ -360,6 +360,7 @@ static int tc_decide(fdas_plan *p, void *planes, int batch, bool want_maps, TcDe
         const long long items = (long long)batch * ((p->M + R - 1) / R);
         if (R == 128 || (smem_total(R) <= smem_cap && items >= 2LL * sms_per_group)) break;
     }
+    R = fdas_tc_balance_items(R, p->M, batch, sms_per_group);
     d.R = R;
     d.smem = smem_total(R);
     if (d.smem > smem_cap) return FDAS_ERR_UNSUPPORTED;

@@ -154,6 +154,22 @@ static inline void tc_fill_params(const fdas_plan *p, TcParams &tp, const void *
     tp.search.cand_span = 8;
 }
 
+// Work-item size against the tail: with a handful of items per CTA the CTAs holding one item more than the others set
+// the launch time (config 2: 512 items of 1024 bins on 148 CTAs = 4 rounds where 3.46 would do).  Halving the item (at
+// most twice, never below 128 bins) is taken when it shortens the longest CTA's share of bins by 8 % or more; long
+// launches keep the largest item (fewer halo rows to load, the store pattern measured fastest).
+static inline int fdas_tc_balance_items(int R, long long M, int batch, int ctas)
+{
+    auto share = [&](int r) {
+        const long long items = (long long)batch * ((M + r - 1) / r);
+        return ((items + ctas - 1) / ctas) * r;
+    };
+    int best = R;
+    for (int r = R >> 1, n = 0; r >= 128 && n < 2; r >>= 1, ++n)
+        if (share(r) * 100 <= share(best) * 92) best = r;
+    return best;
+}
+
 // CTAs of a TB_PLANE / TB_SCAN launch over `items` work items per template group: total returned, tp.cta0 / cta_even
 // filled.  Up to 8 groups share the SMs in proportion to their cost per tile (tensor work or plane stores, whichever
 // bounds the group), at least one CTA and at most `items` each; more groups get the same number each.

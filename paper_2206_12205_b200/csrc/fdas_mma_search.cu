@@ -79,7 +79,7 @@ static int scan_item_bins(const fdas_plan *p, int batch, int split, int sms_per_
         const long long items = (long long)batch * ((p->M + R - 1) / R);
         if (R == 128 || (TbSmem(R, p->tc_KS, p->tc_NT, TC_TILE * 4, split, false).total <= 227u * 1024u && items >= 2LL * sms_per_group)) break;
     }
-    return R;
+    return fdas_tc_balance_items(R, p->M, batch, sms_per_group);
 }
 
 int fdas_tc_describe_noplane(fdas_plan *p, int batch, fdas_kernel_info_t *out)
