@@ -65,6 +65,7 @@ __device__ __forceinline__ Best block_best(Best mine, Best *sh)
     return mine;   // valid in thread 0
 }
 
+constexpr int BM_SLICE = 512;   // columns per block of fdas_band_scan_kernel (two per thread)
 // band n covers bins lo[n]..hi[n] (host-computed, clipped; lo > hi = empty)
 struct BandBounds {
     long long lo[FDAS_MAX_BANDS], hi[FDAS_MAX_BANDS];
@@ -78,37 +79,57 @@ __global__ void __launch_bounds__(256) fdas_band_scan_kernel(const T *__restrict
     const long long r0 = bb.lo[band], r1 = bb.hi[band];
     Best mine{0.0, -1};
     if (r0 <= r1) {
-        const long long width = r1 - r0 + 1;
-        // this block's slice of the band's columns; every row of the slice is read contiguously
-        const long long per = (width + gridDim.x - 1) / gridDim.x;
-        const long long c0 = r0 + (long long)blockIdx.x * per, c1 = min(c0 + per, r1 + 1);
+        // this block's slice of the band's columns: BM_SLICE columns starting at a multiple of BM_SLICE (so that every
+        // row segment starts on a 128-byte line), clipped to the band; every row of the slice is read contiguously
+        const long long a0 = (r0 / BM_SLICE + blockIdx.x) * BM_SLICE;
+        const long long c0 = a0 < r0 ? r0 : a0, c1 = min(a0 + BM_SLICE, r1 + 1);
         // the first cell (in (k, r) order) of the largest value; compared in the plane's own type (float for float and bf16
         // planes: fp64 compares run at a fraction of the rate)
         using CT = typename bm_cmp<T>::type;
         CT bv = 0;
         long long bi = -1;
-        // (the slice is a few hundred columns wide: a thread has one or two cells per row, so the loads of four rows are
-        // put in flight together)
-        for (long long r = c0 + threadIdx.x; r < c1; r += blockDim.x) {
-            int k = 0;
-            for (; k + 4 <= K; k += 4) {
-                CT v[4];
-#pragma unroll
-                for (int j = 0; j < 4; ++j) v[j] = (CT)bm_elem<T>::load(P + (size_t)(k + j) * M + r);
-#pragma unroll
-                for (int j = 0; j < 4; ++j)
-                    if (bi < 0 || v[j] > bv || (v[j] == bv && (long long)(k + j) * M + r < bi)) {
-                        bv = v[j];
-                        bi = (long long)(k + j) * M + r;
-                    }
+        auto take = [&](CT v, long long idx) {
+            if (bi < 0 || v > bv || (v == bv && idx < bi)) {
+                bv = v;
+                bi = idx;
             }
-            for (; k < K; ++k) {
-                const CT v = (CT)bm_elem<T>::load(P + (size_t)k * M + r);
-                if (bi < 0 || v > bv || (v == bv && (long long)k * M + r < bi)) {
-                    bv = v;
-                    bi = (long long)k * M + r;
+        };
+        // a thread owns columns a0 + tid and a0 + tid + 256 and walks down them with the loads of ROWS rows of both in
+        // flight: the walk is bound by the latency of its loads, not by instruction issue.  Measured on the 97 x 2^22 plane,
+        // 16 bands of 1e5 bins: float 0.138 ms with four rows, 0.157 with eight; bf16 0.128 / 0.114 ms.
+        constexpr int ROWS = sizeof(T) == 2 ? 8 : 4;
+        const long long ra = a0 + threadIdx.x, rb = ra + 256;
+        const bool has_a = ra >= c0 && ra < c1, has_b = rb >= c0 && rb < c1;
+        if (has_a && has_b) {
+            int k = 0;
+            for (; k + ROWS <= K; k += ROWS) {
+                CT va[ROWS], vb[ROWS];
+#pragma unroll
+                for (int j = 0; j < ROWS; ++j) {
+                    va[j] = (CT)bm_elem<T>::load(P + (size_t)(k + j) * M + ra);
+                    vb[j] = (CT)bm_elem<T>::load(P + (size_t)(k + j) * M + rb);
+                }
+#pragma unroll
+                for (int j = 0; j < ROWS; ++j) {
+                    take(va[j], (long long)(k + j) * M + ra);
+                    take(vb[j], (long long)(k + j) * M + rb);
                 }
             }
+            for (; k < K; ++k) {
+                take((CT)bm_elem<T>::load(P + (size_t)k * M + ra), (long long)k * M + ra);
+                take((CT)bm_elem<T>::load(P + (size_t)k * M + rb), (long long)k * M + rb);
+            }
+        } else if (has_a || has_b) {
+            const long long r = has_a ? ra : rb;
+            int k = 0;
+            for (; k + ROWS <= K; k += ROWS) {
+                CT v[ROWS];
+#pragma unroll
+                for (int j = 0; j < ROWS; ++j) v[j] = (CT)bm_elem<T>::load(P + (size_t)(k + j) * M + r);
+#pragma unroll
+                for (int j = 0; j < ROWS; ++j) take(v[j], (long long)(k + j) * M + r);
+            }
+            for (; k < K; ++k) take((CT)bm_elem<T>::load(P + (size_t)k * M + r), (long long)k * M + r);
         }
         mine = Best{(double)bv, bi};
     }
@@ -136,7 +157,21 @@ __global__ void __launch_bounds__(256) fdas_band_reduce_kernel(const Best *__res
 
 int fdas_launch_band_max(fdas_plan *p, const void *plane, double f_bin, int n_bands, fdas_peak_t *out, cudaStream_t st)
 {
-    const int nblk = p->num_sms * 2;                               // blocks per band
+    BandBounds bb;
+    for (int n = 0; n < n_bands; ++n) {
+        // Table 3: fundamental [0, 1.5 f]; band n ((n + 0.5) f, (n + 1.5) f], upper bound inclusive
+        bb.lo[n] = n == 0 ? 0 : (long long)floor((n + 0.5) * f_bin) + 1;
+        const long long hi = (long long)floor((n + 1.5) * f_bin);
+        bb.hi[n] = hi > p->M - 1 ? p->M - 1 : hi;
+    }
+    // blocks per band: the slices of BM_SLICE columns the widest band touches (blocks beyond a band's last slice report nothing)
+    long long nblk_ll = 1;
+    for (int n = 0; n < n_bands; ++n)
+        if (bb.lo[n] <= bb.hi[n]) {
+            const long long need_n = bb.hi[n] / BM_SLICE - bb.lo[n] / BM_SLICE + 1;
+            if (need_n > nblk_ll) nblk_ll = need_n;
+        }
+    const int nblk = (int)nblk_ll;
     const size_t need = (size_t)n_bands * nblk * sizeof(Best);
     if (need > p->band_scratch_bytes) {
         cudaFree(p->band_scratch);
@@ -144,13 +179,6 @@ int fdas_launch_band_max(fdas_plan *p, const void *plane, double f_bin, int n_ba
         p->band_scratch_bytes = 0;
         FDAS_CUDA_TRY(p, cudaMalloc(&p->band_scratch, need));
         p->band_scratch_bytes = need;
-    }
-    BandBounds bb;
-    for (int n = 0; n < n_bands; ++n) {
-        // Table 3: fundamental [0, 1.5 f]; band n ((n + 0.5) f, (n + 1.5) f], upper bound inclusive
-        bb.lo[n] = n == 0 ? 0 : (long long)floor((n + 0.5) * f_bin) + 1;
-        const long long hi = (long long)floor((n + 1.5) * f_bin);
-        bb.hi[n] = hi > p->M - 1 ? p->M - 1 : hi;
     }
     Best *partial = static_cast<Best *>(p->band_scratch);
     const dim3 grid((unsigned)nblk, (unsigned)n_bands);
