@@ -250,6 +250,8 @@ fdas_rfft_fast_kernel(const float2 *__restrict__ in, void *__restrict__ out_, in
             im[a] = v.x;
         }
     } else {
+        // launched as a programmatic dependent of the column pass: the twiddle table above is built while that pass drains
+        asm volatile("griddepcontrol.wait;" ::: "memory");
         const int b = blockIdx.x;
         if (b + 1 < (int)gridDim.x) {
             k1 = seq < 2 ? 2 * b + 1 + seq : L1 - 2 * b - 1 - (seq - 2);
@@ -372,8 +374,17 @@ int launch_fast_r(fdas_plan *p, int l1, int l2, const float2 *in, void *out, flo
     const size_t smem = ((size_t)G::N + (size_t)NSEQ * G::SE + (size_t)NSEQ * 16) * sizeof(float2);
     { const int rc = fdas_optin_smem(p, (COLS ? FDAS_OPTIN_RFFT_COLS : sizeof(OT2) == 16 ? FDAS_OPTIN_RFFT_ROWS64 : FDAS_OPTIN_RFFT_ROWS), kern, smem); if (rc) return rc; }
     const int seqs = COLS ? (1 << l2) : (1 << l1);       // columns m2 / rows k1
-    kern<<<seqs / NSEQ, G::T * NSEQ, smem, st>>>(in, out, l1, l2, scale);
-    FDAS_CUDA_TRY(p, cudaGetLastError());
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(seqs / NSEQ);
+    cfg.blockDim = dim3(G::T * NSEQ);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // row pass: set up while the column pass drains
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = COLS ? 0 : 1;
+    FDAS_CUDA_TRY(p, cudaLaunchKernelEx(&cfg, kern, in, out, l1, l2, scale));
     p->launches += 1;
     return FDAS_OK;
 }
