@@ -114,7 +114,7 @@ __global__ void __launch_bounds__(HD_THREADS) fdas_harmonic_drift_kernel(const I
         const int t = h >> 1;
         const int dk0 = kh - t < 0 ? (int)-kh : -t, dk1 = kh + t >= K ? (int)(K - 1 - kh) : t;
         const IT *rowh = P + (size_t)kh * M;
-        const int chunk = (HD_SPAN - 2 * t - 8) / h < HD_TILE ? (HD_SPAN - 2 * t - 8) / h : HD_TILE;   // outputs per span (3 bins of alignment slack)
+        const int chunk = (HD_SPAN - 2 * t - 16) / h < HD_TILE ? (HD_SPAN - 2 * t - 16) / h : HD_TILE;   // outputs per span (7 bins of alignment slack at either end)
         for (int c0 = 0; c0 < HD_TILE; c0 += chunk) {
             const long long rc = r0 + c0;                              // first output bin of this chunk
             if (rc * h >= M) break;
@@ -138,6 +138,39 @@ __global__ void __launch_bounds__(HD_THREADS) fdas_harmonic_drift_kernel(const I
                     reinterpret_cast<float4 *>(buf)[i] = v;
                 }
                 x_base = x_al;
+            } else if (sizeof(IT) == 2 && (M & 7) == 0) {
+                // bf16-stored planes with 16-byte aligned rows: eight elements per load, widened (bits << 16) and compared
+                // as floats (2.78 ms with one 16-bit load per element, the float plane's 1.75 ms being the faster one)
+                if constexpr (sizeof(IT) == 2) {
+                    const long long x_al = x_lo & ~7LL;
+                    const int nq = (int)((x_hi - x_al) / 8 + 1);
+                    const size_t M8 = (size_t)(M >> 3);
+                    for (int i = threadIdx.x; i < nq; i += HD_THREADS) {
+                        const uint4 *src = reinterpret_cast<const uint4 *>(rowh + (long long)dk0 * M + x_al) + i;
+                        float f[8];
+                        {
+                            const uint4 v = __ldg(src);
+                            const unsigned w4[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                            for (int e = 0; e < 4; ++e) {
+                                f[2 * e] = __uint_as_float(w4[e] << 16);
+                                f[2 * e + 1] = __uint_as_float(w4[e] & 0xFFFF0000u);
+                            }
+                        }
+                        for (int dk = dk0 + 1; dk <= dk1; ++dk) {
+                            const uint4 v = __ldg(src + (size_t)(dk - dk0) * M8);
+                            const unsigned w4[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                            for (int e = 0; e < 4; ++e) {
+                                f[2 * e] = fmaxf(f[2 * e], __uint_as_float(w4[e] << 16));
+                                f[2 * e + 1] = fmaxf(f[2 * e + 1], __uint_as_float(w4[e] & 0xFFFF0000u));
+                            }
+                        }
+                        reinterpret_cast<float4 *>(buf)[2 * i] = make_float4(f[0], f[1], f[2], f[3]);
+                        reinterpret_cast<float4 *>(buf)[2 * i + 1] = make_float4(f[4], f[5], f[6], f[7]);
+                    }
+                    x_base = x_al;
+                }
             } else {
                 for (int i = threadIdx.x; i < span; i += HD_THREADS) {
                     OT v = (OT)hs_elem<IT>::load(rowh + (long long)dk0 * M + x_lo + i);
