@@ -371,7 +371,7 @@ int fdas_search_batched(fdas_plan_t *p, const void *spectra_dev, void *planes_de
  *   fdas_search_host     fdas_search in its plane-free form where the plan allows it (no plane is allocated
  *                        anywhere), else with a plane that stays on the device; peaks_host
  *                        receives min(count, capacity) records and *count_host the total.  In the plane-free
- *                        form a spectrum of 8 MB or more is copied in four chunks on a stream of the plan's own
+ *                        form a spectrum of 8 MB or more is copied in five chunks (1/2, 1/4, 1/8, 1/16, 1/16) on a stream of the plan's own
  *                        (ordered after `stream` at entry) and every chunk is scanned as soon as the next one
  *                        has landed, so the search overlaps the copy; the result is the same.
  */

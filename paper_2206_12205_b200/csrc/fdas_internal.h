@@ -76,10 +76,11 @@ struct fdas_plan {
     fdas_peak_t *stage_peaks;
     int *stage_count;
     int stage_peaks_capacity;
+    void *host_tail;               // pinned host: [count | pad to 16 B | FDAS_TAIL_PEAKS records], the first records of a host search's result
     // fdas_search_host_batched: copy stream, events and double-buffered staging of the host pipeline
     cudaStream_t pipe_stream;
     cudaEvent_t pipe_ev[3][2];     // [h2d done | search done | d2h done][buffer]
-    cudaEvent_t chunk_ev[5];       // fdas_search_host: [0] the caller's stream at entry, [1 + c] chunk c of the spectrum on the device
+    cudaEvent_t chunk_ev[6];       // fdas_search_host: [0] the caller's stream at entry, [1 + c] chunk c of the spectrum on the device
     void *pipe_spec[2], *pipe_series[2];
     fdas_peak_t *pipe_peaks[2];
     int *pipe_count[2];
@@ -148,6 +149,7 @@ struct fdas_search_args {
     int capacity;
     int *counts;           // [batch] totals out (cleared by the scan launch)
 };
+#define FDAS_TAIL_PEAKS 1024    // records fetched together with the count by the host search forms (one synchronisation)
 #define FDAS_TC_STRIP 384   // bins per recheck work item: the flagged tile and its two neighbours
 
 #define FDAS_CUDA_TRY(p, call)                                  \

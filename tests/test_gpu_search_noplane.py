@@ -159,3 +159,14 @@ def test_search_host_scans_the_spectrum_in_chunks(F, prec, N):
         n = plan.search_host(sp, THRESH, rec, 1 << 16)
         assert n == n_ref
         assert as_set(rec[:n]) == as_set(rec_ref)
+    # the count and the first 1024 records come back in one copy, the rest (if any) in a second one: a threshold with
+    # thousands of peaks, the snprintf convention on a capacity below and above that split, capacity 0
+    _, n_low, rec_low = plan.search(torch.from_numpy(sp).cuda(), 9.0, capacity=1 << 16)
+    assert 1024 < n_low < (1 << 16)
+    n = plan.search_host(sp, 9.0, rec, 1 << 16)
+    assert n == n_low and as_set(rec[:n]) == as_set(rec_low)
+    for cap in (0, 5, 1024, 1025, 3000):
+        small = np.zeros(max(cap, 1), dtype=rec_ref.dtype)
+        assert plan.search_host(sp, 9.0, small, cap) == n_low
+        assert set(as_set(small[:min(cap, n_low)])) <= set(as_set(rec_low))
+        assert len(set(as_set(small[:min(cap, n_low)]))) == min(cap, n_low)
