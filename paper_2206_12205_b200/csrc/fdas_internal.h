@@ -79,6 +79,7 @@ struct fdas_plan {
     void *host_tail;               // pinned host: [count | pad to 16 B | FDAS_TAIL_PEAKS records], the first records of a host search's result
     // fdas_search_host_batched: copy stream, events and double-buffered staging of the host pipeline
     cudaStream_t pipe_stream;
+    cudaStream_t pipe_stream_back; // device -> host results of the pipelined host search (the host link is full duplex)
     cudaEvent_t pipe_ev[3][2];     // [h2d done | search done | d2h done][buffer]
     cudaEvent_t chunk_ev[6];       // fdas_search_host: [0] the caller's stream at entry, [1 + c] chunk c of the spectrum on the device
     void *pipe_spec[2], *pipe_series[2];

@@ -19,6 +19,7 @@ static void free_device_members(fdas_plan *p)
     cudaFree(p->rfft_scratch);
     if (p->pipe_ready) {
         cudaStreamDestroy(p->pipe_stream);
+        cudaStreamDestroy(p->pipe_stream_back);
         for (int e = 0; e < 3; ++e)
             for (int b = 0; b < 2; ++b) cudaEventDestroy(p->pipe_ev[e][b]);
         for (int c = 0; c < 6; ++c) cudaEventDestroy(p->chunk_ev[c]);
@@ -416,6 +417,7 @@ static int ensure_pipe(fdas_plan *p)
 {
     if (p->pipe_ready) return FDAS_OK;
     FDAS_CUDA_TRY(p, cudaStreamCreateWithFlags(&p->pipe_stream, cudaStreamNonBlocking));
+    FDAS_CUDA_TRY(p, cudaStreamCreateWithFlags(&p->pipe_stream_back, cudaStreamNonBlocking));
     for (int e = 0; e < 3; ++e)
         for (int b = 0; b < 2; ++b) FDAS_CUDA_TRY(p, cudaEventCreateWithFlags(&p->pipe_ev[e][b], cudaEventDisableTiming));
     for (int c = 0; c < 6; ++c) FDAS_CUDA_TRY(p, cudaEventCreateWithFlags(&p->chunk_ev[c], cudaEventDisableTiming));
@@ -521,7 +523,8 @@ extern "C" int fdas_search_host_timeseries(fdas_plan_t *p, const void *timeserie
 }
 
 // Survey form of the host path: series i+1 crosses PCIe while series i is searched.
-//   copy stream:    [wait search(i-1)] H2D spectrum(i+1)            [wait search(i)] D2H count(i), peaks(i)
+//   copy stream:    [wait search(i-1)] H2D spectrum(i+1)
+//   back stream:    [wait search(i)] D2H count(i), peaks(i)
 //   caller stream:  [wait H2D(i)] [wait D2H(i-2)] fdas_search(i)
 static int search_host_pipeline(fdas_plan_t *p, const void *spectra_host, bool timeseries, int n_series, float threshold,
                                 fdas_peak_t *peaks_host, int capacity, int *counts_host, void *stream)
@@ -552,7 +555,7 @@ static int search_host_pipeline(fdas_plan_t *p, const void *spectra_host, bool t
         }
     }
     p->pipe_capacity = capacity;
-    cudaStream_t cs = p->pipe_stream;
+    cudaStream_t cs = p->pipe_stream, bs = p->pipe_stream_back;
     const unsigned char *src = static_cast<const unsigned char *>(spectra_host);
     void *const *in_buf = timeseries ? p->pipe_series : p->pipe_spec;
     // the pipeline starts after whatever the caller queued on `stream` before this call
@@ -581,14 +584,17 @@ static int search_host_pipeline(fdas_plan_t *p, const void *spectra_host, bool t
                                              cudaMemcpyHostToDevice, cs));
             FDAS_CUDA_TRY(p, cudaEventRecord(p->pipe_ev[0][b ^ 1], cs));
         }
-        FDAS_CUDA_TRY(p, cudaStreamWaitEvent(cs, p->pipe_ev[1][b], 0));
-        FDAS_CUDA_TRY(p, cudaMemcpyAsync(counts_host + i, p->pipe_count[b], sizeof(int), cudaMemcpyDeviceToHost, cs));
+        // results of series i go back on a stream of their own: the link is full duplex, and behind the copies of the
+        // next spectra they would cost every series ~20 us of link time
+        FDAS_CUDA_TRY(p, cudaStreamWaitEvent(bs, p->pipe_ev[1][b], 0));
+        FDAS_CUDA_TRY(p, cudaMemcpyAsync(counts_host + i, p->pipe_count[b], sizeof(int), cudaMemcpyDeviceToHost, bs));
         if (capacity > 0)
             FDAS_CUDA_TRY(p, cudaMemcpyAsync(peaks_host + (size_t)i * capacity, p->pipe_peaks[b],
-                                             sizeof(fdas_peak_t) * (size_t)capacity, cudaMemcpyDeviceToHost, cs));
-        FDAS_CUDA_TRY(p, cudaEventRecord(p->pipe_ev[2][b], cs));
+                                             sizeof(fdas_peak_t) * (size_t)capacity, cudaMemcpyDeviceToHost, bs));
+        FDAS_CUDA_TRY(p, cudaEventRecord(p->pipe_ev[2][b], bs));
     }
     FDAS_CUDA_TRY(p, cudaStreamSynchronize(cs));
+    FDAS_CUDA_TRY(p, cudaStreamSynchronize(bs));
     FDAS_CUDA_TRY(p, cudaStreamSynchronize(st));
     return FDAS_OK;
 }
