@@ -341,6 +341,8 @@ int fdas_search(fdas_plan_t *p, const void *spectrum_dev, void *plane_dev, float
  *              call clears what must start at zero (stream-ordered, before its first launch), and two calls that
  *              overlap on the GPU (different streams, no ordering between them) RACE -- order them
  *   device     the plan's device must be current (the array's address is looked up per device, once)
+ *   capture    a plan's first call sets function attributes and looks the address up: make it before a stream capture;
+ *              later calls consist of one memset and two kernel launches and can be captured into a CUDA graph
  * Asynchronous on `stream`.
  * Errors: INVALID_ARG (NULL, capacity < 0, another device current), NOT_BUILT, TOO_LARGE (M beyond the limit),
  * UNSUPPORTED (a plan the plane-free fdas_search does not take, or more than one template group), CUDA.

@@ -119,3 +119,35 @@ def test_static_search_refuses_what_does_not_fit(F):
     assert F.fdas_search_static(ok._h, xs.data_ptr(), 9.0, buf.data_ptr(), 16, cnt.data_ptr(), 0) == 0
     torch.cuda.synchronize()
     assert int(cnt.item()) == 0                                                        # an all-zero spectrum has no peak
+
+
+def test_static_search_can_be_captured_into_a_cuda_graph(F):
+    # what the entry point is for: stream capture rejects cudaMalloc, so a captured call proves there is none.  The
+    # first call of a plan sets up function attributes and the scratch address; it is made before the capture.
+    import torch
+    w = workloads.config2()
+    plan = F.Plan(w.N, w.zmax, w.dz, w.seglen, "bf16")
+    x = torch.from_numpy(w.spectrum).cuda()
+    cap = 1 << 12
+    peaks_buf = torch.empty(3 * cap, dtype=torch.int32, device="cuda")
+    count_buf = torch.zeros(1, dtype=torch.int32, device="cuda")
+    _, n_ref, rec_ref = plan.search(x, THRESH, capacity=cap)
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        assert F.fdas_search_static(plan._h, x.data_ptr(), THRESH, peaks_buf.data_ptr(), cap, count_buf.data_ptr(), s.cuda_stream) == 0
+    s.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=s):
+        rc = F.fdas_search_static(plan._h, x.data_ptr(), THRESH, peaks_buf.data_ptr(), cap, count_buf.data_ptr(), s.cuda_stream)
+    assert rc == 0
+    for _ in range(2):                                   # two replays in a row: the array is cleared inside the graph
+        peaks_buf.zero_()
+        count_buf.zero_()
+        torch.cuda.synchronize()
+        g.replay()
+        torch.cuda.synchronize()
+        n = int(count_buf.item())
+        assert n == n_ref and n >= 8
+        got = sorted((int(a), int(b), float(np.int32(c).view(np.float32))) for a, b, c in peaks_buf[: 3 * n].cpu().numpy().reshape(n, 3))
+        assert got == as_set(rec_ref)
