@@ -97,6 +97,23 @@ def test_drift_tolerant_sum_on_seeded_planes(F, K_zmax, M, prec):
         check_sum(S, oh.harmonic_sum_drift(P.astype(np.float64), H, k0), H, 2.0 ** -52 if prec == "f64" else 2.0 ** -23)
 
 
+@pytest.mark.parametrize("M", [8192, 20000, 20004, 4101])
+def test_drift_tolerant_sum_of_a_bf16_plane(F, M):
+    # bf16-stored planes: rows that are 16-byte aligned (M % 8 == 0) take eight elements per load, the others one; several
+    # 1024-bin tiles, spans that start at bin 0 and end at the plane's last bin, windows clipped at the first / last rows
+    import torch
+    plan = F.Plan(2 * M, 20.0, 2.0, 1024, "bf16", plane="bf16", build=False)
+    K = plan.K
+    rng = np.random.default_rng(M + 7)
+    bits = obf.bf16_plane(rng.standard_exponential((K, M)).astype(np.float32))
+    Pd = torch.from_numpy(bits.view(np.int16)).cuda().view(torch.bfloat16)
+    wide = obf.quick_cast(bits).astype(np.float64)
+    k0 = oh.zero_row(20.0, 2.0)
+    for H in (2, 4, 5, 8):
+        S = plan.harmonic_sum(Pd, H, drift=True).cpu().numpy()
+        check_sum(S, oh.harmonic_sum_drift(wide, H, k0), H, 2.0 ** -23)
+
+
 def test_drift_tolerant_sum_gathers_an_off_grid_pulse_train(F):
     # harmonics drift into adjacent bins; the exact-multiple sum misses them, the window sum does not
     import torch
